@@ -1,0 +1,138 @@
+"""ctypes loader for the CPU parity oracle (oracle/bifrost_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: may be imported by tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs, never by the product package
+paper_2210_02472_b200.  It shares no code with the CUDA path and does not
+import it.  See the header of bifrost_oracle.cpp for what each routine computes,
+the passages of /root/reference/PAPER.md it follows and how it is pinned.
+
+All routines take host numpy arrays (float64 / int32, C-contiguous) and return
+new numpy arrays; per-sink outputs are compact (row k belongs to sink_idx[k]).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "bifrost_oracle.cpp")
+_LIB = os.path.join(_HERE, "libbifrost_oracle.so")
+
+CXXFLAGS = ["-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared"]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (plain IEEE arithmetic: no contraction, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["g++", *CXXFLAGS, _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+_D = ctypes.c_double
+_I64 = ctypes.c_int64
+_P = ctypes.c_void_p
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        common = [_I64, _P, _P, _P, _I64, _P, _I64, _D, _D, _P]
+        for name in ("oracle_acc", "oracle_acc_ld"):
+            getattr(lib, name).argtypes = common
+        for name in ("oracle_grad", "oracle_grad_ld"):
+            getattr(lib, name).argtypes = [_I64, _P, _P, _P, _P, _I64, _P, _I64, _D, _D, _P]
+        lib.oracle_dtmin.argtypes = [_I64, _P, _P, _P, _P, _I64, _P, _I64, _D, _D, _D, _P, _P, _P, _P, _P, _P]
+        for name in ("oracle_pn1", "oracle_pn1_ld"):
+            getattr(lib, name).argtypes = [_I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+        for name in ("oracle_potential", "oracle_potential_ld"):
+            getattr(lib, name).argtypes = [_I64, _P, _P, _D, _D]
+            getattr(lib, name).restype = _D
+        _lib = lib
+    return _lib
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _idx(a: Optional[np.ndarray]):
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data
+
+
+def n_threads() -> int:
+    """Number of OpenMP threads the oracle will use (OMP_NUM_THREADS or all cores)."""
+    env = os.environ.get("OMP_NUM_THREADS")
+    if env:
+        return int(env.split(",")[0])
+    return len(os.sched_getaffinity(0))
+
+
+def acc(pos, mass, G, eps, sink_idx=None, src_idx=None, long_double=False) -> np.ndarray:
+    pos, mass = _f64(pos), _f64(mass)
+    n = mass.shape[0]
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    ns = n if si is None else si.shape[0]
+    nj = n if sj is None else sj.shape[0]
+    out = np.zeros((ns, 3))
+    fn = _load().oracle_acc_ld if long_double else _load().oracle_acc
+    fn(n, pos.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps, out.ctypes.data)
+    return out
+
+
+def grad(pos, mass, acc_in, G, eps, sink_idx=None, src_idx=None, long_double=False) -> np.ndarray:
+    pos, mass, acc_in = _f64(pos), _f64(mass), _f64(acc_in)
+    n = mass.shape[0]
+    assert acc_in.shape == (n, 3)
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    ns = n if si is None else si.shape[0]
+    nj = n if sj is None else sj.shape[0]
+    out = np.zeros((ns, 3))
+    fn = _load().oracle_grad_ld if long_double else _load().oracle_grad
+    fn(n, pos.ctypes.data, mass.ctypes.data, acc_in.ctypes.data, sip, ns, sjp, nj, G, eps, out.ctypes.data)
+    return out
+
+
+def dtmin(pos, vel, mass, G, eta_ff, eta_fb, sink_idx=None, src_idx=None):
+    """Returns dict(dt_ff, dt_fb, j_ff, j_fb, margin_ff, margin_fb)."""
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    ns = n if si is None else si.shape[0]
+    nj = n if sj is None else sj.shape[0]
+    dt_ff, dt_fb = np.zeros(ns), np.zeros(ns)
+    m_ff, m_fb = np.zeros(ns), np.zeros(ns)
+    j_ff, j_fb = np.zeros(ns, dtype=np.int32), np.zeros(ns, dtype=np.int32)
+    _load().oracle_dtmin(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eta_ff, eta_fb,
+                         dt_ff.ctypes.data, dt_fb.ctypes.data, j_ff.ctypes.data, j_fb.ctypes.data,
+                         m_ff.ctypes.data, m_fb.ctypes.data)
+    return dict(dt_ff=dt_ff, dt_fb=dt_fb, j_ff=j_ff, j_fb=j_fb, margin_ff=m_ff, margin_fb=m_fb)
+
+
+def pn1(pos, vel, mass, bh_idx, G, c, long_double=False) -> np.ndarray:
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    bh = np.ascontiguousarray(bh_idx, dtype=np.int32)
+    out = np.zeros((n, 3))
+    fn = _load().oracle_pn1_ld if long_double else _load().oracle_pn1
+    fn(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, bh.ctypes.data, bh.shape[0], G, c, out.ctypes.data)
+    return out
+
+
+def potential(pos, mass, G, eps=0.0, long_double=False) -> float:
+    pos, mass = _f64(pos), _f64(mass)
+    fn = _load().oracle_potential_ld if long_double else _load().oracle_potential
+    return float(fn(mass.shape[0], pos.ctypes.data, mass.ctypes.data, G, eps))
