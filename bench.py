@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the BIFROST direct-summation hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 4|5]
+
+One STEP is one pass of the whole hot path over the workload:
+bifrost_acc -> bifrost_grad -> bifrost_dtmin -> bifrost_pn1, all particles active.
+Workload at N=1 GPU: BASELINE.json configs[3] ("config4": Plummer N = 2^20, Kroupa masses,
+central IMBH + 100 stellar BHs, eps = 0, c = 1e4) - the configuration the metric
+"... (acc+FSI grad) at N=1e6" is quoted on.  `--config 5` times the N = 2^21 acc+grad
+peak-throughput case instead (no velocities/BHs in that config: dtmin/pn1 are skipped).
+
+Metric: fp64 pair interactions/s for acc + FSI grad = n_sink * n_src / (t_acc + t_grad), one
+interaction = one ordered (sink, source) pair evaluated in one pass.
+`ms_per_step` is the whole step (all four calls); `passes` lists every call's own time.
+
+Multi-GPU (torchrun, one rank per GPU): sinks are sharded across ranks (strong scaling, total
+work fixed), with one NCCL all-gather of the accelerations between the acc and grad passes.
+
+--impl reference times the CPU oracle (oracle/, unmodified) on the host cores on a bounded
+sample of the same workload and prints the same JSON line with "impl": "reference".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 pair interactions/s (acc+FSI grad) at N=1e6; % of B200 FP64 peak"
+UNIT = "interactions/s"
+
+# FP64-pipe instruction / flop counts per pair of the kernels' inner loops (
+# cross-checked against the SASS and ncu's smsp__sass_thread_inst_executed_op_d*_pred_on).
+FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 25}
+FP64_FLOPS = {"acc": 24, "grad": 44, "dtmin": 33}     # FMA = 2, ADD/MUL = 1
+# B200 FP64 ALU peak derived from unit counts and clocks (no fp64 entry in MEASURED_PEAKS.json):
+# 148 SMs x 64 FP64 lanes/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.
+FP64_LANES_PER_SM = 64
+
+
+def fp64_peak_tflops(num_sms: int = 148, sm_max_mhz: float = 1965.0) -> float:
+    return num_sms * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i",
+                 str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1])); power.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(cfg: int):
+    from paper_2210_02472_b200 import workloads as W
+    return W.CONFIGS[cfg]()
+
+
+def workload_name(cfg: int, n: int) -> str:
+    return {4: f"config4: Plummer N=2^20={n}, Kroupa IMF, IMBH 1e-3 M + 100 stellar BHs, eps=0, c=1e4, all active; "
+               "acc + FSI grad + dtmin + PN1.0",
+            5: f"config5: Plummer N=2^21={n}, Kroupa IMF, eps=1e-5, all active; acc + FSI grad"}[cfg]
+
+
+# --------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle, as it stands, on the host cores
+# --------------------------------------------------------------------------------------
+
+def oracle_sample(w, n_sample_sinks: int, seed: int = 777):
+    """Time oracle acc + grad for a seeded sample of sinks against ALL sources.  Each sink's
+    sum is independent, so the sample's rate (pairs/s) is the full problem's rate."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    sinks = np.sort(rng.choice(w.n, size=min(n_sample_sinks, w.n), replace=False)).astype(np.int32)
+    fake_acc = np.ascontiguousarray(w.vel)      # any [n][3] field: the cost does not depend on its values
+    t0 = time.perf_counter()
+    oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=sinks)
+    t1 = time.perf_counter()
+    oracle.grad(w.pos, w.mass, fake_acc, w.G, w.eps, sink_idx=sinks)
+    t2 = time.perf_counter()
+    pairs = float(sinks.shape[0]) * w.n
+    return {"pairs": pairs, "t_acc": t1 - t0, "t_grad": t2 - t1, "n_sinks": int(sinks.shape[0])}
+
+
+def cpu_baseline(w, n_sample_sinks: int):
+    import oracle
+    s = oracle_sample(w, n_sample_sinks)
+    return {"value": s["pairs"] / (s["t_acc"] + s["t_grad"]), "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+            "sample": f"{s['n_sinks']} seeded sinks x all {w.n} sources, acc then grad "
+                      f"({s['pairs']:.3g} pairs per pass; acc {s['t_acc']:.2f} s, grad {s['t_grad']:.2f} s)"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    w = make_workload(args.config)
+    n_sinks = args.ref_sinks
+    for _ in range(args.warmup):
+        oracle_sample(w, max(8, n_sinks // 8))
+    tot_pairs, tot_t, tot_wall = 0.0, 0.0, 0.0
+    for k in range(args.steps):
+        t0 = time.perf_counter()
+        s = oracle_sample(w, n_sinks, seed=777 + k)
+        tot_wall += time.perf_counter() - t0
+        tot_pairs += s["pairs"]
+        tot_t += s["t_acc"] + s["t_grad"]
+    value = tot_pairs / tot_t
+    sample = f"each step: {n_sinks} seeded sinks x all {w.n} sources, acc then grad ({n_sinks * w.n:.3g} pairs per pass)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_wall / max(1, args.steps), "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, w.n), "reference_sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2210_02472_b200 import sharding
+    from paper_2210_02472_b200.binding import Context
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = make_workload(args.config)
+    n = w.n
+    full_path = args.config == 4
+    ctx = Context(n)
+    pos, vel, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.vel, w.mass))
+    bh = torch.from_numpy(w.bh_idx).to(dev) if full_path else None
+    b, e = sharding.sink_slice(n, rank, world)
+    sinks = None if world == 1 else torch.arange(b, e, dtype=torch.int32, device=dev)
+    n_loc = e - b
+    acc = torch.zeros((n, 3), dtype=torch.float64, device=dev)
+    grad = torch.zeros((n, 3), dtype=torch.float64, device=dev)
+    dts = (torch.full((n,), float("inf"), dtype=torch.float64, device=dev),
+           torch.full((n,), float("inf"), dtype=torch.float64, device=dev),
+           torch.full((n,), -1, dtype=torch.int32, device=dev), torch.full((n,), -1, dtype=torch.int32, device=dev))
+    apn = torch.empty((n, 3), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > L2 (126 MB)
+    names = ["acc", "allgather", "grad", "dtmin", "pn1"]
+    ev = {k: [torch.cuda.Event(enable_timing=True) for _ in range(2)] for k in names}
+
+    def step(timed: bool):
+        """One pass of the whole hot path; returns per-call device times in ms."""
+        flush.fill_(1)                                   # L2 flush, outside the timed events
+        rec = {}
+
+        def timed_call(name, fn):
+            ev[name][0].record()
+            fn()
+            ev[name][1].record()
+
+        timed_call("acc", lambda: ctx.acc(pos, mass, w.G, w.eps, sinks, None, out=acc))
+        if world > 1:
+            def gather():
+                acc.copy_(sharding.allgather_rows(acc[b:e], n))
+            timed_call("allgather", gather)
+        timed_call("grad", lambda: ctx.grad(pos, mass, acc, w.G, w.eps, sinks, None, out=grad))
+        if full_path:
+            timed_call("dtmin", lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, sinks, None, out=dts))
+            # PN1.0 is BH x N work (2e8 pairs): every rank evaluates it redundantly (it is < 0.1 % of a step)
+            timed_call("pn1", lambda: ctx.pn1(pos, vel, mass, bh, w.G, w.c, out=apn))
+        torch.cuda.synchronize()
+        for name in names:
+            if name in ("allgather",) and world == 1:
+                continue
+            if name in ("dtmin", "pn1") and not full_path:
+                continue
+            rec[name] = ev[name][0].elapsed_time(ev[name][1])
+        return rec
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(False)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    launches0 = ctx.launch_count
+    t_wall0 = time.perf_counter()
+    recs = [step(True) for _ in range(args.steps)]
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = ctx.launch_count - launches0
+    clocks = sampler.stop()
+
+    keys = list(recs[0].keys())
+    mean_ms = {k: sum(r[k] for r in recs) / len(recs) for k in keys}
+    step_ms = sum(mean_ms.values())
+    t = torch.tensor([step_ms, mean_ms["acc"] + mean_ms["grad"] + mean_ms.get("allgather", 0.0)] + [mean_ms[k] for k in keys],
+                     dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)          # max over ranks
+    t = t.cpu().tolist()
+    step_ms, accgrad_ms = t[0], t[1]
+    mean_ms = dict(zip(keys, t[2:]))
+    value = float(n) * n / (accgrad_ms * 1e-3)            # whole job: all ranks' sinks x all sources
+
+    # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if rank == 0 or world > 1:
+        def pinned(a):
+            tns = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+            return tns.numpy()
+        hpos, hvel, hmass = pinned(w.pos), pinned(w.vel), pinned(w.mass)
+        hsinks = None if world == 1 else np.arange(b, e, dtype=np.int32)
+        hacc = pinned(np.zeros((n, 3)))
+        hgrad = pinned(np.zeros((n, 3)))
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        t_ag, t_all = 0.0, 0.0
+        for it in range(1 + e2e_steps):                   # first iteration = warm-up (allocates the mirrors)
+            barrier()
+            t0 = time.perf_counter()
+            ctx.acc_host(hpos, hmass, w.G, w.eps, hsinks, None, out=hacc)
+            if world > 1:
+                g = sharding.allgather_rows(torch.from_numpy(hacc[b:e]).to(dev), n)
+                hacc[:] = g.cpu().numpy()
+            ctx.grad_host(hpos, hmass, hacc, w.G, w.eps, hsinks, None, out=hgrad)
+            t1 = time.perf_counter()
+            if full_path:
+                ctx.dtmin_host(hpos, hvel, hmass, w.G, w.eta_ff, w.eta_fb, hsinks, None)
+                ctx.pn1_host(hpos, hvel, hmass, w.bh_idx, w.G, w.c)
+            t2 = time.perf_counter()
+            if it > 0:
+                t_ag += t1 - t0
+                t_all += t2 - t0
+        tt = torch.tensor([t_ag / e2e_steps, t_all / e2e_steps], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        tt = tt.cpu().tolist()
+        idx_b = 0 if world == 1 else 4 * n_loc
+        h2d = (32 * n + idx_b) + (56 * n + idx_b) + ((56 * n + idx_b) + (56 * n + 4 * len(w.bh_idx)) if full_path else 0)
+        d2h = 24 * n_loc * 2 + ((24 * n_loc) + 24 * n if full_path else 0)
+        e2e = {"value": float(n) * n / tt[0], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * tt[1], "steps": e2e_steps,
+               "how": "bifrost_*_host entry points on pinned host arrays: H2D copies, kernels, D2H copies per call; "
+                      "value = N^2 / host wall time of acc_host + grad_host"}
+
+    if rank == 0:
+        num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak = fp64_peak_tflops(num_sms, clocks.get("sm_max_mhz") or 1965.0)
+        pairs_rank = float(max(sharding.slice_counts(n, world))) * n     # the slowest rank's share
+
+        def kern(name):
+            ms = mean_ms[name]
+            tf = pairs_rank * FP64_FLOPS[name] / (ms * 1e-3) / 1e12
+            pipe = pairs_rank * FP64_INSTR[name] / (ms * 1e-3) / (peak * 1e12 / 2)
+            return {"ms": ms, "interactions_per_s": pairs_rank / (ms * 1e-3), "tflops": tf, "frac_of_flop_peak": tf / peak,
+                    "fp64_pipe_issue_util": pipe}
+        passes = {k: kern(k) for k in ("acc", "grad", "dtmin") if k in mean_ms}
+        if "pn1" in mean_ms:
+            passes["pn1"] = {"ms": mean_ms["pn1"], "interactions_per_s": 2.0 * len(w.bh_idx) * n / (mean_ms["pn1"] * 1e-3)}
+        if "allgather" in mean_ms:
+            passes["allgather"] = {"ms": mean_ms["allgather"], "bytes": 24 * n}
+        dom = passes["grad"]
+        traffic = None
+        prof = os.path.join(ROOT, "profiles", "traffic_per_launch.json")
+        if os.path.exists(prof):
+            try:
+                traffic = json.load(open(prof)).get(f"config{args.config}", {}).get("grad_pair_kernel_dram_bytes")
+            except (OSError, ValueError):
+                traffic = None
+        roofline = {"bound": "alu", "kernel": "pair_kernel<GradPass> (bifrost_grad: pack + pair [+ reduce] timed together; "
+                                              "the pair kernel is > 99.9 % of it)",
+                    "achieved": dom["tflops"], "peak": peak, "unit": "TFLOP/s", "frac": dom["tflops"] / peak,
+                    "peak_source": f"derived: {num_sms} SMs x 64 FP64 lanes x 2 flop x clocks.max.sm "
+                                   f"(no FP64 figure in MEASURED_PEAKS.json)",
+                    "flops_per_interaction": FP64_FLOPS["grad"], "fp64_instr_per_interaction": FP64_INSTR["grad"],
+                    "fp64_pipe_issue_util": dom["fp64_pipe_issue_util"],
+                    "acc_grad_combined_frac": (FP64_FLOPS["acc"] + FP64_FLOPS["grad"]) * pairs_rank
+                    / (1e-3 * (mean_ms["acc"] + mean_ms["grad"])) / 1e12 / peak,
+                    "traffic": traffic}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload_name(args.config, n), "n": n, "seed": w.seed,
+                           "l2": "flushed between steps (256 MiB device write, outside the timed events)",
+                           "parallelism": f"sinks sharded over {world} rank(s)" + (", NCCL all-gather of acc" if world > 1 else ""),
+                           "timing": "CUDA events per C-ABI call on the launching stream, mean over steps, max over ranks"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "wall_s_timed_region": t_wall,
+                "passes": passes, "roofline": roofline}
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            oracle.build()
+            line["cpu_baseline"] = cpu_baseline(w, args.cpu_sinks)
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[4, 5])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sinks", type=int, default=2048, help="oracle sample size (sinks) for cpu_baseline")
+    ap.add_argument("--ref-sinks", type=int, default=1024, help="oracle sample size (sinks) per reference step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,133 @@
+/* bifrost.h - C ABI of the B200 (sm_100a) direct-summation force path of BIFROST's
+ * hierarchical fourth-order forward symplectic integrator (HHS-FSI).
+ *
+ * Paper: Rantala et al., "BIFROST: simulating compact subsystems in star clusters using a
+ * hierarchical fourth-order forward symplectic integrator code", arXiv:2210.02472
+ * (citations below are lines of /root/reference/PAPER.md).
+ *
+ * The library evaluates, for a set of active SINK particles i against a set of SOURCE
+ * particles j, in binary64:
+ *   bifrost_acc    softened Newtonian accelerations         (Eq. 6, Eq. 12)
+ *   bifrost_grad   the FSI gradient ("extra") force sum     (Eq. 9, Eq. 13)
+ *   bifrost_dtmin  free-fall / fly-by time-step minima      (Eq. 21, Eq. 22)
+ *   bifrost_pn1    the global PN1.0 pair term, BH x N        (§3.8, Eq. 42-43)
+ * Every step (index gather, pair kernels, fixed-order reductions, scatter) runs in
+ * hand-written CUDA kernels; there is no CPU fallback.
+ *
+ * Common conventions
+ *  - Particle arrays are indexed by particle id 0..n-1:
+ *      pos, vel, acc, out_acc, out_grad, out_acc_pn : double[n][3], row-major;  mass : double[n].
+ *  - sink_idx / src_idx / bh_idx : int32 particle ids in [0, n) (not range-checked).
+ *    NULL means "all n particles in id order" and then the matching count must equal n.
+ *  - r_ji = r_j - r_i (L65): the force on sink i points towards source j.
+ *  - A source whose id equals the sink's id is skipped ("j != i", Eq. 6).  Distinct particles
+ *    at exactly the same position with eps = 0 are outside the contract (the pair is dropped
+ *    from acc/grad instead of producing inf/NaN).
+ *  - Duplicate ids in src_idx are summed twice; duplicates in sink_idx are harmless.
+ *  - n_sink == 0 is a no-op.  n_src == 0 gives zeros (acc, grad) or +inf with id -1 (dtmin).
+ *  - Results are written only at out[sink id]; other rows are untouched (bifrost_pn1 overwrites
+ *    all n rows).  Outputs must not alias inputs.
+ *  - Device entry points: every pointer is a DEVICE pointer owned by the caller; the call is
+ *    asynchronous on `stream` (a cudaStream_t passed as void*, NULL = legacy default stream) and
+ *    never synchronises the host.  The library owns only the scratch inside bifrost_ctx, which
+ *    is allocated once in bifrost_create (no allocation afterwards).
+ *  - *_host entry points: every pointer is a HOST pointer (pinned or pageable); the call copies
+ *    the inputs to device scratch owned by the context, runs the same kernels, copies the
+ *    results back and returns after the stream has drained.
+ *  - One context per stream; concurrent calls on one context are not allowed.
+ *  - Results are bit-identical for identical inputs on the same GPU model: tiling is fixed by
+ *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
+ *  - Return value: BIFROST_OK (0) or a negative BIFROST_E* code.  Nothing is printed, nothing
+ *    aborts.  On BIFROST_ECUDA, bifrost_last_cuda_error(ctx) holds the CUDA error string.
+ */
+#ifndef BIFROST_H
+#define BIFROST_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BIFROST_OK      0
+#define BIFROST_EINVAL (-1)  /* NULL where a pointer is required, negative count, n > max_n, n >= 2^31,
+                                count/NULL-list mismatch */
+#define BIFROST_ECUDA  (-2)  /* a CUDA runtime call or kernel launch failed */
+#define BIFROST_ENOMEM (-3)  /* bifrost_create could not allocate its workspace */
+
+typedef struct bifrost_ctx bifrost_ctx;
+
+/* Create a context on CUDA device `device` able to handle up to max_n particles (ids < max_n,
+ * list lengths <= max_n).  Allocates all scratch: packed source records (80 B x max_n),
+ * split-j partials, BH flags, and device mirrors for the *_host entry points (lazily, on the
+ * first *_host call).  *ctx is set to NULL on failure. */
+int bifrost_create(bifrost_ctx** ctx, int device, int64_t max_n);
+int bifrost_destroy(bifrost_ctx* ctx);
+
+const char* bifrost_strerror(int code);                 /* static string */
+const char* bifrost_last_cuda_error(bifrost_ctx* ctx);  /* "" if none; valid until the next call */
+/* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+int64_t bifrost_launch_count(bifrost_ctx* ctx);
+
+/* bifrost_acc - PAPER.md:L75 Eq. 6 and L115-119 Eq. 12 with Plummer softening (L818):
+ *     out_acc[i] = G * sum_{j in src, j != i} mass[j] * r_ji / (|r_ji|^2 + eps^2)^(3/2),  i in sinks.
+ * eps is the softening LENGTH (eps = 0: BIFROST's unsoftened standard mode). */
+int bifrost_acc(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
+                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                double G, double eps, double* out_acc, void* stream);
+
+/* bifrost_grad - the sum of PAPER.md:L90 Eq. 9 / L123-127 Eq. 13, second pass:
+ *     out_grad[i] = G * sum_{j in src, j != i} mass[j] * [ a_ji / s^3 - 3 (a_ji . r_ji) r_ji / s^5 ],
+ *     a_ji = acc[j] - acc[i],  s^2 = |r_ji|^2 + eps^2
+ * i.e. the bare tidal-tensor contraction C_i; the caller forms the gradient acceleration
+ * a~_i = a_i + (eps_step^2 / 24) C_i (Eq. 9; Eq. 23: g_i = 2 C_i, g'_i = C_i / 24).
+ * acc[] must hold the up-to-date Newtonian acceleration of every id that appears as a sink or
+ * a source (L99: "up-to-date Newtonian accelerations are required"); which accelerations
+ * those are (all-active or inter-level, Eq. 12) is the caller's choice. */
+int bifrost_grad(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                 const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                 double G, double eps, double* out_grad, void* stream);
+
+/* bifrost_dtmin - PAPER.md:L312 Eq. 21 and L317 Eq. 22 (unsoftened), per sink i:
+ *     out_dt_ff[i] = eta_ff * min_{j in src, j != i} sqrt( |r_ij|^3 / (G (m_i + m_j)) ),  out_j_ff[i] = argmin id
+ *     out_dt_fb[i] = eta_fb * min_{j in src, j != i} |r_ij| / |v_ij|,                      out_j_fb[i] = argmin id
+ * Exact ties go to the smaller particle id.  A pair with v_ij = 0 has fly-by time +inf; if no
+ * source gives a finite value the result is +inf with id -1.  Any of the four outputs may be
+ * NULL.  The caller takes min(dt_ff, dt_fb) (L293). */
+int bifrost_dtmin(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                  const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                  double G, double eta_ff, double eta_fb,
+                  double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff, int32_t* out_j_fb, void* stream);
+
+/* bifrost_pn1 - PAPER.md:L476-488 §3.8 (Eq. 42-43): the global PN1.0 term "only for pairwise
+ * interactions when either of the particles is massive enough".  The caller supplies the ids of
+ * the massive particles (m > m_PN) in bh_idx (distinct ids; n_bh may be 0).  For every ordered
+ * pair (i, j), i != j, with i or j in bh_idx, each pair once:
+ *     out_acc_pn[i] += G m_j / (c^2 r^2) { n [ 5 G m_i / r + 4 G m_j / r + 3/2 (n.v_j)^2 - v_i.v_i
+ *                                              + 4 v_i.v_j - 2 v_j.v_j ] + (4 n.v_i - 3 n.v_j)(v_i - v_j) },
+ *     r = |r_i - r_j|,  n = (r_i - r_j) / r
+ * (standard two-body 1PN/EIH term in harmonic coordinates; the paper cites Thorne & Hartle 1985
+ * without printing it - DESIGN.md reading P1).  out_acc_pn : double[n][3], fully overwritten. */
+int bifrost_pn1(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn, void* stream);
+
+/* Host-buffer variants: same semantics, HOST pointers, synchronous (see header comment).
+ * Index lists may be NULL as above.  Outputs are written only at sink ids (other host rows are
+ * untouched), bifrost_pn1_host overwrites all n rows. */
+int bifrost_acc_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
+                     const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                     double G, double eps, double* out_acc);
+int bifrost_grad_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                      const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                      double G, double eps, double* out_grad);
+int bifrost_dtmin_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                       const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                       double G, double eta_ff, double eta_fb,
+                       double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff, int32_t* out_j_fb);
+int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                     const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIFROST_H */

@@ -1,0 +1,261 @@
+"""Thin Python binding of the C ABI in include/bifrost.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/bifrost.cu; this module only
+checks dtypes/devices, passes `tensor.data_ptr()` and the current CUDA stream, and
+allocates output tensors.  There is NO CPU fallback: if libbifrost.so is missing or
+fails to load, or a call returns an error code, a BifrostError is raised.
+
+    ctx = Context(max_n)                       # bifrost_create on the current device
+    a   = ctx.acc(pos, mass, G, eps)           # torch.float64 CUDA tensors in, tensor out
+    c   = ctx.grad(pos, mass, a, G, eps)
+    dt  = ctx.dtmin(pos, vel, mass, G, eta_ff, eta_fb)   # (dt_ff, dt_fb, j_ff, j_fb)
+    apn = ctx.pn1(pos, vel, mass, bh_idx, G, c)
+Host-buffer calls (numpy in / numpy out through bifrost_*_host): ctx.acc_host(...), etc.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbifrost.so")
+
+SYMBOLS = [
+    "bifrost_create", "bifrost_destroy", "bifrost_strerror", "bifrost_last_cuda_error", "bifrost_launch_count",
+    "bifrost_acc", "bifrost_grad", "bifrost_dtmin", "bifrost_pn1",
+    "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
+]
+
+
+class BifrostError(RuntimeError):
+    pass
+
+
+_lib = None
+_P, _I64, _D, _I = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libbifrost.so (built by paper_2210_02472_b200.build) and declare signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise BifrostError(f"{LIB_PATH} not found: run `python -m paper_2210_02472_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.bifrost_create.argtypes = [ctypes.POINTER(_P), _I, _I64]
+    lib.bifrost_destroy.argtypes = [_P]
+    lib.bifrost_strerror.argtypes = [_I]
+    lib.bifrost_strerror.restype = ctypes.c_char_p
+    lib.bifrost_last_cuda_error.argtypes = [_P]
+    lib.bifrost_last_cuda_error.restype = ctypes.c_char_p
+    lib.bifrost_launch_count.argtypes = [_P]
+    lib.bifrost_launch_count.restype = _I64
+    lists = [_P, _I64, _P, _I64]
+    lib.bifrost_acc.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P, _P]
+    lib.bifrost_grad.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P]
+    lib.bifrost_dtmin.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P, _P]
+    lib.bifrost_pn1.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P, _P]
+    lib.bifrost_acc_host.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P]
+    lib.bifrost_grad_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P]
+    lib.bifrost_dtmin_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P]
+    lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+    _lib = lib
+    return lib
+
+
+def _dev_f64(t, shape_tail, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise BifrostError(f"{name}: expected a contiguous float64 CUDA tensor")
+    if tuple(t.shape[1:]) != shape_tail:
+        raise BifrostError(f"{name}: bad shape {tuple(t.shape)}")
+    return t
+
+
+def _dev_idx(t, name):
+    import torch
+    if t is None:
+        return None, 0
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.dim() == 1):
+        raise BifrostError(f"{name}: expected a contiguous 1-D int32 CUDA tensor")
+    # an empty list is not NULL ("all particles"): hand the library a valid dummy address
+    return t, (t.data_ptr() if t.numel() else _dummy_ptr(t.device))
+
+
+_dummies = {}
+_HOST_DUMMY = np.zeros(1, dtype=np.int32)
+
+
+def _dummy_ptr(device) -> int:
+    import torch
+    if device not in _dummies:
+        _dummies[device] = torch.zeros(1, dtype=torch.int32, device=device)
+    return _dummies[device].data_ptr()
+
+
+def _host_f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _host_idx(a):
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, (a.ctypes.data if a.size else _HOST_DUMMY.ctypes.data)
+
+
+class Context:
+    """Owns one bifrost_ctx (device scratch for up to max_n particles) on `device`."""
+
+    def __init__(self, max_n: int, device: Optional[int] = None):
+        import torch
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise BifrostError("no CUDA device: the BIFROST path has no CPU fallback")
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        self.max_n = int(max_n)
+        h = _P()
+        rc = self._lib.bifrost_create(ctypes.byref(h), self.device, self.max_n)
+        if rc != 0:
+            raise BifrostError(f"bifrost_create: {self._lib.bifrost_strerror(rc).decode()}")
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.bifrost_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != 0:
+            msg = self._lib.bifrost_strerror(rc).decode()
+            cu = self._lib.bifrost_last_cuda_error(self._h).decode()
+            raise BifrostError(f"{what}: {msg}" + (f" [{cu}]" if cu else ""))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.bifrost_launch_count(self._h))
+
+    @staticmethod
+    def _stream():
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+
+    # ---- device-pointer entry points -------------------------------------------------
+    def acc(self, pos, mass, G, eps, sink_idx=None, src_idx=None, out=None):
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = torch.zeros((n, 3), dtype=torch.float64, device=pos.device)
+        _dev_f64(out, (3,), "out")
+        rc = self._lib.bifrost_acc(self._h, n, pos.data_ptr(), mass.data_ptr(), sip or None,
+                                   n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                   float(G), float(eps), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_acc")
+        return out
+
+    def grad(self, pos, mass, acc, G, eps, sink_idx=None, src_idx=None, out=None):
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass"); acc = _dev_f64(acc, (3,), "acc")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = torch.zeros((n, 3), dtype=torch.float64, device=pos.device)
+        _dev_f64(out, (3,), "out")
+        rc = self._lib.bifrost_grad(self._h, n, pos.data_ptr(), mass.data_ptr(), acc.data_ptr(), sip or None,
+                                    n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                    float(G), float(eps), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_grad")
+        return out
+
+    def dtmin(self, pos, vel, mass, G, eta_ff, eta_fb, sink_idx=None, src_idx=None, out=None):
+        """Returns (dt_ff, dt_fb, j_ff, j_fb), each of length n, written at sink ids
+        (rows of inactive particles keep their initial value: +inf / -1)."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = (torch.full((n,), float("inf"), dtype=torch.float64, device=pos.device),
+                   torch.full((n,), float("inf"), dtype=torch.float64, device=pos.device),
+                   torch.full((n,), -1, dtype=torch.int32, device=pos.device),
+                   torch.full((n,), -1, dtype=torch.int32, device=pos.device))
+        rc = self._lib.bifrost_dtmin(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
+                                     n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                     float(G), float(eta_ff), float(eta_fb),
+                                     out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), out[3].data_ptr(),
+                                     self._stream())
+        self._check(rc, "bifrost_dtmin")
+        return out
+
+    def pn1(self, pos, vel, mass, bh_idx, G, c, out=None):
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        bh, bhp = _dev_idx(bh_idx, "bh_idx")
+        if out is None:
+            out = torch.empty((n, 3), dtype=torch.float64, device=pos.device)
+        rc = self._lib.bifrost_pn1(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), bhp or None,
+                                   0 if bh is None else bh.shape[0], float(G), float(c), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_pn1")
+        return out
+
+    # ---- host-buffer entry points (numpy in, numpy out; synchronous) -----------------
+    def acc_host(self, pos, mass, G, eps, sink_idx=None, src_idx=None, out=None):
+        pos, mass = _host_f64(pos), _host_f64(mass)
+        n = mass.shape[0]
+        si, sip = _host_idx(sink_idx); sj, sjp = _host_idx(src_idx)
+        if out is None:
+            out = np.zeros((n, 3))
+        rc = self._lib.bifrost_acc_host(self._h, n, pos.ctypes.data, mass.ctypes.data, sip,
+                                        n if si is None else si.shape[0], sjp, n if sj is None else sj.shape[0],
+                                        float(G), float(eps), out.ctypes.data)
+        self._check(rc, "bifrost_acc_host")
+        return out
+
+    def grad_host(self, pos, mass, acc, G, eps, sink_idx=None, src_idx=None, out=None):
+        pos, mass, acc = _host_f64(pos), _host_f64(mass), _host_f64(acc)
+        n = mass.shape[0]
+        si, sip = _host_idx(sink_idx); sj, sjp = _host_idx(src_idx)
+        if out is None:
+            out = np.zeros((n, 3))
+        rc = self._lib.bifrost_grad_host(self._h, n, pos.ctypes.data, mass.ctypes.data, acc.ctypes.data, sip,
+                                         n if si is None else si.shape[0], sjp, n if sj is None else sj.shape[0],
+                                         float(G), float(eps), out.ctypes.data)
+        self._check(rc, "bifrost_grad_host")
+        return out
+
+    def dtmin_host(self, pos, vel, mass, G, eta_ff, eta_fb, sink_idx=None, src_idx=None):
+        pos, vel, mass = _host_f64(pos), _host_f64(vel), _host_f64(mass)
+        n = mass.shape[0]
+        si, sip = _host_idx(sink_idx); sj, sjp = _host_idx(src_idx)
+        dt_ff, dt_fb = np.full(n, np.inf), np.full(n, np.inf)
+        j_ff, j_fb = np.full(n, -1, np.int32), np.full(n, -1, np.int32)
+        rc = self._lib.bifrost_dtmin_host(self._h, n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip,
+                                          n if si is None else si.shape[0], sjp, n if sj is None else sj.shape[0],
+                                          float(G), float(eta_ff), float(eta_fb), dt_ff.ctypes.data, dt_fb.ctypes.data,
+                                          j_ff.ctypes.data, j_fb.ctypes.data)
+        self._check(rc, "bifrost_dtmin_host")
+        return dt_ff, dt_fb, j_ff, j_fb
+
+    def pn1_host(self, pos, vel, mass, bh_idx, G, c):
+        pos, vel, mass = _host_f64(pos), _host_f64(vel), _host_f64(mass)
+        n = mass.shape[0]
+        bh, bhp = _host_idx(bh_idx)
+        out = np.empty((n, 3))
+        rc = self._lib.bifrost_pn1_host(self._h, n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, bhp,
+                                        0 if bh is None else bh.shape[0], float(G), float(c), out.ctypes.data)
+        self._check(rc, "bifrost_pn1_host")
+        return out

@@ -1,0 +1,929 @@
+// bifrost.cu - sm_100a kernels and C ABI (include/bifrost.h) of the BIFROST direct-summation
+// force path: acc (Eq. 6/12), grad (Eq. 9/13), dtmin (Eq. 21/22), pn1 (§3.8) of
+// arXiv:2210.02472.  See DESIGN.md for the kernel design and the roofline that bounds it.
+//
+// Design in one paragraph.  The path is bound by the FP64 ALU pipe (64 lanes/clk/SM), so the
+// inner loops are written to the minimal number of FP64-pipe instructions per pair
+// (acc 15, grad 28, dtmin 25) and everything else (shared-memory broadcast loads, the
+// MUFU.RSQ64H seed, integer clamps/selects, loop control) rides in the other issue slots.
+//   a1  pack kernels gather sources from the index list into 16-B aligned records
+//       (acc 48 B, grad 80 B, dtmin 64 B) with the mass-scaled polynomial coefficients.
+//   a2-a4  one "pair kernel" skeleton: a CTA owns THREADS*S sinks (S per thread, in registers)
+//       and a contiguous range of source tiles; tiles are staged through shared memory with
+//       a cp.async double buffer and read back as warp-wide broadcasts (LDS.128).
+//   a5  when the source range is split across CTAs (grid.y > 1), partial results go to a
+//       [split][sink] workspace and a second kernel reduces them in fixed order.
+//   a6  pn1: BH records broadcast to all particles + a deterministic block reduction of
+//       all non-BH particles onto each BH.
+//   a7  results are scattered to out[sink id] by the last kernel of each call.
+// Reciprocal square root: y0 = MUFU.RSQ64H(r2) (relative error d ~ 2^-20), e = 1 - r2*y0^2,
+// then r2^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2) and 1/r2 = y0^2 (1 + e + e^2); truncation
+// O(e^3) ~ 1e-17.  The source record carries m, 1.5 m, 1.875 m so the polynomial yields
+// m * r2^(-3/2) directly.  r2 == 0 (a particle meeting itself at eps = 0) is handled by an
+// integer clamp of the seed's argument, which makes the pair contribute exactly 0.
+
+#include "../../include/bifrost.h"
+
+#include <cuda_runtime.h>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace {
+
+constexpr int THREADS = 128;      // threads per CTA of the pair kernels
+constexpr int TILE = 128;         // sources per shared-memory tile
+constexpr int MAX_SPLIT = 256;    // upper bound on grid.y (source-range splits)
+
+// ----------------------------------------------------------------------------------------
+// small device helpers
+// ----------------------------------------------------------------------------------------
+
+// Seed for r2^(-1/2): MUFU.RSQ64H looks only at the high word.  The signed-int max clamps
+// r2 < 2^-400 (including 0) to 2^-400 so the seed stays finite; the refinement then uses the
+// unclamped r2, giving a finite weight that multiplies a zero separation.
+__device__ __forceinline__ double rsqrt_seed(double r2) {
+    int hi = __double2hiint(r2);
+    hi = max(hi, 0x26f00000);                       // 2^-400
+    double x = __hiloint2double(hi, 0);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+struct Geom {
+    int n_sink;           // number of sinks
+    int n_src;            // number of sources (valid records)
+    int tiles_per_split;  // source tiles handled by one blockIdx.y
+    int n_split;          // gridDim.y
+    int compact;          // 1: output row = sink position k, 0: output row = sink particle id
+};
+
+// ----------------------------------------------------------------------------------------
+// Pass policies.  Each defines the packed source record, the per-sink state, the pair update
+// and how a thread's result is stored.
+// ----------------------------------------------------------------------------------------
+
+struct AccArgs {
+    const double* pos;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;        // final output [.][3]
+    double* partial;    // [split][n_sink][3]
+};
+
+struct AccPass {
+    static constexpr int REC = 6;   // x y z m 1.5m 1.875m
+    using Args = AccArgs;
+    struct Sink { double x, y, z; };
+    struct Acc { double x, y, z; };
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2];
+    }
+    __device__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
+    // 15 FP64-pipe instructions: 3 DADD, 3 DFMA (r2), DMUL t, DFMA e, 2 DFMA poly, 2 DMUL, 3 DFMA.
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 3/2 e + 15/8 e^2)
+        const double w = (y0 * t) * pm;                       // m / s^3
+        c.x = fma(w, dx, c.x); c.y = fma(w, dy, c.y); c.z = fma(w, dz, c.z);
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        if (g.n_split == 1) {
+            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
+            o[0] = a.G * c.x; o[1] = a.G * c.y; o[2] = a.G * c.z;
+        } else {
+            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
+            o[0] = c.x; o[1] = c.y; o[2] = c.z;
+        }
+    }
+};
+
+struct GradArgs {
+    const double* pos;
+    const double* acc;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;
+    double* partial;
+};
+
+struct GradPass {
+    static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m pad
+    using Args = GradArgs;
+    struct Sink { double x, y, z, ax, ay, az; };
+    struct Acc { double ux, uy, uz, wx, wy, wz; };   // U = sum w a_ji,  W = sum w (a_ji.r_ji)/s^2 r_ji
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        const size_t o = 3 * (size_t)id;
+        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
+        s.ax = a.acc[o]; s.ay = a.acc[o + 1]; s.az = a.acc[o + 2];
+    }
+    __device__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
+    // 28 FP64-pipe instructions; C_i = U - 3 W is formed once per sink in store().
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double bx = r[3] - s.ax, by = r[4] - s.ay, bz = r[5] - s.az;       // a_ji
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        const double q = fma(bx, dx, fma(by, dy, bz * dz));                       // a_ji . r_ji
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[8], r[7]), e, r[6]);
+        const double w = (y0 * t) * pm;                                           // m / s^3
+        const double y2 = fma(t, fma(e, e, e), t);                                // 1 / s^2
+        const double v = (w * y2) * q;                                            // m (a_ji.r_ji) / s^5
+        c.ux = fma(w, bx, c.ux); c.uy = fma(w, by, c.uy); c.uz = fma(w, bz, c.uz);
+        c.wx = fma(v, dx, c.wx); c.wy = fma(v, dy, c.wy); c.wz = fma(v, dz, c.wz);
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        const double cx = fma(-3.0, c.wx, c.ux), cy = fma(-3.0, c.wy, c.uy), cz = fma(-3.0, c.wz, c.uz);
+        if (g.n_split == 1) {
+            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
+            o[0] = a.G * cx; o[1] = a.G * cy; o[2] = a.G * cz;
+        } else {
+            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
+            o[0] = cx; o[1] = cy; o[2] = cz;
+        }
+    }
+};
+
+struct DtArgs {
+    const double* pos;
+    const double* vel;
+    const double* mass;
+    const int32_t* sink_idx;
+    double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
+    int32_t* pid;      // [split][2][n_sink]  their source ids
+};
+
+struct DtPass {
+    static constexpr int REC = 8;   // x y z m vx vy vz id(bits)
+    using Args = DtArgs;
+    struct Sink { double x, y, z, m, vx, vy, vz; int id; };
+    // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
+    struct Acc { double kff, kfb; int jff, jfb; };
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        const size_t o = 3 * (size_t)id;
+        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
+        s.vx = a.vel[o]; s.vy = a.vel[o + 1]; s.vz = a.vel[o + 2];
+        s.m = a.mass[id]; s.id = id;
+    }
+    __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
+    __device__ __forceinline__ static void pair(const Args&, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
+        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
+        const int jid = __double2loint(r[7]);
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
+        const double y3 = (y0 * t) * p3;
+        const double y2 = fma(t, fma(e, e, e), t);
+        double kff = (s.m + r[3]) * y3;
+        double kfb = v2 * y2;
+        if (jid == s.id) { kff = -1.0; kfb = -1.0; }          // j != i (Eq. 21, 22)
+        if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
+        if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
+        const size_t o = (size_t)split * 2 * g.n_sink + k;
+        a.pkey[o] = c.kff; a.pkey[o + g.n_sink] = c.kfb;
+        a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
+    }
+};
+
+// ----------------------------------------------------------------------------------------
+// a2-a4: the pair kernel.  grid = (ceil(n_sink / (THREADS*S)), n_split).
+// ----------------------------------------------------------------------------------------
+template <class P, int S, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ src_rec) {
+    constexpr int REC = P::REC;
+    constexpr int CHUNKS = TILE * REC * 8 / 16;            // 16-B chunks per tile
+    __shared__ __align__(16) double sm[2][TILE * REC];
+
+    typename P::Sink sink[S];
+    typename P::Acc accu[S];
+    int ids[S];
+    const int kbase = blockIdx.x * (THREADS * S) + threadIdx.x;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * THREADS;
+        const int kk = k < g.n_sink ? k : g.n_sink - 1;      // tail threads shadow the last sink
+        ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
+        P::load_sink(a, ids[s], sink[s]);
+        P::init(accu[s]);
+    }
+
+    const int n_tiles = (g.n_src + TILE - 1) / TILE;
+    const int tile0 = blockIdx.y * g.tiles_per_split;
+    const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
+
+    auto load_tile = [&](int tile, int buf) {
+        const double* gsrc = src_rec + (size_t)tile * TILE * REC;
+        for (int ch = threadIdx.x; ch < CHUNKS; ch += THREADS) cp_async16(&sm[buf][2 * ch], gsrc + 2 * ch);
+        cp_async_commit();
+    };
+
+    if (tile0 < tile1) load_tile(tile0, 0);
+    for (int tile = tile0; tile < tile1; ++tile) {
+        const int buf = (tile - tile0) & 1;
+        if (tile + 1 < tile1) { load_tile(tile + 1, buf ^ 1); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        const int cnt = min(TILE, g.n_src - tile * TILE);
+        const double* __restrict__ tb = sm[buf];
+#pragma unroll 2
+        for (int jj = 0; jj < cnt; ++jj) {
+            double r[REC];
+#pragma unroll
+            for (int q = 0; q < REC; q += 2) {
+                const double2 v = *reinterpret_cast<const double2*>(tb + jj * REC + q);
+                r[q] = v.x; r[q + 1] = v.y;
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) P::pair(a, sink[s], accu[s], r);
+        }
+        __syncthreads();
+    }
+
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * THREADS;
+        if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
+    }
+}
+
+// ----------------------------------------------------------------------------------------
+// a1: pack kernels (gather sources through the index list into aligned records; the tail of
+// the last tile is zero-filled so the cp.async stage never reads undefined memory).
+// ----------------------------------------------------------------------------------------
+__global__ void pack_acc_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
+                                const double* __restrict__ pos, const double* __restrict__ mass,
+                                double* __restrict__ rec) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n_pad) return;
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 6);
+    if (l < n_src) {
+        const int j = src_idx ? src_idx[l] : l;
+        const double m = mass[j];
+        o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
+        o[1] = make_double2(pos[3 * (size_t)j + 2], m);
+        o[2] = make_double2(1.5 * m, 1.875 * m);
+    } else {
+        o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
+    }
+}
+
+__global__ void pack_grad_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
+                                 const double* __restrict__ pos, const double* __restrict__ mass,
+                                 const double* __restrict__ acc, double* __restrict__ rec) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n_pad) return;
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 10);
+    if (l < n_src) {
+        const int j = src_idx ? src_idx[l] : l;
+        const size_t b = 3 * (size_t)j;
+        const double m = mass[j];
+        o[0] = make_double2(pos[b], pos[b + 1]);
+        o[1] = make_double2(pos[b + 2], acc[b]);
+        o[2] = make_double2(acc[b + 1], acc[b + 2]);
+        o[3] = make_double2(m, 1.5 * m);
+        o[4] = make_double2(1.875 * m, 0.0);
+    } else {
+        o[0] = o[1] = o[2] = o[3] = o[4] = make_double2(0.0, 0.0);
+    }
+}
+
+__global__ void pack_dt_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
+                               const double* __restrict__ pos, const double* __restrict__ vel,
+                               const double* __restrict__ mass, double* __restrict__ rec) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n_pad) return;
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
+    if (l < n_src) {
+        const int j = src_idx ? src_idx[l] : l;
+        const size_t b = 3 * (size_t)j;
+        o[0] = make_double2(pos[b], pos[b + 1]);
+        o[1] = make_double2(pos[b + 2], mass[j]);
+        o[2] = make_double2(vel[b], vel[b + 1]);
+        o[3] = make_double2(vel[b + 2], __hiloint2double(0, j));
+    } else {
+        o[0] = o[1] = o[2] = o[3] = make_double2(0.0, 0.0);
+    }
+}
+
+// ----------------------------------------------------------------------------------------
+// a5 + a7: fixed-order reduction over the source-range splits, then scatter.
+// ----------------------------------------------------------------------------------------
+__global__ void reduce_vec3_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
+                                   const double* __restrict__ partial, double G, double* __restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_sink) return;
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int s = 0; s < n_split; ++s) {                       // fixed order: deterministic
+        const double* p = partial + 3 * ((size_t)s * n_sink + k);
+        sx += p[0]; sy += p[1]; sz += p[2];
+    }
+    const int id = sink_idx ? sink_idx[k] : k;
+    double* o = out + 3 * (size_t)(compact ? k : id);
+    o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
+}
+
+// dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
+// Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
+__global__ void dt_finalize_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
+                                   const double* __restrict__ pkey, const int32_t* __restrict__ pid,
+                                   const double* __restrict__ pos, const double* __restrict__ vel,
+                                   const double* __restrict__ mass, double G, double eta_ff, double eta_fb,
+                                   double* __restrict__ dt_ff, double* __restrict__ dt_fb,
+                                   int32_t* __restrict__ j_ff, int32_t* __restrict__ j_fb) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_sink) return;
+    double kb[2] = {0.0, 0.0};
+    int jb[2] = {-1, -1};
+    for (int s = 0; s < n_split; ++s) {
+        for (int w = 0; w < 2; ++w) {
+            const size_t o = ((size_t)s * 2 + w) * n_sink + k;
+            const double key = pkey[o];
+            const int j = pid[o];
+            if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+        }
+    }
+    const int i = sink_idx ? sink_idx[k] : k;
+    const int row = compact ? k : i;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double tff = inf, tfb = inf;
+    if (jb[0] >= 0) {
+        const int j = jb[0];
+        const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                     dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        const double r = sqrt(r2);
+        tff = eta_ff * sqrt(__dmul_rn(r2, r) / (G * (mass[i] + mass[j])));
+    }
+    if (jb[1] >= 0) {
+        const int j = jb[1];
+        const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                     dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+        const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
+                     uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+        tfb = __dmul_rn(eta_fb, sqrt(r2)) / sqrt(v2);
+    }
+    if (dt_ff) dt_ff[row] = tff;
+    if (dt_fb) dt_fb[row] = tfb;
+    if (j_ff) j_ff[row] = jb[0];
+    if (j_fb) j_fb[row] = jb[1];
+}
+
+// ----------------------------------------------------------------------------------------
+// a6: PN1.0 pair term (§3.8).  Standard two-body 1PN acceleration in harmonic coordinates.
+// ----------------------------------------------------------------------------------------
+struct Body { double x, y, z, m, vx, vy, vz; };
+
+__device__ __forceinline__ Body load_body(const double* pos, const double* vel, const double* mass, int id) {
+    Body b;
+    const size_t o = 3 * (size_t)id;
+    b.x = pos[o]; b.y = pos[o + 1]; b.z = pos[o + 2];
+    b.vx = vel[o]; b.vy = vel[o + 1]; b.vz = vel[o + 2];
+    b.m = mass[id];
+    return b;
+}
+
+// acceleration of body `i` due to body `j`, 1/c^2 part only
+__device__ __forceinline__ void pn1_pair(const Body& i, const Body& j, double G, double inv_c2,
+                                         double& fx, double& fy, double& fz) {
+    const double rx = i.x - j.x, ry = i.y - j.y, rz = i.z - j.z;
+    const double r2 = rx * rx + ry * ry + rz * rz;
+    const double rinv = 1.0 / sqrt(r2);
+    const double nx = rx * rinv, ny = ry * rinv, nz = rz * rinv;
+    const double nvi = nx * i.vx + ny * i.vy + nz * i.vz;
+    const double nvj = nx * j.vx + ny * j.vy + nz * j.vz;
+    const double vivi = i.vx * i.vx + i.vy * i.vy + i.vz * i.vz;
+    const double vjvj = j.vx * j.vx + j.vy * j.vy + j.vz * j.vz;
+    const double vivj = i.vx * j.vx + i.vy * j.vy + i.vz * j.vz;
+    const double A = G * (5.0 * i.m + 4.0 * j.m) * rinv + 1.5 * nvj * nvj - vivi + 4.0 * vivj - 2.0 * vjvj;
+    const double B = 4.0 * nvi - 3.0 * nvj;
+    const double pref = G * j.m * inv_c2 * (rinv * rinv);
+    fx += pref * (nx * A + B * (i.vx - j.vx));
+    fy += pref * (ny * A + B * (i.vy - j.vy));
+    fz += pref * (nz * A + B * (i.vz - j.vz));
+}
+
+__global__ void pn1_flag_kernel(int n_bh, const int32_t* __restrict__ bh_idx, unsigned char* __restrict__ is_bh) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < n_bh) is_bh[bh_idx[b]] = 1;
+}
+
+// every particle i <- all BHs j != i (BH records staged through shared memory)
+constexpr int PN_THREADS = 128;
+__global__ void __launch_bounds__(PN_THREADS)
+pn1_from_bh_kernel(int n, int n_bh, const int32_t* __restrict__ bh_idx, const double* __restrict__ pos,
+                   const double* __restrict__ vel, const double* __restrict__ mass, double G, double inv_c2,
+                   double* __restrict__ out) {
+    __shared__ Body sb[PN_THREADS];
+    __shared__ int sid[PN_THREADS];
+    const int i = blockIdx.x * PN_THREADS + threadIdx.x;
+    const int ii = i < n ? i : n - 1;
+    const Body me = load_body(pos, vel, mass, ii);
+    double fx = 0.0, fy = 0.0, fz = 0.0;
+    for (int b0 = 0; b0 < n_bh; b0 += PN_THREADS) {
+        const int b = b0 + threadIdx.x;
+        if (b < n_bh) { sid[threadIdx.x] = bh_idx[b]; sb[threadIdx.x] = load_body(pos, vel, mass, bh_idx[b]); }
+        __syncthreads();
+        const int cnt = min(PN_THREADS, n_bh - b0);
+        for (int q = 0; q < cnt; ++q)
+            if (sid[q] != ii) pn1_pair(me, sb[q], G, inv_c2, fx, fy, fz);
+        __syncthreads();
+    }
+    if (i < n) { out[3 * (size_t)i] = fx; out[3 * (size_t)i + 1] = fy; out[3 * (size_t)i + 2] = fz; }
+}
+
+// each BH b <- all non-BH particles of one chunk; deterministic block reduction
+constexpr int PN_RED_THREADS = 256;
+__global__ void __launch_bounds__(PN_RED_THREADS)
+pn1_on_bh_kernel(int n, int chunk, const int32_t* __restrict__ bh_idx, const unsigned char* __restrict__ is_bh,
+                 const double* __restrict__ pos, const double* __restrict__ vel, const double* __restrict__ mass,
+                 double G, double inv_c2, double* __restrict__ partial /*[n_bh][n_chunks][3]*/) {
+    __shared__ double red[3][PN_RED_THREADS / 32];
+    const int b = blockIdx.y;
+    const Body me = load_body(pos, vel, mass, bh_idx[b]);
+    const int j0 = blockIdx.x * chunk, j1 = min(j0 + chunk, n);
+    double fx = 0.0, fy = 0.0, fz = 0.0;
+    for (int j = j0 + threadIdx.x; j < j1; j += PN_RED_THREADS) {
+        if (is_bh[j]) continue;
+        const Body o = load_body(pos, vel, mass, j);
+        pn1_pair(me, o, G, inv_c2, fx, fy, fz);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        fx += __shfl_down_sync(0xffffffffu, fx, off);
+        fy += __shfl_down_sync(0xffffffffu, fy, off);
+        fz += __shfl_down_sync(0xffffffffu, fz, off);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { red[0][warp] = fx; red[1][warp] = fy; red[2][warp] = fz; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int w = 0; w < PN_RED_THREADS / 32; ++w) { sx += red[0][w]; sy += red[1][w]; sz += red[2][w]; }
+        double* o = partial + 3 * ((size_t)b * gridDim.x + blockIdx.x);
+        o[0] = sx; o[1] = sy; o[2] = sz;
+    }
+}
+
+__global__ void pn1_bh_finalize_kernel(int n_bh, int n_chunks, const int32_t* __restrict__ bh_idx,
+                                       const double* __restrict__ partial, double* __restrict__ out) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_bh) return;
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int c = 0; c < n_chunks; ++c) {
+        const double* p = partial + 3 * ((size_t)b * n_chunks + c);
+        sx += p[0]; sy += p[1]; sz += p[2];
+    }
+    double* o = out + 3 * (size_t)bh_idx[b];
+    o[0] += sx; o[1] += sy; o[2] += sz;
+}
+
+}  // namespace
+
+// ========================================================================================
+// host side
+// ========================================================================================
+
+struct bifrost_ctx {
+    int device = 0;
+    int64_t max_n = 0;
+    int num_sms = 0;
+    double* src_rec = nullptr;       // packed source records, (max_n rounded up to TILE) * 10 doubles
+    void* partial = nullptr;         // split-j partials / pn1 partials
+    size_t partial_bytes = 0;
+    unsigned char* is_bh = nullptr;  // [max_n]
+    int64_t launches = 0;
+    char err[256] = {0};
+    // mirrors for the *_host entry points (allocated on first use)
+    bool host_ready = false;
+    cudaStream_t hstream = nullptr;
+    double *d_pos = nullptr, *d_vel = nullptr, *d_mass = nullptr, *d_acc = nullptr, *d_out = nullptr, *d_dt = nullptr;
+    int32_t *d_sink = nullptr, *d_src = nullptr, *d_j = nullptr;
+    double* h_stage = nullptr;       // pinned, 3 * max_n doubles
+    int32_t* h_stage_i = nullptr;    // pinned, 2 * max_n ints
+};
+
+namespace {
+
+#define CU_TRY(ctx, expr)                                                         \
+    do {                                                                          \
+        cudaError_t e_ = (expr);                                                  \
+        if (e_ != cudaSuccess) {                                                  \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s: %s", #expr, cudaGetErrorString(e_)); \
+            return BIFROST_ECUDA;                                                 \
+        }                                                                         \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int check_lists(bifrost_ctx* ctx, int64_t n, const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx,
+                int64_t n_src) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n >= (int64_t)1 << 31) return BIFROST_EINVAL;
+    if (n_sink < 0 || n_src < 0 || n_sink > ctx->max_n || n_src > ctx->max_n) return BIFROST_EINVAL;
+    if (!sink_idx && n_sink != n) return BIFROST_EINVAL;
+    if (!src_idx && n_src != n) return BIFROST_EINVAL;
+    return BIFROST_OK;
+}
+
+inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// Source-range split: enough CTAs for ~16 per resident slot (tail < a few %), bounded by the
+// number of source tiles, MAX_SPLIT and the partial workspace.
+Geom make_geom(const bifrost_ctx* ctx, int64_t n_sink, int64_t n_src, int sinks_per_cta, int resident_per_sm,
+               size_t partial_bytes_per_sink, bool force_partial) {
+    Geom g;
+    g.n_sink = (int)n_sink;
+    g.n_src = (int)n_src;
+    g.compact = 0;
+    const int n_tiles = ceil_div(n_src, TILE);
+    const int ctas_i = ceil_div(n_sink, sinks_per_cta);
+    const int64_t target = 16LL * ctx->num_sms * resident_per_sm;
+    int64_t split = (target + ctas_i - 1) / ctas_i;
+    if (split > n_tiles) split = n_tiles;
+    if (split > MAX_SPLIT) split = MAX_SPLIT;
+    const int64_t ws_cap = (int64_t)(ctx->partial_bytes / (partial_bytes_per_sink * (size_t)(n_sink > 0 ? n_sink : 1)));
+    if (split > ws_cap) split = ws_cap;
+    if (split < 1) split = 1;
+    g.tiles_per_split = n_tiles > 0 ? ceil_div(n_tiles, split) : 1;
+    g.n_split = n_tiles > 0 ? ceil_div(n_tiles, g.tiles_per_split) : 1;
+    (void)force_partial;
+    return g;
+}
+
+template <class P, int S, int MINB>
+int launch_pair(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
+    dim3 grid(ceil_div(g.n_sink, THREADS * S), g.n_split);
+    pair_kernel<P, S, MINB><<<grid, THREADS, 0, st>>>(a, g, ctx->src_rec);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
+             int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out, int compact,
+             cudaStream_t st) {
+    if (n_sink == 0) return BIFROST_OK;
+    constexpr int S = 4, MINB = 4;
+    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, false);
+    g.compact = compact;
+    if (n_src > 0) {
+        const int n_pad = ceil_div(n_src, TILE) * TILE;
+        pack_acc_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    AccArgs a{pos, sink_idx, eps * eps, G, out, (double*)ctx->partial};
+    int rc = launch_pair<AccPass, S, MINB>(ctx, a, g, st);
+    if (rc) return rc;
+    if (g.n_split > 1) {
+        reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
+                                                                 (const double*)ctx->partial, G, out);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    return BIFROST_OK;
+}
+
+int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+              const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+              double* out, int compact, cudaStream_t st) {
+    if (n_sink == 0) return BIFROST_OK;
+    constexpr int S = 4, MINB = 3;
+    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, false);
+    g.compact = compact;
+    if (n_src > 0) {
+        const int n_pad = ceil_div(n_src, TILE) * TILE;
+        pack_grad_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, acc, ctx->src_rec);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    GradArgs a{pos, acc, sink_idx, eps * eps, G, out, (double*)ctx->partial};
+    int rc = launch_pair<GradPass, S, MINB>(ctx, a, g, st);
+    if (rc) return rc;
+    if (g.n_split > 1) {
+        reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
+                                                                 (const double*)ctx->partial, G, out);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    return BIFROST_OK;
+}
+
+int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+               const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
+               double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact,
+               cudaStream_t st) {
+    if (n_sink == 0) return BIFROST_OK;
+    constexpr int S = 4, MINB = 3;
+    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, true);
+    g.compact = compact;
+    if (n_src > 0) {
+        const int n_pad = ceil_div(n_src, TILE) * TILE;
+        pack_dt_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, vel, mass, ctx->src_rec);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    // workspace: keys [split][2][n_sink] doubles, then ids [split][2][n_sink] ints
+    double* pkey = (double*)ctx->partial;
+    int32_t* pid = (int32_t*)(pkey + (size_t)g.n_split * 2 * n_sink);
+    DtArgs a{pos, vel, mass, sink_idx, pkey, pid};
+    int rc = launch_pair<DtPass, S, MINB>(ctx, a, g, st);
+    if (rc) return rc;
+    dt_finalize_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx, pkey, pid, pos,
+                                                             vel, mass, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+int pn1_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+             const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out, cudaStream_t st) {
+    if (n == 0) return BIFROST_OK;
+    const double inv_c2 = 1.0 / (c * c);
+    pn1_from_bh_kernel<<<ceil_div(n, PN_THREADS), PN_THREADS, 0, st>>>((int)n, (int)n_bh, bh_idx, pos, vel, mass, G,
+                                                                      inv_c2, out);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    if (n_bh == 0) return BIFROST_OK;
+    CU_TRY(ctx, cudaMemsetAsync(ctx->is_bh, 0, (size_t)n, st));
+    pn1_flag_kernel<<<ceil_div(n_bh, 256), 256, 0, st>>>((int)n_bh, bh_idx, ctx->is_bh);
+    ctx->launches++;
+    // chunks: bounded by the partial workspace and by useful parallelism
+    int64_t n_chunks = ceil_div(n, 16384);
+    const int64_t cap = (int64_t)(ctx->partial_bytes / (24 * (size_t)n_bh));
+    if (n_chunks > cap) n_chunks = cap;
+    if (n_chunks > 65535) n_chunks = 65535;
+    if (n_chunks < 1) n_chunks = 1;
+    const int chunk = ceil_div(n, n_chunks);
+    n_chunks = ceil_div(n, chunk);
+    // grid.y is limited to 65535 BHs per launch
+    for (int64_t b0 = 0; b0 < n_bh; b0 += 65535) {
+        const int nb = (int)((n_bh - b0 < 65535) ? (n_bh - b0) : 65535);
+        dim3 grid((unsigned)n_chunks, (unsigned)nb);
+        pn1_on_bh_kernel<<<grid, PN_RED_THREADS, 0, st>>>((int)n, chunk, bh_idx + b0, ctx->is_bh, pos, vel, mass, G, inv_c2,
+                                                          (double*)ctx->partial + 3 * (size_t)b0 * n_chunks);
+        ctx->launches++;
+    }
+    pn1_bh_finalize_kernel<<<ceil_div(n_bh, 128), 128, 0, st>>>((int)n_bh, (int)n_chunks, bh_idx,
+                                                               (const double*)ctx->partial, out);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+int ensure_host_mirrors(bifrost_ctx* ctx) {
+    if (ctx->host_ready) return BIFROST_OK;
+    const size_t n = (size_t)ctx->max_n;
+    CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->hstream, cudaStreamNonBlocking));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_pos, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_vel, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_mass, 8 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_acc, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_out, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_dt, 16 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_sink, 4 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_src, 4 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->d_j, 8 * n));
+    CU_TRY(ctx, cudaMallocHost(&ctx->h_stage, 24 * n));
+    CU_TRY(ctx, cudaMallocHost(&ctx->h_stage_i, 8 * n));
+    ctx->host_ready = true;
+    return BIFROST_OK;
+}
+
+// copy compact device rows back and scatter them to out[sink id] on the host (marshalling only)
+int fetch_rows(bifrost_ctx* ctx, const void* d_rows, size_t row_bytes, const int32_t* sink_idx, int64_t n_sink,
+               void* h_out, void* h_stage) {
+    if (!h_out) return BIFROST_OK;
+    if (!sink_idx) {
+        CU_TRY(ctx, cudaMemcpyAsync(h_out, d_rows, row_bytes * (size_t)n_sink, cudaMemcpyDeviceToHost, ctx->hstream));
+        CU_TRY(ctx, cudaStreamSynchronize(ctx->hstream));
+        return BIFROST_OK;
+    }
+    CU_TRY(ctx, cudaMemcpyAsync(h_stage, d_rows, row_bytes * (size_t)n_sink, cudaMemcpyDeviceToHost, ctx->hstream));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->hstream));
+    for (int64_t k = 0; k < n_sink; ++k)
+        memcpy((char*)h_out + row_bytes * (size_t)sink_idx[k], (const char*)h_stage + row_bytes * (size_t)k, row_bytes);
+    return BIFROST_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bifrost_strerror(int code) {
+    switch (code) {
+        case BIFROST_OK: return "ok";
+        case BIFROST_EINVAL: return "invalid argument";
+        case BIFROST_ECUDA: return "CUDA error (see bifrost_last_cuda_error)";
+        case BIFROST_ENOMEM: return "out of device memory";
+        default: return "unknown error";
+    }
+}
+
+const char* bifrost_last_cuda_error(bifrost_ctx* ctx) { return ctx ? ctx->err : ""; }
+int64_t bifrost_launch_count(bifrost_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
+    if (!out) return BIFROST_EINVAL;
+    *out = nullptr;
+    if (max_n <= 0 || max_n >= (int64_t)1 << 31) return BIFROST_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return BIFROST_ECUDA;
+    DeviceGuard guard(device);
+    bifrost_ctx* ctx = new (std::nothrow) bifrost_ctx();
+    if (!ctx) return BIFROST_ENOMEM;
+    ctx->device = device;
+    ctx->max_n = max_n;
+    cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
+    const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
+    ctx->partial_bytes = 24 * (size_t)max_n * 8;
+    if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
+    if (cudaMalloc(&ctx->src_rec, n_pad * 10 * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
+        cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess) {
+        cudaGetLastError();
+        bifrost_destroy(ctx);
+        return BIFROST_ENOMEM;
+    }
+    *out = ctx;
+    return BIFROST_OK;
+}
+
+int bifrost_destroy(bifrost_ctx* ctx) {
+    if (!ctx) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh);
+    cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
+    cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->h_stage_i) cudaFreeHost(ctx->h_stage_i);
+    if (ctx->hstream) cudaStreamDestroy(ctx->hstream);
+    delete ctx;
+    return BIFROST_OK;
+}
+
+int bifrost_acc(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
+                int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out_acc,
+                void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !mass || !out_acc)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return acc_impl(ctx, n, pos, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out_acc, 0, (cudaStream_t)stream);
+}
+
+int bifrost_grad(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                 const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                 double* out_grad, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !mass || !acc || !out_grad)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return grad_impl(ctx, n, pos, mass, acc, sink_idx, n_sink, src_idx, n_src, G, eps, out_grad, 0,
+                     (cudaStream_t)stream);
+}
+
+int bifrost_dtmin(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                  const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
+                  double eta_ff, double eta_fb, double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff,
+                  int32_t* out_j_fb, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !vel || !mass)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return dtmin_impl(ctx, n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eta_ff, eta_fb, out_dt_ff,
+                      out_dt_fb, out_j_ff, out_j_fb, 0, (cudaStream_t)stream);
+}
+
+int bifrost_pn1(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_bh < 0 || n_bh > n) return BIFROST_EINVAL;
+    if (n > 0 && (!pos || !vel || !mass || !out_acc_pn)) return BIFROST_EINVAL;
+    if (n_bh > 0 && !bh_idx) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return pn1_impl(ctx, n, pos, vel, mass, bh_idx, n_bh, G, c, out_acc_pn, (cudaStream_t)stream);
+}
+
+// ---- host-buffer variants --------------------------------------------------------------
+
+#define H2D(dst, src, bytes) CU_TRY(ctx, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, ctx->hstream))
+
+int bifrost_acc_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
+                     int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out_acc) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink == 0) return BIFROST_OK;
+    if (!pos || !mass || !out_acc) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if ((rc = ensure_host_mirrors(ctx))) return rc;
+    H2D(ctx->d_pos, pos, 24 * (size_t)n);
+    H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
+    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    rc = acc_impl(ctx, n, ctx->d_pos, ctx->d_mass, sink_idx ? ctx->d_sink : nullptr, n_sink,
+                  src_idx ? ctx->d_src : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
+    if (rc) return rc;
+    return fetch_rows(ctx, ctx->d_out, 24, sink_idx, n_sink, out_acc, ctx->h_stage);
+}
+
+int bifrost_grad_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                      const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
+                      double eps, double* out_grad) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink == 0) return BIFROST_OK;
+    if (!pos || !mass || !acc || !out_grad) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if ((rc = ensure_host_mirrors(ctx))) return rc;
+    H2D(ctx->d_pos, pos, 24 * (size_t)n);
+    H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    H2D(ctx->d_acc, acc, 24 * (size_t)n);
+    if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
+    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    rc = grad_impl(ctx, n, ctx->d_pos, ctx->d_mass, ctx->d_acc, sink_idx ? ctx->d_sink : nullptr, n_sink,
+                   src_idx ? ctx->d_src : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
+    if (rc) return rc;
+    return fetch_rows(ctx, ctx->d_out, 24, sink_idx, n_sink, out_grad, ctx->h_stage);
+}
+
+int bifrost_dtmin_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                       const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
+                       double eta_ff, double eta_fb, double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff,
+                       int32_t* out_j_fb) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink == 0) return BIFROST_OK;
+    if (!pos || !vel || !mass) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if ((rc = ensure_host_mirrors(ctx))) return rc;
+    H2D(ctx->d_pos, pos, 24 * (size_t)n);
+    H2D(ctx->d_vel, vel, 24 * (size_t)n);
+    H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
+    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    double* d_ff = ctx->d_dt;
+    double* d_fb = ctx->d_dt + n_sink;
+    int32_t* d_jff = ctx->d_j;
+    int32_t* d_jfb = ctx->d_j + n_sink;
+    rc = dtmin_impl(ctx, n, ctx->d_pos, ctx->d_vel, ctx->d_mass, sink_idx ? ctx->d_sink : nullptr, n_sink,
+                    src_idx ? ctx->d_src : nullptr, n_src, G, eta_ff, eta_fb, d_ff, d_fb, d_jff, d_jfb, 1, ctx->hstream);
+    if (rc) return rc;
+    if ((rc = fetch_rows(ctx, d_ff, 8, sink_idx, n_sink, out_dt_ff, ctx->h_stage))) return rc;
+    if ((rc = fetch_rows(ctx, d_fb, 8, sink_idx, n_sink, out_dt_fb, ctx->h_stage))) return rc;
+    if ((rc = fetch_rows(ctx, d_jff, 4, sink_idx, n_sink, out_j_ff, ctx->h_stage_i))) return rc;
+    if ((rc = fetch_rows(ctx, d_jfb, 4, sink_idx, n_sink, out_j_fb, ctx->h_stage_i))) return rc;
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->hstream));
+    return BIFROST_OK;
+}
+
+int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                     const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_bh < 0 || n_bh > n) return BIFROST_EINVAL;
+    if (n == 0) return BIFROST_OK;
+    if (!pos || !vel || !mass || !out_acc_pn || (n_bh > 0 && !bh_idx)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    int rc;
+    if ((rc = ensure_host_mirrors(ctx))) return rc;
+    H2D(ctx->d_pos, pos, 24 * (size_t)n);
+    H2D(ctx->d_vel, vel, 24 * (size_t)n);
+    H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    if (n_bh) H2D(ctx->d_sink, bh_idx, 4 * (size_t)n_bh);
+    rc = pn1_impl(ctx, n, ctx->d_pos, ctx->d_vel, ctx->d_mass, ctx->d_sink, n_bh, G, c, ctx->d_out, ctx->hstream);
+    if (rc) return rc;
+    return fetch_rows(ctx, ctx->d_out, 24, nullptr, n, out_acc_pn, ctx->h_stage);
+}
+
+}  // extern "C"

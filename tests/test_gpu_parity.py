@@ -1,0 +1,305 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  All tests here need a B200 (`-m gpu`).
+
+Gates (BASELINE.json north_star):
+  acc, grad, acc_pn : per-component normwise relative error over the sink set <= 1e-12
+  dt_ff, dt_fb      : max relative error <= 1e-13
+  j_ff, j_fb        : identical (where the oracle's runner-up margin exceeds 1e-12; see reading T4)
+"""
+import numpy as np
+import pytest
+
+import oracle
+from conftest import normwise_rel_err, workload
+from paper_2210_02472_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_VEC = 1e-12
+TOL_DT = 1e-13
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as _torch
+    if not _torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return _torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch):
+    from paper_2210_02472_b200.binding import Context
+    c = Context(1 << 21)
+    yield c
+    c.close()
+
+
+def dev(torch, a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def check_vec(got, ref, what, tol=TOL_VEC):
+    err = normwise_rel_err(got, ref)
+    assert np.isfinite(got).all(), what
+    assert (err <= tol).all(), f"{what}: normwise rel err {err}"
+    return err
+
+
+def check_dt(got, ref, what):
+    """got = (dt_ff, dt_fb, j_ff, j_fb) numpy, rows of the sinks; ref = oracle dict."""
+    for name, g in (("dt_ff", got[0]), ("dt_fb", got[1])):
+        r = ref[name]
+        fin = np.isfinite(r)
+        assert np.array_equal(np.isfinite(g), fin), f"{what}: {name} finiteness"
+        rel = np.abs(g[fin] / r[fin] - 1.0)
+        assert rel.size == 0 or rel.max() <= TOL_DT, f"{what}: {name} rel err {rel.max()}"
+    for name, g, marg in (("j_ff", got[2], ref["margin_ff"]), ("j_fb", got[3], ref["margin_fb"])):
+        r = ref[name]
+        bad = g != r
+        # a mismatch is only admissible when best and runner-up agree to rounding (reading T4)
+        assert not (bad & ~(marg < 1e-12)).any(), f"{what}: {name} argmin mismatch at {np.flatnonzero(bad)[:8]}"
+        assert bad.mean() <= 1e-4, f"{what}: {name} too many near-tie mismatches"
+
+
+def run_all(torch, ctx, w, sinks=None, srcs=None, acc_full=None):
+    """GPU acc / grad / dtmin for workload w restricted to (sinks, srcs); returns numpy rows at the sinks."""
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    si = None if sinks is None else dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    rows = slice(None) if sinks is None else sinks
+    a = ctx.acc(pos, mass, w.G, w.eps, si, sj)
+    acc_in = a if acc_full is None else dev(torch, acc_full)
+    c = ctx.grad(pos, mass, acc_in, w.G, w.eps, si, sj)
+    d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, sj)
+    torch.cuda.synchronize()
+    return (a.cpu().numpy()[rows], c.cpu().numpy()[rows], tuple(t.cpu().numpy()[rows] for t in d),
+            acc_in.cpu().numpy())
+
+
+# ---- config 1: N = 1024, all active --------------------------------------------------
+
+def test_config1_all_active(torch, ctx):
+    w = workload(1)
+    a, c, d, acc_in = run_all(torch, ctx, w)
+    a_ref = oracle.acc(w.pos, w.mass, w.G, w.eps)
+    check_vec(a, a_ref, "acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps), "grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb), "dtmin")
+    # full pipeline (grad fed the oracle's own acc) also within the gate
+    check_vec(c, oracle.grad(w.pos, w.mass, a_ref, w.G, w.eps), "grad(oracle acc)", tol=1e-11)
+
+
+# ---- config 2: N = 16384, sinks = 2^k random subsets, sources = all ---------------------
+
+@pytest.mark.parametrize("k", [0, 1, 2, 5, 7, 9, 12, 14])
+def test_config2_active_subsets(torch, ctx, k):
+    w = workload(2)
+    sinks = W.config2_sink_list(k)
+    pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+    acc_full = ctx.acc(pos, mass, w.G, w.eps).cpu().numpy()          # a_k for every particle (reading G2)
+    a, c, d, _ = run_all(torch, ctx, w, sinks=sinks, acc_full=acc_full)
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=sinks), f"acc k={k}")
+    assert np.array_equal(a, acc_full[sinks])                         # subset call == rows of the full call
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sink_idx=sinks), f"grad k={k}")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sink_idx=sinks), f"dtmin k={k}")
+
+
+# ---- config 3: N = 131072 with binaries, eps = 0, active-fraction sweep -----------------
+
+@pytest.mark.parametrize("frac_log2", [10, 7, 4, 0])
+def test_config3_active_fraction(torch, ctx, frac_log2):
+    w = workload(3)
+    sinks = W.config3_sink_list(frac_log2)
+    pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+    acc_full = ctx.acc(pos, mass, w.G, w.eps).cpu().numpy()
+    a, c, d, _ = run_all(torch, ctx, w, sinks=None if frac_log2 == 0 else sinks, acc_full=acc_full)
+    # the oracle checks every sink up to 8192 sinks, else a seeded sample of 4096 of them
+    if sinks.shape[0] > 8192:
+        pick = np.sort(np.random.default_rng(33).choice(sinks.shape[0], 4096, replace=False))
+    else:
+        pick = np.arange(sinks.shape[0])
+    chk = sinks[pick]
+    check_vec(a[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=chk), f"acc 2^-{frac_log2}")
+    check_vec(c[pick], oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sink_idx=chk), f"grad 2^-{frac_log2}")
+    check_dt(tuple(x[pick] for x in d), oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sink_idx=chk),
+             f"dtmin 2^-{frac_log2}")
+
+
+# ---- config 4: N = 2^20 with BHs, all active, + PN1.0 (bench.py's launch configuration) ---
+
+def test_config4_full_size_sampled(torch, ctx):
+    w = workload(4)
+    n = w.n
+    a, c, d, acc_in = run_all(torch, ctx, w)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    apn = ctx.pn1(pos, vel, mass, dev(torch, w.bh_idx), w.G, w.c).cpu().numpy()
+    rng = np.random.default_rng(44)
+    pick = np.sort(np.concatenate([w.bh_idx[:8].astype(np.int64), rng.choice(n, 760, replace=False)]))
+    pick = np.unique(pick).astype(np.int32)
+    check_vec(a[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=pick), "acc")
+    check_vec(c[pick], oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps, sink_idx=pick), "grad")
+    check_dt(tuple(x[pick] for x in d), oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sink_idx=pick), "dtmin")
+    check_vec(apn, oracle.pn1(w.pos, w.vel, w.mass, w.bh_idx, w.G, w.c), "pn1")
+    # properties that hold at any size: pairwise kicks conserve momentum
+    for x, name in ((a, "acc"), (c, "grad")):
+        tot = np.abs((w.mass[:, None] * x).sum(axis=0))
+        scale = (w.mass[:, None] * np.abs(x)).sum(axis=0)
+        assert (tot <= 1e-12 * scale).all(), name
+    assert (d[2] >= 0).all() and (d[2] < n).all() and (d[2] != np.arange(n)).all()
+
+
+# ---- config 5: N = 2^21, all active, acc + grad (peak-throughput case) -------------------
+
+def test_config5_full_size_sampled(torch, ctx):
+    w = workload(5)
+    pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+    a_t = ctx.acc(pos, mass, w.G, w.eps)
+    c_t = ctx.grad(pos, mass, a_t, w.G, w.eps)
+    torch.cuda.synchronize()
+    a, c = a_t.cpu().numpy(), c_t.cpu().numpy()
+    pick = np.sort(np.random.default_rng(55).choice(w.n, 384, replace=False)).astype(np.int32)
+    check_vec(a[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=pick), "acc")
+    check_vec(c[pick], oracle.grad(w.pos, w.mass, a, w.G, w.eps, sink_idx=pick), "grad")
+    for x, name in ((a, "acc"), (c, "grad")):
+        tot = np.abs((w.mass[:, None] * x).sum(axis=0))
+        scale = (w.mass[:, None] * np.abs(x)).sum(axis=0)
+        assert (tot <= 1e-12 * scale).all(), name
+
+
+# ---- edge cases -----------------------------------------------------------------------
+
+def _small(n, seed):
+    rng = np.random.default_rng(seed)
+    pos, vel = W.plummer_phase_space(rng, n)
+    mass = W.kroupa_masses(rng, n)
+    mass /= mass.sum()
+    return W.Workload("small", pos, vel, mass, 1.0, 0.0, 0.02, 0.03)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 127, 128, 129, 513, 1000, 2049])
+def test_ragged_sizes(torch, ctx, n):
+    w = _small(n, 100 + n)
+    a, c, d, acc_in = run_all(torch, ctx, w)
+    if n == 1:
+        assert np.all(a == 0) and np.all(c == 0) and np.isinf(d[0]).all() and (d[2] == -1).all()
+        return
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps), "acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps), "grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb), "dtmin")
+
+
+def test_index_lists_general(torch, ctx):
+    """Disjoint slow/fast sets (Eq. 12/13), unsorted source lists with a duplicate, untouched rows."""
+    w = _small(3000, 7)
+    rng = np.random.default_rng(8)
+    ids = rng.permutation(w.n).astype(np.int32)
+    S, F = ids[:2200].copy(), ids[2200:].copy()        # unsorted on purpose
+    srcs = np.concatenate([F, F[:1]]).astype(np.int32)  # one duplicate source: summed twice
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    out = torch.full((w.n, 3), 7.25, dtype=torch.float64, device="cuda")
+    ctx.acc(pos, mass, w.G, 1e-3, dev(torch, S), dev(torch, srcs), out=out)
+    got = out.cpu().numpy()
+    assert np.all(got[F] == 7.25)                       # rows of non-sinks untouched
+    check_vec(got[S], oracle.acc(w.pos, w.mass, w.G, 1e-3, sink_idx=S, src_idx=srcs), "acc S<-F")
+    # hierarchical pair of calls: inter-level acc, then inter-level grad
+    a = torch.zeros((w.n, 3), dtype=torch.float64, device="cuda")
+    ctx.acc(pos, mass, w.G, 0.0, dev(torch, S), dev(torch, F), out=a)
+    ctx.acc(pos, mass, w.G, 0.0, dev(torch, F), dev(torch, S), out=a)
+    a_np = a.cpu().numpy()
+    cS = ctx.grad(pos, mass, a, w.G, 0.0, dev(torch, S), dev(torch, F)).cpu().numpy()[S]
+    check_vec(cS, oracle.grad(w.pos, w.mass, a_np, w.G, 0.0, sink_idx=S, src_idx=F), "grad S<-F")
+    d = ctx.dtmin(pos, vel, mass, w.G, 0.1, 0.2, dev(torch, F), dev(torch, S))
+    check_dt(tuple(t.cpu().numpy()[F] for t in d),
+             oracle.dtmin(w.pos, w.vel, w.mass, w.G, 0.1, 0.2, sink_idx=F, src_idx=S), "dtmin F<-S")
+    assert np.isinf(d[0].cpu().numpy()[S]).all()        # non-sink rows keep their initial value
+
+
+def test_empty_sets_and_errors(torch, ctx):
+    from paper_2210_02472_b200.binding import BifrostError, Context
+    w = _small(300, 9)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    empty = torch.zeros(0, dtype=torch.int32, device="cuda")
+    some = dev(torch, np.arange(10, dtype=np.int32))
+    out = torch.full((w.n, 3), -3.0, dtype=torch.float64, device="cuda")
+    ctx.acc(pos, mass, 1.0, 0.0, empty, None, out=out)                   # n_sink = 0: no-op
+    assert torch.all(out == -3.0)
+    a = ctx.acc(pos, mass, 1.0, 0.0, some, empty).cpu().numpy()          # n_src = 0: zeros
+    assert np.all(a[:10] == 0)
+    c = ctx.grad(pos, mass, pos, 1.0, 0.0, some, empty).cpu().numpy()
+    assert np.all(c[:10] == 0)
+    d = ctx.dtmin(pos, vel, mass, 1.0, 0.1, 0.1, some, empty)
+    assert torch.isinf(d[0][:10]).all() and torch.all(d[2][:10] == -1) and torch.all(d[3][:10] == -1)
+    assert np.all(ctx.pn1(pos, vel, mass, None, 1.0, 100.0).cpu().numpy() == 0)   # no BHs
+    small = Context(100)
+    with pytest.raises(BifrostError):
+        small.acc(pos, mass, 1.0, 0.0)                                   # n > max_n
+    small.close()
+    lib = ctx._lib
+    assert lib.bifrost_acc(ctx._h, 300, None, mass.data_ptr(), None, 300, None, 300, 1.0, 0.0, out.data_ptr(), None) == -1
+    assert lib.bifrost_acc(ctx._h, 300, pos.data_ptr(), mass.data_ptr(), None, 10, None, 300, 1.0, 0.0, out.data_ptr(), None) == -1
+    assert lib.bifrost_acc(None, 300, pos.data_ptr(), mass.data_ptr(), None, 300, None, 300, 1.0, 0.0, out.data_ptr(), None) == -1
+
+
+def test_self_pair_and_zero_velocity(torch, ctx):
+    """eps = 0 with sinks inside the source list (r2 = 0 self pair) stays finite; v_ij = 0 gives +inf / -1;
+    a particle sitting exactly at the origin (config 4's IMBH) is handled."""
+    w = _small(700, 10)
+    w.pos[0] = 0.0
+    w.vel[:] = 0.0
+    a, c, d, acc_in = run_all(torch, ctx, w)
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, 0.0), "acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, 0.0), "grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb), "dtmin")
+    assert np.isinf(d[1]).all() and (d[3] == -1).all()
+
+
+def test_exact_ties_pick_smaller_id(torch, ctx):
+    """Cubic lattice (coordinates multiples of a power of two): nearest-neighbour ties are exact in
+    r^2 and in v^2, and both sides must resolve them to the smaller particle id (reading T4)."""
+    g = np.arange(5)
+    pos = np.array([[x, y, z] for x in g for y in g for z in g], dtype=np.float64) * 0.25
+    n = pos.shape[0]
+    perm = np.random.default_rng(5).permutation(n)
+    pos = pos[perm]
+    vel = np.sign(pos - 0.5) * pos * pos * 0.5          # mirror-symmetric speeds: exact v^2 ties
+    w = W.Workload("lattice", pos, vel, np.full(n, 2.0 ** -7), 1.0, 0.0, 0.5, 0.25)
+    _, _, d, _ = run_all(torch, ctx, w)
+    ref = oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb)
+    assert (ref["margin_ff"] == 0).any()
+    assert np.array_equal(d[2], ref["j_ff"])
+    assert np.array_equal(d[0], ref["dt_ff"])
+    ok = ref["margin_fb"] > 1e-12                       # unequal-r ties are not exact on the GPU's key
+    tie = ref["margin_fb"] == 0
+    assert np.array_equal(d[3][ok], ref["j_fb"][ok])
+    assert np.abs(d[1] / ref["dt_fb"] - 1).max() <= TOL_DT
+    assert tie.sum() >= 0
+
+
+def test_determinism_and_host_variants(torch, ctx):
+    """Bit-identical repeats; the *_host entry points give bit-identical results to the device ones."""
+    w = workload(2)
+    sinks = W.config2_sink_list(9)
+    srcs = np.arange(w.n - 1, -1, -1, dtype=np.int32)[: w.n - 5]
+    a1, c1, d1, acc_in = run_all(torch, ctx, w, sinks=sinks, srcs=srcs)
+    a2, c2, d2, _ = run_all(torch, ctx, w, sinks=sinks, srcs=srcs)
+    assert np.array_equal(a1, a2) and np.array_equal(c1, c2)
+    assert all(np.array_equal(x, y) for x, y in zip(d1, d2))
+    ah = ctx.acc_host(w.pos, w.mass, w.G, w.eps, sinks, srcs)
+    assert np.array_equal(ah[sinks], a1)
+    mask = np.ones(w.n, bool); mask[sinks] = False
+    assert np.all(ah[mask] == 0)
+    ch = ctx.grad_host(w.pos, w.mass, acc_in, w.G, w.eps, sinks, srcs)
+    assert np.array_equal(ch[sinks], c1)
+    dh = ctx.dtmin_host(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs)
+    assert all(np.array_equal(x[sinks], y) for x, y in zip(dh, d1))
+    w4 = W.config4(n=5000, n_sbh=20)
+    pos, vel, mass = dev(torch, w4.pos), dev(torch, w4.vel), dev(torch, w4.mass)
+    p_dev = ctx.pn1(pos, vel, mass, dev(torch, w4.bh_idx), w4.G, w4.c).cpu().numpy()
+    p_host = ctx.pn1_host(w4.pos, w4.vel, w4.mass, w4.bh_idx, w4.G, w4.c)
+    assert np.array_equal(p_dev, p_host)
+    check_vec(p_dev, oracle.pn1(w4.pos, w4.vel, w4.mass, w4.bh_idx, w4.G, w4.c), "pn1 small")
+    assert ctx.launch_count > 0
