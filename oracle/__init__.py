@@ -52,6 +52,10 @@ def _load():
         lib.oracle_dtmin.argtypes = [_I64, _P, _P, _P, _P, _I64, _P, _I64, _D, _D, _D, _P, _P, _P, _P, _P, _P]
         for name in ("oracle_pn1", "oracle_pn1_ld"):
             getattr(lib, name).argtypes = [_I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+        for name in ("oracle_jerk", "oracle_jerk_ld"):
+            getattr(lib, name).argtypes = [_I64, _P, _P, _P, _P, _I64, _P, _I64, _D, _D, _P]
+        lib.oracle_phi.argtypes = common
+        lib.oracle_criteria.argtypes = [_I64, _P, _P, _P, _P, _P, _I64, _D, _D, _D, _P, _P, _P, _P]
         for name in ("oracle_potential", "oracle_potential_ld"):
             getattr(lib, name).argtypes = [_I64, _P, _P, _D, _D]
             getattr(lib, name).restype = _D
@@ -136,3 +140,42 @@ def potential(pos, mass, G, eps=0.0, long_double=False) -> float:
     pos, mass = _f64(pos), _f64(mass)
     fn = _load().oracle_potential_ld if long_double else _load().oracle_potential
     return float(fn(mass.shape[0], pos.ctypes.data, mass.ctypes.data, G, eps))
+
+
+def jerk(pos, vel, mass, G, eps, sink_idx=None, src_idx=None, long_double=False) -> np.ndarray:
+    """Eq. 28, softened; compact rows of the sink list."""
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    ns = n if si is None else si.shape[0]
+    nj = n if sj is None else sj.shape[0]
+    out = np.zeros((ns, 3))
+    fn = _load().oracle_jerk_ld if long_double else _load().oracle_jerk
+    fn(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps, out.ctypes.data)
+    return out
+
+
+def phi(pos, mass, G, eps, sink_idx=None, src_idx=None) -> np.ndarray:
+    """Per-sink potential phi_i = -G sum_j m_j / s_ij (Eq. 4 / Eq. 68); compact rows."""
+    pos, mass = _f64(pos), _f64(mass)
+    n = mass.shape[0]
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    ns = n if si is None else si.shape[0]
+    nj = n if sj is None else sj.shape[0]
+    out = np.zeros(ns)
+    _load().oracle_phi(n, pos.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps, out.ctypes.data)
+    return out
+
+
+def criteria(vel, acc_in, grad_c, jerk_in, eta, eta_grad, eta_jerk, sink_idx=None):
+    """Eq. 24, 26, 27, 29: returns dict(dt_va, dt_gradv, dt_grada, dt_jerk), compact rows."""
+    vel, acc_in, grad_c, jerk_in = _f64(vel), _f64(acc_in), _f64(grad_c), _f64(jerk_in)
+    n = vel.shape[0]
+    si, sip = _idx(sink_idx)
+    ns = n if si is None else si.shape[0]
+    outs = [np.zeros(ns) for _ in range(4)]
+    _load().oracle_criteria(n, vel.ctypes.data, acc_in.ctypes.data, grad_c.ctypes.data, jerk_in.ctypes.data, sip, ns,
+                            eta, eta_grad, eta_jerk, *[o.ctypes.data for o in outs])
+    return dict(dt_va=outs[0], dt_gradv=outs[1], dt_grada=outs[2], dt_jerk=outs[3])

@@ -26,7 +26,11 @@
 // and for pn1: label-swap symmetry, exact c -> 2c scaling, the test-particle
 // limit, the centre-of-mass relative-acceleration identity and the periapsis
 // advance of PAPER.md:L534 Eq. 46.
-// Parity status: acc, grad, dtmin, potential pinned.  pn1: the relative two-body
+// jerk (NEXT-1): central finite difference in time of O-acc along r + v h, two-body closed
+// form, sum_i m_i j_i = 0.  phi: two-body value, W = 1/2 sum m_i phi_i against O-pot and the
+// Plummer value, -m_i a_i = finite difference of W.  criteria: hand-set vectors with integer
+// norms (3-4-5 triangles) evaluated by hand from Eq. 24, 26, 27, 29.
+// Parity status: acc, grad, dtmin, potential, jerk, phi, criteria pinned.  pn1: the relative two-body
 // dynamics are pinned; the paper prints no PN1.0 formula (PAPER.md:L439, L476 cite
 // Thorne & Hartle 1985 / Einstein et al. 1938), so parity with the paper's own
 // implementation of the per-body split is "parity unpinned" (reading P1).
@@ -234,6 +238,100 @@ void pn1_impl(int64_t n, const double* pos, const double* vel, const double* mas
 }
 
 // ---------------------------------------------------------------------------
+// O-jerk.  PAPER.md:L360 Eq. 28 (reading J1: the garbled lhs is j_i = da_i/dt, the
+// sum runs over j != i), softened like the accelerations (exact time derivative
+// of the softened pair acceleration along r_ji(t), dr_ji/dt = v_ji):
+//     j_i = G sum_{j in src, j != i} m_j [ v_ji / s^3 - 3 (r_ji . v_ji) r_ji / s^5 ],
+//     v_ji = v_j - v_i,  s^2 = |r_ji|^2 + eps^2.
+// For eps = 0 this is literally Eq. 28's G m_j/|r|^5 (|r|^2 v_ji - 3 (r_ji.v_ji) r_ji).
+// ---------------------------------------------------------------------------
+template <class T>
+void jerk_impl(int64_t n, const double* pos, const double* vel, const double* mass,
+               const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+               double G, double eps, double* out) {
+    (void)n;
+    const T eps2 = (T)eps * (T)eps;
+#pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
+    for (int64_t k = 0; k < n_sink; ++k) {
+        const int64_t i = pid(sink_idx, k);
+        Neumaier<T> sx, sy, sz;
+        for (int64_t l = 0; l < n_src; ++l) {
+            const int64_t j = pid(src_idx, l);
+            if (j == i) continue;
+            const T dx = (T)pos[3 * j] - (T)pos[3 * i], dy = (T)pos[3 * j + 1] - (T)pos[3 * i + 1],
+                    dz = (T)pos[3 * j + 2] - (T)pos[3 * i + 2];
+            const T ux = (T)vel[3 * j] - (T)vel[3 * i], uy = (T)vel[3 * j + 1] - (T)vel[3 * i + 1],
+                    uz = (T)vel[3 * j + 2] - (T)vel[3 * i + 2];
+            const T s2 = dx * dx + dy * dy + dz * dz + eps2;
+            const T s = std::sqrt(s2);
+            const T s3 = s2 * s, s5 = s3 * s2;
+            const T rv = dx * ux + dy * uy + dz * uz;       // r_ji . v_ji
+            const T m = mass[j];
+            sx.add(m * (ux / s3 - (T)3 * rv * dx / s5));
+            sy.add(m * (uy / s3 - (T)3 * rv * dy / s5));
+            sz.add(m * (uz / s3 - (T)3 * rv * dz / s5));
+        }
+        out[3 * k]     = (double)((T)G * sx.value());
+        out[3 * k + 1] = (double)((T)G * sy.value());
+        out[3 * k + 2] = (double)((T)G * sz.value());
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O-phi.  Per-sink potential of PAPER.md:L63 Eq. 4 (second term) / L724 Eq. 68, softened
+// like the accelerations:  phi_i = -G sum_{j in src, j != i} m_j / sqrt(|r_ji|^2 + eps^2),
+// so that W = 1/2 sum_i m_i phi_i when sinks = sources = all.
+// ---------------------------------------------------------------------------
+template <class T>
+void phi_impl(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx, int64_t n_sink,
+              const int32_t* src_idx, int64_t n_src, double G, double eps, double* out) {
+    (void)n;
+    const T eps2 = (T)eps * (T)eps;
+#pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
+    for (int64_t k = 0; k < n_sink; ++k) {
+        const int64_t i = pid(sink_idx, k);
+        Neumaier<T> s;
+        for (int64_t l = 0; l < n_src; ++l) {
+            const int64_t j = pid(src_idx, l);
+            if (j == i) continue;
+            const T dx = (T)pos[3 * j] - (T)pos[3 * i], dy = (T)pos[3 * j + 1] - (T)pos[3 * i + 1],
+                    dz = (T)pos[3 * j + 2] - (T)pos[3 * i + 2];
+            s.add((T)mass[j] / std::sqrt(dx * dx + dy * dy + dz * dz + eps2));
+        }
+        out[k] = (double)(-(T)G * s.value());
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O-crit.  The O(N) per-particle time-step criteria of PAPER.md §3.5.4-3.5.5:
+//     dt_va    = eta      |v_i| / |a_i|                 (L338 Eq. 24)
+//     dt_gradv = eta_grad (|v_i| / |g'_i|)^(1/3)        (L346 Eq. 26)
+//     dt_grada = eta_grad (|a_i| / |g'_i|)^(1/2)        (L350 Eq. 27)
+//     dt_jerk  = eta_jerk |a_i| / |j_i|                 (L365 Eq. 29)
+// with g'_i = C_i / 24 (L327-332 Eq. 23), C_i the bare gradient sum (O-grad).
+// A zero denominator gives +inf (reading J2).  Inputs are indexed by particle id;
+// outputs are compact rows of the sink list.
+// ---------------------------------------------------------------------------
+inline double norm3(const double* p) { return std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2]); }
+
+void criteria_impl(int64_t n, const double* vel, const double* acc, const double* grad_c, const double* jerk,
+                   const int32_t* sink_idx, int64_t n_sink, double eta, double eta_grad, double eta_jerk,
+                   double* dt_va, double* dt_gradv, double* dt_grada, double* dt_jerk) {
+    (void)n;
+    const double inf = std::numeric_limits<double>::infinity();
+    for (int64_t k = 0; k < n_sink; ++k) {
+        const int64_t i = pid(sink_idx, k);
+        const double v = norm3(vel + 3 * i), a = norm3(acc + 3 * i);
+        const double gp = norm3(grad_c + 3 * i) / 24.0;
+        const double j = norm3(jerk + 3 * i);
+        dt_va[k]    = (a == 0.0) ? inf : eta * v / a;
+        dt_gradv[k] = (gp == 0.0) ? inf : eta_grad * std::cbrt(v / gp);
+        dt_grada[k] = (gp == 0.0) ? inf : eta_grad * std::sqrt(a / gp);
+        dt_jerk[k]  = (j == 0.0) ? inf : eta_jerk * a / j;
+    }
+}
+
+// ---------------------------------------------------------------------------
 // O-pot.  PAPER.md:L63 Eq. 4 (second term), softened like the accelerations:
 //     W = -G sum_{i<j} m_i m_j / sqrt(|r_ji|^2 + eps^2).   Self-check only.
 // ---------------------------------------------------------------------------
@@ -296,6 +394,27 @@ int oracle_pn1(int64_t n, const double* pos, const double* vel, const double* ma
 int oracle_pn1_ld(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* bh_idx,
                   int64_t n_bh, double G, double c, double* out) {
     pn1_impl<long double>(n, pos, vel, mass, bh_idx, n_bh, G, c, out);
+    return 0;
+}
+int oracle_jerk(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+                int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out) {
+    jerk_impl<double>(n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out);
+    return 0;
+}
+int oracle_jerk_ld(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+                   int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out) {
+    jerk_impl<long double>(n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out);
+    return 0;
+}
+int oracle_phi(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx, int64_t n_sink,
+               const int32_t* src_idx, int64_t n_src, double G, double eps, double* out) {
+    phi_impl<double>(n, pos, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out);
+    return 0;
+}
+int oracle_criteria(int64_t n, const double* vel, const double* acc, const double* grad_c, const double* jerk,
+                    const int32_t* sink_idx, int64_t n_sink, double eta, double eta_grad, double eta_jerk,
+                    double* dt_va, double* dt_gradv, double* dt_grada, double* dt_jerk) {
+    criteria_impl(n, vel, acc, grad_c, jerk, sink_idx, n_sink, eta, eta_grad, eta_jerk, dt_va, dt_gradv, dt_grada, dt_jerk);
     return 0;
 }
 double oracle_potential(int64_t n, const double* pos, const double* mass, double G, double eps) {
