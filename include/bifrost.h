@@ -111,6 +111,46 @@ int bifrost_dtmin(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
 int bifrost_pn1(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
                 const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn, void* stream);
 
+/* ---- NEXT rows, built on the same kernels.  Device pointers, asynchronous. ---- */
+
+/* bifrost_jerk - PAPER.md:L360 Eq. 28 (lhs garbled in the extraction; reading J1: j_i = da_i/dt,
+ * sum over j != i), softened like bifrost_acc so that it is the exact time derivative of it:
+ *     out_jerk[i] = G * sum_{j in src, j != i} mass[j] * [ v_ji / s^3 - 3 (r_ji . v_ji) r_ji / s^5 ],
+ *     v_ji = vel[j] - vel[i],  s^2 = |r_ji|^2 + eps^2.
+ * Same tensor contraction as bifrost_grad with v_ji for a_ji (one kernel serves both).
+ * Index-list, self-pair and output conventions as for bifrost_acc. */
+int bifrost_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                 const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                 double G, double eps, double* out_jerk, void* stream);
+
+/* bifrost_potential - the potential term of PAPER.md:L63 Eq. 4 (and the first two terms' potential
+ * part of the energy book-keeping, L724 Eq. 68), softened like bifrost_acc:
+ *     out_phi[i] = -G * sum_{j in src, j != i} mass[j] / sqrt(|r_ji|^2 + eps^2)      (i in sinks; double[n])
+ *     *out_W     = 1/2 * sum_{i in sinks} mass[i] * phi_i                             (one DEVICE double)
+ * With sinks = sources = all, *out_W = -sum_{i<j} G m_i m_j / s_ij.  Either output may be NULL (not
+ * both).  The self pair is dropped by particle id.  The sum over sinks runs in a fixed order
+ * (two-stage block reduction), so *out_W is bit-reproducible. */
+int bifrost_potential(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
+                      const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                      double G, double eps, double* out_phi, double* out_W, void* stream);
+
+/* bifrost_timestep_criteria - the O(N) per-particle criteria of PAPER.md §3.5.4-3.5.5, for i in sinks:
+ *     out_dt_va[i]    = eta      * |vel_i| / |acc_i|                      (L338 Eq. 24)
+ *     out_dt_gradv[i] = eta_grad * (|vel_i| / |g'_i|)^(1/3)               (L346 Eq. 26)
+ *     out_dt_grada[i] = eta_grad * (|acc_i| / |g'_i|)^(1/2)               (L350 Eq. 27)
+ *     out_dt_jerk[i]  = eta_jerk * |acc_i| / |jerk_i|                     (L365 Eq. 29)
+ * with g'_i = grad_i / 24 (L327-332 Eq. 23), grad = the output of bifrost_grad, jerk = the output of
+ * bifrost_jerk; all double[n][3] indexed by particle id.  A zero denominator gives +inf.
+ * grad and/or jerk may be NULL (their criteria are skipped; the matching outputs must be NULL).
+ * Any out_* may be NULL.  If inout_dt (double[n]) is not NULL, inout_dt[i] = min(inout_dt[i], every
+ * criterion evaluated) - "the final time-step of a particle is the minimum of the set of its
+ * different time-steps" (L293); seed it with min(dt_ff, dt_fb) from bifrost_dtmin or with +inf. */
+int bifrost_timestep_criteria(bifrost_ctx* ctx, int64_t n, const double* vel, const double* acc,
+                              const double* grad, const double* jerk, const int32_t* sink_idx, int64_t n_sink,
+                              double eta, double eta_grad, double eta_jerk,
+                              double* out_dt_va, double* out_dt_gradv, double* out_dt_grada, double* out_dt_jerk,
+                              double* inout_dt, void* stream);
+
 /* Host-buffer variants: same semantics, HOST pointers, synchronous (see header comment).
  * Index lists may be NULL as above.  Outputs are written only at sink ids (other host rows are
  * untouched), bifrost_pn1_host overwrites all n rows. */

@@ -26,6 +26,7 @@ LIB_PATH = os.path.join(_HERE, "libbifrost.so")
 SYMBOLS = [
     "bifrost_create", "bifrost_destroy", "bifrost_strerror", "bifrost_last_cuda_error", "bifrost_launch_count",
     "bifrost_acc", "bifrost_grad", "bifrost_dtmin", "bifrost_pn1",
+    "bifrost_jerk", "bifrost_potential", "bifrost_timestep_criteria",
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
 ]
 
@@ -60,6 +61,9 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_grad.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P]
     lib.bifrost_dtmin.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P, _P]
     lib.bifrost_pn1.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P, _P]
+    lib.bifrost_jerk.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P]
+    lib.bifrost_potential.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P, _P, _P]
+    lib.bifrost_timestep_criteria.argtypes = [_P, _I64, _P, _P, _P, _P, _P, _I64, _D, _D, _D, _P, _P, _P, _P, _P, _P]
     lib.bifrost_acc_host.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P]
     lib.bifrost_grad_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P]
     lib.bifrost_dtmin_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P]
@@ -211,6 +215,60 @@ class Context:
                                    0 if bh is None else bh.shape[0], float(G), float(c), out.data_ptr(), self._stream())
         self._check(rc, "bifrost_pn1")
         return out
+
+    # ---- NEXT rows ------------------------------------------------------------------
+    def jerk(self, pos, vel, mass, G, eps, sink_idx=None, src_idx=None, out=None):
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = torch.zeros((n, 3), dtype=torch.float64, device=pos.device)
+        _dev_f64(out, (3,), "out")
+        rc = self._lib.bifrost_jerk(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
+                                    n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                    float(G), float(eps), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_jerk")
+        return out
+
+    def potential(self, pos, mass, G, eps, sink_idx=None, src_idx=None, want_phi=True, want_W=True):
+        """Returns (phi [n] or None, W 0-dim device tensor or None)."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        phi = torch.zeros(n, dtype=torch.float64, device=pos.device) if want_phi else None
+        W = torch.zeros((), dtype=torch.float64, device=pos.device) if want_W else None
+        rc = self._lib.bifrost_potential(self._h, n, pos.data_ptr(), mass.data_ptr(), sip or None,
+                                         n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                         float(G), float(eps), phi.data_ptr() if want_phi else None,
+                                         W.data_ptr() if want_W else None, self._stream())
+        self._check(rc, "bifrost_potential")
+        return phi, W
+
+    def timestep_criteria(self, vel, acc, grad, jerk, eta, eta_grad, eta_jerk, sink_idx=None, inout_dt=None):
+        """Returns dict(dt_va, dt_gradv, dt_grada, dt_jerk) of [n] tensors (+inf at non-sinks; gradv/grada/jerk
+        entries are None when grad / jerk is None).  inout_dt, if given, is min-updated in place."""
+        import torch
+        vel = _dev_f64(vel, (3,), "vel"); acc = _dev_f64(acc, (3,), "acc")
+        if grad is not None:
+            grad = _dev_f64(grad, (3,), "grad")
+        if jerk is not None:
+            jerk = _dev_f64(jerk, (3,), "jerk")
+        n = vel.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx")
+
+        def new():
+            return torch.full((n,), float("inf"), dtype=torch.float64, device=vel.device)
+        o = dict(dt_va=new(), dt_gradv=new() if grad is not None else None,
+                 dt_grada=new() if grad is not None else None, dt_jerk=new() if jerk is not None else None)
+        ptr = lambda t: None if t is None else t.data_ptr()
+        rc = self._lib.bifrost_timestep_criteria(self._h, n, vel.data_ptr(), acc.data_ptr(), ptr(grad), ptr(jerk),
+                                                 sip or None, n if si is None else si.shape[0], float(eta),
+                                                 float(eta_grad), float(eta_jerk), ptr(o["dt_va"]), ptr(o["dt_gradv"]),
+                                                 ptr(o["dt_grada"]), ptr(o["dt_jerk"]), ptr(inout_dt), self._stream())
+        self._check(rc, "bifrost_timestep_criteria")
+        return o
 
     # ---- host-buffer entry points (numpy in, numpy out; synchronous) -----------------
     def acc_host(self, pos, mass, G, eps, sink_idx=None, src_idx=None, out=None):

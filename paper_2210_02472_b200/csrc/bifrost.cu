@@ -206,6 +206,44 @@ struct DtPass {
     }
 };
 
+struct PotArgs {
+    const double* pos;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;        // phi at [.]
+    double* partial;    // [split][n_sink]
+};
+
+// Potential (Eq. 4 second term, Eq. 68): p_i = sum_j m_j / s_ij; phi_i = -G p_i.
+// 1/s = y0 (1 + e/2 + 3/8 e^2); the record carries m, m/2, 3m/8 and the source id, because here
+// the self pair does not multiply a zero separation and must be dropped by id (integer select).
+struct PotPass {
+    static constexpr int REC = 8;   // x y z m 0.5m 0.375m id(bits) pad
+    using Args = PotArgs;
+    struct Sink { double x, y, z; int id; };
+    struct Acc { double p; };
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2]; s.id = id;
+    }
+    __device__ static void init(Acc& c) { c.p = 0.0; }
+    // 12 FP64-pipe instructions: 3 DADD, 3 DFMA, DMUL, DFMA, 2 DFMA, DMUL, DADD.
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 1/2 e + 3/8 e^2)
+        double w = y0 * pm;                                   // m / s
+        if (__double2loint(r[6]) == s.id) w = 0.0;            // j != i
+        c.p += w;
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        if (g.n_split == 1) a.out[g.compact ? k : id] = -a.G * c.p;
+        else a.partial[(size_t)split * g.n_sink + k] = c.p;
+    }
+};
+
 // ----------------------------------------------------------------------------------------
 // a2-a4: the pair kernel.  grid = (ceil(n_sink / (THREADS*S)), n_split).
 // ----------------------------------------------------------------------------------------
@@ -342,6 +380,108 @@ __global__ void reduce_vec3_kernel(int n_sink, int n_split, int compact, const i
     const int id = sink_idx ? sink_idx[k] : k;
     double* o = out + 3 * (size_t)(compact ? k : id);
     o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
+}
+
+__global__ void pack_pot_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
+                                const double* __restrict__ pos, const double* __restrict__ mass,
+                                double* __restrict__ rec) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n_pad) return;
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
+    if (l < n_src) {
+        const int j = src_idx ? src_idx[l] : l;
+        const double m = mass[j];
+        o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
+        o[1] = make_double2(pos[3 * (size_t)j + 2], m);
+        o[2] = make_double2(0.5 * m, 0.375 * m);
+        o[3] = make_double2(__hiloint2double(0, j), 0.0);
+    } else {
+        o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
+        o[3] = make_double2(__hiloint2double(0, -1), 0.0);
+    }
+}
+
+__global__ void reduce_scalar_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
+                                     const double* __restrict__ partial, double scale, double* __restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_sink) return;
+    double s = 0.0;
+    for (int q = 0; q < n_split; ++q) s += partial[(size_t)q * n_sink + k];     // fixed order
+    const int id = sink_idx ? sink_idx[k] : k;
+    out[compact ? k : id] = scale * s;
+}
+
+// W = 1/2 sum_{i in sinks} m_i phi_i in two fixed-order stages (deterministic; no atomics).
+constexpr int WSUM_THREADS = 256;
+constexpr int WSUM_PER_BLOCK = 4096;
+__device__ __forceinline__ double block_sum_fixed(double v) {
+    __shared__ double red[WSUM_THREADS / 32];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < WSUM_THREADS / 32; ++w) s += red[w];
+    return s;   // valid in thread 0
+}
+__global__ void __launch_bounds__(WSUM_THREADS)
+wsum_stage1_kernel(int n_sink, const int32_t* __restrict__ sink_idx, int compact_phi, const double* __restrict__ mass,
+                   const double* __restrict__ phi, double* __restrict__ block_part) {
+    const int base = blockIdx.x * WSUM_PER_BLOCK;
+    double v = 0.0;
+    for (int q = threadIdx.x; q < WSUM_PER_BLOCK; q += WSUM_THREADS) {
+        const int k = base + q;
+        if (k < n_sink) {
+            const int id = sink_idx ? sink_idx[k] : k;
+            v += mass[id] * phi[compact_phi ? k : id];
+        }
+    }
+    const double s = block_sum_fixed(v);
+    if (threadIdx.x == 0) block_part[blockIdx.x] = s;
+}
+__global__ void __launch_bounds__(WSUM_THREADS)
+wsum_stage2_kernel(int n_blocks, const double* __restrict__ block_part, double* __restrict__ out_W) {
+    double v = 0.0;
+    for (int q = threadIdx.x; q < n_blocks; q += WSUM_THREADS) v += block_part[q];
+    const double s = block_sum_fixed(v);
+    if (threadIdx.x == 0) *out_W = 0.5 * s;
+}
+
+// O(N) time-step criteria, Eq. 24, 26, 27, 29; IEEE sqrt / cbrt / division.
+__global__ void criteria_kernel(int n_sink, const int32_t* __restrict__ sink_idx, const double* __restrict__ vel,
+                                const double* __restrict__ acc, const double* __restrict__ grad,
+                                const double* __restrict__ jerk, double eta, double eta_grad, double eta_jerk,
+                                double* __restrict__ dt_va, double* __restrict__ dt_gradv, double* __restrict__ dt_grada,
+                                double* __restrict__ dt_jerk, double* __restrict__ inout_dt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_sink) return;
+    const int i = sink_idx ? sink_idx[k] : k;
+    const size_t o = 3 * (size_t)i;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    auto norm = [](const double* p) {
+        return sqrt(__dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2])));
+    };
+    const double v = norm(vel + o), a = norm(acc + o);
+    double best = inout_dt ? inout_dt[i] : inf;
+    const double t_va = (a == 0.0) ? inf : __dmul_rn(eta, v) / a;
+    if (dt_va) dt_va[i] = t_va;
+    best = fmin(best, t_va);
+    if (grad) {
+        const double gp = norm(grad + o) / 24.0;
+        const double t_gv = (gp == 0.0) ? inf : eta_grad * cbrt(v / gp);
+        const double t_ga = (gp == 0.0) ? inf : eta_grad * sqrt(a / gp);
+        if (dt_gradv) dt_gradv[i] = t_gv;
+        if (dt_grada) dt_grada[i] = t_ga;
+        best = fmin(best, fmin(t_gv, t_ga));
+    }
+    if (jerk) {
+        const double j = norm(jerk + o);
+        const double t_j = (j == 0.0) ? inf : __dmul_rn(eta_jerk, a) / j;
+        if (dt_jerk) dt_jerk[i] = t_j;
+        best = fmin(best, t_j);
+    }
+    if (inout_dt) inout_dt[i] = best;
 }
 
 // dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
@@ -515,6 +655,8 @@ struct bifrost_ctx {
     void* partial = nullptr;         // split-j partials / pn1 partials
     size_t partial_bytes = 0;
     unsigned char* is_bh = nullptr;  // [max_n]
+    double* phi_scratch = nullptr;   // [max_n]   (bifrost_potential with out_phi == NULL)
+    double* wpart = nullptr;         // [ceil(max_n / 4096)] block partials of the W reduction
     int64_t launches = 0;
     char err[256] = {0};
     // mirrors for the *_host entry points (allocated on first use)
@@ -665,6 +807,43 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     return BIFROST_OK;
 }
 
+int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
+             int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out_phi,
+             double* out_W, cudaStream_t st) {
+    if (n_sink == 0) {
+        if (out_W) CU_TRY(ctx, cudaMemsetAsync(out_W, 0, sizeof(double), st));
+        return BIFROST_OK;
+    }
+    constexpr int S = 4, MINB = 4;
+    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 8, false);
+    const int compact = out_phi ? 0 : 1;           // the scratch holds compact rows
+    double* phi = out_phi ? out_phi : ctx->phi_scratch;
+    g.compact = compact;
+    if (n_src > 0) {
+        const int n_pad = ceil_div(n_src, TILE) * TILE;
+        pack_pot_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    PotArgs a{pos, sink_idx, eps * eps, G, phi, (double*)ctx->partial};
+    int rc = launch_pair<PotPass, S, MINB>(ctx, a, g, st);
+    if (rc) return rc;
+    if (g.n_split > 1) {
+        reduce_scalar_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
+                                                                   (const double*)ctx->partial, -G, phi);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    if (out_W) {
+        const int nb = ceil_div(n_sink, WSUM_PER_BLOCK);
+        wsum_stage1_kernel<<<nb, WSUM_THREADS, 0, st>>>((int)n_sink, sink_idx, compact, mass, phi, ctx->wpart);
+        wsum_stage2_kernel<<<1, WSUM_THREADS, 0, st>>>(nb, ctx->wpart, out_W);
+        ctx->launches += 2;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    return BIFROST_OK;
+}
+
 int pn1_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
              const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out, cudaStream_t st) {
     if (n == 0) return BIFROST_OK;
@@ -769,7 +948,9 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
     if (cudaMalloc(&ctx->src_rec, n_pad * 10 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
-        cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess) {
+        cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess ||
+        cudaMalloc(&ctx->phi_scratch, 8 * (size_t)max_n) != cudaSuccess ||
+        cudaMalloc(&ctx->wpart, 8 * ((size_t)max_n / WSUM_PER_BLOCK + 1)) != cudaSuccess) {
         cudaGetLastError();
         bifrost_destroy(ctx);
         return BIFROST_ENOMEM;
@@ -781,7 +962,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
 int bifrost_destroy(bifrost_ctx* ctx) {
     if (!ctx) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh);
+    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
@@ -833,6 +1014,50 @@ int bifrost_pn1(bifrost_ctx* ctx, int64_t n, const double* pos, const double* ve
     if (n_bh > 0 && !bh_idx) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
     return pn1_impl(ctx, n, pos, vel, mass, bh_idx, n_bh, G, c, out_acc_pn, (cudaStream_t)stream);
+}
+
+// ---- NEXT-1 / NEXT-4 rows ---------------------------------------------------
+
+int bifrost_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                 const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                 double* out_jerk, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !vel || !mass || !out_jerk)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    // Eq. 28 is Eq. 9's tensor contraction with v_ji in place of a_ji: the same kernel.
+    return grad_impl(ctx, n, pos, mass, vel, sink_idx, n_sink, src_idx, n_src, G, eps, out_jerk, 0, (cudaStream_t)stream);
+}
+
+int bifrost_potential(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
+                      int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out_phi,
+                      double* out_W, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !mass)) return BIFROST_EINVAL;
+    if (!out_phi && !out_W) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return pot_impl(ctx, n, pos, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out_phi, out_W, (cudaStream_t)stream);
+}
+
+int bifrost_timestep_criteria(bifrost_ctx* ctx, int64_t n, const double* vel, const double* acc, const double* grad,
+                              const double* jerk, const int32_t* sink_idx, int64_t n_sink, double eta, double eta_grad,
+                              double eta_jerk, double* out_dt_va, double* out_dt_gradv, double* out_dt_grada,
+                              double* out_dt_jerk, double* inout_dt, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_sink < 0 || n_sink > ctx->max_n) return BIFROST_EINVAL;
+    if (!sink_idx && n_sink != n) return BIFROST_EINVAL;
+    if (n_sink == 0) return BIFROST_OK;
+    if (!vel || !acc) return BIFROST_EINVAL;
+    if ((!grad && (out_dt_gradv || out_dt_grada)) || (!jerk && out_dt_jerk)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    criteria_kernel<<<ceil_div(n_sink, 256), 256, 0, (cudaStream_t)stream>>>(
+        (int)n_sink, sink_idx, vel, acc, grad, jerk, eta, eta_grad, eta_jerk, out_dt_va, out_dt_gradv, out_dt_grada,
+        out_dt_jerk, inout_dt);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
 }
 
 // ---- host-buffer variants --------------------------------------------------------------
