@@ -42,7 +42,7 @@ UNIT = "interactions/s"
 
 # FP64-pipe instruction / flop counts per pair of the kernels' inner loops (
 # cross-checked against the SASS and ncu's smsp__sass_thread_inst_executed_op_d*_pred_on).
-FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 25}
+FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 25}     # dtmin: 23 arithmetic + 2 DSETP (ascending source ids)
 FP64_FLOPS = {"acc": 24, "grad": 44, "dtmin": 33}     # FMA = 2, ADD/MUL = 1
 # B200 FP64 ALU peak derived from unit counts and clocks (no fp64 entry in MEASURED_PEAKS.json):
 # 148 SMs x 64 FP64 lanes/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.
@@ -312,6 +312,12 @@ def run_cuda(args):
     if rank == 0:
         num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
         peak = fp64_peak_tflops(num_sms, clocks.get("sm_max_mhz") or 1965.0)
+        # measured FP64-pipe rates of a register-only kernel (outside the timed region; ~0.3 s each)
+        probe = {}
+        if not args.no_fp64_probe:
+            for mix, name in ((0, "dfma"), (1, "acc_mix")):
+                ms, rate = ctx.fp64_probe(mix=mix, iters=1 << 15, ctas_per_sm=32)
+                probe[name] = {"ms": ms, "lane_instr_per_s": rate, "frac_of_derived_pipe_peak": rate / (peak * 1e12 / 2)}
         pairs_rank = float(max(sharding.slice_counts(n, world))) * n     # the slowest rank's share
 
         def kern(name):
@@ -343,6 +349,10 @@ def run_cuda(args):
                     "acc_grad_combined_frac": (FP64_FLOPS["acc"] + FP64_FLOPS["grad"]) * pairs_rank
                     / (1e-3 * (mean_ms["acc"] + mean_ms["grad"])) / 1e12 / peak,
                     "traffic": traffic}
+        if probe:
+            roofline["measured_fp64_pipe"] = probe
+            roofline["pipe_util_vs_measured_dfma"] = (
+                dom["fp64_pipe_issue_util"] / probe["dfma"]["frac_of_derived_pipe_peak"])
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
@@ -374,6 +384,7 @@ def main():
     ap.add_argument("--cpu-sinks", type=int, default=2048, help="oracle sample size (sinks) for cpu_baseline")
     ap.add_argument("--ref-sinks", type=int, default=1024, help="oracle sample size (sinks) per reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fp64-probe", action="store_true", help="skip the register-only FP64-pipe peak probe")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

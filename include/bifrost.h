@@ -167,6 +167,17 @@ int bifrost_dtmin_host(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
 int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
                      const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out_acc_pn);
 
+/* Measurement aid, not part of the paper's path: runs a register-only kernel of independent FP64
+ * chains (no memory traffic) on the context's device, on the legacy default stream, synchronously,
+ * so that bench.py can quote a MEASURED FP64-pipe peak beside the derived one.
+ *   mix = 0: pure DFMA;  mix = 1: 3 DADD + 9 DFMA + 3 DMUL per 15 instructions (the acc pair's mix).
+ *   iters: loop trips per thread (32 (mix 0) or 120 (mix 1) FP64 instructions each);
+ *   ctas_per_sm: grid = SM count x ctas_per_sm CTAs of 128 threads (4 are resident per SM).
+ * HOST outputs: *out_ms = device time of one launch (CUDA events, after a warm-up launch);
+ * *out_lane_instr = FP64-pipe lane-instructions that launch executed (threads x instructions). */
+int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm, double* out_ms,
+                       double* out_lane_instr);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,6 +28,7 @@ SYMBOLS = [
     "bifrost_acc", "bifrost_grad", "bifrost_dtmin", "bifrost_pn1",
     "bifrost_jerk", "bifrost_potential", "bifrost_timestep_criteria",
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
+    "bifrost_fp64_probe",
 ]
 
 
@@ -68,6 +69,7 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_grad_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P]
     lib.bifrost_dtmin_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P]
     lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+    lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
     _lib = lib
     return lib
 
@@ -317,3 +319,12 @@ class Context:
                                         0 if bh is None else bh.shape[0], float(G), float(c), out.ctypes.data)
         self._check(rc, "bifrost_pn1_host")
         return out
+
+    # ---- measurement aid --------------------------------------------------------------
+    def fp64_probe(self, mix: int = 0, iters: int = 1 << 16, ctas_per_sm: int = 16):
+        """Measured FP64-pipe rate of a register-only kernel: (ms, lane_instructions_per_s)."""
+        ms, cnt = _D(0.0), _D(0.0)
+        rc = self._lib.bifrost_fp64_probe(self._h, int(mix), int(iters), int(ctas_per_sm), ctypes.byref(ms),
+                                          ctypes.byref(cnt))
+        self._check(rc, "bifrost_fp64_probe")
+        return ms.value, cnt.value / (ms.value * 1e-3)

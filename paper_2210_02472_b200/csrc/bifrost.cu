@@ -8,7 +8,7 @@
 // MUFU.RSQ64H seed, integer clamps/selects, loop control) rides in the other issue slots.
 //   a1  pack kernels gather sources from the index list into 16-B aligned records
 //       (acc 48 B, grad 80 B, dtmin 64 B) with the mass-scaled polynomial coefficients.
-//   a2-a4  one "pair kernel" skeleton: a CTA owns THREADS*S sinks (S per thread, in registers)
+//   a2-a4  one "pair kernel" skeleton: a CTA owns T*S sinks (S per thread, in registers)
 //       and a contiguous range of source tiles; tiles are staged through shared memory with
 //       a cp.async double buffer and read back as warp-wide broadcasts (LDS.128).
 //   a5  when the source range is split across CTAs (grid.y > 1), partial results go to a
@@ -31,7 +31,6 @@
 
 namespace {
 
-constexpr int THREADS = 128;      // threads per CTA of the pair kernels
 constexpr int TILE = 128;         // sources per shared-memory tile
 constexpr int MAX_SPLIT = 256;    // upper bound on grid.y (source-range splits)
 
@@ -39,15 +38,13 @@ constexpr int MAX_SPLIT = 256;    // upper bound on grid.y (source-range splits)
 // small device helpers
 // ----------------------------------------------------------------------------------------
 
-// Seed for r2^(-1/2): MUFU.RSQ64H looks only at the high word.  The signed-int max clamps
-// r2 < 2^-400 (including 0) to 2^-400 so the seed stays finite; the refinement then uses the
-// unclamped r2, giving a finite weight that multiplies a zero separation.
+// Seed for r2^(-1/2): MUFU.RSQ64H looks only at the high word.  Every caller adds R2_FLOOR (or a
+// larger eps^2) to r2, so the argument is a positive normal number and the seed is finite even
+// for the self pair (r_ji = 0 exactly), whose finite weight then multiplies a zero separation.
+constexpr double R2_FLOOR = 4.909093465297727e-91;    // 2^-300: below any representable |r_ji|^2 of interest
 __device__ __forceinline__ double rsqrt_seed(double r2) {
-    int hi = __double2hiint(r2);
-    hi = max(hi, 0x26f00000);                       // 2^-400
-    double x = __hiloint2double(hi, 0);
     double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
     return y;
 }
 
@@ -168,7 +165,10 @@ struct DtArgs {
     int32_t* pid;      // [split][2][n_sink]  their source ids
 };
 
-struct DtPass {
+// ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
+// the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
+template <bool ASC>
+struct DtPassT {
     static constexpr int REC = 8;   // x y z m vx vy vz id(bits)
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id; };
@@ -181,10 +181,12 @@ struct DtPass {
         s.m = a.mass[id]; s.id = id;
     }
     __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
+    // FP64-pipe instructions: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
+    // 2 DMUL keys = 23, plus 2 (ASC) or 4 DSETP.
     __device__ __forceinline__ static void pair(const Args&, const Sink& s, Acc& c, const double* __restrict__ r) {
         const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
         const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
-        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
         const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
         const int jid = __double2loint(r[7]);
         const double y0 = rsqrt_seed(r2);
@@ -195,9 +197,16 @@ struct DtPass {
         const double y2 = fma(t, fma(e, e, e), t);
         double kff = (s.m + r[3]) * y3;
         double kfb = v2 * y2;
-        if (jid == s.id) { kff = -1.0; kfb = -1.0; }          // j != i (Eq. 21, 22)
-        if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
-        if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+        if (ASC) {
+            const bool other = jid != s.id;                   // j != i (Eq. 21, 22)
+            const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
+            c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
+            c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
+        } else {
+            if (jid == s.id) { kff = -1.0; kfb = -1.0; }          // j != i (Eq. 21, 22)
+            if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
+            if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+        }
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
         const size_t o = (size_t)split * 2 * g.n_sink + k;
@@ -205,6 +214,9 @@ struct DtPass {
         a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
     }
 };
+
+using DtPass = DtPassT<false>;
+using DtPassAsc = DtPassT<true>;
 
 struct PotArgs {
     const double* pos;
@@ -245,10 +257,11 @@ struct PotPass {
 };
 
 // ----------------------------------------------------------------------------------------
-// a2-a4: the pair kernel.  grid = (ceil(n_sink / (THREADS*S)), n_split).
+// a2-a4: the pair kernel.  grid = (ceil(n_sink / (T*S)), n_split); T threads, S sinks per thread,
+// MINB resident CTAs per SM, inner loop unrolled UNR times.
 // ----------------------------------------------------------------------------------------
-template <class P, int S, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
+template <class P, int S, int T, int MINB, int UNR>
+__global__ void __launch_bounds__(T, MINB)
 pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ src_rec) {
     constexpr int REC = P::REC;
     constexpr int CHUNKS = TILE * REC * 8 / 16;            // 16-B chunks per tile
@@ -257,10 +270,10 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
     typename P::Sink sink[S];
     typename P::Acc accu[S];
     int ids[S];
-    const int kbase = blockIdx.x * (THREADS * S) + threadIdx.x;
+    const int kbase = blockIdx.x * (T * S) + threadIdx.x;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * THREADS;
+        const int k = kbase + s * T;
         const int kk = k < g.n_sink ? k : g.n_sink - 1;      // tail threads shadow the last sink
         ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
         P::load_sink(a, ids[s], sink[s]);
@@ -273,7 +286,7 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
 
     auto load_tile = [&](int tile, int buf) {
         const double* gsrc = src_rec + (size_t)tile * TILE * REC;
-        for (int ch = threadIdx.x; ch < CHUNKS; ch += THREADS) cp_async16(&sm[buf][2 * ch], gsrc + 2 * ch);
+        for (int ch = threadIdx.x; ch < CHUNKS; ch += T) cp_async16(&sm[buf][2 * ch], gsrc + 2 * ch);
         cp_async_commit();
     };
 
@@ -285,7 +298,7 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
         __syncthreads();
         const int cnt = min(TILE, g.n_src - tile * TILE);
         const double* __restrict__ tb = sm[buf];
-#pragma unroll 2
+#pragma unroll UNR
         for (int jj = 0; jj < cnt; ++jj) {
             double r[REC];
 #pragma unroll
@@ -301,7 +314,7 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
 
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * THREADS;
+        const int k = kbase + s * T;
         if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
     }
 }
@@ -641,6 +654,43 @@ __global__ void pn1_bh_finalize_kernel(int n_bh, int n_chunks, const int32_t* __
     o[0] += sx; o[1] += sy; o[2] += sz;
 }
 
+// ----------------------------------------------------------------------------------------
+// Measurement aid: register-only FP64 chains (no memory traffic), to MEASURE the FP64-pipe peak
+// that bench.py's roofline quotes next to the derived 64 lanes/clk/SM figure.
+//   MIX 0: 8 independent DFMA chains per thread (pure DFMA peak).
+//   MIX 1: per 15 instructions 3 DADD + 9 DFMA + 3 DMUL (the acc pair's instruction mix).
+// ----------------------------------------------------------------------------------------
+constexpr int PROBE_THREADS = 128;
+constexpr int PROBE_CHAINS = 8;
+template <int MIX>
+__global__ void __launch_bounds__(PROBE_THREADS, 4)
+fp64_probe_kernel(int iters, double b, double c, double* __restrict__ sink) {
+    double a[PROBE_CHAINS];
+#pragma unroll
+    for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = 1.0 + 1e-9 * (double)(threadIdx.x + k);
+    for (int it = 0; it < iters; ++it) {
+        if (MIX == 0) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = fma(a[k], b, c);          // 32 DFMA
+        } else {
+#pragma unroll
+            for (int k = 0; k < PROBE_CHAINS; ++k) {                                     // 8 x 15 instructions
+                double x = a[k];
+                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                a[k] = x;
+            }
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < PROBE_CHAINS; ++k) s += a[k];
+    if (s == 123.456) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chains alive
+}
+
 }  // namespace
 
 // ========================================================================================
@@ -696,55 +746,89 @@ int check_lists(bifrost_ctx* ctx, int64_t n, const int32_t* sink_idx, int64_t n_
     return BIFROST_OK;
 }
 
+// eps^2 as the kernels use it: never below R2_FLOOR (see rsqrt_seed)
+inline double soft2(double eps) { const double e2 = eps * eps; return e2 > R2_FLOOR ? e2 : R2_FLOOR; }
+
 inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // Source-range split: enough CTAs for ~16 per resident slot (tail < a few %), bounded by the
 // number of source tiles, MAX_SPLIT and the partial workspace.
 Geom make_geom(const bifrost_ctx* ctx, int64_t n_sink, int64_t n_src, int sinks_per_cta, int resident_per_sm,
-               size_t partial_bytes_per_sink, bool force_partial) {
+               size_t partial_bytes_per_sink) {
     Geom g;
     g.n_sink = (int)n_sink;
     g.n_src = (int)n_src;
     g.compact = 0;
     const int n_tiles = ceil_div(n_src, TILE);
     const int ctas_i = ceil_div(n_sink, sinks_per_cta);
-    const int64_t target = 16LL * ctx->num_sms * resident_per_sm;
-    int64_t split = (target + ctas_i - 1) / ctas_i;
-    if (split > n_tiles) split = n_tiles;
-    if (split > MAX_SPLIT) split = MAX_SPLIT;
+    const int64_t slots = (int64_t)ctx->num_sms * resident_per_sm;
+    const int64_t target = 16LL * slots;
+    int64_t cap = (target + ctas_i - 1) / ctas_i;
+    if (cap < 16) cap = 16;                 // room to search for a balanced wave count
+    if (cap > n_tiles) cap = n_tiles;
+    if (cap > MAX_SPLIT) cap = MAX_SPLIT;
     const int64_t ws_cap = (int64_t)(ctx->partial_bytes / (partial_bytes_per_sink * (size_t)(n_sink > 0 ? n_sink : 1)));
-    if (split > ws_cap) split = ws_cap;
-    if (split < 1) split = 1;
+    if (cap > ws_cap) cap = ws_cap;
+    if (cap < 1) cap = 1;
+    // Wave quantisation: all CTAs cost ~tiles_per_split tile-times (+ a fixed prologue), and the
+    // grid runs in ceil(CTAs / slots) waves.  Pick the split with the least modelled time.
+    int64_t split = 1;
+    double best_t = 0.0;
+    for (int64_t s = 1; n_tiles > 0 && s <= cap; ++s) {
+        const int64_t tps = (n_tiles + s - 1) / s;
+        const int64_t ns = (n_tiles + tps - 1) / tps;
+        if (ns != s) continue;
+        const int64_t waves = (ctas_i * ns + slots - 1) / slots;
+        const double t = (double)waves * ((double)tps + 0.25);
+        if (s == 1 || t < best_t * (1.0 - 1e-3)) { best_t = t; split = s; }
+    }
     g.tiles_per_split = n_tiles > 0 ? ceil_div(n_tiles, split) : 1;
     g.n_split = n_tiles > 0 ? ceil_div(n_tiles, g.tiles_per_split) : 1;
-    (void)force_partial;
     return g;
 }
 
-template <class P, int S, int MINB>
-int launch_pair(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
-    dim3 grid(ceil_div(g.n_sink, THREADS * S), g.n_split);
-    pair_kernel<P, S, MINB><<<grid, THREADS, 0, st>>>(a, g, ctx->src_rec);
+// Kernel shapes (S sinks per thread, T threads, MINB resident CTAs per SM, unroll), chosen on B200
+// with the steady-state sweep recorded in profiles/ (DESIGN.md §7): large sink sets want the most
+// sinks per shared-memory broadcast that the register file allows; small sets want every thread
+// to own a distinct sink.
+template <int S_, int T_, int MINB_, int UNR_>
+struct Shape { static constexpr int S = S_, T = T_, MINB = MINB_, UNR = UNR_; };
+using ShapeTiny = Shape<1, 128, 8, 4>;
+
+template <class P, class Sh>
+int launch_pair(bifrost_ctx* ctx, const typename P::Args& a, Geom& g, int64_t n_sink, int64_t n_src,
+                size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
+    g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
+    g.compact = compact;
+    dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
+    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
+}
+
+// Big: n_sink >= 4096; Mid: 256 <= n_sink < 4096; Tiny: below.
+template <class P, class Big, class Mid, class Tiny = ShapeTiny>
+int run_pair(bifrost_ctx* ctx, const typename P::Args& a, Geom& g, int64_t n_sink, int64_t n_src,
+             size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
+    if (n_sink >= 4096) return launch_pair<P, Big>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
+    if (n_sink >= 256) return launch_pair<P, Mid>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
+    return launch_pair<P, Tiny>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
 }
 
 int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
              int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out, int compact,
              cudaStream_t st) {
     if (n_sink == 0) return BIFROST_OK;
-    constexpr int S = 4, MINB = 4;
-    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, false);
-    g.compact = compact;
+    Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
         pack_acc_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    AccArgs a{pos, sink_idx, eps * eps, G, out, (double*)ctx->partial};
-    int rc = launch_pair<AccPass, S, MINB>(ctx, a, g, st);
+    AccArgs a{pos, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    int rc = run_pair<AccPass, Shape<8, 256, 1, 1>, Shape<4, 128, 4, 2>>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -759,17 +843,15 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
               const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
               double* out, int compact, cudaStream_t st) {
     if (n_sink == 0) return BIFROST_OK;
-    constexpr int S = 4, MINB = 3;
-    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, false);
-    g.compact = compact;
+    Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
         pack_grad_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, acc, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    GradArgs a{pos, acc, sink_idx, eps * eps, G, out, (double*)ctx->partial};
-    int rc = launch_pair<GradPass, S, MINB>(ctx, a, g, st);
+    GradArgs a{pos, acc, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    int rc = run_pair<GradPass, Shape<4, 256, 1, 2>, Shape<4, 128, 3, 2>, Shape<1, 128, 5, 2>>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -785,20 +867,21 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
                double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact,
                cudaStream_t st) {
     if (n_sink == 0) return BIFROST_OK;
-    constexpr int S = 4, MINB = 3;
-    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 24, true);
-    g.compact = compact;
+    Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
         pack_dt_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, vel, mass, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    // workspace: keys [split][2][n_sink] doubles, then ids [split][2][n_sink] ints
+    // workspace (24 B per sink and split): keys [split][2][n_sink] doubles in the first two thirds,
+    // ids [split][2][n_sink] ints in the last third
     double* pkey = (double*)ctx->partial;
-    int32_t* pid = (int32_t*)(pkey + (size_t)g.n_split * 2 * n_sink);
+    int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
     DtArgs a{pos, vel, mass, sink_idx, pkey, pid};
-    int rc = launch_pair<DtPass, S, MINB>(ctx, a, g, st);
+    using Big = Shape<4, 128, 3, 2>;
+    int rc = src_idx ? run_pair<DtPass, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
+                     : run_pair<DtPassAsc, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     dt_finalize_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx, pkey, pid, pos,
                                                              vel, mass, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb);
@@ -814,19 +897,17 @@ int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
         if (out_W) CU_TRY(ctx, cudaMemsetAsync(out_W, 0, sizeof(double), st));
         return BIFROST_OK;
     }
-    constexpr int S = 4, MINB = 4;
-    Geom g = make_geom(ctx, n_sink, n_src, THREADS * S, MINB, 8, false);
+    Geom g;
     const int compact = out_phi ? 0 : 1;           // the scratch holds compact rows
     double* phi = out_phi ? out_phi : ctx->phi_scratch;
-    g.compact = compact;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
         pack_pot_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    PotArgs a{pos, sink_idx, eps * eps, G, phi, (double*)ctx->partial};
-    int rc = launch_pair<PotPass, S, MINB>(ctx, a, g, st);
+    PotArgs a{pos, sink_idx, soft2(eps), G, phi, (double*)ctx->partial};
+    int rc = run_pair<PotPass, Shape<4, 128, 4, 2>, Shape<4, 128, 4, 2>>(ctx, a, g, n_sink, n_src, 8, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_scalar_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -944,7 +1025,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     ctx->max_n = max_n;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
-    ctx->partial_bytes = 24 * (size_t)max_n * 8;
+    ctx->partial_bytes = 24 * (size_t)max_n * 16;   // up to 16 source-range splits at n_sink = max_n
     if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
     if (cudaMalloc(&ctx->src_rec, n_pad * 10 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
@@ -1149,6 +1230,38 @@ int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
     rc = pn1_impl(ctx, n, ctx->d_pos, ctx->d_vel, ctx->d_mass, ctx->d_sink, n_bh, G, c, ctx->d_out, ctx->hstream);
     if (rc) return rc;
     return fetch_rows(ctx, ctx->d_out, 24, nullptr, n, out_acc_pn, ctx->h_stage);
+}
+
+// ---- measurement aid -------------------------------------------------------------------
+
+int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm, double* out_ms,
+                       double* out_lane_instr) {
+    if (!ctx || !out_ms || !out_lane_instr || iters <= 0 || iters > (1 << 30) || ctas_per_sm <= 0 || ctas_per_sm > 64 ||
+        (mix != 0 && mix != 1))
+        return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    DeviceGuard guard(ctx->device);
+    cudaEvent_t e0, e1;
+    CU_TRY(ctx, cudaEventCreate(&e0));
+    CU_TRY(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->num_sms * ctas_per_sm;
+    const double b = 0.999999999, c = 1e-9;
+    double* sink = (double*)ctx->partial;      // never written (see kernel); >= 64 MiB
+    for (int rep = 0; rep < 2; ++rep) {        // first launch = warm-up
+        cudaEventRecord(e0, 0);
+        if (mix == 0) fp64_probe_kernel<0><<<grid, PROBE_THREADS>>>((int)iters, b, c, sink);
+        else fp64_probe_kernel<1><<<grid, PROBE_THREADS>>>((int)iters, b, c, sink);
+        cudaEventRecord(e1, 0);
+        ctx->launches++;
+        CU_TRY(ctx, cudaEventSynchronize(e1));
+    }
+    float ms = 0.f;
+    CU_TRY(ctx, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *out_ms = ms;
+    const double per_thread = (double)iters * (mix == 0 ? 32.0 : 120.0);
+    *out_lane_instr = per_thread * (double)grid * PROBE_THREADS;
+    return BIFROST_OK;
 }
 
 }  // extern "C"
