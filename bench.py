@@ -102,12 +102,15 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def make_workload(cfg: int):
+def make_workload(cfg: int, n: int = 0):
     from paper_2210_02472_b200 import workloads as W
-    return W.CONFIGS[cfg]()
+    return W.CONFIGS[cfg](n=n) if n else W.CONFIGS[cfg]()
 
 
 def workload_name(cfg: int, n: int) -> str:
+    full = {4: 1 << 20, 5: 1 << 21}[cfg]
+    if n != full:
+        return f"config{cfg} recipe at a REDUCED N={n} (profiling aid, not the benchmark configuration)"
     return {4: f"config4: Plummer N=2^20={n}, Kroupa IMF, IMBH 1e-3 M + 100 stellar BHs, eps=0, c=1e4, all active; "
                "acc + FSI grad + dtmin + PN1.0",
             5: f"config5: Plummer N=2^21={n}, Kroupa IMF, eps=1e-5, all active; acc + FSI grad"}[cfg]
@@ -147,7 +150,7 @@ def run_reference(args):
         return 0
     import oracle
     oracle.build()
-    w = make_workload(args.config)
+    w = make_workload(args.config, args.n)
     n_sinks = args.ref_sinks
     for _ in range(args.warmup):
         oracle_sample(w, max(8, n_sinks // 8))
@@ -191,7 +194,7 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    w = make_workload(args.config)
+    w = make_workload(args.config, args.n)
     n = w.n
     full_path = args.config == 4
     ctx = Context(n)
@@ -373,6 +376,56 @@ def run_cuda(args):
     return 0
 
 
+# --------------------------------------------------------------------------------------
+# small-active-set sweep (configs 2 and 3): us per call, launch-bound / L2-bound regime
+# --------------------------------------------------------------------------------------
+
+def run_sweep(args):
+    import torch
+    from paper_2210_02472_b200 import workloads as W
+    from paper_2210_02472_b200.binding import Context
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    out = {"metric": "us per C-ABI call vs active-set size (configs 2, 3)", "unit": "us", "data": "synthetic",
+           "timing": "CUDA events around 20 back-to-back calls after 3 warm-ups, sources L2-resident", "cases": []}
+    for cfg, sizes in ((2, [W.config2_sink_list(k) for k in range(0, 15)]),
+                       (3, [W.config3_sink_list(k) for k in range(10, -1, -1)])):
+        w = W.CONFIGS[cfg]()
+        ctx = Context(w.n)
+        pos, vel, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.vel, w.mass))
+        acc = ctx.acc(pos, mass, w.G, w.eps)
+        outs = {"acc": torch.zeros_like(acc), "grad": torch.zeros_like(acc)}
+        for sinks in sizes:
+            si = torch.from_numpy(sinks).to(dev)
+            ns = int(sinks.shape[0])
+            calls = {"acc": lambda: ctx.acc(pos, mass, w.G, w.eps, si, None, out=outs["acc"]),
+                     "grad": lambda: ctx.grad(pos, mass, acc, w.G, w.eps, si, None, out=outs["grad"]),
+                     "dtmin": lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None)}
+            rec = {"config": cfg, "n_src": w.n, "n_sink": ns}
+            reps = 20 if ns * w.n < 2e9 else 3
+            for name, fn in calls.items():
+                for _ in range(3):
+                    fn()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                for _ in range(reps):
+                    fn()
+                e1.record()
+                torch.cuda.synchronize()
+                us = 1e3 * e0.elapsed_time(e1) / reps
+                rec[name + "_us"] = round(us, 2)
+                rec[name + "_pairs_per_s"] = ns * float(w.n) / (us * 1e-6)
+            # a1 gather traffic: the acc pack reads 32 B and writes 48 B per source
+            rec["acc_source_bytes"] = 80 * w.n
+            out["cases"].append(rec)
+        ctx.close()
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -384,10 +437,14 @@ def main():
     ap.add_argument("--cpu-sinks", type=int, default=2048, help="oracle sample size (sinks) for cpu_baseline")
     ap.add_argument("--ref-sinks", type=int, default=1024, help="oracle sample size (sinks) per reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--n", type=int, default=0, help="override the workload's N (profiling aid; NOT the benchmark configuration)")
+    ap.add_argument("--sweep", action="store_true", help="small-active-set sweep of configs 2 and 3 (us per call); prints one JSON line")
     ap.add_argument("--no-fp64-probe", action="store_true", help="skip the register-only FP64-pipe peak probe")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_cuda(args)
 
 

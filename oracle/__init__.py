@@ -179,3 +179,112 @@ def criteria(vel, acc_in, grad_c, jerk_in, eta, eta_grad, eta_jerk, sink_idx=Non
     _load().oracle_criteria(n, vel.ctypes.data, acc_in.ctypes.data, grad_c.ctypes.data, jerk_in.ctypes.data, sip, ns,
                             eta, eta_grad, eta_jerk, *[o.ctypes.data for o in outs])
     return dict(dt_va=outs[0], dt_gradv=outs[1], dt_grada=outs[2], dt_jerk=outs[3])
+
+
+# ---- NEXT-2: subsystem-aware variants -------------------------
+
+def _sub_arr(subsys, n):
+    s = np.ascontiguousarray(subsys, dtype=np.int32)
+    assert s.shape == (n,)
+    return s
+
+
+def _lists(n, sink_idx, src_idx):
+    si, sip = _idx(sink_idx)
+    sj, sjp = _idx(src_idx)
+    return si, sip, (n if si is None else si.shape[0]), sj, sjp, (n if sj is None else sj.shape[0])
+
+
+def _sub_sigs():
+    lib = _load()
+    if not getattr(lib, "_sub_ready", False):
+        lists = [_P, _I64, _P, _I64]
+        lib.oracle_acc_sub.argtypes = [_I64, _P, _P, *lists, _D, _D, _P, _P]
+        lib.oracle_phi_sub.argtypes = [_I64, _P, _P, *lists, _D, _D, _P, _P]
+        lib.oracle_grad_sub.argtypes = [_I64, _P, _P, _P, *lists, _D, _D, _P, _P]
+        lib.oracle_jerk_sub.argtypes = [_I64, _P, _P, _P, *lists, _D, _D, _P, _P]
+        lib.oracle_dtmin_sub.argtypes = [_I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P, _P, _P, _P]
+        lib.oracle_pn1_sub.argtypes = [_I64, _P, _P, _P, _P, _I64, _D, _D, _P, _P]
+        lib.oracle_subsys_min.argtypes = [_I64, _P, _P, _P]
+        lib._sub_ready = True
+    return lib
+
+
+def acc_sub(pos, mass, G, eps, subsys, sink_idx=None, src_idx=None) -> np.ndarray:
+    """O-acc with pairs inside one subsystem dropped (Alg. 1)."""
+    pos, mass = _f64(pos), _f64(mass)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    out = np.zeros((ns, 3))
+    _sub_sigs().oracle_acc_sub(n, pos.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps, sub.ctypes.data,
+                               out.ctypes.data)
+    return out
+
+
+def phi_sub(pos, mass, G, eps, subsys, sink_idx=None, src_idx=None) -> np.ndarray:
+    pos, mass = _f64(pos), _f64(mass)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    out = np.zeros(ns)
+    _sub_sigs().oracle_phi_sub(n, pos.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps, sub.ctypes.data,
+                               out.ctypes.data)
+    return out
+
+
+def grad_sub(pos, mass, acc_in, G, eps, subsys, sink_idx=None, src_idx=None) -> np.ndarray:
+    pos, mass, acc_in = _f64(pos), _f64(mass), _f64(acc_in)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    out = np.zeros((ns, 3))
+    _sub_sigs().oracle_grad_sub(n, pos.ctypes.data, mass.ctypes.data, acc_in.ctypes.data, sip, ns, sjp, nj, G, eps,
+                                sub.ctypes.data, out.ctypes.data)
+    return out
+
+
+def jerk_sub(pos, vel, mass, G, eps, subsys, sink_idx=None, src_idx=None) -> np.ndarray:
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    out = np.zeros((ns, 3))
+    _sub_sigs().oracle_jerk_sub(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eps,
+                                sub.ctypes.data, out.ctypes.data)
+    return out
+
+
+def dtmin_sub(pos, vel, mass, G, eta_ff, eta_fb, subsys, sink_idx=None, src_idx=None):
+    """O-dt with same-subsystem sources excluded (§3.5.2); dict like dtmin()."""
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    dt_ff, dt_fb, m_ff, m_fb = np.zeros(ns), np.zeros(ns), np.zeros(ns), np.zeros(ns)
+    j_ff, j_fb = np.zeros(ns, dtype=np.int32), np.zeros(ns, dtype=np.int32)
+    _sub_sigs().oracle_dtmin_sub(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, eta_ff,
+                                 eta_fb, sub.ctypes.data, dt_ff.ctypes.data, dt_fb.ctypes.data, j_ff.ctypes.data,
+                                 j_fb.ctypes.data, m_ff.ctypes.data, m_fb.ctypes.data)
+    return dict(dt_ff=dt_ff, dt_fb=dt_fb, j_ff=j_ff, j_fb=j_fb, margin_ff=m_ff, margin_fb=m_fb)
+
+
+def pn1_sub(pos, vel, mass, bh_idx, G, c, subsys) -> np.ndarray:
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    sub = _sub_arr(subsys, n)
+    bh = np.ascontiguousarray(bh_idx, dtype=np.int32)
+    out = np.zeros((n, 3))
+    _sub_sigs().oracle_pn1_sub(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, bh.ctypes.data, bh.shape[0], G, c,
+                               sub.ctypes.data, out.ctypes.data)
+    return out
+
+
+def subsys_min(subsys, dt) -> np.ndarray:
+    """Eq. 20: every member of a subsystem gets the minimum time-step of its members."""
+    dt = _f64(dt)
+    n = dt.shape[0]
+    sub = _sub_arr(subsys, n)
+    out = np.zeros(n)
+    _sub_sigs().oracle_subsys_min(n, sub.ctypes.data, dt.ctypes.data, out.ctypes.data)
+    return out

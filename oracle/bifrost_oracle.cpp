@@ -30,6 +30,9 @@
 // form, sum_i m_i j_i = 0.  phi: two-body value, W = 1/2 sum m_i phi_i against O-pot and the
 // Plummer value, -m_i a_i = finite difference of W.  criteria: hand-set vectors with integer
 // norms (3-4-5 triangles) evaluated by hand from Eq. 24, 26, 27, 29.
+// NEXT-2 (subsystem exclusion): all-(-1) ids reproduce the plain routines bit for bit; excluded +
+// intra-subsystem partial sums (index lists) = full sums; one all-embracing subsystem gives 0 / +inf;
+// numpy brute force with an explicit mask for dtmin; Eq. 20 against numpy minimum.reduceat.
 // Parity status: acc, grad, dtmin, potential, jerk, phi, criteria pinned.  pn1: the relative two-body
 // dynamics are pinned; the paper prints no PN1.0 formula (PAPER.md:L439, L476 cite
 // Thorne & Hartle 1985 / Einstein et al. 1938), so parity with the paper's own
@@ -61,6 +64,15 @@ struct Neumaier {  // compensated running sum (Neumaier 1974)
 
 inline int64_t pid(const int32_t* idx, int64_t k) { return idx ? (int64_t)idx[k] : k; }
 
+// NEXT-2, subsystem-aware sums.  PAPER.md:L233 Alg. 1 "Acceleration calculations ignore
+// intra-subsystem contributions"; L299 §3.5.2 "the other particles j in the same subsystem are
+// excluded from the time-step assignment"; L488 §3.8 (PN kicks exclude the same subsystem).
+// subsys[k] >= 0 is the subsystem particle k belongs to, -1 marks a single particle; a NULL
+// array means "no subsystems".  A pair (i, j) is dropped iff both carry the same id >= 0.
+inline bool same_subsystem(const int32_t* subsys, int64_t i, int64_t j) {
+    return subsys && subsys[i] >= 0 && subsys[i] == subsys[j];
+}
+
 // ---------------------------------------------------------------------------
 // O-acc.  PAPER.md:L75 Eq. 6 (all pairs) and PAPER.md:L115-119 Eq. 12 (inter-level:
 // the same sum restricted to a source set), with Plummer softening
@@ -70,7 +82,7 @@ inline int64_t pid(const int32_t* idx, int64_t k) { return idx ? (int64_t)idx[k]
 template <class T>
 void acc_impl(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
               int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
-              double* out) {
+              double* out, const int32_t* subsys = nullptr) {
     (void)n;
     const T eps2 = (T)eps * (T)eps;
 #pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
@@ -80,7 +92,7 @@ void acc_impl(int64_t n, const double* pos, const double* mass, const int32_t* s
         Neumaier<T> sx, sy, sz;
         for (int64_t l = 0; l < n_src; ++l) {
             const int64_t j = pid(src_idx, l);
-            if (j == i) continue;
+            if (j == i || same_subsystem(subsys, i, j)) continue;
             const T dx = (T)pos[3 * j] - xi, dy = (T)pos[3 * j + 1] - yi, dz = (T)pos[3 * j + 2] - zi;
             const T s2 = dx * dx + dy * dy + dz * dz + eps2;
             const T w = (T)mass[j] / (s2 * std::sqrt(s2));
@@ -106,7 +118,7 @@ void acc_impl(int64_t n, const double* pos, const double* mass, const int32_t* s
 template <class T>
 void grad_impl(int64_t n, const double* pos, const double* mass, const double* acc,
                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
-               double G, double eps, double* out) {
+               double G, double eps, double* out, const int32_t* subsys = nullptr) {
     (void)n;
     const T eps2 = (T)eps * (T)eps;
 #pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
@@ -117,7 +129,7 @@ void grad_impl(int64_t n, const double* pos, const double* mass, const double* a
         Neumaier<T> sx, sy, sz;
         for (int64_t l = 0; l < n_src; ++l) {
             const int64_t j = pid(src_idx, l);
-            if (j == i) continue;
+            if (j == i || same_subsystem(subsys, i, j)) continue;
             const T dx = (T)pos[3 * j] - xi, dy = (T)pos[3 * j + 1] - yi, dz = (T)pos[3 * j + 2] - zi;
             const T dax = (T)acc[3 * j] - axi, day = (T)acc[3 * j + 1] - ayi, daz = (T)acc[3 * j + 2] - azi;
             const T s2 = dx * dx + dy * dy + dz * dz + eps2;
@@ -147,7 +159,8 @@ void grad_impl(int64_t n, const double* pos, const double* mass, const double* a
 void dtmin_impl(int64_t n, const double* pos, const double* vel, const double* mass,
                 const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
                 double G, double eta_ff, double eta_fb, double* dt_ff, double* dt_fb,
-                int32_t* j_ff, int32_t* j_fb, double* margin_ff, double* margin_fb) {
+                int32_t* j_ff, int32_t* j_fb, double* margin_ff, double* margin_fb,
+                const int32_t* subsys = nullptr) {
     (void)n;
     const double inf = std::numeric_limits<double>::infinity();
 #pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
@@ -157,7 +170,7 @@ void dtmin_impl(int64_t n, const double* pos, const double* vel, const double* m
         int64_t iff = -1, ifb = -1;
         for (int64_t l = 0; l < n_src; ++l) {
             const int64_t j = pid(src_idx, l);
-            if (j == i) continue;
+            if (j == i || same_subsystem(subsys, i, j)) continue;
             const double dx = pos[3 * j] - pos[3 * i], dy = pos[3 * j + 1] - pos[3 * i + 1],
                          dz = pos[3 * j + 2] - pos[3 * i + 2];
             const double r2 = dx * dx + dy * dy + dz * dz;
@@ -219,7 +232,8 @@ inline void pn1_pair(const double* pos, const double* vel, const double* mass, i
 
 template <class T>
 void pn1_impl(int64_t n, const double* pos, const double* vel, const double* mass,
-              const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out) {
+              const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out,
+              const int32_t* subsys = nullptr) {
     std::vector<char> is_bh((size_t)n, 0);
     for (int64_t b = 0; b < n_bh; ++b) is_bh[(size_t)bh_idx[b]] = 1;
     const T c2inv = (T)1 / ((T)c * (T)c);
@@ -228,10 +242,11 @@ void pn1_impl(int64_t n, const double* pos, const double* vel, const double* mas
         Neumaier<T> sx, sy, sz;
         if (is_bh[(size_t)i]) {
             for (int64_t j = 0; j < n; ++j)
-                if (j != i) pn1_pair<T>(pos, vel, mass, i, j, (T)G, c2inv, sx, sy, sz);
+                if (j != i && !same_subsystem(subsys, i, j)) pn1_pair<T>(pos, vel, mass, i, j, (T)G, c2inv, sx, sy, sz);
         } else {
             for (int64_t b = 0; b < n_bh; ++b)
-                pn1_pair<T>(pos, vel, mass, i, (int64_t)bh_idx[b], (T)G, c2inv, sx, sy, sz);
+                if (!same_subsystem(subsys, i, (int64_t)bh_idx[b]))
+                    pn1_pair<T>(pos, vel, mass, i, (int64_t)bh_idx[b], (T)G, c2inv, sx, sy, sz);
         }
         out[3 * i] = (double)sx.value(); out[3 * i + 1] = (double)sy.value(); out[3 * i + 2] = (double)sz.value();
     }
@@ -248,7 +263,7 @@ void pn1_impl(int64_t n, const double* pos, const double* vel, const double* mas
 template <class T>
 void jerk_impl(int64_t n, const double* pos, const double* vel, const double* mass,
                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
-               double G, double eps, double* out) {
+               double G, double eps, double* out, const int32_t* subsys = nullptr) {
     (void)n;
     const T eps2 = (T)eps * (T)eps;
 #pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
@@ -257,7 +272,7 @@ void jerk_impl(int64_t n, const double* pos, const double* vel, const double* ma
         Neumaier<T> sx, sy, sz;
         for (int64_t l = 0; l < n_src; ++l) {
             const int64_t j = pid(src_idx, l);
-            if (j == i) continue;
+            if (j == i || same_subsystem(subsys, i, j)) continue;
             const T dx = (T)pos[3 * j] - (T)pos[3 * i], dy = (T)pos[3 * j + 1] - (T)pos[3 * i + 1],
                     dz = (T)pos[3 * j + 2] - (T)pos[3 * i + 2];
             const T ux = (T)vel[3 * j] - (T)vel[3 * i], uy = (T)vel[3 * j + 1] - (T)vel[3 * i + 1],
@@ -284,7 +299,8 @@ void jerk_impl(int64_t n, const double* pos, const double* vel, const double* ma
 // ---------------------------------------------------------------------------
 template <class T>
 void phi_impl(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx, int64_t n_sink,
-              const int32_t* src_idx, int64_t n_src, double G, double eps, double* out) {
+              const int32_t* src_idx, int64_t n_src, double G, double eps, double* out,
+              const int32_t* subsys = nullptr) {
     (void)n;
     const T eps2 = (T)eps * (T)eps;
 #pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
@@ -293,7 +309,7 @@ void phi_impl(int64_t n, const double* pos, const double* mass, const int32_t* s
         Neumaier<T> s;
         for (int64_t l = 0; l < n_src; ++l) {
             const int64_t j = pid(src_idx, l);
-            if (j == i) continue;
+            if (j == i || same_subsystem(subsys, i, j)) continue;
             const T dx = (T)pos[3 * j] - (T)pos[3 * i], dy = (T)pos[3 * j + 1] - (T)pos[3 * i + 1],
                     dz = (T)pos[3 * j + 2] - (T)pos[3 * i + 2];
             s.add((T)mass[j] / std::sqrt(dx * dx + dy * dy + dz * dz + eps2));
@@ -352,6 +368,21 @@ double potential_impl(int64_t n, const double* pos, const double* mass, double G
     Neumaier<T> tot;
     for (int64_t i = 0; i < n; ++i) tot.add((T)row[(size_t)i]);
     return (double)(-(T)G * tot.value());
+}
+
+// ---------------------------------------------------------------------------
+// O-share.  PAPER.md:L303 Eq. 20: "Each particle in the same subsystem shares the same
+// time-step": eps_i = min_{j in S} eps_j for every member i of subsystem S; single particles
+// (subsys = -1) keep their own value.  Written as the definition: for each i, a loop over all j.
+// ---------------------------------------------------------------------------
+void subsys_min_impl(int64_t n, const int32_t* subsys, const double* dt, double* out) {
+    for (int64_t i = 0; i < n; ++i) {
+        double best = dt[i];
+        if (subsys[i] >= 0)
+            for (int64_t j = 0; j < n; ++j)
+                if (subsys[j] == subsys[i] && dt[j] < best) best = dt[j];
+        out[i] = best;
+    }
 }
 
 }  // namespace
@@ -422,6 +453,47 @@ double oracle_potential(int64_t n, const double* pos, const double* mass, double
 }
 double oracle_potential_ld(int64_t n, const double* pos, const double* mass, double G, double eps) {
     return potential_impl<long double>(n, pos, mass, G, eps);
+}
+
+// ---- NEXT-2: subsystem-aware variants (same routines, pairs inside one subsystem dropped) ----
+int oracle_acc_sub(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx, int64_t n_sink,
+                   const int32_t* src_idx, int64_t n_src, double G, double eps, const int32_t* subsys, double* out) {
+    acc_impl<double>(n, pos, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out, subsys);
+    return 0;
+}
+int oracle_grad_sub(int64_t n, const double* pos, const double* mass, const double* acc, const int32_t* sink_idx,
+                    int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                    const int32_t* subsys, double* out) {
+    grad_impl<double>(n, pos, mass, acc, sink_idx, n_sink, src_idx, n_src, G, eps, out, subsys);
+    return 0;
+}
+int oracle_jerk_sub(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+                    int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                    const int32_t* subsys, double* out) {
+    jerk_impl<double>(n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out, subsys);
+    return 0;
+}
+int oracle_phi_sub(int64_t n, const double* pos, const double* mass, const int32_t* sink_idx, int64_t n_sink,
+                   const int32_t* src_idx, int64_t n_src, double G, double eps, const int32_t* subsys, double* out) {
+    phi_impl<double>(n, pos, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out, subsys);
+    return 0;
+}
+int oracle_dtmin_sub(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+                     int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eta_ff, double eta_fb,
+                     const int32_t* subsys, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb,
+                     double* margin_ff, double* margin_fb) {
+    dtmin_impl(n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb,
+               margin_ff, margin_fb, subsys);
+    return 0;
+}
+int oracle_pn1_sub(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* bh_idx,
+                   int64_t n_bh, double G, double c, const int32_t* subsys, double* out) {
+    pn1_impl<double>(n, pos, vel, mass, bh_idx, n_bh, G, c, out, subsys);
+    return 0;
+}
+int oracle_subsys_min(int64_t n, const int32_t* subsys, const double* dt, double* out) {
+    subsys_min_impl(n, subsys, dt, out);
+    return 0;
 }
 
 }  // extern "C"
