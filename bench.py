@@ -318,8 +318,8 @@ def run_cuda(args):
         # measured FP64-pipe rates of a register-only kernel (outside the timed region; ~0.3 s each)
         probe = {}
         if not args.no_fp64_probe:
-            for mix, name in ((0, "dfma"), (1, "acc_mix")):
-                ms, rate = ctx.fp64_probe(mix=mix, iters=1 << 15, ctas_per_sm=32)
+            for mix, name in ((0, "dfma"), (1, "acc_mix"), (2, "dfma_3_distinct_operands"), (3, "dfma_accumulate_pattern")):
+                ms, rate = ctx.fp64_probe(mix=mix, iters=(1 << 15) if mix < 2 else (1 << 16), ctas_per_sm=32)
                 probe[name] = {"ms": ms, "lane_instr_per_s": rate, "frac_of_derived_pipe_peak": rate / (peak * 1e12 / 2)}
         pairs_rank = float(max(sharding.slice_counts(n, world))) * n     # the slowest rank's share
 

@@ -151,6 +151,25 @@ int bifrost_timestep_criteria(bifrost_ctx* ctx, int64_t n, const double* vel, co
                               double* out_dt_va, double* out_dt_gradv, double* out_dt_grada, double* out_dt_jerk,
                               double* inout_dt, void* stream);
 
+/* ---- NEXT-2: subsystem-aware sums ----
+ * bifrost_set_subsystems - PAPER.md:L233 Alg. 1 ("Acceleration calculations ignore intra-subsystem
+ * contributions"), L299 §3.5.2 (same-subsystem particles are excluded from the time-step assignment)
+ * and L488 §3.8 (no PN kick between members of one subsystem).  subsys : DEVICE int32[n]; subsys[k] is
+ * the subsystem particle k belongs to (0 <= id < n) or -1 for a single particle.  While set, EVERY
+ * pair routine of this context (acc, grad, jerk, potential, dtmin, pn1 and their *_host variants)
+ * drops each pair (i, j) whose members carry the same id >= 0, in addition to j == i; calls must then
+ * use the same n (else BIFROST_EINVAL).  The pointer is BORROWED: the caller keeps the array alive and
+ * unchanged until it is replaced or reset with subsys = NULL (which restores the plain sums).
+ * The exclusion is decided inside the pair kernels (an integer compare and a select per pair; the
+ * excluded term is never formed, so there is no cancellation against the huge intra-subsystem force). */
+int bifrost_set_subsystems(bifrost_ctx* ctx, const int32_t* subsys, int64_t n);
+
+/* bifrost_subsys_min - PAPER.md:L303 Eq. 20: every member of a subsystem shares the minimum time-step
+ * of its members: inout_dt[i] = min_{j : subsys[j] == subsys[i]} inout_dt[j] for subsys[i] >= 0; single
+ * particles keep their value.  DEVICE pointers, asynchronous on stream; inout_dt : double[n] >= 0.
+ * Exact and order-independent (integer atomic minimum on the bit patterns). */
+int bifrost_subsys_min(bifrost_ctx* ctx, int64_t n, const int32_t* subsys, double* inout_dt, void* stream);
+
 /* Host-buffer variants: same semantics, HOST pointers, synchronous (see header comment).
  * Index lists may be NULL as above.  Outputs are written only at sink ids (other host rows are
  * untouched), bifrost_pn1_host overwrites all n rows. */
@@ -170,8 +189,10 @@ int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
 /* Measurement aid, not part of the paper's path: runs a register-only kernel of independent FP64
  * chains (no memory traffic) on the context's device, on the legacy default stream, synchronously,
  * so that bench.py can quote a MEASURED FP64-pipe peak beside the derived one.
- *   mix = 0: pure DFMA;  mix = 1: 3 DADD + 9 DFMA + 3 DMUL per 15 instructions (the acc pair's mix).
- *   iters: loop trips per thread (32 (mix 0) or 120 (mix 1) FP64 instructions each);
+ *   mix = 0: pure DFMA;  mix = 1: 3 DADD + 9 DFMA + 3 DMUL per 15 instructions (the acc pair's mix);
+ *   mix = 2: DFMA with three distinct register operands;  mix = 3: groups of three DFMAs sharing one
+ *   operand (the pair kernels' accumulate pattern) - these two expose the register-file operand limit.
+ *   iters: loop trips per thread (32 (mix 0), 120 (mix 1) or 12 (mix 2, 3) FP64 instructions each);
  *   ctas_per_sm: grid = SM count x ctas_per_sm CTAs of 128 threads (4 are resident per SM).
  * HOST outputs: *out_ms = device time of one launch (CUDA events, after a warm-up launch);
  * *out_lane_instr = FP64-pipe lane-instructions that launch executed (threads x instructions). */

@@ -28,7 +28,7 @@ SYMBOLS = [
     "bifrost_acc", "bifrost_grad", "bifrost_dtmin", "bifrost_pn1",
     "bifrost_jerk", "bifrost_potential", "bifrost_timestep_criteria",
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
-    "bifrost_fp64_probe",
+    "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
 ]
 
 
@@ -69,6 +69,8 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_grad_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P]
     lib.bifrost_dtmin_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P]
     lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+    lib.bifrost_set_subsystems.argtypes = [_P, _P, _I64]
+    lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
     lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
     _lib = lib
     return lib
@@ -328,3 +330,22 @@ class Context:
                                           ctypes.byref(cnt))
         self._check(rc, "bifrost_fp64_probe")
         return ms.value, cnt.value / (ms.value * 1e-3)
+
+    # ---- NEXT-2 ----------------------------------------------------------------------
+    def set_subsystems(self, subsys):
+        """subsys: int32 CUDA tensor [n] (-1 = single) or None.  The tensor is kept alive here."""
+        if subsys is None:
+            self._subsys = None
+            self._check(self._lib.bifrost_set_subsystems(self._h, None, 0), "bifrost_set_subsystems")
+            return
+        _dev_idx(subsys, "subsys")
+        self._subsys = subsys
+        self._check(self._lib.bifrost_set_subsystems(self._h, subsys.data_ptr(), subsys.shape[0]),
+                    "bifrost_set_subsystems")
+
+    def subsys_min(self, subsys, inout_dt):
+        _dev_idx(subsys, "subsys")
+        _dev_f64(inout_dt, (), "inout_dt")
+        rc = self._lib.bifrost_subsys_min(self._h, subsys.shape[0], subsys.data_ptr(), inout_dt.data_ptr(), self._stream())
+        self._check(rc, "bifrost_subsys_min")
+        return inout_dt

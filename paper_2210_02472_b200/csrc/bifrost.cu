@@ -69,28 +69,44 @@ struct Geom {
 // and how a thread's result is stored.
 // ----------------------------------------------------------------------------------------
 
+// NEXT-2: with EXCL = true every record carries the subsystem code of
+// its source (-1 for a single particle) and every sink its own (-2 for a single particle, so that it
+// never matches); a pair with equal codes gets the seed y0 = 0, hence the weight 0 - one integer
+// compare and one 32-bit select per pair, nothing on the FP64 pipe.
+__device__ __forceinline__ double mask_seed(double y0, bool same) {
+    return __hiloint2double(same ? 0 : __double2hiint(y0), 0);
+}
+__device__ __forceinline__ int sink_code(const int32_t* subsys, int id) {
+    const int c = subsys[id];
+    return c < 0 ? -2 : c;
+}
+
 struct AccArgs {
     const double* pos;
+    const int32_t* subsys;
     const int32_t* sink_idx;
     double eps2, G;
     double* out;        // final output [.][3]
     double* partial;    // [split][n_sink][3]
 };
 
-struct AccPass {
-    static constexpr int REC = 6;   // x y z m 1.5m 1.875m
+template <bool EXCL>
+struct AccPassT {
+    static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
     using Args = AccArgs;
-    struct Sink { double x, y, z; };
+    struct Sink { double x, y, z; int sub; };
     struct Acc { double x, y, z; };
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2];
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
     __device__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
     // 15 FP64-pipe instructions: 3 DADD, 3 DFMA (r2), DMUL t, DFMA e, 2 DFMA poly, 2 DMUL, 3 DFMA.
     __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
         const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
         const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
-        const double y0 = rsqrt_seed(r2);
+        double y0 = rsqrt_seed(r2);
+        if (EXCL) y0 = mask_seed(y0, __double2loint(r[6]) == s.sub);
         const double t = y0 * y0;
         const double e = fma(-r2, t, 1.0);
         const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 3/2 e + 15/8 e^2)
@@ -108,24 +124,29 @@ struct AccPass {
     }
 };
 
+using AccPass = AccPassT<false>;
+
 struct GradArgs {
     const double* pos;
     const double* acc;
+    const int32_t* subsys;
     const int32_t* sink_idx;
     double eps2, G;
     double* out;
     double* partial;
 };
 
-struct GradPass {
-    static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m pad
+template <bool EXCL>
+struct GradPassT {
+    static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
     using Args = GradArgs;
-    struct Sink { double x, y, z, ax, ay, az; };
+    struct Sink { double x, y, z, ax, ay, az; int sub; };
     struct Acc { double ux, uy, uz, wx, wy, wz; };   // U = sum w a_ji,  W = sum w (a_ji.r_ji)/s^2 r_ji
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         const size_t o = 3 * (size_t)id;
         s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
         s.ax = a.acc[o]; s.ay = a.acc[o + 1]; s.az = a.acc[o + 2];
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
     __device__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
     // 28 FP64-pipe instructions; C_i = U - 3 W is formed once per sink in store().
@@ -134,7 +155,8 @@ struct GradPass {
         const double bx = r[3] - s.ax, by = r[4] - s.ay, bz = r[5] - s.az;       // a_ji
         const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
         const double q = fma(bx, dx, fma(by, dy, bz * dz));                       // a_ji . r_ji
-        const double y0 = rsqrt_seed(r2);
+        double y0 = rsqrt_seed(r2);
+        if (EXCL) y0 = mask_seed(y0, __double2loint(r[9]) == s.sub);
         const double t = y0 * y0;
         const double e = fma(-r2, t, 1.0);
         const double pm = fma(fma(e, r[8], r[7]), e, r[6]);
@@ -156,10 +178,13 @@ struct GradPass {
     }
 };
 
+using GradPass = GradPassT<false>;
+
 struct DtArgs {
     const double* pos;
     const double* vel;
     const double* mass;
+    const int32_t* subsys;
     const int32_t* sink_idx;
     double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
     int32_t* pid;      // [split][2][n_sink]  their source ids
@@ -167,11 +192,11 @@ struct DtArgs {
 
 // ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
 // the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
-template <bool ASC>
+template <bool ASC, bool EXCL>
 struct DtPassT {
-    static constexpr int REC = 8;   // x y z m vx vy vz id(bits)
+    static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
     using Args = DtArgs;
-    struct Sink { double x, y, z, m, vx, vy, vz; int id; };
+    struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
     // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
     struct Acc { double kff, kfb; int jff, jfb; };
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
@@ -179,6 +204,7 @@ struct DtPassT {
         s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
         s.vx = a.vel[o]; s.vy = a.vel[o + 1]; s.vz = a.vel[o + 2];
         s.m = a.mass[id]; s.id = id;
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
     __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
     // FP64-pipe instructions: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
@@ -197,13 +223,14 @@ struct DtPassT {
         const double y2 = fma(t, fma(e, e, e), t);
         double kff = (s.m + r[3]) * y3;
         double kfb = v2 * y2;
+        // j != i (Eq. 21, 22) and, with EXCL, not in the sink's subsystem
+        const bool other = EXCL ? ((jid != s.id) & (__double2hiint(r[7]) != s.sub)) : (jid != s.id);
         if (ASC) {
-            const bool other = jid != s.id;                   // j != i (Eq. 21, 22)
             const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
             c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
             c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
         } else {
-            if (jid == s.id) { kff = -1.0; kfb = -1.0; }          // j != i (Eq. 21, 22)
+            if (!other) { kff = -1.0; kfb = -1.0; }
             if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
             if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
         }
@@ -215,11 +242,12 @@ struct DtPassT {
     }
 };
 
-using DtPass = DtPassT<false>;
-using DtPassAsc = DtPassT<true>;
+using DtPass = DtPassT<false, false>;
+using DtPassAsc = DtPassT<true, false>;
 
 struct PotArgs {
     const double* pos;
+    const int32_t* subsys;
     const int32_t* sink_idx;
     double eps2, G;
     double* out;        // phi at [.]
@@ -229,13 +257,15 @@ struct PotArgs {
 // Potential (Eq. 4 second term, Eq. 68): p_i = sum_j m_j / s_ij; phi_i = -G p_i.
 // 1/s = y0 (1 + e/2 + 3/8 e^2); the record carries m, m/2, 3m/8 and the source id, because here
 // the self pair does not multiply a zero separation and must be dropped by id (integer select).
-struct PotPass {
-    static constexpr int REC = 8;   // x y z m 0.5m 0.375m id(bits) pad
+template <bool EXCL>
+struct PotPassT {
+    static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
     using Args = PotArgs;
-    struct Sink { double x, y, z; int id; };
+    struct Sink { double x, y, z; int id, sub; };
     struct Acc { double p; };
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2]; s.id = id;
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
     __device__ static void init(Acc& c) { c.p = 0.0; }
     // 12 FP64-pipe instructions: 3 DADD, 3 DFMA, DMUL, DFMA, 2 DFMA, DMUL, DADD.
@@ -248,6 +278,7 @@ struct PotPass {
         const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 1/2 e + 3/8 e^2)
         double w = y0 * pm;                                   // m / s
         if (__double2loint(r[6]) == s.id) w = 0.0;            // j != i
+        if (EXCL && __double2hiint(r[6]) == s.sub) w = 0.0;   // same subsystem
         c.p += w;
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
@@ -255,6 +286,8 @@ struct PotPass {
         else a.partial[(size_t)split * g.n_sink + k] = c.p;
     }
 };
+
+using PotPass = PotPassT<false>;
 
 // ----------------------------------------------------------------------------------------
 // a2-a4: the pair kernel.  grid = (ceil(n_sink / (T*S)), n_split); T threads, S sinks per thread,
@@ -323,26 +356,38 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
 // a1: pack kernels (gather sources through the index list into aligned records; the tail of
 // the last tile is zero-filled so the cp.async stage never reads undefined memory).
 // ----------------------------------------------------------------------------------------
+// source-side subsystem code: -1 for a single particle (never equal to a sink's code, which is
+// -2 for a single particle), the subsystem id otherwise
+__device__ __forceinline__ int src_code(const int32_t* subsys, int j) {
+    if (!subsys) return -1;
+    const int c = subsys[j];
+    return c < 0 ? -1 : c;
+}
+
+template <bool EXCL>
 __global__ void pack_acc_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
                                 const double* __restrict__ pos, const double* __restrict__ mass,
-                                double* __restrict__ rec) {
+                                const int32_t* __restrict__ subsys, double* __restrict__ rec) {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= n_pad) return;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 6);
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * (EXCL ? 8 : 6));
     if (l < n_src) {
         const int j = src_idx ? src_idx[l] : l;
         const double m = mass[j];
         o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
         o[1] = make_double2(pos[3 * (size_t)j + 2], m);
         o[2] = make_double2(1.5 * m, 1.875 * m);
+        if (EXCL) o[3] = make_double2(__hiloint2double(0, src_code(subsys, j)), 0.0);
     } else {
         o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
+        if (EXCL) o[3] = make_double2(0.0, 0.0);
     }
 }
 
 __global__ void pack_grad_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
                                  const double* __restrict__ pos, const double* __restrict__ mass,
-                                 const double* __restrict__ acc, double* __restrict__ rec) {
+                                 const double* __restrict__ acc, const int32_t* __restrict__ subsys,
+                                 double* __restrict__ rec) {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= n_pad) return;
     double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 10);
@@ -354,7 +399,7 @@ __global__ void pack_grad_kernel(int n_src, int n_pad, const int32_t* __restrict
         o[1] = make_double2(pos[b + 2], acc[b]);
         o[2] = make_double2(acc[b + 1], acc[b + 2]);
         o[3] = make_double2(m, 1.5 * m);
-        o[4] = make_double2(1.875 * m, 0.0);
+        o[4] = make_double2(1.875 * m, __hiloint2double(0, src_code(subsys, j)));
     } else {
         o[0] = o[1] = o[2] = o[3] = o[4] = make_double2(0.0, 0.0);
     }
@@ -362,7 +407,8 @@ __global__ void pack_grad_kernel(int n_src, int n_pad, const int32_t* __restrict
 
 __global__ void pack_dt_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
                                const double* __restrict__ pos, const double* __restrict__ vel,
-                               const double* __restrict__ mass, double* __restrict__ rec) {
+                               const double* __restrict__ mass, const int32_t* __restrict__ subsys,
+                               double* __restrict__ rec) {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= n_pad) return;
     double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
@@ -372,7 +418,7 @@ __global__ void pack_dt_kernel(int n_src, int n_pad, const int32_t* __restrict__
         o[0] = make_double2(pos[b], pos[b + 1]);
         o[1] = make_double2(pos[b + 2], mass[j]);
         o[2] = make_double2(vel[b], vel[b + 1]);
-        o[3] = make_double2(vel[b + 2], __hiloint2double(0, j));
+        o[3] = make_double2(vel[b + 2], __hiloint2double(src_code(subsys, j), j));
     } else {
         o[0] = o[1] = o[2] = o[3] = make_double2(0.0, 0.0);
     }
@@ -397,7 +443,7 @@ __global__ void reduce_vec3_kernel(int n_sink, int n_split, int compact, const i
 
 __global__ void pack_pot_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
                                 const double* __restrict__ pos, const double* __restrict__ mass,
-                                double* __restrict__ rec) {
+                                const int32_t* __restrict__ subsys, double* __restrict__ rec) {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= n_pad) return;
     double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
@@ -407,7 +453,7 @@ __global__ void pack_pot_kernel(int n_src, int n_pad, const int32_t* __restrict_
         o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
         o[1] = make_double2(pos[3 * (size_t)j + 2], m);
         o[2] = make_double2(0.5 * m, 0.375 * m);
-        o[3] = make_double2(__hiloint2double(0, j), 0.0);
+        o[3] = make_double2(__hiloint2double(src_code(subsys, j), j), 0.0);
     } else {
         o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
         o[3] = make_double2(__hiloint2double(0, -1), 0.0);
@@ -588,21 +634,27 @@ __global__ void pn1_flag_kernel(int n_bh, const int32_t* __restrict__ bh_idx, un
 constexpr int PN_THREADS = 128;
 __global__ void __launch_bounds__(PN_THREADS)
 pn1_from_bh_kernel(int n, int n_bh, const int32_t* __restrict__ bh_idx, const double* __restrict__ pos,
-                   const double* __restrict__ vel, const double* __restrict__ mass, double G, double inv_c2,
-                   double* __restrict__ out) {
+                   const double* __restrict__ vel, const double* __restrict__ mass,
+                   const int32_t* __restrict__ subsys, double G, double inv_c2, double* __restrict__ out) {
     __shared__ Body sb[PN_THREADS];
     __shared__ int sid[PN_THREADS];
+    __shared__ int ssub[PN_THREADS];
     const int i = blockIdx.x * PN_THREADS + threadIdx.x;
     const int ii = i < n ? i : n - 1;
     const Body me = load_body(pos, vel, mass, ii);
+    const int my_sub = subsys ? sink_code(subsys, ii) : -2;
     double fx = 0.0, fy = 0.0, fz = 0.0;
     for (int b0 = 0; b0 < n_bh; b0 += PN_THREADS) {
         const int b = b0 + threadIdx.x;
-        if (b < n_bh) { sid[threadIdx.x] = bh_idx[b]; sb[threadIdx.x] = load_body(pos, vel, mass, bh_idx[b]); }
+        if (b < n_bh) {
+            sid[threadIdx.x] = bh_idx[b];
+            sb[threadIdx.x] = load_body(pos, vel, mass, bh_idx[b]);
+            ssub[threadIdx.x] = src_code(subsys, bh_idx[b]);
+        }
         __syncthreads();
         const int cnt = min(PN_THREADS, n_bh - b0);
         for (int q = 0; q < cnt; ++q)
-            if (sid[q] != ii) pn1_pair(me, sb[q], G, inv_c2, fx, fy, fz);
+            if (sid[q] != ii && ssub[q] != my_sub) pn1_pair(me, sb[q], G, inv_c2, fx, fy, fz);
         __syncthreads();
     }
     if (i < n) { out[3 * (size_t)i] = fx; out[3 * (size_t)i + 1] = fy; out[3 * (size_t)i + 2] = fz; }
@@ -613,14 +665,16 @@ constexpr int PN_RED_THREADS = 256;
 __global__ void __launch_bounds__(PN_RED_THREADS)
 pn1_on_bh_kernel(int n, int chunk, const int32_t* __restrict__ bh_idx, const unsigned char* __restrict__ is_bh,
                  const double* __restrict__ pos, const double* __restrict__ vel, const double* __restrict__ mass,
-                 double G, double inv_c2, double* __restrict__ partial /*[n_bh][n_chunks][3]*/) {
+                 const int32_t* __restrict__ subsys, double G, double inv_c2,
+                 double* __restrict__ partial /*[n_bh][n_chunks][3]*/) {
     __shared__ double red[3][PN_RED_THREADS / 32];
     const int b = blockIdx.y;
     const Body me = load_body(pos, vel, mass, bh_idx[b]);
+    const int my_sub = subsys ? sink_code(subsys, bh_idx[b]) : -2;
     const int j0 = blockIdx.x * chunk, j1 = min(j0 + chunk, n);
     double fx = 0.0, fy = 0.0, fz = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += PN_RED_THREADS) {
-        if (is_bh[j]) continue;
+        if (is_bh[j] || src_code(subsys, j) == my_sub) continue;
         const Body o = load_body(pos, vel, mass, j);
         pn1_pair(me, o, G, inv_c2, fx, fy, fz);
     }
@@ -654,6 +708,28 @@ __global__ void pn1_bh_finalize_kernel(int n_bh, int n_chunks, const int32_t* __
     o[0] += sx; o[1] += sy; o[2] += sz;
 }
 
+// NEXT-2, Eq. 20: eps_i = min_{j in S} eps_j.  Non-negative doubles order like their
+// bit patterns read as unsigned integers, so the segment minimum is an integer atomicMin: exact and
+// independent of the order in which members arrive (deterministic).
+__global__ void smin_fill_kernel(int n, unsigned long long* __restrict__ smin) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) smin[i] = 0x7ff0000000000000ULL;     // +inf
+}
+__global__ void smin_reduce_kernel(int n, const int32_t* __restrict__ subsys, const double* __restrict__ dt,
+                                   unsigned long long* __restrict__ smin) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int s = subsys[i];
+    if (s >= 0) atomicMin(&smin[s], (unsigned long long)__double_as_longlong(dt[i]));
+}
+__global__ void smin_apply_kernel(int n, const int32_t* __restrict__ subsys, const unsigned long long* __restrict__ smin,
+                                  double* __restrict__ dt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int s = subsys[i];
+    if (s >= 0) dt[i] = __longlong_as_double((long long)smin[s]);
+}
+
 // ----------------------------------------------------------------------------------------
 // Measurement aid: register-only FP64 chains (no memory traffic), to MEASURE the FP64-pipe peak
 // that bench.py's roofline quotes next to the derived 64 lanes/clk/SM figure.
@@ -662,26 +738,56 @@ __global__ void pn1_bh_finalize_kernel(int n_bh, int n_chunks, const int32_t* __
 // ----------------------------------------------------------------------------------------
 constexpr int PROBE_THREADS = 128;
 constexpr int PROBE_CHAINS = 8;
+//   MIX 2: DFMA with three DISTINCT register operands, x = fma(y, z, x) (no reuse possible).
+//   MIX 3: the pair kernels' accumulate pattern: groups of three DFMAs sharing one operand,
+//          x0 = fma(w, y0, x0); x1 = fma(w, y1, x1); x2 = fma(w, y2, x2).
+// MIX 2 and 3 show the register-file operand limit (one 64-bit operand per clock per SM
+// sub-partition): 2/3 and 6/7 of the MIX 0 rate.
 template <int MIX>
 __global__ void __launch_bounds__(PROBE_THREADS, 4)
-fp64_probe_kernel(int iters, double b, double c, double* __restrict__ sink) {
+fp64_probe_kernel(int iters, double b, double c, const double* __restrict__ in, double* __restrict__ sink) {
     double a[PROBE_CHAINS];
 #pragma unroll
     for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = 1.0 + 1e-9 * (double)(threadIdx.x + k);
-    for (int it = 0; it < iters; ++it) {
-        if (MIX == 0) {
+    if (MIX == 2 || MIX == 3) {
+        // operands that the compiler cannot fold: loaded from memory (all 1 + O(1e-6))
+        double x[12], y[12], w[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+        for (int k = 0; k < 12; ++k) { x[k] = in[threadIdx.x + 128 * k]; y[k] = in[threadIdx.x + 128 * (k + 12)]; }
 #pragma unroll
-                for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = fma(a[k], b, c);          // 32 DFMA
-        } else {
+        for (int k = 0; k < 4; ++k) w[k] = in[threadIdx.x + 128 * (k + 24)];
+        for (int it = 0; it < iters; ++it) {
 #pragma unroll
-            for (int k = 0; k < PROBE_CHAINS; ++k) {                                     // 8 x 15 instructions
-                double x = a[k];
-                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                a[k] = x;
+            for (int g = 0; g < 4; ++g) {
+                if (MIX == 2) {
+                    x[3 * g] = fma(y[3 * g], w[g], x[3 * g]);
+                    x[3 * g + 1] = fma(y[3 * g + 1], y[(3 * g + 5) % 12], x[3 * g + 1]);
+                    x[3 * g + 2] = fma(y[3 * g + 2], y[(3 * g + 7) % 12], x[3 * g + 2]);
+                } else {
+                    x[3 * g] = fma(w[g], y[3 * g], x[3 * g]);
+                    x[3 * g + 1] = fma(w[g], y[3 * g + 1], x[3 * g + 1]);
+                    x[3 * g + 2] = fma(w[g], y[3 * g + 2], x[3 * g + 2]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 12; ++k) a[k % PROBE_CHAINS] += x[k] + y[k];
+    } else {
+        for (int it = 0; it < iters; ++it) {
+            if (MIX == 0) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = fma(a[k], b, c);          // 32 DFMA
+            } else {
+#pragma unroll
+                for (int k = 0; k < PROBE_CHAINS; ++k) {                                     // 8 x 15 instructions
+                    double x = a[k];
+                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
+                    a[k] = x;
+                }
             }
         }
     }
@@ -707,6 +813,9 @@ struct bifrost_ctx {
     unsigned char* is_bh = nullptr;  // [max_n]
     double* phi_scratch = nullptr;   // [max_n]   (bifrost_potential with out_phi == NULL)
     double* wpart = nullptr;         // [ceil(max_n / 4096)] block partials of the W reduction
+    unsigned long long* smin = nullptr;   // [max_n] per-subsystem minima (bifrost_subsys_min)
+    const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
+    int64_t subsys_n = 0;
     int64_t launches = 0;
     char err[256] = {0};
     // mirrors for the *_host entry points (allocated on first use)
@@ -743,6 +852,7 @@ int check_lists(bifrost_ctx* ctx, int64_t n, const int32_t* sink_idx, int64_t n_
     if (n_sink < 0 || n_src < 0 || n_sink > ctx->max_n || n_src > ctx->max_n) return BIFROST_EINVAL;
     if (!sink_idx && n_sink != n) return BIFROST_EINVAL;
     if (!src_idx && n_src != n) return BIFROST_EINVAL;
+    if (ctx->subsys && ctx->subsys_n != n) return BIFROST_EINVAL;
     return BIFROST_OK;
 }
 
@@ -819,16 +929,21 @@ int run_pair(bifrost_ctx* ctx, const typename P::Args& a, Geom& g, int64_t n_sin
 int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
              int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out, int compact,
              cudaStream_t st) {
+    const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_acc_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
+        if (sub) pack_acc_kernel<true><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
+        else pack_acc_kernel<false><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    AccArgs a{pos, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
-    int rc = run_pair<AccPass, Shape<8, 256, 1, 1>, Shape<4, 128, 4, 2>>(ctx, a, g, n_sink, n_src, 24, compact, st);
+    AccArgs a{pos, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    using Big = Shape<8, 256, 1, 1>;
+    using Mid = Shape<4, 128, 4, 2>;
+    int rc = sub ? run_pair<AccPassT<true>, Big, Mid>(ctx, a, g, n_sink, n_src, 24, compact, st)
+                 : run_pair<AccPassT<false>, Big, Mid>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -842,16 +957,21 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
 int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
               const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
               double* out, int compact, cudaStream_t st) {
+    const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_grad_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, acc, ctx->src_rec);
+        pack_grad_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, acc, sub, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    GradArgs a{pos, acc, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
-    int rc = run_pair<GradPass, Shape<4, 256, 1, 2>, Shape<4, 128, 3, 2>, Shape<1, 128, 5, 2>>(ctx, a, g, n_sink, n_src, 24, compact, st);
+    GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    using Big = Shape<4, 256, 1, 2>;
+    using Mid = Shape<4, 128, 3, 2>;
+    using Tiny = Shape<1, 128, 5, 2>;
+    int rc = sub ? run_pair<GradPassT<true>, Big, Mid, Tiny>(ctx, a, g, n_sink, n_src, 24, compact, st)
+                 : run_pair<GradPassT<false>, Big, Mid, Tiny>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -866,11 +986,12 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
                double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact,
                cudaStream_t st) {
+    const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     Geom g;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_dt_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, vel, mass, ctx->src_rec);
+        pack_dt_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, vel, mass, sub, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
@@ -878,10 +999,13 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     // ids [split][2][n_sink] ints in the last third
     double* pkey = (double*)ctx->partial;
     int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
-    DtArgs a{pos, vel, mass, sink_idx, pkey, pid};
+    DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid};
     using Big = Shape<4, 128, 3, 2>;
-    int rc = src_idx ? run_pair<DtPass, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
-                     : run_pair<DtPassAsc, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
+    int rc;
+    if (sub) rc = src_idx ? run_pair<DtPassT<false, true>, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
+                          : run_pair<DtPassT<true, true>, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
+    else rc = src_idx ? run_pair<DtPass, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
+                      : run_pair<DtPassAsc, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
     if (rc) return rc;
     dt_finalize_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx, pkey, pid, pos,
                                                              vel, mass, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb);
@@ -893,6 +1017,7 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
 int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
              int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out_phi,
              double* out_W, cudaStream_t st) {
+    const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) {
         if (out_W) CU_TRY(ctx, cudaMemsetAsync(out_W, 0, sizeof(double), st));
         return BIFROST_OK;
@@ -902,12 +1027,14 @@ int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     double* phi = out_phi ? out_phi : ctx->phi_scratch;
     if (n_src > 0) {
         const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_pot_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, ctx->src_rec);
+        pack_pot_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    PotArgs a{pos, sink_idx, soft2(eps), G, phi, (double*)ctx->partial};
-    int rc = run_pair<PotPass, Shape<4, 128, 4, 2>, Shape<4, 128, 4, 2>>(ctx, a, g, n_sink, n_src, 8, compact, st);
+    PotArgs a{pos, sub, sink_idx, soft2(eps), G, phi, (double*)ctx->partial};
+    using Big = Shape<4, 128, 4, 2>;
+    int rc = sub ? run_pair<PotPassT<true>, Big, Big>(ctx, a, g, n_sink, n_src, 8, compact, st)
+                 : run_pair<PotPassT<false>, Big, Big>(ctx, a, g, n_sink, n_src, 8, compact, st);
     if (rc) return rc;
     if (g.n_split > 1) {
         reduce_scalar_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
@@ -929,7 +1056,8 @@ int pn1_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, 
              const int32_t* bh_idx, int64_t n_bh, double G, double c, double* out, cudaStream_t st) {
     if (n == 0) return BIFROST_OK;
     const double inv_c2 = 1.0 / (c * c);
-    pn1_from_bh_kernel<<<ceil_div(n, PN_THREADS), PN_THREADS, 0, st>>>((int)n, (int)n_bh, bh_idx, pos, vel, mass, G,
+    const int32_t* sub = ctx->subsys;   // NEXT-2; length checked by the caller
+    pn1_from_bh_kernel<<<ceil_div(n, PN_THREADS), PN_THREADS, 0, st>>>((int)n, (int)n_bh, bh_idx, pos, vel, mass, sub, G,
                                                                       inv_c2, out);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
@@ -949,7 +1077,7 @@ int pn1_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, 
     for (int64_t b0 = 0; b0 < n_bh; b0 += 65535) {
         const int nb = (int)((n_bh - b0 < 65535) ? (n_bh - b0) : 65535);
         dim3 grid((unsigned)n_chunks, (unsigned)nb);
-        pn1_on_bh_kernel<<<grid, PN_RED_THREADS, 0, st>>>((int)n, chunk, bh_idx + b0, ctx->is_bh, pos, vel, mass, G, inv_c2,
+        pn1_on_bh_kernel<<<grid, PN_RED_THREADS, 0, st>>>((int)n, chunk, bh_idx + b0, ctx->is_bh, pos, vel, mass, sub, G, inv_c2,
                                                           (double*)ctx->partial + 3 * (size_t)b0 * n_chunks);
         ctx->launches++;
     }
@@ -1031,7 +1159,8 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
         cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
         cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess ||
         cudaMalloc(&ctx->phi_scratch, 8 * (size_t)max_n) != cudaSuccess ||
-        cudaMalloc(&ctx->wpart, 8 * ((size_t)max_n / WSUM_PER_BLOCK + 1)) != cudaSuccess) {
+        cudaMalloc(&ctx->wpart, 8 * ((size_t)max_n / WSUM_PER_BLOCK + 1)) != cudaSuccess ||
+        cudaMalloc(&ctx->smin, 8 * (size_t)max_n) != cudaSuccess) {
         cudaGetLastError();
         bifrost_destroy(ctx);
         return BIFROST_ENOMEM;
@@ -1043,7 +1172,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
 int bifrost_destroy(bifrost_ctx* ctx) {
     if (!ctx) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart);
+    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
@@ -1093,6 +1222,7 @@ int bifrost_pn1(bifrost_ctx* ctx, int64_t n, const double* pos, const double* ve
     if (n < 0 || n > ctx->max_n || n_bh < 0 || n_bh > n) return BIFROST_EINVAL;
     if (n > 0 && (!pos || !vel || !mass || !out_acc_pn)) return BIFROST_EINVAL;
     if (n_bh > 0 && !bh_idx) return BIFROST_EINVAL;
+    if (ctx->subsys && ctx->subsys_n != n) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
     return pn1_impl(ctx, n, pos, vel, mass, bh_idx, n_bh, G, c, out_acc_pn, (cudaStream_t)stream);
 }
@@ -1220,6 +1350,7 @@ int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
     if (n < 0 || n > ctx->max_n || n_bh < 0 || n_bh > n) return BIFROST_EINVAL;
     if (n == 0) return BIFROST_OK;
     if (!pos || !vel || !mass || !out_acc_pn || (n_bh > 0 && !bh_idx)) return BIFROST_EINVAL;
+    if (ctx->subsys && ctx->subsys_n != n) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
     int rc;
     if ((rc = ensure_host_mirrors(ctx))) return rc;
@@ -1232,12 +1363,40 @@ int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
     return fetch_rows(ctx, ctx->d_out, 24, nullptr, n, out_acc_pn, ctx->h_stage);
 }
 
+// ---- NEXT-2: subsystem-aware sums ------------------------------------------
+
+int bifrost_set_subsystems(bifrost_ctx* ctx, const int32_t* subsys, int64_t n) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (subsys && (n <= 0 || n > ctx->max_n)) return BIFROST_EINVAL;
+    ctx->subsys = subsys;
+    ctx->subsys_n = subsys ? n : 0;
+    return BIFROST_OK;
+}
+
+int bifrost_subsys_min(bifrost_ctx* ctx, int64_t n, const int32_t* subsys, double* inout_dt, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n) return BIFROST_EINVAL;
+    if (n == 0) return BIFROST_OK;
+    if (!subsys || !inout_dt) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nb = ceil_div(n, 256);
+    smin_fill_kernel<<<nb, 256, 0, st>>>((int)n, ctx->smin);
+    smin_reduce_kernel<<<nb, 256, 0, st>>>((int)n, subsys, inout_dt, ctx->smin);
+    smin_apply_kernel<<<nb, 256, 0, st>>>((int)n, subsys, ctx->smin, inout_dt);
+    ctx->launches += 3;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
 // ---- measurement aid -------------------------------------------------------------------
 
 int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm, double* out_ms,
                        double* out_lane_instr) {
     if (!ctx || !out_ms || !out_lane_instr || iters <= 0 || iters > (1 << 30) || ctas_per_sm <= 0 || ctas_per_sm > 64 ||
-        (mix != 0 && mix != 1))
+        mix < 0 || mix > 3)
         return BIFROST_EINVAL;
     ctx->err[0] = 0;
     DeviceGuard guard(ctx->device);
@@ -1247,10 +1406,18 @@ int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm
     const int grid = ctx->num_sms * ctas_per_sm;
     const double b = 0.999999999, c = 1e-9;
     double* sink = (double*)ctx->partial;      // never written (see kernel); >= 64 MiB
+    double* in = ctx->src_rec;                 // operands of mix 2/3: 28 x 128 doubles, set to 1 + O(1e-6)
+    {
+        static double h[28 * 128];
+        for (int i = 0; i < 28 * 128; ++i) h[i] = 1.0 + 1e-6 * i;
+        CU_TRY(ctx, cudaMemcpy(in, h, sizeof(h), cudaMemcpyHostToDevice));
+    }
     for (int rep = 0; rep < 2; ++rep) {        // first launch = warm-up
         cudaEventRecord(e0, 0);
-        if (mix == 0) fp64_probe_kernel<0><<<grid, PROBE_THREADS>>>((int)iters, b, c, sink);
-        else fp64_probe_kernel<1><<<grid, PROBE_THREADS>>>((int)iters, b, c, sink);
+        if (mix == 0) fp64_probe_kernel<0><<<grid, PROBE_THREADS>>>((int)iters, b, c, in, sink);
+        else if (mix == 1) fp64_probe_kernel<1><<<grid, PROBE_THREADS>>>((int)iters, b, c, in, sink);
+        else if (mix == 2) fp64_probe_kernel<2><<<grid, PROBE_THREADS>>>((int)iters, b, c, in, sink);
+        else fp64_probe_kernel<3><<<grid, PROBE_THREADS>>>((int)iters, b, c, in, sink);
         cudaEventRecord(e1, 0);
         ctx->launches++;
         CU_TRY(ctx, cudaEventSynchronize(e1));
@@ -1259,7 +1426,7 @@ int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm
     CU_TRY(ctx, cudaEventElapsedTime(&ms, e0, e1));
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     *out_ms = ms;
-    const double per_thread = (double)iters * (mix == 0 ? 32.0 : 120.0);
+    const double per_thread = (double)iters * (mix == 0 ? 32.0 : mix == 1 ? 120.0 : 12.0);
     *out_lane_instr = per_thread * (double)grid * PROBE_THREADS;
     return BIFROST_OK;
 }

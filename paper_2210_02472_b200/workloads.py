@@ -41,6 +41,7 @@ class Workload:
     c: Optional[float] = None          # speed of light (config 4 only)
     bh_idx: Optional[np.ndarray] = None  # int32 ids of PN particles (config 4 only)
     seed: int = 0
+    subsys: Optional[np.ndarray] = None  # int32 [n]: binary (subsystem) index of each star, -1 = single (config 3)
 
     @property
     def n(self) -> int:
@@ -268,9 +269,12 @@ def config3(n: int = 131072, seed: int = 2) -> Workload:
     vel[2 * n_b:] = com_vel[n_b:]
     perm = rng.permutation(n)           # binary members are not neighbours in memory
     pos, vel, mass = pos[perm], vel[perm], mass[perm]
+    # the binaries double as the subsystems of the NEXT-2 (subsystem-aware) parity cases
+    subsys = np.concatenate([np.arange(n_b), np.arange(n_b), np.full(n_s, -1)]).astype(np.int32)[perm]
     recentre(pos, vel, mass)
     return Workload("config3", np.ascontiguousarray(pos), np.ascontiguousarray(vel),
-                    np.ascontiguousarray(mass), G_NBODY, 0.0, 0.01, 0.01, seed=seed)
+                    np.ascontiguousarray(mass), G_NBODY, 0.0, 0.01, 0.01, seed=seed,
+                    subsys=np.ascontiguousarray(subsys))
 
 
 def config3_sink_list(frac_log2: int, n: int = 131072) -> np.ndarray:

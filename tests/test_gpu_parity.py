@@ -377,3 +377,81 @@ def test_timestep_criteria(torch, ctx):
     o2 = ctx.timestep_criteria(vel, a, None, None, 0.02, 0.1, 0.1)
     assert o2["dt_gradv"] is None and o2["dt_jerk"] is None
     assert np.abs(o2["dt_va"].cpu().numpy()[sinks] / ref["dt_va"] - 1).max() <= 1e-13
+
+
+# ---- NEXT-2: subsystem-aware sums (Alg. 1, §3.5.2, §3.8) -------------------------
+
+def _with_subsystems(n, seed, n_bh=0):
+    """config-3 recipe at a small N: binaries are the subsystems; optionally some members are BHs."""
+    w = W.config3(n=n, seed=seed)
+    assert w.subsys is not None and (w.subsys >= 0).sum() == 2 * (n // 4)
+    return w
+
+
+@pytest.mark.parametrize("n,sel", [(3000, None), (3000, "subset"), (20000, "subset")])
+def test_subsystem_exclusion_parity(torch, ctx, n, sel):
+    w = _with_subsystems(n, 40 + n)
+    rng = np.random.default_rng(n)
+    sinks = None if sel is None else np.sort(rng.choice(n, size=min(n, 777), replace=False)).astype(np.int32)
+    srcs = None if sel is None else rng.permutation(n).astype(np.int32)[: n - 11]
+    pos, vel, mass, sub = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), dev(torch, w.subsys)
+    si = None if sinks is None else dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    rows = slice(None) if sinks is None else sinks
+    a_plain = ctx.acc(pos, mass, w.G, w.eps, si, sj).cpu().numpy()[rows]
+    ctx.set_subsystems(sub)
+    try:
+        a = ctx.acc(pos, mass, w.G, w.eps, si, sj)
+        acc_in = ctx.acc(pos, mass, w.G, w.eps)                       # a_k of every particle, subsystem-aware
+        c = ctx.grad(pos, mass, acc_in, w.G, w.eps, si, sj)
+        j = ctx.jerk(pos, vel, mass, w.G, w.eps, si, sj)
+        d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, sj)
+        phi, _ = ctx.potential(pos, mass, w.G, w.eps, si, sj)
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_subsystems(None)
+    a = a.cpu().numpy()[rows]
+    acc_np = acc_in.cpu().numpy()
+    check_vec(a, oracle.acc_sub(w.pos, w.mass, w.G, w.eps, w.subsys, sink_idx=sinks, src_idx=srcs), "acc_sub")
+    check_vec(c.cpu().numpy()[rows], oracle.grad_sub(w.pos, w.mass, acc_np, w.G, w.eps, w.subsys, sink_idx=sinks, src_idx=srcs),
+              "grad_sub")
+    check_vec(j.cpu().numpy()[rows], oracle.jerk_sub(w.pos, w.vel, w.mass, w.G, w.eps, w.subsys, sink_idx=sinks, src_idx=srcs),
+              "jerk_sub")
+    check_dt(tuple(t.cpu().numpy()[rows] for t in d),
+             oracle.dtmin_sub(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, w.subsys, sink_idx=sinks, src_idx=srcs), "dtmin_sub")
+    phi_ref = oracle.phi_sub(w.pos, w.mass, w.G, w.eps, w.subsys, sink_idx=sinks, src_idx=srcs)
+    assert np.abs(phi.cpu().numpy()[rows] / phi_ref - 1).max() <= 1e-13
+    # the binary partner dominates the plain acceleration of a member: the exclusion really removed it
+    in_sub = (w.subsys >= 0) if sinks is None else (w.subsys[sinks] >= 0)
+    ratio = np.linalg.norm(a_plain[in_sub], axis=1) / np.linalg.norm(a[in_sub], axis=1)
+    assert np.median(ratio) > 10
+    # after the reset the plain sums are back, bit for bit
+    assert np.array_equal(ctx.acc(pos, mass, w.G, w.eps, si, sj).cpu().numpy()[rows], a_plain)
+
+
+def test_subsystem_pn1_and_shared_timestep(torch, ctx):
+    w = _with_subsystems(4000, 77)
+    n = w.n
+    members = np.flatnonzero(w.subsys >= 0)
+    singles = np.flatnonzero(w.subsys < 0)
+    bh = np.concatenate([members[:7], singles[:5]]).astype(np.int32)      # BHs inside binaries and single BHs
+    pos, vel, mass, sub = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), dev(torch, w.subsys)
+    ctx.set_subsystems(sub)
+    try:
+        p = ctx.pn1(pos, vel, mass, dev(torch, bh), w.G, 1e3).cpu().numpy()
+        d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+        # a call with another n while subsystems are set is refused (the id array would not match)
+        from paper_2210_02472_b200.binding import BifrostError
+        with pytest.raises(BifrostError):
+            ctx.acc(pos[:100].contiguous(), mass[:100].contiguous(), w.G, w.eps)
+    finally:
+        ctx.set_subsystems(None)
+    check_vec(p, oracle.pn1_sub(w.pos, w.vel, w.mass, bh, w.G, 1e3, w.subsys), "pn1_sub")
+    plain = oracle.pn1(w.pos, w.vel, w.mass, bh, w.G, 1e3)
+    assert np.abs(plain[bh[:7]]).max() > 10 * np.abs(p[bh[:7]]).max()       # the partner's PN kick is gone
+    # Eq. 20: members share the minimum of their time-steps
+    dt = torch.minimum(d[0], d[1]).clone()
+    dt_np = dt.cpu().numpy().copy()
+    ctx.subsys_min(sub, dt)
+    assert np.array_equal(dt.cpu().numpy(), oracle.subsys_min(w.subsys, dt_np))
+    assert n == dt_np.shape[0]
