@@ -336,12 +336,12 @@ def run_cuda(args):
             passes["allgather"] = {"ms": mean_ms["allgather"], "bytes": 24 * n}
         dom = passes["grad"]
         traffic = None
-        prof = os.path.join(ROOT, "profiles", "traffic_per_launch.json")
+        prof = os.path.join(ROOT, "profiles", "r1_traffic_per_launch.csv")   # ncu dram__bytes_* of the bench launch
         if os.path.exists(prof):
-            try:
-                traffic = json.load(open(prof)).get(f"config{args.config}", {}).get("grad_pair_kernel_dram_bytes")
-            except (OSError, ValueError):
-                traffic = None
+            for row in open(prof).read().splitlines()[1:]:
+                f = row.split(",")
+                if len(f) >= 4 and f[0] == str(args.config) and f[1] == "grad_pair_kernel" and n == {4: 1 << 20, 5: 1 << 21}[args.config]:
+                    traffic = int(f[2]) + int(f[3])
         roofline = {"bound": "alu", "kernel": "pair_kernel<GradPass> (bifrost_grad: pack + pair [+ reduce] timed together; "
                                               "the pair kernel is > 99.9 % of it)",
                     "achieved": dom["tflops"], "peak": peak, "unit": "TFLOP/s", "frac": dom["tflops"] / peak,

@@ -288,3 +288,40 @@ def subsys_min(subsys, dt) -> np.ndarray:
     out = np.zeros(n)
     _sub_sigs().oracle_subsys_min(n, sub.ctypes.data, dt.ctypes.data, out.ctypes.data)
     return out
+
+
+# ---- NEXT-3: neighbour search (§3.4, Eq. 18-19) and subsystem construction ------------
+
+def ngb(pos, vel, mass, G, r_ngb, r_ngb_max, tau, C, cap=16, sink_idx=None, src_idx=None):
+    """Returns (count[n_sink], list[n_sink][cap]) - neighbour ids in source-list order, -1 padded."""
+    pos, vel, mass = _f64(pos), _f64(vel), _f64(mass)
+    n = mass.shape[0]
+    si, sip, ns, sj, sjp, nj = _lists(n, sink_idx, src_idx)
+    lib = _load()
+    lib.oracle_ngb.argtypes = [_I64, _P, _P, _P, _P, _I64, _P, _I64, _D, _D, _D, _D, _D, _I64, _P, _P]
+    count = np.zeros(ns, dtype=np.int32)
+    lst = np.full((ns, cap), -1, dtype=np.int32)
+    lib.oracle_ngb(n, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, sip, ns, sjp, nj, G, r_ngb, r_ngb_max, tau, C,
+                   cap, count.ctypes.data, lst.ctypes.data)
+    return count, lst
+
+
+def components(n, edge_i, edge_j) -> np.ndarray:
+    """Subsystem id (smallest member id) of every particle, -1 for particles without an edge."""
+    ei = np.ascontiguousarray(edge_i, dtype=np.int32)
+    ej = np.ascontiguousarray(edge_j, dtype=np.int32)
+    lib = _load()
+    lib.oracle_components.argtypes = [_I64, _P, _P, _I64, _P]
+    out = np.zeros(n, dtype=np.int32)
+    lib.oracle_components(n, ei.ctypes.data, ej.ctypes.data, ei.shape[0], out.ctypes.data)
+    return out
+
+
+def edges_from_lists(sinks, count, lst):
+    """(edge_i, edge_j) arrays from per-sink neighbour lists (each listed pair once per direction)."""
+    sinks = np.arange(count.shape[0], dtype=np.int32) if sinks is None else np.asarray(sinks, dtype=np.int32)
+    ei, ej = [], []
+    for k, i in enumerate(sinks):
+        for q in range(min(int(count[k]), lst.shape[1])):
+            ei.append(int(i)); ej.append(int(lst[k, q]))
+    return np.asarray(ei, dtype=np.int32), np.asarray(ej, dtype=np.int32)

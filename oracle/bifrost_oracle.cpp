@@ -33,6 +33,10 @@
 // NEXT-2 (subsystem exclusion): all-(-1) ids reproduce the plain routines bit for bit; excluded +
 // intra-subsystem partial sums (index lists) = full sums; one all-embracing subsystem gives 0 / +inf;
 // numpy brute force with an explicit mask for dtmin; Eq. 20 against numpy minimum.reduceat.
+// NEXT-3 (neighbour search, Eq. 18-19; components): circular / eccentric binaries and hyperbolic
+// fly-bys built from chosen (a, e, true anomaly) so that every branch of Eq. 18-19 is hit with a known
+// answer; Fig. 1's chain F-G (shared neighbour) for the components; numpy re-derivation of a, e from
+// the vis-viva and Laplace-Runge-Lenz vector; brute-force union-find.
 // Parity status: acc, grad, dtmin, potential, jerk, phi, criteria pinned.  pn1: the relative two-body
 // dynamics are pinned; the paper prints no PN1.0 formula (PAPER.md:L439, L476 cite
 // Thorne & Hartle 1985 / Einstein et al. 1938), so parity with the paper's own
@@ -385,6 +389,95 @@ void subsys_min_impl(int64_t n, const int32_t* subsys, const double* dt, double*
     }
 }
 
+// ---------------------------------------------------------------------------
+// O-ngb (NEXT-3).  PAPER.md:L227-281 §3.4 "Finding subsystems", Eq. 18-19, in the paper's order:
+// for each pair (i, j) with r_ij = |r_j - r_i| < r_ngb_max compute the two-body orbital elements
+// a (semi-major axis) and e (eccentricity) from the relative orbit,
+//     mu = G (m_i + m_j),  E = v_ij^2/2 - mu/r_ij,  a = -mu/(2E),
+//     h = r_ij x v_ij,     e = sqrt(1 + 2 E h^2/mu^2),
+// then
+//   bound   (E <  0):  neighbours iff  a < r_ngb  or  (a >= r_ngb and r_ij < r_ngb)             (Eq. 18)
+//   unbound (E >= 0):  r_peri = a (1 - e); reject if r_peri >= r_ngb; otherwise neighbours iff
+//                      r_ij < r_ngb  or  (r_ij >= r_ngb and C r_ij/|v_ij| < tau)                  (Eq. 19)
+// Readings (N1-N3): r_peri is evaluated as p/(1+e) with p = h^2/mu, which equals a(1-e)
+// for every conic and stays finite for the parabolic case E = 0 (a infinite); 1 + 2Eh^2/mu^2 is
+// clamped at 0 before the square root; a pair with v_ij = 0 is bound (E < 0).  The relation is
+// exactly symmetric in floating point (every quantity is even in the pair order).
+// Output: for sink k, count[k] neighbours among the sources, their ids in source-list order in
+// list[k*cap .. k*cap+min(count,cap)-1] (cap = capacity per sink; count itself is never truncated).
+// ---------------------------------------------------------------------------
+inline bool ngb_pair(const double* pos, const double* vel, const double* mass, int64_t i, int64_t j, double G,
+                     double r_ngb, double r_ngb_max, double tau, double C) {
+    const double dx = pos[3 * j] - pos[3 * i], dy = pos[3 * j + 1] - pos[3 * i + 1], dz = pos[3 * j + 2] - pos[3 * i + 2];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r = std::sqrt(r2);
+    if (!(r < r_ngb_max)) return false;
+    const double ux = vel[3 * j] - vel[3 * i], uy = vel[3 * j + 1] - vel[3 * i + 1], uz = vel[3 * j + 2] - vel[3 * i + 2];
+    const double v2 = ux * ux + uy * uy + uz * uz;
+    const double mu = G * (mass[i] + mass[j]);
+    const double E = 0.5 * v2 - mu / r;
+    if (E < 0.0) {
+        const double a = -mu / (2.0 * E);
+        return (a < r_ngb) || (r < r_ngb);
+    }
+    const double hx = dy * uz - dz * uy, hy = dz * ux - dx * uz, hz = dx * uy - dy * ux;
+    const double h2 = hx * hx + hy * hy + hz * hz;
+    double e2 = 1.0 + 2.0 * E * h2 / (mu * mu);
+    if (e2 < 0.0) e2 = 0.0;
+    const double e = std::sqrt(e2);
+    const double r_peri = (h2 / mu) / (1.0 + e);
+    if (!(r_peri < r_ngb)) return false;
+    if (r < r_ngb) return true;
+    return C * r / std::sqrt(v2) < tau;
+}
+
+void ngb_impl(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+              int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double r_ngb, double r_ngb_max,
+              double tau, double C, int64_t cap, int32_t* count, int32_t* list) {
+    (void)n;
+#pragma omp parallel for schedule(dynamic, 8) if (n_sink * n_src > 16384)
+    for (int64_t k = 0; k < n_sink; ++k) {
+        const int64_t i = pid(sink_idx, k);
+        int64_t c = 0;
+        for (int64_t l = 0; l < n_src; ++l) {
+            const int64_t j = pid(src_idx, l);
+            if (j == i) continue;
+            if (ngb_pair(pos, vel, mass, i, j, G, r_ngb, r_ngb_max, tau, C)) {
+                if (c < cap) list[k * cap + c] = (int32_t)j;
+                ++c;
+            }
+        }
+        count[k] = (int32_t)c;
+    }
+}
+
+// O-comp.  PAPER.md:L279: subsystems = connected components of the neighbour graph ("finding the
+// components of a finite graph", depth-first search).  label = smallest particle id of the
+// component; a particle without any edge is single (-1).  edges: n_edge pairs (i, j).
+void components_impl(int64_t n, const int32_t* edge_i, const int32_t* edge_j, int64_t n_edge, int32_t* subsys) {
+    std::vector<std::vector<int32_t>> adj((size_t)n);
+    for (int64_t q = 0; q < n_edge; ++q) {
+        adj[(size_t)edge_i[q]].push_back(edge_j[q]);
+        adj[(size_t)edge_j[q]].push_back(edge_i[q]);
+    }
+    for (int64_t i = 0; i < n; ++i) subsys[i] = -1;
+    std::vector<char> seen((size_t)n, 0);
+    std::vector<int32_t> stack, members;
+    for (int64_t s = 0; s < n; ++s) {
+        if (seen[(size_t)s] || adj[(size_t)s].empty()) continue;
+        stack.assign(1, (int32_t)s); members.clear(); seen[(size_t)s] = 1;
+        while (!stack.empty()) {                      // depth-first traversal
+            const int32_t u = stack.back(); stack.pop_back();
+            members.push_back(u);
+            for (int32_t v : adj[(size_t)u])
+                if (!seen[(size_t)v]) { seen[(size_t)v] = 1; stack.push_back(v); }
+        }
+        int32_t lab = members[0];
+        for (int32_t u : members) if (u < lab) lab = u;
+        for (int32_t u : members) subsys[(size_t)u] = lab;
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -493,6 +586,18 @@ int oracle_pn1_sub(int64_t n, const double* pos, const double* vel, const double
 }
 int oracle_subsys_min(int64_t n, const int32_t* subsys, const double* dt, double* out) {
     subsys_min_impl(n, subsys, dt, out);
+    return 0;
+}
+
+// ---- NEXT-3: neighbour search and subsystem construction (§3.4) ----
+int oracle_ngb(int64_t n, const double* pos, const double* vel, const double* mass, const int32_t* sink_idx,
+               int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double r_ngb, double r_ngb_max,
+               double tau, double C, int64_t cap, int32_t* count, int32_t* list) {
+    ngb_impl(n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, r_ngb, r_ngb_max, tau, C, cap, count, list);
+    return 0;
+}
+int oracle_components(int64_t n, const int32_t* edge_i, const int32_t* edge_j, int64_t n_edge, int32_t* subsys) {
+    components_impl(n, edge_i, edge_j, n_edge, subsys);
     return 0;
 }
 
