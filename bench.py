@@ -389,7 +389,7 @@ def run_sweep(args):
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     out = {"metric": "us per C-ABI call vs active-set size (configs 2, 3)", "unit": "us", "data": "synthetic",
-           "timing": "CUDA events around 20 back-to-back calls after 3 warm-ups, sources L2-resident", "cases": []}
+           "timing": "CUDA events around 20 back-to-back calls after 3 warm-ups, sources L2-resident; *_graph_us = the same 20 calls captured in one CUDA graph and replayed", "cases": []}
     for cfg, sizes in ((2, [W.config2_sink_list(k) for k in range(0, 15)]),
                        (3, [W.config3_sink_list(k) for k in range(10, -1, -1)])):
         w = W.CONFIGS[cfg]()
@@ -397,12 +397,14 @@ def run_sweep(args):
         pos, vel, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.vel, w.mass))
         acc = ctx.acc(pos, mass, w.G, w.eps)
         outs = {"acc": torch.zeros_like(acc), "grad": torch.zeros_like(acc)}
+        dt_out = (torch.empty(w.n, dtype=torch.float64, device=dev), torch.empty(w.n, dtype=torch.float64, device=dev),
+                  torch.empty(w.n, dtype=torch.int32, device=dev), torch.empty(w.n, dtype=torch.int32, device=dev))
         for sinks in sizes:
             si = torch.from_numpy(sinks).to(dev)
             ns = int(sinks.shape[0])
             calls = {"acc": lambda: ctx.acc(pos, mass, w.G, w.eps, si, None, out=outs["acc"]),
                      "grad": lambda: ctx.grad(pos, mass, acc, w.G, w.eps, si, None, out=outs["grad"]),
-                     "dtmin": lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None)}
+                     "dtmin": lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None, out=dt_out)}
             rec = {"config": cfg, "n_src": w.n, "n_sink": ns}
             reps = 20 if ns * w.n < 2e9 else 3
             for name, fn in calls.items():
@@ -418,6 +420,20 @@ def run_sweep(args):
                 us = 1e3 * e0.elapsed_time(e1) / reps
                 rec[name + "_us"] = round(us, 2)
                 rec[name + "_pairs_per_s"] = ns * float(w.n) / (us * 1e-6)
+                # the same calls captured in a CUDA graph and replayed: device time without the
+                # host's launch cost (the calls are asynchronous and capture-safe)
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph):
+                    for _ in range(reps):
+                        fn()
+                graph.replay()
+                torch.cuda.synchronize()
+                e0.record()
+                graph.replay()
+                e1.record()
+                torch.cuda.synchronize()
+                rec[name + "_graph_us"] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
+                del graph
             # a1 gather traffic: the acc pack reads 32 B and writes 48 B per source
             rec["acc_source_bytes"] = 80 * w.n
             out["cases"].append(rec)

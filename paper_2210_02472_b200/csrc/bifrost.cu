@@ -27,12 +27,15 @@
 #include <cuda_runtime.h>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
+#include <algorithm>
 #include <new>
 
 namespace {
 
 constexpr int TILE = 128;         // sources per shared-memory tile
 constexpr int MAX_SPLIT = 256;    // upper bound on grid.y (source-range splits)
+constexpr int TICKETS = 1024;     // >= the largest grid.x of pair_fused_kernel
 
 // ----------------------------------------------------------------------------------------
 // small device helpers
@@ -55,6 +58,16 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// a1 inputs: the caller's arrays a source record is gathered from (aux = acc for grad, vel for
+// dtmin / jerk, unused otherwise); src_idx == NULL means sources are particles 0..n_src-1.
+struct SrcArrays {
+    const double* pos;
+    const double* aux;
+    const double* mass;
+    const int32_t* subsys;
+    const int32_t* src_idx;
+};
 
 struct Geom {
     int n_sink;           // number of sinks
@@ -81,6 +94,37 @@ __device__ __forceinline__ int sink_code(const int32_t* subsys, int id) {
     return c < 0 ? -2 : c;
 }
 
+// source-side subsystem code: -1 for a single particle (never equal to a sink's code, which is
+// -2 for a single particle), the subsystem id otherwise
+__device__ __forceinline__ int src_code(const int32_t* subsys, int j) {
+    if (!subsys) return -1;
+    const int c = subsys[j];
+    return c < 0 ? -1 : c;
+}
+
+// a5 + a7: reduction of one sink's partials in a FIXED order, then scatter.  A group of L lanes
+// (L = 1, 2, .. 32, a power of two; lane = index in the group) shares one sink: lane l adds the
+// partials of splits l, l+L, ... in that order and a butterfly adds the lanes - an order that
+// depends only on (n_split, L), never on which CTA runs it.  All 32 lanes of a warp must call
+// (write = false for a group that shadows a sink).  The partials come from other CTAs: L2 loads.
+__device__ __forceinline__ double group_add(double v, int L) {
+    for (int off = L >> 1; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v;
+}
+__device__ __forceinline__ void finish_vec3(const double* partial, double* out, double G, const Geom& g, int k, int id,
+                                            int lane, int L, bool write) {
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int s = lane; s < g.n_split; s += L) {
+        const double* p = partial + 3 * ((size_t)s * g.n_sink + k);
+        sx += __ldcg(p); sy += __ldcg(p + 1); sz += __ldcg(p + 2);
+    }
+    if (L > 1) { sx = group_add(sx, L); sy = group_add(sy, L); sz = group_add(sz, L); }
+    if (write && lane == 0) {
+        double* o = out + 3 * (size_t)(g.compact ? k : id);
+        o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
+    }
+}
+
 struct AccArgs {
     const double* pos;
     const int32_t* subsys;
@@ -96,6 +140,20 @@ struct AccPassT {
     using Args = AccArgs;
     struct Sink { double x, y, z; int sub; };
     struct Acc { double x, y, z; };
+    struct Raw { double x, y, z, m; int code; };
+    // a1: gather one source (j < 0: padding record) and write its packed record
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
+            w.m = s.mass[j]; w.code = EXCL ? src_code(s.subsys, j) : 0;
+        } else { w.x = w.y = w.z = w.m = 0.0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(1.5 * w.m, 1.875 * w.m);
+        if (EXCL) o[3] = make_double2(__hiloint2double(0, w.code), 0.0);
+    }
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2];
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
@@ -122,6 +180,10 @@ struct AccPassT {
             o[0] = c.x; o[1] = c.y; o[2] = c.z;
         }
     }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
+    }
 };
 
 using AccPass = AccPassT<false>;
@@ -142,6 +204,22 @@ struct GradPassT {
     using Args = GradArgs;
     struct Sink { double x, y, z, ax, ay, az; int sub; };
     struct Acc { double ux, uy, uz, wx, wy, wz; };   // U = sum w a_ji,  W = sum w (a_ji.r_ji)/s^2 r_ji
+    struct Raw { double x, y, z, ax, ay, az, m; int code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            const size_t b = 3 * (size_t)j;
+            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
+            w.ax = s.aux[b]; w.ay = s.aux[b + 1]; w.az = s.aux[b + 2];
+            w.m = s.mass[j]; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.ax = w.ay = w.az = w.m = 0.0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.ax);
+        o[2] = make_double2(w.ay, w.az);
+        o[3] = make_double2(w.m, 1.5 * w.m);
+        o[4] = make_double2(1.875 * w.m, __hiloint2double(0, w.code));
+    }
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         const size_t o = 3 * (size_t)id;
         s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
@@ -176,6 +254,10 @@ struct GradPassT {
             o[0] = cx; o[1] = cy; o[2] = cz;
         }
     }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
+    }
 };
 
 using GradPass = GradPassT<false>;
@@ -188,6 +270,8 @@ struct DtArgs {
     const int32_t* sink_idx;
     double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
     int32_t* pid;      // [split][2][n_sink]  their source ids
+    double G, eta_ff, eta_fb;
+    double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
 };
 
 // ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
@@ -199,6 +283,21 @@ struct DtPassT {
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
     // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
     struct Acc { double kff, kfb; int jff, jfb; };
+    struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            const size_t b = 3 * (size_t)j;
+            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
+            w.vx = s.aux[b]; w.vy = s.aux[b + 1]; w.vz = s.aux[b + 2];
+            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.vx = w.vy = w.vz = w.m = 0.0; w.j = 0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(w.vx, w.vy);
+        o[3] = make_double2(w.vz, __hiloint2double(w.code, w.j));
+    }
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         const size_t o = 3 * (size_t)id;
         s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
@@ -240,6 +339,55 @@ struct DtPassT {
         a.pkey[o] = c.kff; a.pkey[o + g.n_sink] = c.kfb;
         a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
     }
+    // dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
+    // Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
+    static constexpr bool ALWAYS_FINISH = true;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int i, int lane, int L, bool write) {
+        double kb[2] = {0.0, 0.0};
+        int jb[2] = {-1, -1};
+        for (int s = lane; s < g.n_split; s += L) {
+            for (int w = 0; w < 2; ++w) {
+                const size_t o = ((size_t)s * 2 + w) * g.n_sink + k;
+                const double key = __ldcg(a.pkey + o);
+                const int j = __ldcg(a.pid + o);
+                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+            }
+        }
+        for (int off = L >> 1; off > 0; off >>= 1) {      // (max key, then min id) is order-independent
+            for (int w = 0; w < 2; ++w) {
+                const double key = __shfl_xor_sync(0xffffffffu, kb[w], off);
+                const int j = __shfl_xor_sync(0xffffffffu, jb[w], off);
+                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+            }
+        }
+        if (!write || lane != 0) return;
+        const double* pos = a.pos; const double* vel = a.vel;
+        const int row = g.compact ? k : i;
+        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+        double tff = inf, tfb = inf;
+        if (jb[0] >= 0) {
+            const int j = jb[0];
+            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            const double r = sqrt(r2);
+            tff = a.eta_ff * sqrt(__dmul_rn(r2, r) / (a.G * (a.mass[i] + a.mass[j])));
+        }
+        if (jb[1] >= 0) {
+            const int j = jb[1];
+            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+            const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
+                         uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+            tfb = __dmul_rn(a.eta_fb, sqrt(r2)) / sqrt(v2);
+        }
+        if (a.dt_ff) a.dt_ff[row] = tff;
+        if (a.dt_fb) a.dt_fb[row] = tfb;
+        if (a.j_ff) a.j_ff[row] = jb[0];
+        if (a.j_fb) a.j_fb[row] = jb[1];
+    }
 };
 
 using DtPass = DtPassT<false, false>;
@@ -263,6 +411,19 @@ struct PotPassT {
     using Args = PotArgs;
     struct Sink { double x, y, z; int id, sub; };
     struct Acc { double p; };
+    struct Raw { double x, y, z, m; int j, code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
+            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.m = 0.0; w.j = -1; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(0.5 * w.m, 0.375 * w.m);
+        o[3] = make_double2(__hiloint2double(w.code, w.j), 0.0);
+    }
     __device__ static void load_sink(const Args& a, int id, Sink& s) {
         s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2]; s.id = id;
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
@@ -284,6 +445,13 @@ struct PotPassT {
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         if (g.n_split == 1) a.out[g.compact ? k : id] = -a.G * c.p;
         else a.partial[(size_t)split * g.n_sink + k] = c.p;
+    }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        double s = 0.0;
+        for (int q = lane; q < g.n_split; q += L) s += __ldcg(a.partial + (size_t)q * g.n_sink + k);     // fixed order
+        if (L > 1) s = group_add(s, L);
+        if (write && lane == 0) a.out[g.compact ? k : id] = -a.G * s;
     }
 };
 
@@ -356,118 +524,129 @@ pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ s
 // a1: pack kernels (gather sources through the index list into aligned records; the tail of
 // the last tile is zero-filled so the cp.async stage never reads undefined memory).
 // ----------------------------------------------------------------------------------------
-// source-side subsystem code: -1 for a single particle (never equal to a sink's code, which is
-// -2 for a single particle), the subsystem id otherwise
-__device__ __forceinline__ int src_code(const int32_t* subsys, int j) {
-    if (!subsys) return -1;
-    const int c = subsys[j];
-    return c < 0 ? -1 : c;
-}
 
-template <bool EXCL>
-__global__ void pack_acc_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
-                                const double* __restrict__ pos, const double* __restrict__ mass,
-                                const int32_t* __restrict__ subsys, double* __restrict__ rec) {
+template <class P>
+__global__ void pack_kernel(int n_src, int n_pad, const SrcArrays src, double* __restrict__ rec) {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= n_pad) return;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * (EXCL ? 8 : 6));
-    if (l < n_src) {
-        const int j = src_idx ? src_idx[l] : l;
-        const double m = mass[j];
-        o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
-        o[1] = make_double2(pos[3 * (size_t)j + 2], m);
-        o[2] = make_double2(1.5 * m, 1.875 * m);
-        if (EXCL) o[3] = make_double2(__hiloint2double(0, src_code(subsys, j)), 0.0);
-    } else {
-        o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
-        if (EXCL) o[3] = make_double2(0.0, 0.0);
-    }
-}
-
-__global__ void pack_grad_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
-                                 const double* __restrict__ pos, const double* __restrict__ mass,
-                                 const double* __restrict__ acc, const int32_t* __restrict__ subsys,
-                                 double* __restrict__ rec) {
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l >= n_pad) return;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 10);
-    if (l < n_src) {
-        const int j = src_idx ? src_idx[l] : l;
-        const size_t b = 3 * (size_t)j;
-        const double m = mass[j];
-        o[0] = make_double2(pos[b], pos[b + 1]);
-        o[1] = make_double2(pos[b + 2], acc[b]);
-        o[2] = make_double2(acc[b + 1], acc[b + 2]);
-        o[3] = make_double2(m, 1.5 * m);
-        o[4] = make_double2(1.875 * m, __hiloint2double(0, src_code(subsys, j)));
-    } else {
-        o[0] = o[1] = o[2] = o[3] = o[4] = make_double2(0.0, 0.0);
-    }
-}
-
-__global__ void pack_dt_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
-                               const double* __restrict__ pos, const double* __restrict__ vel,
-                               const double* __restrict__ mass, const int32_t* __restrict__ subsys,
-                               double* __restrict__ rec) {
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l >= n_pad) return;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
-    if (l < n_src) {
-        const int j = src_idx ? src_idx[l] : l;
-        const size_t b = 3 * (size_t)j;
-        o[0] = make_double2(pos[b], pos[b + 1]);
-        o[1] = make_double2(pos[b + 2], mass[j]);
-        o[2] = make_double2(vel[b], vel[b + 1]);
-        o[3] = make_double2(vel[b + 2], __hiloint2double(src_code(subsys, j), j));
-    } else {
-        o[0] = o[1] = o[2] = o[3] = make_double2(0.0, 0.0);
-    }
+    typename P::Raw w;
+    P::fetch(src, l < n_src ? (src.src_idx ? src.src_idx[l] : l) : -1, w);
+    P::emit(w, reinterpret_cast<double2*>(rec + (size_t)l * P::REC));
 }
 
 // ----------------------------------------------------------------------------------------
-// a5 + a7: fixed-order reduction over the source-range splits, then scatter.
+// a5 + a7 as a kernel of its own (large sink sets): P::finish for every sink.
 // ----------------------------------------------------------------------------------------
-__global__ void reduce_vec3_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
-                                   const double* __restrict__ partial, double G, double* __restrict__ out) {
+template <class P>
+__global__ void finish_kernel(const typename P::Args a, const Geom g) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_sink) return;
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    for (int s = 0; s < n_split; ++s) {                       // fixed order: deterministic
-        const double* p = partial + 3 * ((size_t)s * n_sink + k);
-        sx += p[0]; sy += p[1]; sz += p[2];
-    }
-    const int id = sink_idx ? sink_idx[k] : k;
-    double* o = out + 3 * (size_t)(compact ? k : id);
-    o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
+    if (k >= g.n_sink) return;
+    P::finish(a, g, k, a.sink_idx ? a.sink_idx[k] : k, 0, 1, true);
 }
 
-__global__ void pack_pot_kernel(int n_src, int n_pad, const int32_t* __restrict__ src_idx,
-                                const double* __restrict__ pos, const double* __restrict__ mass,
-                                const int32_t* __restrict__ subsys, double* __restrict__ rec) {
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l >= n_pad) return;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * 8);
-    if (l < n_src) {
-        const int j = src_idx ? src_idx[l] : l;
-        const double m = mass[j];
-        o[0] = make_double2(pos[3 * (size_t)j], pos[3 * (size_t)j + 1]);
-        o[1] = make_double2(pos[3 * (size_t)j + 2], m);
-        o[2] = make_double2(0.5 * m, 0.375 * m);
-        o[3] = make_double2(__hiloint2double(src_code(subsys, j), j), 0.0);
+// ----------------------------------------------------------------------------------------
+// a1-a7 in ONE launch for small sink sets (the faster levels of the time-step hierarchy,
+// PAPER.md:L295): each CTA gathers its source tiles straight from the caller's arrays (the next
+// tile's loads are in flight while the current one is evaluated), and when the source range is
+// split across blockIdx.y the CTA that arrives last at a ticket (one per blockIdx.x) reduces all
+// partials in split order - so the result does not depend on which CTA that is (deterministic) and
+// no second or third launch is needed.  The ticket resets itself (CUDA-graph replay safe).
+// ----------------------------------------------------------------------------------------
+template <class P, int S, int T, int MINB, int UNR>
+__global__ void __launch_bounds__(T, MINB)
+pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, unsigned* __restrict__ ticket) {
+    static_assert(T >= TILE, "one gathering thread per source of a tile");
+    constexpr int REC = P::REC;
+    __shared__ __align__(16) double sm[2][TILE * REC];
+    __shared__ int s_last;
+
+    typename P::Sink sink[S];
+    typename P::Acc accu[S];
+    int ids[S];
+    const int kbase = blockIdx.x * (T * S) + threadIdx.x;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * T;
+        const int kk = k < g.n_sink ? k : g.n_sink - 1;
+        ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
+        P::load_sink(a, ids[s], sink[s]);
+        P::init(accu[s]);
+    }
+
+    const int n_tiles = (g.n_src + TILE - 1) / TILE;
+    const int tile0 = blockIdx.y * g.tiles_per_split;
+    const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
+
+    typename P::Raw raw;
+    auto fetch_tile = [&](int tile) {
+        const int l = tile * TILE + threadIdx.x;
+        if (threadIdx.x < TILE) P::fetch(src, l < g.n_src ? (src.src_idx ? src.src_idx[l] : l) : -1, raw);
+    };
+    auto emit_tile = [&](int buf) {
+        if (threadIdx.x < TILE) P::emit(raw, reinterpret_cast<double2*>(sm[buf] + threadIdx.x * REC));
+    };
+
+    if (tile0 < tile1) { fetch_tile(tile0); emit_tile(0); }
+    for (int tile = tile0; tile < tile1; ++tile) {
+        const int buf = (tile - tile0) & 1;
+        __syncthreads();                       // sm[buf] complete; everyone is done with sm[buf ^ 1]
+        const bool more = tile + 1 < tile1;
+        if (more) fetch_tile(tile + 1);
+        const int cnt = min(TILE, g.n_src - tile * TILE);
+        const double* __restrict__ tb = sm[buf];
+#pragma unroll UNR
+        for (int jj = 0; jj < cnt; ++jj) {
+            double r[REC];
+#pragma unroll
+            for (int q = 0; q < REC; q += 2) {
+                const double2 v = *reinterpret_cast<const double2*>(tb + jj * REC + q);
+                r[q] = v.x; r[q + 1] = v.y;
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) P::pair(a, sink[s], accu[s], r);
+        }
+        if (more) emit_tile(buf ^ 1);
+    }
+
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * T;
+        if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
+    }
+    if (g.n_split == 1) {
+        if (P::ALWAYS_FINISH) {                // a thread finishes the sinks it stored itself
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const int k = kbase + s * T;
+                if (k < g.n_sink) P::finish(a, g, k, ids[s], 0, 1, true);
+            }
+        }
+        return;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&ticket[blockIdx.x], 1u) == gridDim.y - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // the last CTA reduces: L lanes per sink when this CTA's sinks leave threads to spare
+    const int base = blockIdx.x * (T * S);
+    const int n_local = min(T * S, g.n_sink - base);
+    int L = 1;
+    while (L < 32 && n_local * (2 * L) <= T) L *= 2;
+    if (L == 1) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const int k = kbase + s * T;
+            if (k < g.n_sink) P::finish(a, g, k, ids[s], 0, 1, true);
+        }
     } else {
-        o[0] = o[1] = o[2] = make_double2(0.0, 0.0);
-        o[3] = make_double2(__hiloint2double(0, -1), 0.0);
+        const int q = threadIdx.x / L;
+        const bool live = q < n_local;
+        const int k = base + (live ? q : 0);
+        P::finish(a, g, k, a.sink_idx ? a.sink_idx[k] : k, threadIdx.x % L, L, live);
     }
-}
-
-__global__ void reduce_scalar_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
-                                     const double* __restrict__ partial, double scale, double* __restrict__ out) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_sink) return;
-    double s = 0.0;
-    for (int q = 0; q < n_split; ++q) s += partial[(size_t)q * n_sink + k];     // fixed order
-    const int id = sink_idx ? sink_idx[k] : k;
-    out[compact ? k : id] = scale * s;
+    if (threadIdx.x == 0) ticket[blockIdx.x] = 0;
 }
 
 // W = 1/2 sum_{i in sinks} m_i phi_i in two fixed-order stages (deterministic; no atomics).
@@ -541,54 +720,6 @@ __global__ void criteria_kernel(int n_sink, const int32_t* __restrict__ sink_idx
         best = fmin(best, t_j);
     }
     if (inout_dt) inout_dt[i] = best;
-}
-
-// dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
-// Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
-__global__ void dt_finalize_kernel(int n_sink, int n_split, int compact, const int32_t* __restrict__ sink_idx,
-                                   const double* __restrict__ pkey, const int32_t* __restrict__ pid,
-                                   const double* __restrict__ pos, const double* __restrict__ vel,
-                                   const double* __restrict__ mass, double G, double eta_ff, double eta_fb,
-                                   double* __restrict__ dt_ff, double* __restrict__ dt_fb,
-                                   int32_t* __restrict__ j_ff, int32_t* __restrict__ j_fb) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_sink) return;
-    double kb[2] = {0.0, 0.0};
-    int jb[2] = {-1, -1};
-    for (int s = 0; s < n_split; ++s) {
-        for (int w = 0; w < 2; ++w) {
-            const size_t o = ((size_t)s * 2 + w) * n_sink + k;
-            const double key = pkey[o];
-            const int j = pid[o];
-            if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
-        }
-    }
-    const int i = sink_idx ? sink_idx[k] : k;
-    const int row = compact ? k : i;
-    const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    double tff = inf, tfb = inf;
-    if (jb[0] >= 0) {
-        const int j = jb[0];
-        const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                     dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-        const double r = sqrt(r2);
-        tff = eta_ff * sqrt(__dmul_rn(r2, r) / (G * (mass[i] + mass[j])));
-    }
-    if (jb[1] >= 0) {
-        const int j = jb[1];
-        const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                     dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-        const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
-                     uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
-        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-        const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
-        tfb = __dmul_rn(eta_fb, sqrt(r2)) / sqrt(v2);
-    }
-    if (dt_ff) dt_ff[row] = tff;
-    if (dt_fb) dt_fb[row] = tfb;
-    if (j_ff) j_ff[row] = jb[0];
-    if (j_fb) j_fb[row] = jb[1];
 }
 
 // ----------------------------------------------------------------------------------------
@@ -814,6 +945,8 @@ struct bifrost_ctx {
     double* phi_scratch = nullptr;   // [max_n]   (bifrost_potential with out_phi == NULL)
     double* wpart = nullptr;         // [ceil(max_n / 4096)] block partials of the W reduction
     unsigned long long* smin = nullptr;   // [max_n] per-subsystem minima (bifrost_subsys_min)
+    int64_t fused_max_sinks = 4096;  // below: one fused launch per call (env BIFROST_FUSED_MAX_SINKS overrides; tuning aid)
+    unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel (zero between launches)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
     int64_t subsys_n = 0;
     int64_t launches = 0;
@@ -906,24 +1039,53 @@ struct Shape { static constexpr int S = S_, T = T_, MINB = MINB_, UNR = UNR_; };
 using ShapeTiny = Shape<1, 128, 8, 4>;
 
 template <class P, class Sh>
-int launch_pair(bifrost_ctx* ctx, const typename P::Args& a, Geom& g, int64_t n_sink, int64_t n_src,
-                size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
-    g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
+int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src,
+                 size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
+    Geom g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
     g.compact = compact;
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
 }
 
-// Big: n_sink >= 4096; Mid: 256 <= n_sink < 4096; Tiny: below.
-template <class P, class Big, class Mid, class Tiny = ShapeTiny>
-int run_pair(bifrost_ctx* ctx, const typename P::Args& a, Geom& g, int64_t n_sink, int64_t n_src,
+// One pass (a1-a7) of policy P.
+//   n_sink >= fused_max_sinks: pack -> pair_kernel<Big> -> finish (three launches at most).
+//   below: ONE fused launch with 128 threads and S = 4, 2 or 1 sinks per thread - the largest S
+//   that still yields >= 4 CTAs per SM (sink blocks x source-range splits), because a small set
+//   is short of parallelism, not of registers.
+template <class P, class Big, class F4, class F2, class F1>
+int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src,
              size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
-    if (n_sink >= 4096) return launch_pair<P, Big>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
-    if (n_sink >= 256) return launch_pair<P, Mid>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
-    return launch_pair<P, Tiny>(ctx, a, g, n_sink, n_src, partial_bytes_per_sink, compact, st);
+    Geom g;
+    if (n_sink < ctx->fused_max_sinks) {
+        const int64_t splits = std::max<int64_t>(1, std::min<int64_t>(ceil_div(n_src, TILE), MAX_SPLIT));
+        const int64_t want = 4LL * ctx->num_sms;
+        if ((int64_t)ceil_div(n_sink, 128 * 4) * splits >= want)
+            return launch_fused<P, F4>(ctx, a, src, n_sink, n_src, partial_bytes_per_sink, compact, st);
+        if ((int64_t)ceil_div(n_sink, 128 * 2) * splits >= want)
+            return launch_fused<P, F2>(ctx, a, src, n_sink, n_src, partial_bytes_per_sink, compact, st);
+        return launch_fused<P, F1>(ctx, a, src, n_sink, n_src, partial_bytes_per_sink, compact, st);
+    }
+    if (n_src > 0) {
+        const int n_pad = ceil_div(n_src, TILE) * TILE;
+        pack_kernel<P><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src, ctx->src_rec);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    g = make_geom(ctx, n_sink, n_src, Big::T * Big::S, Big::MINB, partial_bytes_per_sink);
+    g.compact = compact;
+    dim3 grid(ceil_div(g.n_sink, Big::T * Big::S), g.n_split);
+    pair_kernel<P, Big::S, Big::T, Big::MINB, Big::UNR><<<grid, Big::T, 0, st>>>(a, g, ctx->src_rec);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    if (g.n_split > 1 || P::ALWAYS_FINISH) {
+        finish_kernel<P><<<ceil_div(n_sink, 256), 256, 0, st>>>(a, g);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    return BIFROST_OK;
 }
 
 int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
@@ -931,27 +1093,14 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
              cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
-    Geom g;
-    if (n_src > 0) {
-        const int n_pad = ceil_div(n_src, TILE) * TILE;
-        if (sub) pack_acc_kernel<true><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
-        else pack_acc_kernel<false><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
-    AccArgs a{pos, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    const SrcArrays src{pos, nullptr, mass, sub, src_idx};
+    const AccArgs a{pos, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
     using Big = Shape<8, 256, 1, 1>;
-    using Mid = Shape<4, 128, 4, 2>;
-    int rc = sub ? run_pair<AccPassT<true>, Big, Mid>(ctx, a, g, n_sink, n_src, 24, compact, st)
-                 : run_pair<AccPassT<false>, Big, Mid>(ctx, a, g, n_sink, n_src, 24, compact, st);
-    if (rc) return rc;
-    if (g.n_split > 1) {
-        reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
-                                                                 (const double*)ctx->partial, G, out);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
-    return BIFROST_OK;
+    using F4 = Shape<4, 128, 4, 2>;
+    using F2 = Shape<2, 128, 6, 2>;
+    using F1 = Shape<1, 128, 8, 4>;
+    return sub ? run_pass<AccPassT<true>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<AccPassT<false>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
@@ -959,27 +1108,14 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
               double* out, int compact, cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
-    Geom g;
-    if (n_src > 0) {
-        const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_grad_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, acc, sub, ctx->src_rec);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
-    GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    const SrcArrays src{pos, acc, mass, sub, src_idx};
+    const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
     using Big = Shape<4, 256, 1, 2>;
-    using Mid = Shape<4, 128, 3, 2>;
-    using Tiny = Shape<1, 128, 5, 2>;
-    int rc = sub ? run_pair<GradPassT<true>, Big, Mid, Tiny>(ctx, a, g, n_sink, n_src, 24, compact, st)
-                 : run_pair<GradPassT<false>, Big, Mid, Tiny>(ctx, a, g, n_sink, n_src, 24, compact, st);
-    if (rc) return rc;
-    if (g.n_split > 1) {
-        reduce_vec3_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
-                                                                 (const double*)ctx->partial, G, out);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
-    return BIFROST_OK;
+    using F4 = Shape<4, 128, 3, 2>;
+    using F2 = Shape<2, 128, 4, 2>;
+    using F1 = Shape<1, 128, 5, 2>;
+    return sub ? run_pass<GradPassT<true>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<GradPassT<false>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
@@ -988,30 +1124,19 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
                cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
-    Geom g;
-    if (n_src > 0) {
-        const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_dt_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, vel, mass, sub, ctx->src_rec);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
     // workspace (24 B per sink and split): keys [split][2][n_sink] doubles in the first two thirds,
     // ids [split][2][n_sink] ints in the last third
     double* pkey = (double*)ctx->partial;
     int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
-    DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid};
+    const SrcArrays src{pos, vel, mass, sub, src_idx};
+    const DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb};
     using Big = Shape<4, 128, 3, 2>;
-    int rc;
-    if (sub) rc = src_idx ? run_pair<DtPassT<false, true>, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
-                          : run_pair<DtPassT<true, true>, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
-    else rc = src_idx ? run_pair<DtPass, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st)
-                      : run_pair<DtPassAsc, Big, Big>(ctx, a, g, n_sink, n_src, 24, compact, st);
-    if (rc) return rc;
-    dt_finalize_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx, pkey, pid, pos,
-                                                             vel, mass, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb);
-    ctx->launches++;
-    CU_TRY(ctx, cudaGetLastError());
-    return BIFROST_OK;
+    using F2 = Shape<2, 128, 4, 2>;
+    using F1 = Shape<1, 128, 5, 2>;
+    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                            : run_pass<DtPassT<true, true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return src_idx ? run_pass<DtPass, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                   : run_pass<DtPassAsc, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
@@ -1022,26 +1147,16 @@ int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
         if (out_W) CU_TRY(ctx, cudaMemsetAsync(out_W, 0, sizeof(double), st));
         return BIFROST_OK;
     }
-    Geom g;
     const int compact = out_phi ? 0 : 1;           // the scratch holds compact rows
     double* phi = out_phi ? out_phi : ctx->phi_scratch;
-    if (n_src > 0) {
-        const int n_pad = ceil_div(n_src, TILE) * TILE;
-        pack_pot_kernel<<<ceil_div(n_pad, 256), 256, 0, st>>>((int)n_src, n_pad, src_idx, pos, mass, sub, ctx->src_rec);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
-    PotArgs a{pos, sub, sink_idx, soft2(eps), G, phi, (double*)ctx->partial};
+    const SrcArrays src{pos, nullptr, mass, sub, src_idx};
+    const PotArgs a{pos, sub, sink_idx, soft2(eps), G, phi, (double*)ctx->partial};
     using Big = Shape<4, 128, 4, 2>;
-    int rc = sub ? run_pair<PotPassT<true>, Big, Big>(ctx, a, g, n_sink, n_src, 8, compact, st)
-                 : run_pair<PotPassT<false>, Big, Big>(ctx, a, g, n_sink, n_src, 8, compact, st);
+    using F2 = Shape<2, 128, 6, 2>;
+    using F1 = Shape<1, 128, 8, 4>;
+    int rc = sub ? run_pass<PotPassT<true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st)
+                 : run_pass<PotPassT<false>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st);
     if (rc) return rc;
-    if (g.n_split > 1) {
-        reduce_scalar_kernel<<<ceil_div(n_sink, 256), 256, 0, st>>>((int)n_sink, g.n_split, compact, sink_idx,
-                                                                   (const double*)ctx->partial, -G, phi);
-        ctx->launches++;
-        CU_TRY(ctx, cudaGetLastError());
-    }
     if (out_W) {
         const int nb = ceil_div(n_sink, WSUM_PER_BLOCK);
         wsum_stage1_kernel<<<nb, WSUM_THREADS, 0, st>>>((int)n_sink, sink_idx, compact, mass, phi, ctx->wpart);
@@ -1152,6 +1267,10 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     ctx->device = device;
     ctx->max_n = max_n;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
+    if (const char* e = getenv("BIFROST_FUSED_MAX_SINKS")) {
+        const long long v = atoll(e);
+        if (v >= 0 && v <= (long long)TICKETS * 128) ctx->fused_max_sinks = v;
+    }
     const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
     ctx->partial_bytes = 24 * (size_t)max_n * 16;   // up to 16 source-range splits at n_sink = max_n
     if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
@@ -1160,7 +1279,9 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
         cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess ||
         cudaMalloc(&ctx->phi_scratch, 8 * (size_t)max_n) != cudaSuccess ||
         cudaMalloc(&ctx->wpart, 8 * ((size_t)max_n / WSUM_PER_BLOCK + 1)) != cudaSuccess ||
-        cudaMalloc(&ctx->smin, 8 * (size_t)max_n) != cudaSuccess) {
+        cudaMalloc(&ctx->smin, 8 * (size_t)max_n) != cudaSuccess ||
+        cudaMalloc(&ctx->tickets, TICKETS * sizeof(unsigned)) != cudaSuccess ||
+        cudaMemset(ctx->tickets, 0, TICKETS * sizeof(unsigned)) != cudaSuccess) {
         cudaGetLastError();
         bifrost_destroy(ctx);
         return BIFROST_ENOMEM;
@@ -1172,7 +1293,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
 int bifrost_destroy(bifrost_ctx* ctx) {
     if (!ctx) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin);
+    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);

@@ -455,3 +455,45 @@ def test_subsystem_pn1_and_shared_timestep(torch, ctx):
     ctx.subsys_min(sub, dt)
     assert np.array_equal(dt.cpu().numpy(), oracle.subsys_min(w.subsys, dt_np))
     assert n == dt_np.shape[0]
+
+
+# ---- small sink sets: one fused launch (gather + pairs + last-CTA reduction) -----------------------
+
+@pytest.mark.parametrize("k", [0, 3, 6, 8, 11])
+def test_small_sets_single_launch_repeatable_and_graph_safe(torch, ctx, k):
+    """Below 4096 sinks a call is ONE launch (pair_fused_kernel); its split-j reduction is done by
+    whichever CTA arrives last, in split order, so repeats are bit-identical; the arrival tickets
+    reset themselves, so the calls replay from a CUDA graph with identical results."""
+    w = workload(2)
+    sinks = W.config2_sink_list(k)
+    si = dev(torch, sinks)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    acc_full = ctx.acc(pos, mass, w.G, w.eps)
+    l0 = ctx.launch_count
+    a = ctx.acc(pos, mass, w.G, w.eps, si, None)
+    assert ctx.launch_count - l0 == 1
+    c = ctx.grad(pos, mass, acc_full, w.G, w.eps, si, None)
+    d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None)
+    assert ctx.launch_count - l0 == 3
+    torch.cuda.synchronize()
+    ref = [x.clone() for x in (a, c, *d)]
+    a2, c2 = torch.zeros_like(a), torch.zeros_like(c)
+    d2 = tuple(torch.full_like(x, -1) if x.dtype == torch.int32 else torch.full_like(x, float("inf")) for x in d)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):      # warm-up outside capture, as torch requires
+        ctx.acc(pos, mass, w.G, w.eps, si, None, out=a2)
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        ctx.acc(pos, mass, w.G, w.eps, si, None, out=a2)
+        ctx.grad(pos, mass, acc_full, w.G, w.eps, si, None, out=c2)
+        ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None, out=d2)
+    for _ in range(3):
+        a2.zero_(); c2.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for got, want in zip((a2, c2, *d2), ref):
+            assert torch.equal(got, want)
+    sk = sinks
+    check_vec(a.cpu().numpy()[sk], oracle.acc(w.pos, w.mass, w.G, w.eps, sk, None), f"acc k={k}")
