@@ -170,6 +170,35 @@ int bifrost_set_subsystems(bifrost_ctx* ctx, const int32_t* subsys, int64_t n);
  * Exact and order-independent (integer atomic minimum on the bit patterns). */
 int bifrost_subsys_min(bifrost_ctx* ctx, int64_t n, const int32_t* subsys, double* inout_dt, void* stream);
 
+/* bifrost_neighbours - NEXT-3, §3.4 "Finding subsystems", Eq. 18-19.  For every sink i
+ * and every source j != i with r_ij = |r_j - r_i| < r_ngb_max the two-body orbital elements of the pair
+ * are formed (mu = G (m_i + m_j), E = v_ij^2/2 - mu/r_ij, a = -mu/(2E), h = r_ij x v_ij,
+ * e = sqrt(max(0, 1 + 2 E h^2/mu^2))) and j is a neighbour of i iff
+ *   bound   (E <  0): a < r_ngb  or  r_ij < r_ngb                                              (Eq. 18)
+ *   unbound (E >= 0): r_peri < r_ngb  and  ( r_ij < r_ngb  or  C r_ij/|v_ij| < tau )           (Eq. 19)
+ * with r_peri = a (1 - e) evaluated as (h^2/mu)/(1 + e) (finite for the parabolic case).  tau is the
+ * pivot time-step of the hierarchy level, C < 1 the safety factor.  The relation is symmetric.
+ * The decision is taken in IEEE fp64, operation by operation (no contraction; correctly rounded sqrt
+ * and division), so it is reproducible bit for bit; only a conservative distance pre-filter runs in
+ * the fast path.  DEVICE pointers, asynchronous on stream.
+ *   out_count : int32[n]        number of neighbours of sink i among the sources, at row i (never truncated)
+ *   out_list  : int32[n][cap]   their ids in source-list order, the first min(count, cap) of them, at row i;
+ *                               entries beyond that and rows of non-sinks are untouched.  1 <= cap <= 1024. */
+int bifrost_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                       const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                       double G, double r_ngb, double r_ngb_max, double tau, double C, int64_t cap,
+                       int32_t* out_count, int32_t* out_list, void* stream);
+
+/* bifrost_components - NEXT-3: subsystems are the connected components of the neighbour
+ * graph.  count / list are bifrost_neighbours' outputs (rows of particles that were not sinks must have
+ * count = 0; ids outside [0, n) and self edges are ignored; an edge listed in one direction only still
+ * joins its two ends).  out_subsys[i] = smallest particle id of i's component, or -1 if no edge touches i
+ * - the array bifrost_set_subsystems and bifrost_subsys_min take.  The paper traverses the graph
+ * depth-first on the host; here it is a lock-free union-find on the device whose result does not
+ * depend on the order of the edges.  DEVICE pointers, asynchronous on stream. */
+int bifrost_components(bifrost_ctx* ctx, int64_t n, const int32_t* count, const int32_t* list, int64_t cap,
+                       int32_t* out_subsys, void* stream);
+
 /* Host-buffer variants: same semantics, HOST pointers, synchronous (see header comment).
  * Index lists may be NULL as above.  Outputs are written only at sink ids (other host rows are
  * untouched), bifrost_pn1_host overwrites all n rows. */

@@ -29,6 +29,7 @@ SYMBOLS = [
     "bifrost_jerk", "bifrost_potential", "bifrost_timestep_criteria",
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
     "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
+    "bifrost_neighbours", "bifrost_components",
 ]
 
 
@@ -71,6 +72,8 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
     lib.bifrost_set_subsystems.argtypes = [_P, _P, _I64]
     lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
+    lib.bifrost_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _I64, _P, _P, _P]
+    lib.bifrost_components.argtypes = [_P, _I64, _P, _P, _I64, _P, _P]
     lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
     _lib = lib
     return lib
@@ -349,3 +352,32 @@ class Context:
         rc = self._lib.bifrost_subsys_min(self._h, subsys.shape[0], subsys.data_ptr(), inout_dt.data_ptr(), self._stream())
         self._check(rc, "bifrost_subsys_min")
         return inout_dt
+
+    # ---- NEXT-3 ----------------------------------------------------------------------
+    def neighbours(self, pos, vel, mass, G, r_ngb, r_ngb_max, tau, C, cap=16, sink_idx=None, src_idx=None, out=None):
+        """Returns (count [n] int32, list [n, cap] int32) written at sink rows; other rows keep
+        count = 0 / list = -1 (the initial values of freshly allocated outputs)."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = (torch.zeros((n,), dtype=torch.int32, device=pos.device),
+                   torch.full((n, int(cap)), -1, dtype=torch.int32, device=pos.device))
+        rc = self._lib.bifrost_neighbours(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
+                                          n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                          float(G), float(r_ngb), float(r_ngb_max), float(tau), float(C), int(cap),
+                                          out[0].data_ptr(), out[1].data_ptr(), self._stream())
+        self._check(rc, "bifrost_neighbours")
+        return out
+
+    def components(self, count, lst, out=None):
+        """Subsystem id (smallest member id; -1 = single) of every particle from neighbour lists."""
+        import torch
+        _dev_idx(count, "count")
+        n, cap = int(lst.shape[0]), int(lst.shape[1])
+        if out is None:
+            out = torch.empty((n,), dtype=torch.int32, device=count.device)
+        rc = self._lib.bifrost_components(self._h, n, count.data_ptr(), lst.data_ptr(), cap, out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_components")
+        return out

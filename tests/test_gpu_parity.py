@@ -497,3 +497,106 @@ def test_small_sets_single_launch_repeatable_and_graph_safe(torch, ctx, k):
             assert torch.equal(got, want)
     sk = sinks
     check_vec(a.cpu().numpy()[sk], oracle.acc(w.pos, w.mass, w.G, w.eps, sk, None), f"acc k={k}")
+
+
+# ---- NEXT-3: neighbour search (Eq. 18-19) and subsystem construction (§3.4) ----------------
+
+NGB = dict(r_ngb=1.5e-3, r_ngb_max=8e-3, tau=2e-4, C=0.5)
+
+
+def _ngb_both(torch, ctx, pos, vel, mass, G, cap, sinks=None, srcs=None, **par):
+    par = {**NGB, **par}
+    ref_count, ref_list = oracle.ngb(pos, vel, mass, G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"], cap=cap,
+                                     sink_idx=sinks, src_idx=srcs)
+    si = None if sinks is None else dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    count, lst = ctx.neighbours(dev(torch, pos), dev(torch, vel), dev(torch, mass), G, par["r_ngb"], par["r_ngb_max"],
+                                par["tau"], par["C"], cap=cap, sink_idx=si, src_idx=sj)
+    torch.cuda.synchronize()
+    return (count, lst), (ref_count, ref_list)
+
+
+def _check_ngb(got, ref, sinks, n, cap):
+    count, lst = got[0].cpu().numpy(), got[1].cpu().numpy()
+    rows = np.arange(n) if sinks is None else sinks
+    assert np.array_equal(count[rows], ref[0])                       # bit-exact decisions
+    for k, i in enumerate(rows):
+        m = min(int(ref[0][k]), cap)
+        assert np.array_equal(lst[i, :m], ref[1][k, :m]), (i, lst[i], ref[1][k])   # same ids, source-list order
+        assert (lst[i, m:] == -1).all()
+    other = np.ones(n, bool); other[rows] = False
+    assert (count[other] == 0).all() and (lst[other] == -1).all()    # rows of non-sinks untouched
+
+
+def test_neighbours_dense_cluster_every_branch(torch, ctx):
+    """A dense cluster in which every branch of Eq. 18-19 fires; cap = 64 holds every list."""
+    rng = np.random.default_rng(5)
+    n = 300
+    pos = rng.normal(size=(n, 3)) * 4e-3
+    vel = rng.normal(size=(n, 3)) * 8.0
+    mass = rng.uniform(0.05, 0.5, n)
+    got, ref = _ngb_both(torch, ctx, pos, vel, mass, 1.0, 64)
+    assert ref[0].sum() > 200
+    _check_ngb(got, ref, None, n, 64)
+    # truncating capacity: counts stay complete, lists hold the first cap ids
+    got, ref = _ngb_both(torch, ctx, pos, vel, mass, 1.0, 2)
+    assert (ref[0] > 2).any()
+    _check_ngb(got, ref, None, n, 2)
+
+
+@pytest.mark.parametrize("n,sel", [(20000, None), (20000, "subset"), (131072, "subset")])
+def test_neighbours_config3_binaries(torch, ctx, n, sel):
+    """Config 3's binaries (a log-uniform in 1e-4..1e-2 r_h, thermal e): all-active (split-j partial
+    lists, concatenated in split order), and random sink subsets against a permuted source list."""
+    w = workload(3) if n == 131072 else workload(3, n=n)
+    sinks = srcs = None
+    if sel == "subset":
+        rng = np.random.default_rng(31)
+        sinks = np.sort(rng.choice(w.n, 777, replace=False)).astype(np.int32)
+        srcs = rng.permutation(w.n).astype(np.int32)[: w.n - 3]
+    got, ref = _ngb_both(torch, ctx, w.pos, w.vel, w.mass, w.G, 8, sinks, srcs)
+    assert ref[0].sum() > (100 if sel else 2000)                     # the binaries are found
+    _check_ngb(got, ref, sinks, w.n, 8)
+
+
+def test_components_and_subsystem_chain(torch, ctx):
+    """neighbours -> components -> set_subsystems, all device-resident, against the oracle chain."""
+    w = workload(3, n=20000)
+    (count, lst), ref = _ngb_both(torch, ctx, w.pos, w.vel, w.mass, w.G, 8)
+    sub = ctx.components(count, lst)
+    torch.cuda.synchronize()
+    ei, ej = oracle.edges_from_lists(None, ref[0], ref[1])
+    ref_sub = oracle.components(w.n, ei, ej)
+    assert np.array_equal(sub.cpu().numpy(), ref_sub)
+    assert (ref_sub >= 0).sum() > 2000 and len(np.unique(ref_sub[ref_sub >= 0])) > 1000
+    # a chain (Fig. 1: target - F - G) listed in ONE direction only, a self edge and a bad id
+    n = 10
+    cnt = np.zeros(n, np.int32); l2 = np.full((n, 3), -1, np.int32)
+    cnt[7] = 1; l2[7, 0] = 4            # 7 - 4
+    cnt[4] = 2; l2[4, :2] = (9, 4)      # 4 - 9, and a self edge
+    cnt[2] = 3; l2[2, :3] = (5, 99, 2)  # 2 - 5, an id out of range
+    s2 = ctx.components(dev(torch, cnt), dev(torch, l2)).cpu().numpy()
+    assert s2.tolist() == [-1, -1, 2, -1, 4, 2, -1, 4, -1, 4]
+    assert np.array_equal(s2, oracle.components(n, [7, 4, 2], [4, 9, 5]))
+    # feed the labels to the pair kernels: the excluded sums match the subsystem-aware oracle
+    ctx.set_subsystems(sub)
+    try:
+        pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+        a = ctx.acc(pos, mass, w.G, w.eps).cpu().numpy()
+    finally:
+        ctx.set_subsystems(None)
+    check_vec(a, oracle.acc_sub(w.pos, w.mass, w.G, w.eps, ref_sub), "acc with device-built subsystems")
+
+
+def test_components_long_chain_and_big_component(torch, ctx):
+    """Worst cases for a union-find: one path through all particles in a scrambled order, and a star."""
+    n = 50000
+    rng = np.random.default_rng(8)
+    perm = rng.permutation(n).astype(np.int32)
+    cnt = np.zeros(n, np.int32); lst = np.full((n, 2), -1, np.int32)
+    cnt[perm[:-1]] = 1; lst[perm[:-1], 0] = perm[1:]
+    got = ctx.components(dev(torch, cnt), dev(torch, lst)).cpu().numpy()
+    assert (got == 0).all()
+    cnt[:] = 1; lst[:, 0] = 12345; cnt[12345] = 0
+    got = ctx.components(dev(torch, cnt), dev(torch, lst)).cpu().numpy()
+    assert (got == 0).all()
