@@ -199,6 +199,51 @@ int bifrost_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
 int bifrost_components(bifrost_ctx* ctx, int64_t n, const int32_t* count, const int32_t* list, int64_t cap,
                        int32_t* out_subsys, void* stream);
 
+/* ---- NEXT-4: the integrator built on the sums above (§2.1-2.2) -------------------------
+ * Scratch for these calls (2 x double[max_n][3], 3 x double[max_n], 2 x int32[max_n]) is allocated on
+ * their first use, not in bifrost_create. */
+
+/* bifrost_kick - Eq. 5 / Eq. 8-9: vel[i] += h * (acc[i] + c * grad[i]) for i in idx
+ * (grad == NULL: vel[i] += h * acc[i]).  The gradient kick of a cycle of length eps is h = 2 eps/3,
+ * c = eps^2/24 with grad = bifrost_grad's output.  idx == NULL means all n (n_idx must equal n).
+ * DEVICE pointers, asynchronous on stream. */
+int bifrost_kick(bifrost_ctx* ctx, int64_t n, const int32_t* idx, int64_t n_idx, const double* acc,
+                 const double* grad, double h, double c, double* vel, void* stream);
+
+/* bifrost_drift - Eq. 7: pos[i] += h * vel[i] for i in idx.  As bifrost_kick. */
+int bifrost_drift(bifrost_ctx* ctx, int64_t n, const int32_t* idx, int64_t n_idx, const double* vel, double h,
+                  double* pos, void* stream);
+
+/* bifrost_fsi_step - one FSI cycle, Eq. 10: kick(eps/6) drift(eps/2) gradient kick(2 eps/3)
+ * drift(eps/2) kick(eps/6) over the particles idx interacting ONLY among themselves (sinks = sources = idx;
+ * idx == NULL: all n): four O(N^2) sums (acc, acc, grad, acc) and five O(N) updates, all on
+ * stream, no host synchronisation.  pos and vel (double[n][3]) are updated in place at the rows in idx.
+ * eps_soft is the Plummer softening of the sums, eps the time-step. */
+int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass,
+                     const int32_t* idx, int64_t n_idx, double G, double eps_soft, double eps, void* stream);
+
+/* bifrost_hhs_fsi - one HHS-FSI integration interval of length tau, Eq. 11-13, without
+ * subsystem integration (the "softened FROST-like" mode of PAPER.md:L818).  At every level: time-steps
+ * eps_i = min(eps_ff, eps_fb) (Eq. 21-22 with eta_ff, eta_fb) of the level's particles among themselves,
+ * capped by the particle's level-0 value; fast F = {eps_i < tau}, slow S = the rest (stable
+ * partition, S first); then  U_SF(tau/6) H_S(tau/2) H_F(tau/2) U~_SF(2 tau/3) H_F(tau/2) H_S(tau/2) U_SF(tau/6)
+ * with the inter-level accelerations of Eq. 12, the gradient accelerations of Eq. 13, H_S = bifrost_fsi_step
+ * over S and H_F = this procedure over F with tau/2.  A level without fast particles (or at depth max_depth,
+ * 0 <= max_depth <= 62) is one FSI cycle of length tau.  Every sum and update runs on the device; the host
+ * reads one integer (|S|) per level to steer the recursion, so the call is SYNCHRONOUS.
+ *   out_level_log : HOST int64[log_cap][3] or NULL - (depth, |S|, |F|) of the first log_cap levels, in the
+ *                   order they are entered;   out_summary : HOST int64[3] or NULL - levels entered, deepest
+ *                   depth, FSI cycles run.  pos, vel : DEVICE double[n][3], updated in place. */
+int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G,
+                    double eps_soft, double eta_ff, double eta_fb, double tau, int max_depth,
+                    int64_t* out_level_log, int64_t log_cap, int64_t* out_summary, void* stream);
+
+/* bifrost_kinetic_energy - first term of Eq. 4: *out_T = 1/2 sum_{i in idx} m_i |v_i|^2
+ * (DEVICE double, fixed-order two-stage reduction: deterministic).  With bifrost_potential's out_W this
+ * is the total energy of the relative-energy-error check, Eq. 72-73. */
+int bifrost_kinetic_energy(bifrost_ctx* ctx, int64_t n, const double* vel, const double* mass,
+                           const int32_t* idx, int64_t n_idx, double* out_T, void* stream);
+
 /* Host-buffer variants: same semantics, HOST pointers, synchronous (see header comment).
  * Index lists may be NULL as above.  Outputs are written only at sink ids (other host rows are
  * untouched), bifrost_pn1_host overwrites all n rows. */

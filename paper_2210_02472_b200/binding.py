@@ -30,6 +30,7 @@ SYMBOLS = [
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
     "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
     "bifrost_neighbours", "bifrost_components",
+    "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
 ]
 
 
@@ -74,6 +75,11 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
     lib.bifrost_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _I64, _P, _P, _P]
     lib.bifrost_components.argtypes = [_P, _I64, _P, _P, _I64, _P, _P]
+    lib.bifrost_kick.argtypes = [_P, _I64, _P, _I64, _P, _P, _D, _D, _P, _P]
+    lib.bifrost_drift.argtypes = [_P, _I64, _P, _I64, _P, _D, _P, _P]
+    lib.bifrost_fsi_step.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _D, _P]
+    lib.bifrost_hhs_fsi.argtypes = [_P, _I64, _P, _P, _P, _D, _D, _D, _D, _D, _I, _P, _I64, _P, _P]
+    lib.bifrost_kinetic_energy.argtypes = [_P, _I64, _P, _P, _P, _I64, _P, _P]
     lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
     _lib = lib
     return lib
@@ -380,4 +386,60 @@ class Context:
             out = torch.empty((n,), dtype=torch.int32, device=count.device)
         rc = self._lib.bifrost_components(self._h, n, count.data_ptr(), lst.data_ptr(), cap, out.data_ptr(), self._stream())
         self._check(rc, "bifrost_components")
+        return out
+
+    # ---- NEXT-4 ----------------------------------------------------------------------
+    def kick(self, vel, acc, h, grad=None, c=0.0, idx=None):
+        vel = _dev_f64(vel, (3,), "vel"); acc = _dev_f64(acc, (3,), "acc")
+        if grad is not None:
+            _dev_f64(grad, (3,), "grad")
+        n = vel.shape[0]
+        ix, ixp = _dev_idx(idx, "idx")
+        rc = self._lib.bifrost_kick(self._h, n, ixp or None, n if ix is None else ix.shape[0], acc.data_ptr(),
+                                    None if grad is None else grad.data_ptr(), float(h), float(c), vel.data_ptr(),
+                                    self._stream())
+        self._check(rc, "bifrost_kick")
+        return vel
+
+    def drift(self, pos, vel, h, idx=None):
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel")
+        n = pos.shape[0]
+        ix, ixp = _dev_idx(idx, "idx")
+        rc = self._lib.bifrost_drift(self._h, n, ixp or None, n if ix is None else ix.shape[0], vel.data_ptr(), float(h),
+                                     pos.data_ptr(), self._stream())
+        self._check(rc, "bifrost_drift")
+        return pos
+
+    def fsi_step(self, pos, vel, mass, G, eps_soft, eps, idx=None):
+        """One FSI cycle (Eq. 10) in place over idx (None: all)."""
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        ix, ixp = _dev_idx(idx, "idx")
+        rc = self._lib.bifrost_fsi_step(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), ixp or None,
+                                        n if ix is None else ix.shape[0], float(G), float(eps_soft), float(eps),
+                                        self._stream())
+        self._check(rc, "bifrost_fsi_step")
+
+    def hhs_fsi(self, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, log_cap=0):
+        """One HHS-FSI interval (Eq. 11) in place.  Returns (summary dict, level log as an int64 array [k, 3])."""
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        log = np.zeros((max(int(log_cap), 1), 3), dtype=np.int64)
+        summ = np.zeros(3, dtype=np.int64)
+        rc = self._lib.bifrost_hhs_fsi(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), float(G),
+                                       float(eps_soft), float(eta_ff), float(eta_fb), float(tau), int(max_depth),
+                                       log.ctypes.data if log_cap else None, int(log_cap), summ.ctypes.data, self._stream())
+        self._check(rc, "bifrost_hhs_fsi")
+        k = min(int(summ[0]), int(log_cap))
+        return {"levels": int(summ[0]), "deepest": int(summ[1]), "fsi_steps": int(summ[2])}, log[:k]
+
+    def kinetic_energy(self, vel, mass, idx=None):
+        import torch
+        vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        ix, ixp = _dev_idx(idx, "idx")
+        out = torch.zeros(1, dtype=torch.float64, device=vel.device)
+        rc = self._lib.bifrost_kinetic_energy(self._h, n, vel.data_ptr(), mass.data_ptr(), ixp or None,
+                                              n if ix is None else ix.shape[0], out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_kinetic_energy")
         return out

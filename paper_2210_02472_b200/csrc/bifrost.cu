@@ -28,6 +28,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <cmath>
 #include <algorithm>
 #include <new>
 
@@ -1031,6 +1032,109 @@ __global__ void comp_label_kernel(int n, int* parent, const unsigned char* __res
 }
 
 // ----------------------------------------------------------------------------------------
+// NEXT-4: the O(N) operators of the FSI cycle (Eq. 5, 7, 8) and the slow/fast
+// split of a hierarchy level.
+// ----------------------------------------------------------------------------------------
+__global__ void kick_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ acc,
+                            const double* __restrict__ grad, double h, double c, double* __restrict__ vel) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const size_t o = 3 * (size_t)(idx ? idx[k] : k);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double a = acc[o + d];
+        if (grad) a = __dadd_rn(a, __dmul_rn(c, grad[o + d]));        // a~ = a + (eps^2/24) C   (Eq. 9)
+        vel[o + d] = __dadd_rn(vel[o + d], __dmul_rn(h, a));          // v += h a                (Eq. 5, 8)
+    }
+}
+__global__ void drift_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ vel, double h,
+                             double* __restrict__ pos) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const size_t o = 3 * (size_t)(idx ? idx[k] : k);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) pos[o + d] = __dadd_rn(pos[o + d], __dmul_rn(h, vel[o + d]));   // r += h v (Eq. 7)
+}
+
+// eps_i = min(eps_ff, eps_fb), never above the level-0 value; fast iff eps_i < tau
+__global__ void level_flag_kernel(int m, const int32_t* __restrict__ seg, const double* __restrict__ dt_ff,
+                                  const double* __restrict__ dt_fb, double* __restrict__ dt0, int depth, double tau,
+                                  int all_slow, unsigned char* __restrict__ fast) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    if (all_slow) { fast[k] = 0; return; }
+    const int i = seg[k];
+    double dt = fmin(dt_ff[i], dt_fb[i]);
+    if (depth == 0) dt0[i] = dt;
+    dt = fmin(dt, dt0[i]);
+    fast[k] = dt < tau ? 1 : 0;
+}
+
+// stable partition of a segment into [slow | fast]: block counts -> scan -> scatter
+constexpr int PART_T = 256;
+__global__ void __launch_bounds__(PART_T)
+part_count_kernel(int m, const unsigned char* __restrict__ fast, int* __restrict__ block_slow) {
+    const int k = blockIdx.x * PART_T + threadIdx.x;
+    const int slow = (k < m) && !fast[k];
+    const int c = __syncthreads_count(slow);
+    if (threadIdx.x == 0) block_slow[blockIdx.x] = c;
+}
+__global__ void part_scan_kernel(int nb, int* __restrict__ block_slow, int* __restrict__ n_slow) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int run = 0;
+    for (int b = 0; b < nb; ++b) { const int c = block_slow[b]; block_slow[b] = run; run += c; }
+    *n_slow = run;
+}
+__global__ void __launch_bounds__(PART_T)
+part_scatter_kernel(int m, const int32_t* __restrict__ seg, const unsigned char* __restrict__ fast,
+                    const int* __restrict__ block_slow, const int* __restrict__ n_slow, int32_t* __restrict__ out) {
+    __shared__ int warp_slow[PART_T / 32];
+    const int k = blockIdx.x * PART_T + threadIdx.x;
+    const int live = k < m;
+    const int slow = live && !fast[k];
+    const unsigned bal = __ballot_sync(0xffffffffu, slow);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) warp_slow[warp] = __popc(bal);
+    __syncthreads();
+    int before = 0;                                           // slow elements of this block before this warp
+    for (int w = 0; w < warp; ++w) before += warp_slow[w];
+    const int rank_slow = before + __popc(bal & ((1u << lane) - 1u));
+    if (!live) return;
+    const int slow_before_block = block_slow[blockIdx.x];
+    if (slow) out[slow_before_block + rank_slow] = seg[k];
+    else {
+        const int fast_before = (blockIdx.x * PART_T - slow_before_block) + (threadIdx.x - rank_slow);
+        out[*n_slow + fast_before] = seg[k];
+    }
+}
+__global__ void iota_kernel(int n, int32_t* __restrict__ a) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = i;
+}
+__global__ void fill_f64_kernel(int n, double v, double* __restrict__ a) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = v;
+}
+
+// T = 1/2 sum m v^2 over a set, fixed order (stage 1 of the W reduction with another integrand)
+__global__ void __launch_bounds__(WSUM_THREADS)
+ksum_stage1_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ mass,
+                   const double* __restrict__ vel, double* __restrict__ block_part) {
+    const int base = blockIdx.x * WSUM_PER_BLOCK;
+    double v = 0.0;
+    for (int q = threadIdx.x; q < WSUM_PER_BLOCK; q += WSUM_THREADS) {
+        const int k = base + q;
+        if (k < m) {
+            const int id = idx ? idx[k] : k;
+            const double* u = vel + 3 * (size_t)id;
+            v += mass[id] * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+        }
+    }
+    const double s = block_sum_fixed(v);
+    if (threadIdx.x == 0) block_part[blockIdx.x] = s;
+}
+
+// ----------------------------------------------------------------------------------------
 // Measurement aid: register-only FP64 chains (no memory traffic), to MEASURE the FP64-pipe peak
 // that bench.py's roofline quotes next to the derived 64 lanes/clk/SM figure.
 //   MIX 0: 8 independent DFMA chains per thread (pure DFMA peak).
@@ -1120,6 +1224,12 @@ struct bifrost_ctx {
     int64_t subsys_n = 0;
     int64_t launches = 0;
     char err[256] = {0};
+    // NEXT-4 integrator scratch (allocated on first use of bifrost_fsi_step / bifrost_hhs_fsi)
+    bool integ_ready = false;
+    double *w_acc = nullptr, *w_grad = nullptr, *w_dtff = nullptr, *w_dtfb = nullptr, *w_dt0 = nullptr;
+    int32_t *w_order = nullptr, *w_tmp = nullptr;
+    int *w_bcount = nullptr, *w_nslow = nullptr;
+    int* h_nslow = nullptr;          // pinned
     // mirrors for the *_host entry points (allocated on first use)
     bool host_ready = false;
     cudaStream_t hstream = nullptr;
@@ -1407,6 +1517,134 @@ int fetch_rows(bifrost_ctx* ctx, const void* d_rows, size_t row_bytes, const int
     return BIFROST_OK;
 }
 
+// ---- NEXT-4: FSI cycle and HHS-FSI driver (host logic around the kernels above) ------------
+
+int ensure_integrator(bifrost_ctx* ctx) {
+    if (ctx->integ_ready) return BIFROST_OK;
+    const size_t n = (size_t)ctx->max_n;
+    CU_TRY(ctx, cudaMalloc(&ctx->w_acc, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_grad, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_dtff, 8 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_dtfb, 8 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_dt0, 8 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_order, 4 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_tmp, 4 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_bcount, 4 * (n / PART_T + 1)));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_nslow, 4));
+    CU_TRY(ctx, cudaMallocHost(&ctx->h_nslow, 4));
+    ctx->integ_ready = true;
+    return BIFROST_OK;
+}
+
+int kick_impl(bifrost_ctx* ctx, const int32_t* idx, int64_t m, const double* acc, const double* grad, double h, double c,
+              double* vel, cudaStream_t st) {
+    if (m == 0) return BIFROST_OK;
+    kick_kernel<<<ceil_div(m, 256), 256, 0, st>>>((int)m, idx, acc, grad, h, c, vel);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+int drift_impl(bifrost_ctx* ctx, const int32_t* idx, int64_t m, const double* vel, double h, double* pos, cudaStream_t st) {
+    if (m == 0) return BIFROST_OK;
+    drift_kernel<<<ceil_div(m, 256), 256, 0, st>>>((int)m, idx, vel, h, pos);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+#define RC_TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
+
+// Eq. 10 over the particles idx[0..m) interacting among themselves (idx == NULL: all n).
+int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, const int32_t* idx, int64_t m,
+             double G, double eps_soft, double eps, cudaStream_t st) {
+    if (m == 0) return BIFROST_OK;
+    double* a = ctx->w_acc;
+    double* g = ctx->w_grad;
+    RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
+    RC_TRY(kick_impl(ctx, idx, m, a, nullptr, eps / 6.0, 0.0, vel, st));
+    RC_TRY(drift_impl(ctx, idx, m, vel, eps / 2.0, pos, st));
+    RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
+    RC_TRY(grad_impl(ctx, n, pos, mass, a, idx, m, idx, m, G, eps_soft, g, 0, st));
+    RC_TRY(kick_impl(ctx, idx, m, a, g, 2.0 * eps / 3.0, eps * eps / 24.0, vel, st));
+    RC_TRY(drift_impl(ctx, idx, m, vel, eps / 2.0, pos, st));
+    RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
+    RC_TRY(kick_impl(ctx, idx, m, a, nullptr, eps / 6.0, 0.0, vel, st));
+    return BIFROST_OK;
+}
+
+struct Hhs {
+    bifrost_ctx* ctx; int64_t n; double* pos; double* vel; const double* mass;
+    double G, eps_soft, eta_ff, eta_fb; int max_depth; cudaStream_t st;
+    int64_t* log; int64_t log_cap; int64_t n_levels; int64_t deepest; int64_t fsi_steps;
+};
+
+// One level of Eq. 11 over order[lo, hi) for an interval tau.
+int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
+    bifrost_ctx* ctx = h.ctx;
+    const int64_t m = hi - lo;
+    if (m == 0) return BIFROST_OK;
+    cudaStream_t st = h.st;
+    int32_t* seg = ctx->w_order + lo;
+    const int all_slow = depth >= h.max_depth;
+    if (!all_slow)   // time-steps of the level's particles among themselves (Eq. 21-22)
+        RC_TRY(dtmin_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eta_ff, h.eta_fb, ctx->w_dtff, ctx->w_dtfb,
+                          nullptr, nullptr, 0, st));
+    const int nb = ceil_div(m, PART_T);
+    unsigned char* fast = ctx->is_bh;                      // scratch shared with bifrost_pn1 (one call at a time per ctx)
+    level_flag_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow, fast);
+    part_count_kernel<<<nb, PART_T, 0, st>>>((int)m, fast, ctx->w_bcount);
+    part_scan_kernel<<<1, 32, 0, st>>>(nb, ctx->w_bcount, ctx->w_nslow);
+    part_scatter_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, fast, ctx->w_bcount, ctx->w_nslow, ctx->w_tmp);
+    ctx->launches += 4;
+    CU_TRY(ctx, cudaGetLastError());
+    CU_TRY(ctx, cudaMemcpyAsync(seg, ctx->w_tmp, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->h_nslow, ctx->w_nslow, 4, cudaMemcpyDeviceToHost, st));
+    CU_TRY(ctx, cudaStreamSynchronize(st));                // the host decides the recursion (as in the paper)
+    const int64_t ns = *ctx->h_nslow, nf = m - ns;
+    if (h.log && h.n_levels < h.log_cap) {
+        int64_t* e = h.log + 3 * h.n_levels;
+        e[0] = depth; e[1] = ns; e[2] = nf;
+    }
+    h.n_levels++;
+    if (depth > h.deepest) h.deepest = depth;
+    const int32_t* S = seg;
+    const int32_t* F = seg + ns;
+    if (nf == 0) {
+        h.fsi_steps++;
+        return fsi_impl(ctx, h.n, h.pos, h.vel, h.mass, S, ns, h.G, h.eps_soft, tau, st);
+    }
+    double* a = ctx->w_acc;
+    double* g = ctx->w_grad;
+    auto inter_level_acc = [&]() -> int {                  // Eq. 12
+        if (ns == 0) return BIFROST_OK;
+        RC_TRY(acc_impl(ctx, h.n, h.pos, h.mass, S, ns, F, nf, h.G, h.eps_soft, a, 0, st));
+        RC_TRY(acc_impl(ctx, h.n, h.pos, h.mass, F, nf, S, ns, h.G, h.eps_soft, a, 0, st));
+        return BIFROST_OK;
+    };
+    auto H_S = [&]() -> int {
+        if (ns == 0) return BIFROST_OK;
+        h.fsi_steps++;
+        return fsi_impl(ctx, h.n, h.pos, h.vel, h.mass, S, ns, h.G, h.eps_soft, tau / 2.0, st);
+    };
+    auto H_F = [&]() -> int { return hhs_level(h, lo + ns, hi, tau / 2.0, depth + 1); };
+
+    RC_TRY(inter_level_acc());
+    if (ns) RC_TRY(kick_impl(ctx, seg, m, a, nullptr, tau / 6.0, 0.0, h.vel, st));
+    RC_TRY(H_S());
+    RC_TRY(H_F());
+    RC_TRY(inter_level_acc());
+    if (ns) {                                              // Eq. 13
+        RC_TRY(grad_impl(ctx, h.n, h.pos, h.mass, a, S, ns, F, nf, h.G, h.eps_soft, g, 0, st));
+        RC_TRY(grad_impl(ctx, h.n, h.pos, h.mass, a, F, nf, S, ns, h.G, h.eps_soft, g, 0, st));
+        RC_TRY(kick_impl(ctx, seg, m, a, g, 2.0 * tau / 3.0, tau * tau / 24.0, h.vel, st));
+    }
+    RC_TRY(H_F());
+    RC_TRY(H_S());
+    RC_TRY(inter_level_acc());
+    if (ns) RC_TRY(kick_impl(ctx, seg, m, a, nullptr, tau / 6.0, 0.0, h.vel, st));
+    return BIFROST_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -1465,6 +1703,9 @@ int bifrost_destroy(bifrost_ctx* ctx) {
     cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
+    cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
+    cudaFree(ctx->w_order); cudaFree(ctx->w_tmp); cudaFree(ctx->w_bcount); cudaFree(ctx->w_nslow);
+    if (ctx->h_nslow) cudaFreeHost(ctx->h_nslow);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->h_stage_i) cudaFreeHost(ctx->h_stage_i);
     if (ctx->hstream) cudaStreamDestroy(ctx->hstream);
@@ -1737,6 +1978,84 @@ int bifrost_components(bifrost_ctx* ctx, int64_t n, const int32_t* count, const 
     comp_hook_kernel<<<ceil_div(n * cap, 256), 256, 0, st>>>((int)n, (int)cap, count, list, parent, flag);
     comp_label_kernel<<<ceil_div(n, 256), 256, 0, st>>>((int)n, parent, flag, out_subsys);
     ctx->launches += 3;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+// ---- NEXT-4: integrator operators, FSI cycle, HHS-FSI driver -----------------
+
+int bifrost_kick(bifrost_ctx* ctx, int64_t n, const int32_t* idx, int64_t n_idx, const double* acc, const double* grad,
+                 double h, double c, double* vel, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_idx < 0 || n_idx > ctx->max_n || (!idx && n_idx != n)) return BIFROST_EINVAL;
+    if (n_idx == 0) return BIFROST_OK;
+    if (!acc || !vel) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return kick_impl(ctx, idx, n_idx, acc, grad, h, c, vel, (cudaStream_t)stream);
+}
+
+int bifrost_drift(bifrost_ctx* ctx, int64_t n, const int32_t* idx, int64_t n_idx, const double* vel, double h,
+                  double* pos, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_idx < 0 || n_idx > ctx->max_n || (!idx && n_idx != n)) return BIFROST_EINVAL;
+    if (n_idx == 0) return BIFROST_OK;
+    if (!vel || !pos) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return drift_impl(ctx, idx, n_idx, vel, h, pos, (cudaStream_t)stream);
+}
+
+int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, const int32_t* idx,
+                     int64_t n_idx, double G, double eps_soft, double eps, void* stream) {
+    int rc = check_lists(ctx, n, idx, n_idx, idx, n_idx);
+    if (rc) return rc;
+    if (n_idx == 0) return BIFROST_OK;
+    if (!pos || !vel || !mass) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if ((rc = ensure_integrator(ctx))) return rc;
+    return fsi_impl(ctx, n, pos, vel, mass, idx, n_idx, G, eps_soft, eps, (cudaStream_t)stream);
+}
+
+int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G, double eps_soft,
+                    double eta_ff, double eta_fb, double tau, int max_depth, int64_t* out_level_log, int64_t log_cap,
+                    int64_t* out_summary, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || max_depth < 0 || max_depth > 62 || log_cap < 0 || !(tau > 0.0)) return BIFROST_EINVAL;
+    if (ctx->subsys && ctx->subsys_n != n) return BIFROST_EINVAL;
+    if (out_summary) out_summary[0] = out_summary[1] = out_summary[2] = 0;
+    if (n == 0) return BIFROST_OK;
+    if (!pos || !vel || !mass) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    int rc;
+    if ((rc = ensure_integrator(ctx))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    iota_kernel<<<ceil_div(n, 256), 256, 0, st>>>((int)n, ctx->w_order);
+    fill_f64_kernel<<<ceil_div(n, 256), 256, 0, st>>>((int)n, HUGE_VAL, ctx->w_dt0);
+    ctx->launches += 2;
+    CU_TRY(ctx, cudaGetLastError());
+    Hhs h{ctx, n, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, max_depth, st, out_level_log, log_cap, 0, 0, 0};
+    rc = hhs_level(h, 0, n, tau, 0);
+    if (out_summary) { out_summary[0] = h.n_levels; out_summary[1] = h.deepest; out_summary[2] = h.fsi_steps; }
+    if (rc) return rc;
+    CU_TRY(ctx, cudaStreamSynchronize(st));
+    return BIFROST_OK;
+}
+
+int bifrost_kinetic_energy(bifrost_ctx* ctx, int64_t n, const double* vel, const double* mass, const int32_t* idx,
+                           int64_t n_idx, double* out_T, void* stream) {
+    if (!ctx) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (n < 0 || n > ctx->max_n || n_idx < 0 || n_idx > ctx->max_n || (!idx && n_idx != n) || !out_T) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_idx == 0) { CU_TRY(ctx, cudaMemsetAsync(out_T, 0, sizeof(double), st)); return BIFROST_OK; }
+    if (!vel || !mass) return BIFROST_EINVAL;
+    const int nb = ceil_div(n_idx, WSUM_PER_BLOCK);
+    ksum_stage1_kernel<<<nb, WSUM_THREADS, 0, st>>>((int)n_idx, idx, mass, vel, ctx->wpart);
+    wsum_stage2_kernel<<<1, WSUM_THREADS, 0, st>>>(nb, ctx->wpart, out_T);
+    ctx->launches += 2;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
 }

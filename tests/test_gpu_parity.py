@@ -600,3 +600,116 @@ def test_components_long_chain_and_big_component(torch, ctx):
     cnt[:] = 1; lst[:, 0] = 12345; cnt[12345] = 0
     got = ctx.components(dev(torch, cnt), dev(torch, lst)).cpu().numpy()
     assert (got == 0).all()
+
+
+# ---- NEXT-4: FSI cycle (Eq. 10) and HHS-FSI (Eq. 11-13) on the device ------------------------------
+
+def _state_err(pos_g, vel_g, pos_r, vel_r):
+    return max(float(np.abs(pos_g - pos_r).max() / np.abs(pos_r).max()),
+               float(np.abs(vel_g - vel_r).max() / np.abs(vel_r).max()))
+
+
+@pytest.mark.parametrize("cfg,k", [(1, None), (2, 7), (2, 12)])
+def test_fsi_step_parity(torch, ctx, cfg, k):
+    """One FSI cycle over all particles (config 1) and over active subsets (config 2), three cycles."""
+    from oracle import integrator as I
+    w = workload(cfg)
+    idx = None if k is None else W.config2_sink_list(k)
+    eps = 1e-3
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    ix = None if idx is None else dev(torch, idx)
+    for _ in range(3):
+        ctx.fsi_step(pos, vel, mass, w.G, w.eps, eps, ix)
+    torch.cuda.synchronize()
+    rp, rv = w.pos.copy(), w.vel.copy()
+    ridx = np.arange(w.n, dtype=np.int32) if idx is None else idx
+    for _ in range(3):
+        I.fsi_step(rp, rv, w.mass, ridx, w.G, w.eps, eps)
+    assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
+    if idx is not None:                                          # particles outside the set are untouched
+        rest = np.setdiff1d(np.arange(w.n), idx)
+        assert np.array_equal(pos.cpu().numpy()[rest], w.pos[rest]) and np.array_equal(vel.cpu().numpy()[rest], w.vel[rest])
+
+
+def test_kick_drift_operators(torch, ctx):
+    rng = np.random.default_rng(3)
+    n = 1000
+    v, a, g, p = (rng.normal(size=(n, 3)) for _ in range(4))
+    idx = np.sort(rng.choice(n, 300, replace=False)).astype(np.int32)
+    vd = ctx.kick(dev(torch, v), dev(torch, a), 0.3, dev(torch, g), 0.01, dev(torch, idx)).cpu().numpy()
+    ref = v.copy(); ref[idx] += 0.3 * (a[idx] + 0.01 * g[idx])
+    assert np.array_equal(vd, ref)
+    vd = ctx.kick(dev(torch, v), dev(torch, a), 0.3).cpu().numpy()
+    assert np.array_equal(vd, v + 0.3 * a)
+    pd = ctx.drift(dev(torch, p), dev(torch, v), 0.7, dev(torch, idx)).cpu().numpy()
+    ref = p.copy(); ref[idx] += 0.7 * v[idx]
+    assert np.array_equal(pd, ref)
+    m = rng.uniform(0.1, 1, n)
+    T = float(ctx.kinetic_energy(dev(torch, v), dev(torch, m)).cpu()[0])
+    assert abs(T / (0.5 * (m * (v * v).sum(1)).sum()) - 1) < 1e-14
+
+
+def _binary_cluster(n_cl=400, seed=7):
+    """A Plummer cluster with two hard binaries and a triple-ish close pair: several hierarchy levels."""
+    rng = np.random.default_rng(seed)
+    pos, vel = W.plummer_phase_space(rng, n_cl)
+    mass = np.full(n_cl, 1.0 / n_cl)
+    extra_p, extra_v, extra_m = [], [], []
+    for (a, e, off) in ((2e-3, 0.3, (0.05, 0.02, -0.01)), (5e-4, 0.6, (-0.3, 0.1, 0.2))):
+        M = 0.01
+        rp = a * (1 - e); vp = np.sqrt(M * (1 + e) / (a * (1 - e)))
+        extra_p += [np.array([-0.5 * rp, 0, 0]) + off, np.array([0.5 * rp, 0, 0]) + off]
+        extra_v += [np.array([0, -0.5 * vp, 0]), np.array([0, 0.5 * vp, 0])]
+        extra_m += [M / 2, M / 2]
+    pos = np.vstack([pos, np.array(extra_p)]); vel = np.vstack([vel, np.array(extra_v)])
+    mass = np.concatenate([mass, extra_m])
+    W.recentre(pos, vel, mass)
+    return pos, vel, mass
+
+
+def test_hhs_fsi_parity_level_structure_and_energy(torch, ctx):
+    """The hierarchy (which particles are fast at which level: integer decisions) equals the oracle's
+    level by level; the state after the interval agrees to 1e-12; momentum and energy behave."""
+    from oracle import integrator as I
+    pos0, vel0, mass = _binary_cluster()
+    G, eps_soft, eta, tau = 1.0, 1e-4, 0.05, 1e-3
+    rp, rv = pos0.copy(), vel0.copy()
+    stats = {}
+    I.hhs_fsi(rp, rv, mass, G, eps_soft, eta, eta, tau, stats=stats)
+    ref_levels = np.array([(d, s, f) for d, s, f, _ in stats["levels"]], dtype=np.int64)
+    assert ref_levels[:, 0].max() >= 3
+    pos, vel, m = dev(torch, pos0), dev(torch, vel0), dev(torch, mass)
+    e0 = float(ctx.kinetic_energy(vel, m).cpu()[0]) + float(ctx.potential(pos, m, G, eps_soft, want_phi=False)[1].cpu())
+    summ, log = ctx.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, log_cap=len(ref_levels) + 10)
+    assert summ["levels"] == len(ref_levels) and np.array_equal(log, ref_levels)
+    assert summ["deepest"] == int(ref_levels[:, 0].max())
+    pg, vg = pos.cpu().numpy(), vel.cpu().numpy()
+    assert _state_err(pg, vg, rp, rv) < 1e-12
+    e1 = float(ctx.kinetic_energy(vel, m).cpu()[0]) + float(ctx.potential(pos, m, G, eps_soft, want_phi=False)[1].cpu())
+    assert abs(e1 / e0 - 1) < 1e-7
+    assert abs(e1 / I.total_energy(rp, rv, mass, G, eps_soft) - 1) < 1e-12
+    assert np.abs((mass[:, None] * vg).sum(0) - (mass[:, None] * vel0).sum(0)).max() < 1e-15
+    # max_depth = 0: the interval is one FSI cycle over everything
+    pos, vel = dev(torch, pos0), dev(torch, vel0)
+    summ, log = ctx.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=0, log_cap=4)
+    assert summ == {"levels": 1, "deepest": 0, "fsi_steps": 1} and log.tolist() == [[0, len(mass), 0]]
+    p2, v2 = dev(torch, pos0), dev(torch, vel0)
+    ctx.fsi_step(p2, v2, m, G, eps_soft, tau)
+    assert torch.equal(pos, p2) and torch.equal(vel, v2)
+
+
+def test_hhs_fsi_config2_full_size(torch, ctx):
+    """Config 2 (N = 16384, Kroupa masses): the level populations are the hierarchical time-bin sizes the
+    paper's active-subset sweep stands for; checked against the oracle at full size."""
+    from oracle import integrator as I
+    w = workload(2)
+    tau, eta = 2.0 ** -9, 0.1
+    rp, rv = w.pos.copy(), w.vel.copy()
+    stats = {}
+    I.hhs_fsi(rp, rv, w.mass, w.G, w.eps, eta, eta, tau, max_depth=3, stats=stats)
+    ref_levels = np.array([(d, s, f) for d, s, f, _ in stats["levels"]], dtype=np.int64)
+    pos, vel, m = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    summ, log = ctx.hhs_fsi(pos, vel, m, w.G, w.eps, eta, eta, tau, max_depth=3, log_cap=64)
+    assert np.array_equal(log, ref_levels), (log, ref_levels)
+    assert ref_levels[0, 2] > 0 and ref_levels[0, 1] > 0
+    assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
