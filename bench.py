@@ -365,6 +365,8 @@ def run_cuda(args):
                            "timing": "CUDA events per C-ABI call on the launching stream, mean over steps, max over ranks"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "wall_s_timed_region": t_wall,
                 "passes": passes, "roofline": roofline}
+        if world == 1 and args.extras:
+            line["extras"] = run_extras(torch, ctx, w, pos, vel, mass, acc)
         if world == 1 and not args.no_cpu_baseline:
             import oracle
             oracle.build()
@@ -374,6 +376,45 @@ def run_cuda(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def run_extras(torch, ctx, w, pos, vel, mass, acc):
+    """Device times of the NEXT rows (SURVEY.md §8f) on the same workload, outside the timed step:
+    jerk, potential, neighbour search + components, one FSI cycle.  ms per call, 2 calls each after
+    one warm-up, CUDA events on the launching stream."""
+    n = w.n
+    r_h = 1.30477                                       # Plummer half-mass radius for a_p = 1
+    # r_ngb = 1e-3 pc, r_ngb,max = 0.1 pc (PAPER.md:L255) in a cluster of r_h = 3.1 pc (PAPER.md:L820)
+    par = dict(r_ngb=1e-3 / 3.1 * r_h, r_ngb_max=0.1 / 3.1 * r_h, tau=2.0 ** -10, C=0.5)
+    out = {"n": n, "neighbour_parameters": par}
+    cnt = torch.zeros(n, dtype=torch.int32, device=pos.device)
+    lst = torch.full((n, 16), -1, dtype=torch.int32, device=pos.device)
+    jerk = torch.zeros_like(acc)
+    p2, v2 = pos.clone(), vel.clone()
+    calls = {
+        "jerk": lambda: ctx.jerk(pos, vel, mass, w.G, w.eps, out=jerk),
+        "potential": lambda: ctx.potential(pos, mass, w.G, w.eps, want_phi=False),
+        "neighbours": lambda: ctx.neighbours(pos, vel, mass, w.G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"],
+                                             cap=16, out=(cnt, lst)),
+        "components": lambda: ctx.components(cnt, lst),
+        "fsi_step": lambda: ctx.fsi_step(p2, v2, mass, w.G, max(w.eps, 1e-4), 2.0 ** -12),
+    }
+    for name, fn in calls.items():
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        fn(); fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 2
+        out[name] = {"ms": ms}
+        if name in ("jerk", "potential", "neighbours"):
+            out[name]["interactions_per_s"] = float(n) * n / (ms * 1e-3)
+        if name == "fsi_step":
+            out[name]["interactions_per_s"] = 4.0 * n * n / (ms * 1e-3)     # four O(N^2) sums (PAPER.md:L99)
+    out["neighbours"]["pairs_found"] = int(cnt.sum().item())
+    return out
 
 
 # --------------------------------------------------------------------------------------
@@ -454,6 +495,7 @@ def main():
     ap.add_argument("--ref-sinks", type=int, default=1024, help="oracle sample size (sinks) per reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--n", type=int, default=0, help="override the workload's N (profiling aid; NOT the benchmark configuration)")
+    ap.add_argument("--extras", action="store_true", help="also time the NEXT rows (jerk, potential, neighbours, components, one FSI cycle) once, outside the timed step")
     ap.add_argument("--sweep", action="store_true", help="small-active-set sweep of configs 2 and 3 (us per call); prints one JSON line")
     ap.add_argument("--no-fp64-probe", action="store_true", help="skip the register-only FP64-pipe peak probe")
     args = ap.parse_args()
