@@ -1,26 +1,32 @@
-// bifrost.cu - sm_100a kernels and C ABI (include/bifrost.h) of the BIFROST direct-summation
-// force path: acc (Eq. 6/12), grad (Eq. 9/13), dtmin (Eq. 21/22), pn1 (§3.8) of
-// arXiv:2210.02472.  See DESIGN.md for the kernel design and the roofline that bounds it.
+// bifrost.cu - the single translation unit of libbifrost.so: sm_100a kernels and the C ABI
+// (include/bifrost.h) of the BIFROST direct-summation force path of arXiv:2210.02472 - acc
+// (Eq. 6/12), grad (Eq. 9/13), dtmin (Eq. 21/22), pn1 (§3.8) - and the NEXT rows built on them.
+// See DESIGN.md for the kernel design and the roofline that bounds it.
+//
+// Layout of the source (all device code lives in anonymous namespaces of this one TU):
+//   common.cuh        constants, rsqrt seed, cp.async helpers, SrcArrays, Geom
+//   policies.cuh      AccPassT / GradPassT / DtPassT / PotPassT: record, pair(), store(), finish()
+//   pair_kernels.cuh  pair_kernel (a2-a4, large sets), pack_kernel (a1), finish_kernel (a5+a7),
+//                     pair_fused_kernel (a1-a7 in one launch, small sets)
+//   epilogues.cuh     fixed-order W reduction, O(N) time-step criteria
+//   pn1.cuh           a6
+//   subsystems.cuh    Eq. 20 segment minimum, neighbour search (Eq. 18-19), union-find components
+//   integrator.cuh    kick / drift, level split, single-CTA FSI cycle, kinetic energy
+//   fp64_probe.cuh    measurement aid
+//   bifrost.cu        bifrost_ctx, launch geometry, the *_impl host drivers, the extern "C" API
 //
 // Design in one paragraph.  The path is bound by the FP64 ALU pipe (64 lanes/clk/SM), so the
 // inner loops are written to the minimal number of FP64-pipe instructions per pair
 // (acc 15, grad 28, dtmin 25) and everything else (shared-memory broadcast loads, the
-// MUFU.RSQ64H seed, integer clamps/selects, loop control) rides in the other issue slots.
-//   a1  pack kernels gather sources from the index list into 16-B aligned records
-//       (acc 48 B, grad 80 B, dtmin 64 B) with the mass-scaled polynomial coefficients.
-//   a2-a4  one "pair kernel" skeleton: a CTA owns T*S sinks (S per thread, in registers)
-//       and a contiguous range of source tiles; tiles are staged through shared memory with
-//       a cp.async double buffer and read back as warp-wide broadcasts (LDS.128).
-//   a5  when the source range is split across CTAs (grid.y > 1), partial results go to a
-//       [split][sink] workspace and a second kernel reduces them in fixed order.
-//   a6  pn1: BH records broadcast to all particles + a deterministic block reduction of
-//       all non-BH particles onto each BH.
-//   a7  results are scattered to out[sink id] by the last kernel of each call.
-// Reciprocal square root: y0 = MUFU.RSQ64H(r2) (relative error d ~ 2^-20), e = 1 - r2*y0^2,
-// then r2^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2) and 1/r2 = y0^2 (1 + e + e^2); truncation
-// O(e^3) ~ 1e-17.  The source record carries m, 1.5 m, 1.875 m so the polynomial yields
-// m * r2^(-3/2) directly.  r2 == 0 (a particle meeting itself at eps = 0) is handled by an
-// integer clamp of the seed's argument, which makes the pair contribute exactly 0.
+// MUFU.RSQ64H seed, integer selects, loop control) rides in the other issue slots.  A CTA owns
+// T*S sinks (S per thread, in registers) and a contiguous range of source tiles staged through
+// shared memory (cp.async double buffer, warp-wide LDS.128 broadcasts).  When the source range is
+// split across CTAs, partials go to a [split][sink] workspace and are reduced in a fixed order
+// (deterministic).  Reciprocal square root: y0 = MUFU.RSQ64H(r2) (relative error ~ 2^-20),
+// e = 1 - r2*y0^2, then r2^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2) and 1/r2 = y0^2 (1 + e + e^2);
+// truncation O(e^3) ~ 1e-17.  The source record carries m, 1.5 m, 1.875 m so the polynomial
+// yields m * r2^(-3/2) directly.  r2 never reaches 0: R2_FLOOR (or eps^2) is added, so the self
+// pair has a finite weight that multiplies a zero separation and contributes exactly 0.
 
 #include "../../include/bifrost.h"
 
@@ -30,1178 +36,17 @@
 #include <cstdlib>
 #include <cmath>
 #include <algorithm>
+#include <type_traits>
 #include <new>
 
-namespace {
-
-constexpr int TILE = 128;         // sources per shared-memory tile
-constexpr int MAX_SPLIT = 256;    // upper bound on grid.y (source-range splits)
-constexpr int TICKETS = 1024;     // >= the largest grid.x of pair_fused_kernel
-
-// ----------------------------------------------------------------------------------------
-// small device helpers
-// ----------------------------------------------------------------------------------------
-
-// Seed for r2^(-1/2): MUFU.RSQ64H looks only at the high word.  Every caller adds R2_FLOOR (or a
-// larger eps^2) to r2, so the argument is a positive normal number and the seed is finite even
-// for the self pair (r_ji = 0 exactly), whose finite weight then multiplies a zero separation.
-constexpr double R2_FLOOR = 4.909093465297727e-91;    // 2^-300: below any representable |r_ji|^2 of interest
-__device__ __forceinline__ double rsqrt_seed(double r2) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-    return y;
-}
-
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// a1 inputs: the caller's arrays a source record is gathered from (aux = acc for grad, vel for
-// dtmin / jerk, unused otherwise); src_idx == NULL means sources are particles 0..n_src-1.
-struct SrcArrays {
-    const double* pos;
-    const double* aux;
-    const double* mass;
-    const int32_t* subsys;
-    const int32_t* src_idx;
-};
-
-struct Geom {
-    int n_sink;           // number of sinks
-    int n_src;            // number of sources (valid records)
-    int tiles_per_split;  // source tiles handled by one blockIdx.y
-    int n_split;          // gridDim.y
-    int compact;          // 1: output row = sink position k, 0: output row = sink particle id
-};
-
-// ----------------------------------------------------------------------------------------
-// Pass policies.  Each defines the packed source record, the per-sink state, the pair update
-// and how a thread's result is stored.
-// ----------------------------------------------------------------------------------------
-
-// NEXT-2: with EXCL = true every record carries the subsystem code of
-// its source (-1 for a single particle) and every sink its own (-2 for a single particle, so that it
-// never matches); a pair with equal codes gets the seed y0 = 0, hence the weight 0 - one integer
-// compare and one 32-bit select per pair, nothing on the FP64 pipe.
-__device__ __forceinline__ double mask_seed(double y0, bool same) {
-    return __hiloint2double(same ? 0 : __double2hiint(y0), 0);
-}
-__device__ __forceinline__ int sink_code(const int32_t* subsys, int id) {
-    const int c = subsys[id];
-    return c < 0 ? -2 : c;
-}
-
-// source-side subsystem code: -1 for a single particle (never equal to a sink's code, which is
-// -2 for a single particle), the subsystem id otherwise
-__device__ __forceinline__ int src_code(const int32_t* subsys, int j) {
-    if (!subsys) return -1;
-    const int c = subsys[j];
-    return c < 0 ? -1 : c;
-}
-
-// a5 + a7: reduction of one sink's partials in a FIXED order, then scatter.  A group of L lanes
-// (L = 1, 2, .. 32, a power of two; lane = index in the group) shares one sink: lane l adds the
-// partials of splits l, l+L, ... in that order and a butterfly adds the lanes - an order that
-// depends only on (n_split, L), never on which CTA runs it.  All 32 lanes of a warp must call
-// (write = false for a group that shadows a sink).  The partials come from other CTAs: L2 loads.
-__device__ __forceinline__ double group_add(double v, int L) {
-    for (int off = L >> 1; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-    return v;
-}
-__device__ __forceinline__ void finish_vec3(const double* partial, double* out, double G, const Geom& g, int k, int id,
-                                            int lane, int L, bool write) {
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    for (int s = lane; s < g.n_split; s += L) {
-        const double* p = partial + 3 * ((size_t)s * g.n_sink + k);
-        sx += __ldcg(p); sy += __ldcg(p + 1); sz += __ldcg(p + 2);
-    }
-    if (L > 1) { sx = group_add(sx, L); sy = group_add(sy, L); sz = group_add(sz, L); }
-    if (write && lane == 0) {
-        double* o = out + 3 * (size_t)(g.compact ? k : id);
-        o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
-    }
-}
-
-struct AccArgs {
-    const double* pos;
-    const int32_t* subsys;
-    const int32_t* sink_idx;
-    double eps2, G;
-    double* out;        // final output [.][3]
-    double* partial;    // [split][n_sink][3]
-};
-
-template <bool EXCL>
-struct AccPassT {
-    static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
-    using Args = AccArgs;
-    struct Sink { double x, y, z; int sub; };
-    struct Acc { double x, y, z; };
-    struct Raw { double x, y, z, m; int code; };
-    // a1: gather one source (j < 0: padding record) and write its packed record
-    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
-        if (j >= 0) {
-            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
-            w.m = s.mass[j]; w.code = EXCL ? src_code(s.subsys, j) : 0;
-        } else { w.x = w.y = w.z = w.m = 0.0; w.code = 0; }
-    }
-    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
-        o[0] = make_double2(w.x, w.y);
-        o[1] = make_double2(w.z, w.m);
-        o[2] = make_double2(1.5 * w.m, 1.875 * w.m);
-        if (EXCL) o[3] = make_double2(__hiloint2double(0, w.code), 0.0);
-    }
-    __device__ static void load_sink(const Args& a, int id, Sink& s) {
-        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2];
-        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
-    }
-    __device__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
-    // 15 FP64-pipe instructions: 3 DADD, 3 DFMA (r2), DMUL t, DFMA e, 2 DFMA poly, 2 DMUL, 3 DFMA.
-    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
-        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
-        double y0 = rsqrt_seed(r2);
-        if (EXCL) y0 = mask_seed(y0, __double2loint(r[6]) == s.sub);
-        const double t = y0 * y0;
-        const double e = fma(-r2, t, 1.0);
-        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 3/2 e + 15/8 e^2)
-        const double w = (y0 * t) * pm;                       // m / s^3
-        c.x = fma(w, dx, c.x); c.y = fma(w, dy, c.y); c.z = fma(w, dz, c.z);
-    }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
-        if (g.n_split == 1) {
-            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
-            o[0] = a.G * c.x; o[1] = a.G * c.y; o[2] = a.G * c.z;
-        } else {
-            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
-            o[0] = c.x; o[1] = c.y; o[2] = c.z;
-        }
-    }
-    static constexpr bool ALWAYS_FINISH = false;
-    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
-        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
-    }
-};
-
-using AccPass = AccPassT<false>;
-
-struct GradArgs {
-    const double* pos;
-    const double* acc;
-    const int32_t* subsys;
-    const int32_t* sink_idx;
-    double eps2, G;
-    double* out;
-    double* partial;
-};
-
-template <bool EXCL>
-struct GradPassT {
-    static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
-    using Args = GradArgs;
-    struct Sink { double x, y, z, ax, ay, az; int sub; };
-    struct Acc { double ux, uy, uz, wx, wy, wz; };   // U = sum w a_ji,  W = sum w (a_ji.r_ji)/s^2 r_ji
-    struct Raw { double x, y, z, ax, ay, az, m; int code; };
-    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
-        if (j >= 0) {
-            const size_t b = 3 * (size_t)j;
-            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
-            w.ax = s.aux[b]; w.ay = s.aux[b + 1]; w.az = s.aux[b + 2];
-            w.m = s.mass[j]; w.code = src_code(s.subsys, j);
-        } else { w.x = w.y = w.z = w.ax = w.ay = w.az = w.m = 0.0; w.code = 0; }
-    }
-    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
-        o[0] = make_double2(w.x, w.y);
-        o[1] = make_double2(w.z, w.ax);
-        o[2] = make_double2(w.ay, w.az);
-        o[3] = make_double2(w.m, 1.5 * w.m);
-        o[4] = make_double2(1.875 * w.m, __hiloint2double(0, w.code));
-    }
-    __device__ static void load_sink(const Args& a, int id, Sink& s) {
-        const size_t o = 3 * (size_t)id;
-        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
-        s.ax = a.acc[o]; s.ay = a.acc[o + 1]; s.az = a.acc[o + 2];
-        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
-    }
-    __device__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
-    // 28 FP64-pipe instructions; C_i = U - 3 W is formed once per sink in store().
-    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
-        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
-        const double bx = r[3] - s.ax, by = r[4] - s.ay, bz = r[5] - s.az;       // a_ji
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
-        const double q = fma(bx, dx, fma(by, dy, bz * dz));                       // a_ji . r_ji
-        double y0 = rsqrt_seed(r2);
-        if (EXCL) y0 = mask_seed(y0, __double2loint(r[9]) == s.sub);
-        const double t = y0 * y0;
-        const double e = fma(-r2, t, 1.0);
-        const double pm = fma(fma(e, r[8], r[7]), e, r[6]);
-        const double w = (y0 * t) * pm;                                           // m / s^3
-        const double y2 = fma(t, fma(e, e, e), t);                                // 1 / s^2
-        const double v = (w * y2) * q;                                            // m (a_ji.r_ji) / s^5
-        c.ux = fma(w, bx, c.ux); c.uy = fma(w, by, c.uy); c.uz = fma(w, bz, c.uz);
-        c.wx = fma(v, dx, c.wx); c.wy = fma(v, dy, c.wy); c.wz = fma(v, dz, c.wz);
-    }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
-        const double cx = fma(-3.0, c.wx, c.ux), cy = fma(-3.0, c.wy, c.uy), cz = fma(-3.0, c.wz, c.uz);
-        if (g.n_split == 1) {
-            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
-            o[0] = a.G * cx; o[1] = a.G * cy; o[2] = a.G * cz;
-        } else {
-            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
-            o[0] = cx; o[1] = cy; o[2] = cz;
-        }
-    }
-    static constexpr bool ALWAYS_FINISH = false;
-    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
-        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
-    }
-};
-
-using GradPass = GradPassT<false>;
-
-struct DtArgs {
-    const double* pos;
-    const double* vel;
-    const double* mass;
-    const int32_t* subsys;
-    const int32_t* sink_idx;
-    double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
-    int32_t* pid;      // [split][2][n_sink]  their source ids
-    double G, eta_ff, eta_fb;
-    double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
-};
-
-// ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
-// the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
-template <bool ASC, bool EXCL>
-struct DtPassT {
-    static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
-    using Args = DtArgs;
-    struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
-    // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
-    struct Acc { double kff, kfb; int jff, jfb; };
-    struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
-    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
-        if (j >= 0) {
-            const size_t b = 3 * (size_t)j;
-            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
-            w.vx = s.aux[b]; w.vy = s.aux[b + 1]; w.vz = s.aux[b + 2];
-            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
-        } else { w.x = w.y = w.z = w.vx = w.vy = w.vz = w.m = 0.0; w.j = 0; w.code = 0; }
-    }
-    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
-        o[0] = make_double2(w.x, w.y);
-        o[1] = make_double2(w.z, w.m);
-        o[2] = make_double2(w.vx, w.vy);
-        o[3] = make_double2(w.vz, __hiloint2double(w.code, w.j));
-    }
-    __device__ static void load_sink(const Args& a, int id, Sink& s) {
-        const size_t o = 3 * (size_t)id;
-        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
-        s.vx = a.vel[o]; s.vy = a.vel[o + 1]; s.vz = a.vel[o + 2];
-        s.m = a.mass[id]; s.id = id;
-        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
-    }
-    __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
-    // FP64-pipe instructions: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
-    // 2 DMUL keys = 23, plus 2 (ASC) or 4 DSETP.
-    __device__ __forceinline__ static void pair(const Args&, const Sink& s, Acc& c, const double* __restrict__ r) {
-        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
-        const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
-        const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
-        const int jid = __double2loint(r[7]);
-        const double y0 = rsqrt_seed(r2);
-        const double t = y0 * y0;
-        const double e = fma(-r2, t, 1.0);
-        const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
-        const double y3 = (y0 * t) * p3;
-        const double y2 = fma(t, fma(e, e, e), t);
-        double kff = (s.m + r[3]) * y3;
-        double kfb = v2 * y2;
-        // j != i (Eq. 21, 22) and, with EXCL, not in the sink's subsystem
-        const bool other = EXCL ? ((jid != s.id) & (__double2hiint(r[7]) != s.sub)) : (jid != s.id);
-        if (ASC) {
-            const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
-            c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
-            c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
-        } else {
-            if (!other) { kff = -1.0; kfb = -1.0; }
-            if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
-            if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
-        }
-    }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
-        const size_t o = (size_t)split * 2 * g.n_sink + k;
-        a.pkey[o] = c.kff; a.pkey[o + g.n_sink] = c.kfb;
-        a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
-    }
-    // dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
-    // Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
-    static constexpr bool ALWAYS_FINISH = true;
-    __device__ static void finish(const Args& a, const Geom& g, int k, int i, int lane, int L, bool write) {
-        double kb[2] = {0.0, 0.0};
-        int jb[2] = {-1, -1};
-        for (int s = lane; s < g.n_split; s += L) {
-            for (int w = 0; w < 2; ++w) {
-                const size_t o = ((size_t)s * 2 + w) * g.n_sink + k;
-                const double key = __ldcg(a.pkey + o);
-                const int j = __ldcg(a.pid + o);
-                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
-            }
-        }
-        for (int off = L >> 1; off > 0; off >>= 1) {      // (max key, then min id) is order-independent
-            for (int w = 0; w < 2; ++w) {
-                const double key = __shfl_xor_sync(0xffffffffu, kb[w], off);
-                const int j = __shfl_xor_sync(0xffffffffu, jb[w], off);
-                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
-            }
-        }
-        if (!write || lane != 0) return;
-        const double* pos = a.pos; const double* vel = a.vel;
-        const int row = g.compact ? k : i;
-        const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        double tff = inf, tfb = inf;
-        if (jb[0] >= 0) {
-            const int j = jb[0];
-            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            const double r = sqrt(r2);
-            tff = a.eta_ff * sqrt(__dmul_rn(r2, r) / (a.G * (a.mass[i] + a.mass[j])));
-        }
-        if (jb[1] >= 0) {
-            const int j = jb[1];
-            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-            const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
-                         uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
-            tfb = __dmul_rn(a.eta_fb, sqrt(r2)) / sqrt(v2);
-        }
-        if (a.dt_ff) a.dt_ff[row] = tff;
-        if (a.dt_fb) a.dt_fb[row] = tfb;
-        if (a.j_ff) a.j_ff[row] = jb[0];
-        if (a.j_fb) a.j_fb[row] = jb[1];
-    }
-};
-
-using DtPass = DtPassT<false, false>;
-using DtPassAsc = DtPassT<true, false>;
-
-struct PotArgs {
-    const double* pos;
-    const int32_t* subsys;
-    const int32_t* sink_idx;
-    double eps2, G;
-    double* out;        // phi at [.]
-    double* partial;    // [split][n_sink]
-};
-
-// Potential (Eq. 4 second term, Eq. 68): p_i = sum_j m_j / s_ij; phi_i = -G p_i.
-// 1/s = y0 (1 + e/2 + 3/8 e^2); the record carries m, m/2, 3m/8 and the source id, because here
-// the self pair does not multiply a zero separation and must be dropped by id (integer select).
-template <bool EXCL>
-struct PotPassT {
-    static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
-    using Args = PotArgs;
-    struct Sink { double x, y, z; int id, sub; };
-    struct Acc { double p; };
-    struct Raw { double x, y, z, m; int j, code; };
-    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
-        if (j >= 0) {
-            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
-            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
-        } else { w.x = w.y = w.z = w.m = 0.0; w.j = -1; w.code = 0; }
-    }
-    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
-        o[0] = make_double2(w.x, w.y);
-        o[1] = make_double2(w.z, w.m);
-        o[2] = make_double2(0.5 * w.m, 0.375 * w.m);
-        o[3] = make_double2(__hiloint2double(w.code, w.j), 0.0);
-    }
-    __device__ static void load_sink(const Args& a, int id, Sink& s) {
-        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2]; s.id = id;
-        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
-    }
-    __device__ static void init(Acc& c) { c.p = 0.0; }
-    // 12 FP64-pipe instructions: 3 DADD, 3 DFMA, DMUL, DFMA, 2 DFMA, DMUL, DADD.
-    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
-        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
-        const double y0 = rsqrt_seed(r2);
-        const double t = y0 * y0;
-        const double e = fma(-r2, t, 1.0);
-        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 1/2 e + 3/8 e^2)
-        double w = y0 * pm;                                   // m / s
-        if (__double2loint(r[6]) == s.id) w = 0.0;            // j != i
-        if (EXCL && __double2hiint(r[6]) == s.sub) w = 0.0;   // same subsystem
-        c.p += w;
-    }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
-        if (g.n_split == 1) a.out[g.compact ? k : id] = -a.G * c.p;
-        else a.partial[(size_t)split * g.n_sink + k] = c.p;
-    }
-    static constexpr bool ALWAYS_FINISH = false;
-    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
-        double s = 0.0;
-        for (int q = lane; q < g.n_split; q += L) s += __ldcg(a.partial + (size_t)q * g.n_sink + k);     // fixed order
-        if (L > 1) s = group_add(s, L);
-        if (write && lane == 0) a.out[g.compact ? k : id] = -a.G * s;
-    }
-};
-
-using PotPass = PotPassT<false>;
-
-// ----------------------------------------------------------------------------------------
-// a2-a4: the pair kernel.  grid = (ceil(n_sink / (T*S)), n_split); T threads, S sinks per thread,
-// MINB resident CTAs per SM, inner loop unrolled UNR times.
-// ----------------------------------------------------------------------------------------
-template <class P, int S, int T, int MINB, int UNR>
-__global__ void __launch_bounds__(T, MINB)
-pair_kernel(const typename P::Args a, const Geom g, const double* __restrict__ src_rec) {
-    constexpr int REC = P::REC;
-    constexpr int CHUNKS = TILE * REC * 8 / 16;            // 16-B chunks per tile
-    __shared__ __align__(16) double sm[2][TILE * REC];
-
-    typename P::Sink sink[S];
-    typename P::Acc accu[S];
-    int ids[S];
-    const int kbase = blockIdx.x * (T * S) + threadIdx.x;
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        const int kk = k < g.n_sink ? k : g.n_sink - 1;      // tail threads shadow the last sink
-        ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
-        P::load_sink(a, ids[s], sink[s]);
-        P::init(accu[s]);
-    }
-
-    const int n_tiles = (g.n_src + TILE - 1) / TILE;
-    const int tile0 = blockIdx.y * g.tiles_per_split;
-    const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
-
-    auto load_tile = [&](int tile, int buf) {
-        const double* gsrc = src_rec + (size_t)tile * TILE * REC;
-        for (int ch = threadIdx.x; ch < CHUNKS; ch += T) cp_async16(&sm[buf][2 * ch], gsrc + 2 * ch);
-        cp_async_commit();
-    };
-
-    if (tile0 < tile1) load_tile(tile0, 0);
-    for (int tile = tile0; tile < tile1; ++tile) {
-        const int buf = (tile - tile0) & 1;
-        if (tile + 1 < tile1) { load_tile(tile + 1, buf ^ 1); cp_async_wait<1>(); }
-        else cp_async_wait<0>();
-        __syncthreads();
-        const int cnt = min(TILE, g.n_src - tile * TILE);
-        const double* __restrict__ tb = sm[buf];
-#pragma unroll UNR
-        for (int jj = 0; jj < cnt; ++jj) {
-            double r[REC];
-#pragma unroll
-            for (int q = 0; q < REC; q += 2) {
-                const double2 v = *reinterpret_cast<const double2*>(tb + jj * REC + q);
-                r[q] = v.x; r[q + 1] = v.y;
-            }
-#pragma unroll
-            for (int s = 0; s < S; ++s) P::pair(a, sink[s], accu[s], r);
-        }
-        __syncthreads();
-    }
-
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
-    }
-}
-
-// ----------------------------------------------------------------------------------------
-// a1: pack kernels (gather sources through the index list into aligned records; the tail of
-// the last tile is zero-filled so the cp.async stage never reads undefined memory).
-// ----------------------------------------------------------------------------------------
-
-template <class P>
-__global__ void pack_kernel(int n_src, int n_pad, const SrcArrays src, double* __restrict__ rec) {
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l >= n_pad) return;
-    typename P::Raw w;
-    P::fetch(src, l < n_src ? (src.src_idx ? src.src_idx[l] : l) : -1, w);
-    P::emit(w, reinterpret_cast<double2*>(rec + (size_t)l * P::REC));
-}
-
-// ----------------------------------------------------------------------------------------
-// a5 + a7 as a kernel of its own (large sink sets): P::finish for every sink.
-// ----------------------------------------------------------------------------------------
-template <class P>
-__global__ void finish_kernel(const typename P::Args a, const Geom g) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= g.n_sink) return;
-    P::finish(a, g, k, a.sink_idx ? a.sink_idx[k] : k, 0, 1, true);
-}
-
-// ----------------------------------------------------------------------------------------
-// a1-a7 in ONE launch for small sink sets (the faster levels of the time-step hierarchy,
-// PAPER.md:L295): each CTA gathers its source tiles straight from the caller's arrays (the next
-// tile's loads are in flight while the current one is evaluated), and when the source range is
-// split across blockIdx.y the CTA that arrives last at a ticket (one per blockIdx.x) reduces all
-// partials in split order - so the result does not depend on which CTA that is (deterministic) and
-// no second or third launch is needed.  The ticket resets itself (CUDA-graph replay safe).
-// ----------------------------------------------------------------------------------------
-template <class P, int S, int T, int MINB, int UNR>
-__global__ void __launch_bounds__(T, MINB)
-pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, unsigned* __restrict__ ticket) {
-    static_assert(T >= TILE, "one gathering thread per source of a tile");
-    constexpr int REC = P::REC;
-    __shared__ __align__(16) double sm[2][TILE * REC];
-    __shared__ int s_last;
-
-    typename P::Sink sink[S];
-    typename P::Acc accu[S];
-    int ids[S];
-    const int kbase = blockIdx.x * (T * S) + threadIdx.x;
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        const int kk = k < g.n_sink ? k : g.n_sink - 1;
-        ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
-        P::load_sink(a, ids[s], sink[s]);
-        P::init(accu[s]);
-    }
-
-    const int n_tiles = (g.n_src + TILE - 1) / TILE;
-    const int tile0 = blockIdx.y * g.tiles_per_split;
-    const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
-
-    typename P::Raw raw;
-    auto fetch_tile = [&](int tile) {
-        const int l = tile * TILE + threadIdx.x;
-        if (threadIdx.x < TILE) P::fetch(src, l < g.n_src ? (src.src_idx ? src.src_idx[l] : l) : -1, raw);
-    };
-    auto emit_tile = [&](int buf) {
-        if (threadIdx.x < TILE) P::emit(raw, reinterpret_cast<double2*>(sm[buf] + threadIdx.x * REC));
-    };
-
-    if (tile0 < tile1) { fetch_tile(tile0); emit_tile(0); }
-    for (int tile = tile0; tile < tile1; ++tile) {
-        const int buf = (tile - tile0) & 1;
-        __syncthreads();                       // sm[buf] complete; everyone is done with sm[buf ^ 1]
-        const bool more = tile + 1 < tile1;
-        if (more) fetch_tile(tile + 1);
-        const int cnt = min(TILE, g.n_src - tile * TILE);
-        const double* __restrict__ tb = sm[buf];
-#pragma unroll UNR
-        for (int jj = 0; jj < cnt; ++jj) {
-            double r[REC];
-#pragma unroll
-            for (int q = 0; q < REC; q += 2) {
-                const double2 v = *reinterpret_cast<const double2*>(tb + jj * REC + q);
-                r[q] = v.x; r[q + 1] = v.y;
-            }
-#pragma unroll
-            for (int s = 0; s < S; ++s) P::pair(a, sink[s], accu[s], r);
-        }
-        if (more) emit_tile(buf ^ 1);
-    }
-
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
-    }
-    if (g.n_split == 1) {
-        if (P::ALWAYS_FINISH) {                // a thread finishes the sinks it stored itself
-#pragma unroll
-            for (int s = 0; s < S; ++s) {
-                const int k = kbase + s * T;
-                if (k < g.n_sink) P::finish(a, g, k, ids[s], 0, 1, true);
-            }
-        }
-        return;
-    }
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(&ticket[blockIdx.x], 1u) == gridDim.y - 1);
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    // the last CTA reduces: L lanes per sink when this CTA's sinks leave threads to spare
-    const int base = blockIdx.x * (T * S);
-    const int n_local = min(T * S, g.n_sink - base);
-    int L = 1;
-    while (L < 32 && n_local * (2 * L) <= T) L *= 2;
-    if (L == 1) {
-#pragma unroll
-        for (int s = 0; s < S; ++s) {
-            const int k = kbase + s * T;
-            if (k < g.n_sink) P::finish(a, g, k, ids[s], 0, 1, true);
-        }
-    } else {
-        const int q = threadIdx.x / L;
-        const bool live = q < n_local;
-        const int k = base + (live ? q : 0);
-        P::finish(a, g, k, a.sink_idx ? a.sink_idx[k] : k, threadIdx.x % L, L, live);
-    }
-    if (threadIdx.x == 0) ticket[blockIdx.x] = 0;
-}
-
-// W = 1/2 sum_{i in sinks} m_i phi_i in two fixed-order stages (deterministic; no atomics).
-constexpr int WSUM_THREADS = 256;
-constexpr int WSUM_PER_BLOCK = 4096;
-__device__ __forceinline__ double block_sum_fixed(double v) {
-    __shared__ double red[WSUM_THREADS / 32];
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double s = 0.0;
-    if (threadIdx.x == 0)
-        for (int w = 0; w < WSUM_THREADS / 32; ++w) s += red[w];
-    return s;   // valid in thread 0
-}
-__global__ void __launch_bounds__(WSUM_THREADS)
-wsum_stage1_kernel(int n_sink, const int32_t* __restrict__ sink_idx, int compact_phi, const double* __restrict__ mass,
-                   const double* __restrict__ phi, double* __restrict__ block_part) {
-    const int base = blockIdx.x * WSUM_PER_BLOCK;
-    double v = 0.0;
-    for (int q = threadIdx.x; q < WSUM_PER_BLOCK; q += WSUM_THREADS) {
-        const int k = base + q;
-        if (k < n_sink) {
-            const int id = sink_idx ? sink_idx[k] : k;
-            v += mass[id] * phi[compact_phi ? k : id];
-        }
-    }
-    const double s = block_sum_fixed(v);
-    if (threadIdx.x == 0) block_part[blockIdx.x] = s;
-}
-__global__ void __launch_bounds__(WSUM_THREADS)
-wsum_stage2_kernel(int n_blocks, const double* __restrict__ block_part, double* __restrict__ out_W) {
-    double v = 0.0;
-    for (int q = threadIdx.x; q < n_blocks; q += WSUM_THREADS) v += block_part[q];
-    const double s = block_sum_fixed(v);
-    if (threadIdx.x == 0) *out_W = 0.5 * s;
-}
-
-// O(N) time-step criteria, Eq. 24, 26, 27, 29; IEEE sqrt / cbrt / division.
-__global__ void criteria_kernel(int n_sink, const int32_t* __restrict__ sink_idx, const double* __restrict__ vel,
-                                const double* __restrict__ acc, const double* __restrict__ grad,
-                                const double* __restrict__ jerk, double eta, double eta_grad, double eta_jerk,
-                                double* __restrict__ dt_va, double* __restrict__ dt_gradv, double* __restrict__ dt_grada,
-                                double* __restrict__ dt_jerk, double* __restrict__ inout_dt) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_sink) return;
-    const int i = sink_idx ? sink_idx[k] : k;
-    const size_t o = 3 * (size_t)i;
-    const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    auto norm = [](const double* p) {
-        return sqrt(__dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2])));
-    };
-    const double v = norm(vel + o), a = norm(acc + o);
-    double best = inout_dt ? inout_dt[i] : inf;
-    const double t_va = (a == 0.0) ? inf : __dmul_rn(eta, v) / a;
-    if (dt_va) dt_va[i] = t_va;
-    best = fmin(best, t_va);
-    if (grad) {
-        const double gp = norm(grad + o) / 24.0;
-        const double t_gv = (gp == 0.0) ? inf : eta_grad * cbrt(v / gp);
-        const double t_ga = (gp == 0.0) ? inf : eta_grad * sqrt(a / gp);
-        if (dt_gradv) dt_gradv[i] = t_gv;
-        if (dt_grada) dt_grada[i] = t_ga;
-        best = fmin(best, fmin(t_gv, t_ga));
-    }
-    if (jerk) {
-        const double j = norm(jerk + o);
-        const double t_j = (j == 0.0) ? inf : __dmul_rn(eta_jerk, a) / j;
-        if (dt_jerk) dt_jerk[i] = t_j;
-        best = fmin(best, t_j);
-    }
-    if (inout_dt) inout_dt[i] = best;
-}
-
-// ----------------------------------------------------------------------------------------
-// a6: PN1.0 pair term (§3.8).  Standard two-body 1PN acceleration in harmonic coordinates.
-// ----------------------------------------------------------------------------------------
-struct Body { double x, y, z, m, vx, vy, vz; };
-
-__device__ __forceinline__ Body load_body(const double* pos, const double* vel, const double* mass, int id) {
-    Body b;
-    const size_t o = 3 * (size_t)id;
-    b.x = pos[o]; b.y = pos[o + 1]; b.z = pos[o + 2];
-    b.vx = vel[o]; b.vy = vel[o + 1]; b.vz = vel[o + 2];
-    b.m = mass[id];
-    return b;
-}
-
-// acceleration of body `i` due to body `j`, 1/c^2 part only
-__device__ __forceinline__ void pn1_pair(const Body& i, const Body& j, double G, double inv_c2,
-                                         double& fx, double& fy, double& fz) {
-    const double rx = i.x - j.x, ry = i.y - j.y, rz = i.z - j.z;
-    const double r2 = rx * rx + ry * ry + rz * rz;
-    const double rinv = 1.0 / sqrt(r2);
-    const double nx = rx * rinv, ny = ry * rinv, nz = rz * rinv;
-    const double nvi = nx * i.vx + ny * i.vy + nz * i.vz;
-    const double nvj = nx * j.vx + ny * j.vy + nz * j.vz;
-    const double vivi = i.vx * i.vx + i.vy * i.vy + i.vz * i.vz;
-    const double vjvj = j.vx * j.vx + j.vy * j.vy + j.vz * j.vz;
-    const double vivj = i.vx * j.vx + i.vy * j.vy + i.vz * j.vz;
-    const double A = G * (5.0 * i.m + 4.0 * j.m) * rinv + 1.5 * nvj * nvj - vivi + 4.0 * vivj - 2.0 * vjvj;
-    const double B = 4.0 * nvi - 3.0 * nvj;
-    const double pref = G * j.m * inv_c2 * (rinv * rinv);
-    fx += pref * (nx * A + B * (i.vx - j.vx));
-    fy += pref * (ny * A + B * (i.vy - j.vy));
-    fz += pref * (nz * A + B * (i.vz - j.vz));
-}
-
-__global__ void pn1_flag_kernel(int n_bh, const int32_t* __restrict__ bh_idx, unsigned char* __restrict__ is_bh) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < n_bh) is_bh[bh_idx[b]] = 1;
-}
-
-// every particle i <- all BHs j != i (BH records staged through shared memory)
-constexpr int PN_THREADS = 128;
-__global__ void __launch_bounds__(PN_THREADS)
-pn1_from_bh_kernel(int n, int n_bh, const int32_t* __restrict__ bh_idx, const double* __restrict__ pos,
-                   const double* __restrict__ vel, const double* __restrict__ mass,
-                   const int32_t* __restrict__ subsys, double G, double inv_c2, double* __restrict__ out) {
-    __shared__ Body sb[PN_THREADS];
-    __shared__ int sid[PN_THREADS];
-    __shared__ int ssub[PN_THREADS];
-    const int i = blockIdx.x * PN_THREADS + threadIdx.x;
-    const int ii = i < n ? i : n - 1;
-    const Body me = load_body(pos, vel, mass, ii);
-    const int my_sub = subsys ? sink_code(subsys, ii) : -2;
-    double fx = 0.0, fy = 0.0, fz = 0.0;
-    for (int b0 = 0; b0 < n_bh; b0 += PN_THREADS) {
-        const int b = b0 + threadIdx.x;
-        if (b < n_bh) {
-            sid[threadIdx.x] = bh_idx[b];
-            sb[threadIdx.x] = load_body(pos, vel, mass, bh_idx[b]);
-            ssub[threadIdx.x] = src_code(subsys, bh_idx[b]);
-        }
-        __syncthreads();
-        const int cnt = min(PN_THREADS, n_bh - b0);
-        for (int q = 0; q < cnt; ++q)
-            if (sid[q] != ii && ssub[q] != my_sub) pn1_pair(me, sb[q], G, inv_c2, fx, fy, fz);
-        __syncthreads();
-    }
-    if (i < n) { out[3 * (size_t)i] = fx; out[3 * (size_t)i + 1] = fy; out[3 * (size_t)i + 2] = fz; }
-}
-
-// each BH b <- all non-BH particles of one chunk; deterministic block reduction
-constexpr int PN_RED_THREADS = 256;
-__global__ void __launch_bounds__(PN_RED_THREADS)
-pn1_on_bh_kernel(int n, int chunk, const int32_t* __restrict__ bh_idx, const unsigned char* __restrict__ is_bh,
-                 const double* __restrict__ pos, const double* __restrict__ vel, const double* __restrict__ mass,
-                 const int32_t* __restrict__ subsys, double G, double inv_c2,
-                 double* __restrict__ partial /*[n_bh][n_chunks][3]*/) {
-    __shared__ double red[3][PN_RED_THREADS / 32];
-    const int b = blockIdx.y;
-    const Body me = load_body(pos, vel, mass, bh_idx[b]);
-    const int my_sub = subsys ? sink_code(subsys, bh_idx[b]) : -2;
-    const int j0 = blockIdx.x * chunk, j1 = min(j0 + chunk, n);
-    double fx = 0.0, fy = 0.0, fz = 0.0;
-    for (int j = j0 + threadIdx.x; j < j1; j += PN_RED_THREADS) {
-        if (is_bh[j] || src_code(subsys, j) == my_sub) continue;
-        const Body o = load_body(pos, vel, mass, j);
-        pn1_pair(me, o, G, inv_c2, fx, fy, fz);
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        fx += __shfl_down_sync(0xffffffffu, fx, off);
-        fy += __shfl_down_sync(0xffffffffu, fy, off);
-        fz += __shfl_down_sync(0xffffffffu, fz, off);
-    }
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { red[0][warp] = fx; red[1][warp] = fy; red[2][warp] = fz; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double sx = 0.0, sy = 0.0, sz = 0.0;
-        for (int w = 0; w < PN_RED_THREADS / 32; ++w) { sx += red[0][w]; sy += red[1][w]; sz += red[2][w]; }
-        double* o = partial + 3 * ((size_t)b * gridDim.x + blockIdx.x);
-        o[0] = sx; o[1] = sy; o[2] = sz;
-    }
-}
-
-__global__ void pn1_bh_finalize_kernel(int n_bh, int n_chunks, const int32_t* __restrict__ bh_idx,
-                                       const double* __restrict__ partial, double* __restrict__ out) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= n_bh) return;
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    for (int c = 0; c < n_chunks; ++c) {
-        const double* p = partial + 3 * ((size_t)b * n_chunks + c);
-        sx += p[0]; sy += p[1]; sz += p[2];
-    }
-    double* o = out + 3 * (size_t)bh_idx[b];
-    o[0] += sx; o[1] += sy; o[2] += sz;
-}
-
-// NEXT-2, Eq. 20: eps_i = min_{j in S} eps_j.  Non-negative doubles order like their
-// bit patterns read as unsigned integers, so the segment minimum is an integer atomicMin: exact and
-// independent of the order in which members arrive (deterministic).
-__global__ void smin_fill_kernel(int n, unsigned long long* __restrict__ smin) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) smin[i] = 0x7ff0000000000000ULL;     // +inf
-}
-__global__ void smin_reduce_kernel(int n, const int32_t* __restrict__ subsys, const double* __restrict__ dt,
-                                   unsigned long long* __restrict__ smin) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int s = subsys[i];
-    if (s >= 0) atomicMin(&smin[s], (unsigned long long)__double_as_longlong(dt[i]));
-}
-__global__ void smin_apply_kernel(int n, const int32_t* __restrict__ subsys, const unsigned long long* __restrict__ smin,
-                                  double* __restrict__ dt) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int s = subsys[i];
-    if (s >= 0) dt[i] = __longlong_as_double((long long)smin[s]);
-}
-
-// ----------------------------------------------------------------------------------------
-// NEXT-3: neighbour search, §3.4, Eq. 18-19, and subsystem construction.
-// A floating-point test decides an integer result here (is j a neighbour of i), so the decision is
-// taken in plain IEEE fp64 operation by operation (no contraction, correctly rounded sqrt and
-// division) in the order the paper states it: r_ij < r_ngb,max first, then the two-body a, e,
-// then Eq. 18 (bound) or Eq. 19 (unbound).  Only a conservative distance pre-filter runs on the
-// fast path (7 FP64 instructions per pair: the contracted r^2 against r_ngb,max^2 (1 + 1e-10)).
-// ----------------------------------------------------------------------------------------
-struct NgbArgs {
-    const double* pos; const double* vel; const double* mass;
-    const int32_t* sink_idx;
-    double G, r_ngb, r_ngb_max, tau, C, r2_guard;
-    int cap;
-    int32_t* out_count; int32_t* out_list;     // rows at sink ids (or sink positions when compact)
-    int32_t* pcount; int32_t* plist;           // [split][n_sink], [split][n_sink][cap]
-};
-
-__device__ __noinline__ bool ngb_exact(const NgbArgs& a, double dx, double dy, double dz, double ux, double uy, double uz,
-                                       double mi, double mj) {
-    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-    const double r = sqrt(r2);
-    if (!(r < a.r_ngb_max)) return false;
-    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
-    const double mu = __dmul_rn(a.G, __dadd_rn(mi, mj));
-    const double E = __dsub_rn(__dmul_rn(0.5, v2), mu / r);             // two-body orbital energy per reduced mass
-    if (E < 0.0) {                                                       // bound: Eq. 18
-        const double sma = -mu / __dmul_rn(2.0, E);
-        return (sma < a.r_ngb) || (r < a.r_ngb);
-    }
-    const double hx = __dsub_rn(__dmul_rn(dy, uz), __dmul_rn(dz, uy));   // h = r x v
-    const double hy = __dsub_rn(__dmul_rn(dz, ux), __dmul_rn(dx, uz));
-    const double hz = __dsub_rn(__dmul_rn(dx, uy), __dmul_rn(dy, ux));
-    const double h2 = __dadd_rn(__dadd_rn(__dmul_rn(hx, hx), __dmul_rn(hy, hy)), __dmul_rn(hz, hz));
-    double e2 = __dadd_rn(1.0, __dmul_rn(__dmul_rn(2.0, E), h2) / __dmul_rn(mu, mu));
-    if (e2 < 0.0) e2 = 0.0;
-    const double ecc = sqrt(e2);
-    const double r_peri = (h2 / mu) / __dadd_rn(1.0, ecc);               // = a (1 - e), finite for E = 0
-    if (!(r_peri < a.r_ngb)) return false;                               // Eq. 19
-    if (r < a.r_ngb) return true;
-    return __dmul_rn(a.C, r) / sqrt(v2) < a.tau;
-}
-
-template <int S, int T, int MINB>
-__global__ void __launch_bounds__(T, MINB)
-ngb_kernel(const NgbArgs a, const Geom g, const double* __restrict__ src_rec) {
-    constexpr int REC = 8;                                  // DtPass records: x y z m vx vy vz {id}
-    constexpr int CHUNKS = TILE * REC * 8 / 16;
-    __shared__ __align__(16) double sm[2][TILE * REC];
-    double sx[S], sy[S], sz[S];
-    int ids[S], cnt[S];
-    int32_t* lst[S];
-    const int kbase = blockIdx.x * (T * S) + threadIdx.x;
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        const int kk = k < g.n_sink ? k : g.n_sink - 1;
-        ids[s] = a.sink_idx ? a.sink_idx[kk] : kk;
-        sx[s] = a.pos[3 * (size_t)ids[s]]; sy[s] = a.pos[3 * (size_t)ids[s] + 1]; sz[s] = a.pos[3 * (size_t)ids[s] + 2];
-        cnt[s] = 0;
-        if (k >= g.n_sink) lst[s] = nullptr;                // tail threads shadow the last sink and write nothing
-        else if (g.n_split == 1) lst[s] = a.out_list + (size_t)(g.compact ? k : ids[s]) * a.cap;
-        else lst[s] = a.plist + ((size_t)blockIdx.y * g.n_sink + k) * a.cap;
-    }
-    const int n_tiles = (g.n_src + TILE - 1) / TILE;
-    const int tile0 = blockIdx.y * g.tiles_per_split;
-    const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
-    auto load_tile = [&](int tile, int buf) {
-        const double* gsrc = src_rec + (size_t)tile * TILE * REC;
-        for (int ch = threadIdx.x; ch < CHUNKS; ch += T) cp_async16(&sm[buf][2 * ch], gsrc + 2 * ch);
-        cp_async_commit();
-    };
-    if (tile0 < tile1) load_tile(tile0, 0);
-    for (int tile = tile0; tile < tile1; ++tile) {
-        const int buf = (tile - tile0) & 1;
-        if (tile + 1 < tile1) { load_tile(tile + 1, buf ^ 1); cp_async_wait<1>(); }
-        else cp_async_wait<0>();
-        __syncthreads();
-        const int cnt_t = min(TILE, g.n_src - tile * TILE);
-        const double* __restrict__ tb = sm[buf];
-#pragma unroll 2
-        for (int jj = 0; jj < cnt_t; ++jj) {
-            const double2 p0 = *reinterpret_cast<const double2*>(tb + jj * REC);
-            const double pz = tb[jj * REC + 2];
-#pragma unroll
-            for (int s = 0; s < S; ++s) {
-                const double dx = p0.x - sx[s], dy = p0.y - sy[s], dz = pz - sz[s];
-                const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-                if (r2 < a.r2_guard) {                      // rare: candidate pair, exact evaluation
-                    const int j = __double2loint(tb[jj * REC + 7]);
-                    if (j != ids[s]) {
-                        const size_t o = 3 * (size_t)ids[s];
-                        const double ux = tb[jj * REC + 4] - a.vel[o], uy = tb[jj * REC + 5] - a.vel[o + 1],
-                                     uz = tb[jj * REC + 6] - a.vel[o + 2];
-                        if (ngb_exact(a, dx, dy, dz, ux, uy, uz, a.mass[ids[s]], tb[jj * REC + 3])) {
-                            if (lst[s] && cnt[s] < a.cap) lst[s][cnt[s]] = j;
-                            ++cnt[s];
-                        }
-                    }
-                }
-            }
-        }
-        __syncthreads();
-    }
-#pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        if (k >= g.n_sink) continue;
-        if (g.n_split == 1) a.out_count[g.compact ? k : ids[s]] = cnt[s];
-        else a.pcount[(size_t)blockIdx.y * g.n_sink + k] = cnt[s];
-    }
-}
-
-// concatenate the per-split lists in split order (= source-list order); the count is never truncated
-__global__ void ngb_finish_kernel(const NgbArgs a, const Geom g) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= g.n_sink) return;
-    const int id = a.sink_idx ? a.sink_idx[k] : k;
-    const size_t row = g.compact ? k : id;
-    int total = 0;
-    for (int s = 0; s < g.n_split; ++s) {
-        const int c = a.pcount[(size_t)s * g.n_sink + k];
-        const int32_t* l = a.plist + ((size_t)s * g.n_sink + k) * a.cap;
-        for (int q = 0; q < c && q < a.cap && total + q < a.cap; ++q) a.out_list[row * a.cap + total + q] = l[q];
-        total += c;
-    }
-    a.out_count[row] = total;
-}
-
-// Subsystems = connected components of the neighbour graph.  The paper traverses
-// the graph depth-first on the host; here a lock-free union-find: every edge hooks the larger root
-// under the smaller one with an integer compare-and-swap, so the root of a component ends up as its
-// smallest particle id whatever the order of the edges (deterministic), then paths are flattened.
-__device__ __forceinline__ int uf_find(int* parent, int x) {
-    int p = parent[x];
-    while (p != x) {
-        const int gp = parent[p];
-        if (gp != p) parent[x] = gp;            // path halving (benign race: only ever shortens)
-        x = p; p = gp;
-    }
-    return x;
-}
-__global__ void comp_init_kernel(int n, int* __restrict__ parent, unsigned char* __restrict__ flag) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) { parent[i] = i; flag[i] = 0; }
-}
-__global__ void comp_hook_kernel(int n, int cap, const int32_t* __restrict__ count, const int32_t* __restrict__ list,
-                                 int* parent, unsigned char* __restrict__ flag) {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int i = (int)(t / cap), q = (int)(t % cap);
-    if (i >= n || q >= count[i]) return;
-    const int j = list[(size_t)i * cap + q];
-    if (j < 0 || j >= n || j == i) return;
-    flag[i] = 1; flag[j] = 1;
-    int x = i, y = j;
-    while (true) {
-        x = uf_find(parent, x); y = uf_find(parent, y);
-        if (x == y) break;
-        if (x < y) { const int t2 = x; x = y; y = t2; }     // x = larger root
-        const int old = atomicCAS(&parent[x], x, y);
-        if (old == x) break;                                // x was still a root: hooked under the smaller root
-        x = old;                                            // someone else hooked x first: retry from there
-    }
-}
-__global__ void comp_label_kernel(int n, int* parent, const unsigned char* __restrict__ flag, int32_t* __restrict__ subsys) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    subsys[i] = flag[i] ? uf_find(parent, i) : -1;
-}
-
-// ----------------------------------------------------------------------------------------
-// NEXT-4: the O(N) operators of the FSI cycle (Eq. 5, 7, 8) and the slow/fast
-// split of a hierarchy level.
-// ----------------------------------------------------------------------------------------
-__global__ void kick_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ acc,
-                            const double* __restrict__ grad, double h, double c, double* __restrict__ vel) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= m) return;
-    const size_t o = 3 * (size_t)(idx ? idx[k] : k);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        double a = acc[o + d];
-        if (grad) a = __dadd_rn(a, __dmul_rn(c, grad[o + d]));        // a~ = a + (eps^2/24) C   (Eq. 9)
-        vel[o + d] = __dadd_rn(vel[o + d], __dmul_rn(h, a));          // v += h a                (Eq. 5, 8)
-    }
-}
-__global__ void drift_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ vel, double h,
-                             double* __restrict__ pos) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= m) return;
-    const size_t o = 3 * (size_t)(idx ? idx[k] : k);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) pos[o + d] = __dadd_rn(pos[o + d], __dmul_rn(h, vel[o + d]));   // r += h v (Eq. 7)
-}
-
-// eps_i = min(eps_ff, eps_fb), never above the level-0 value; fast iff eps_i < tau
-__global__ void level_flag_kernel(int m, const int32_t* __restrict__ seg, const double* __restrict__ dt_ff,
-                                  const double* __restrict__ dt_fb, double* __restrict__ dt0, int depth, double tau,
-                                  int all_slow, unsigned char* __restrict__ fast) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= m) return;
-    if (all_slow) { fast[k] = 0; return; }
-    const int i = seg[k];
-    double dt = fmin(dt_ff[i], dt_fb[i]);
-    if (depth == 0) dt0[i] = dt;
-    dt = fmin(dt, dt0[i]);
-    fast[k] = dt < tau ? 1 : 0;
-}
-
-// stable partition of a segment into [slow | fast]: block counts -> scan -> scatter
-constexpr int PART_T = 256;
-__global__ void __launch_bounds__(PART_T)
-part_count_kernel(int m, const unsigned char* __restrict__ fast, int* __restrict__ block_slow) {
-    const int k = blockIdx.x * PART_T + threadIdx.x;
-    const int slow = (k < m) && !fast[k];
-    const int c = __syncthreads_count(slow);
-    if (threadIdx.x == 0) block_slow[blockIdx.x] = c;
-}
-__global__ void part_scan_kernel(int nb, int* __restrict__ block_slow, int* __restrict__ n_slow) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    int run = 0;
-    for (int b = 0; b < nb; ++b) { const int c = block_slow[b]; block_slow[b] = run; run += c; }
-    *n_slow = run;
-}
-__global__ void __launch_bounds__(PART_T)
-part_scatter_kernel(int m, const int32_t* __restrict__ seg, const unsigned char* __restrict__ fast,
-                    const int* __restrict__ block_slow, const int* __restrict__ n_slow, int32_t* __restrict__ out) {
-    __shared__ int warp_slow[PART_T / 32];
-    const int k = blockIdx.x * PART_T + threadIdx.x;
-    const int live = k < m;
-    const int slow = live && !fast[k];
-    const unsigned bal = __ballot_sync(0xffffffffu, slow);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (lane == 0) warp_slow[warp] = __popc(bal);
-    __syncthreads();
-    int before = 0;                                           // slow elements of this block before this warp
-    for (int w = 0; w < warp; ++w) before += warp_slow[w];
-    const int rank_slow = before + __popc(bal & ((1u << lane) - 1u));
-    if (!live) return;
-    const int slow_before_block = block_slow[blockIdx.x];
-    if (slow) out[slow_before_block + rank_slow] = seg[k];
-    else {
-        const int fast_before = (blockIdx.x * PART_T - slow_before_block) + (threadIdx.x - rank_slow);
-        out[*n_slow + fast_before] = seg[k];
-    }
-}
-__global__ void iota_kernel(int n, int32_t* __restrict__ a) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) a[i] = i;
-}
-__global__ void fill_f64_kernel(int n, double v, double* __restrict__ a) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) a[i] = v;
-}
-
-// T = 1/2 sum m v^2 over a set, fixed order (stage 1 of the W reduction with another integrand)
-__global__ void __launch_bounds__(WSUM_THREADS)
-ksum_stage1_kernel(int m, const int32_t* __restrict__ idx, const double* __restrict__ mass,
-                   const double* __restrict__ vel, double* __restrict__ block_part) {
-    const int base = blockIdx.x * WSUM_PER_BLOCK;
-    double v = 0.0;
-    for (int q = threadIdx.x; q < WSUM_PER_BLOCK; q += WSUM_THREADS) {
-        const int k = base + q;
-        if (k < m) {
-            const int id = idx ? idx[k] : k;
-            const double* u = vel + 3 * (size_t)id;
-            v += mass[id] * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-        }
-    }
-    const double s = block_sum_fixed(v);
-    if (threadIdx.x == 0) block_part[blockIdx.x] = s;
-}
-
-// ----------------------------------------------------------------------------------------
-// Measurement aid: register-only FP64 chains (no memory traffic), to MEASURE the FP64-pipe peak
-// that bench.py's roofline quotes next to the derived 64 lanes/clk/SM figure.
-//   MIX 0: 8 independent DFMA chains per thread (pure DFMA peak).
-//   MIX 1: per 15 instructions 3 DADD + 9 DFMA + 3 DMUL (the acc pair's instruction mix).
-// ----------------------------------------------------------------------------------------
-constexpr int PROBE_THREADS = 128;
-constexpr int PROBE_CHAINS = 8;
-//   MIX 2: DFMA with three DISTINCT register operands, x = fma(y, z, x) (no reuse possible).
-//   MIX 3: the pair kernels' accumulate pattern: groups of three DFMAs sharing one operand,
-//          x0 = fma(w, y0, x0); x1 = fma(w, y1, x1); x2 = fma(w, y2, x2).
-// MIX 2 and 3 show the register-file operand limit (one 64-bit operand per clock per SM
-// sub-partition): 2/3 and 6/7 of the MIX 0 rate.
-template <int MIX>
-__global__ void __launch_bounds__(PROBE_THREADS, 4)
-fp64_probe_kernel(int iters, double b, double c, const double* __restrict__ in, double* __restrict__ sink) {
-    double a[PROBE_CHAINS];
-#pragma unroll
-    for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = 1.0 + 1e-9 * (double)(threadIdx.x + k);
-    if (MIX == 2 || MIX == 3) {
-        // operands that the compiler cannot fold: loaded from memory (all 1 + O(1e-6))
-        double x[12], y[12], w[4];
-#pragma unroll
-        for (int k = 0; k < 12; ++k) { x[k] = in[threadIdx.x + 128 * k]; y[k] = in[threadIdx.x + 128 * (k + 12)]; }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) w[k] = in[threadIdx.x + 128 * (k + 24)];
-        for (int it = 0; it < iters; ++it) {
-#pragma unroll
-            for (int g = 0; g < 4; ++g) {
-                if (MIX == 2) {
-                    x[3 * g] = fma(y[3 * g], w[g], x[3 * g]);
-                    x[3 * g + 1] = fma(y[3 * g + 1], y[(3 * g + 5) % 12], x[3 * g + 1]);
-                    x[3 * g + 2] = fma(y[3 * g + 2], y[(3 * g + 7) % 12], x[3 * g + 2]);
-                } else {
-                    x[3 * g] = fma(w[g], y[3 * g], x[3 * g]);
-                    x[3 * g + 1] = fma(w[g], y[3 * g + 1], x[3 * g + 1]);
-                    x[3 * g + 2] = fma(w[g], y[3 * g + 2], x[3 * g + 2]);
-                }
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 12; ++k) a[k % PROBE_CHAINS] += x[k] + y[k];
-    } else {
-        for (int it = 0; it < iters; ++it) {
-            if (MIX == 0) {
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-#pragma unroll
-                    for (int k = 0; k < PROBE_CHAINS; ++k) a[k] = fma(a[k], b, c);          // 32 DFMA
-            } else {
-#pragma unroll
-                for (int k = 0; k < PROBE_CHAINS; ++k) {                                     // 8 x 15 instructions
-                    double x = a[k];
-                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                    x = x + c; x = fma(x, b, c); x = fma(x, b, c); x = x * b; x = fma(x, b, c);
-                    a[k] = x;
-                }
-            }
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < PROBE_CHAINS; ++k) s += a[k];
-    if (s == 123.456) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chains alive
-}
-
-}  // namespace
+#include "common.cuh"
+#include "policies.cuh"
+#include "pair_kernels.cuh"
+#include "epilogues.cuh"
+#include "pn1.cuh"
+#include "subsystems.cuh"
+#include "integrator.cuh"
+#include "fp64_probe.cuh"
 
 // ========================================================================================
 // host side
@@ -1218,6 +63,8 @@ struct bifrost_ctx {
     double* phi_scratch = nullptr;   // [max_n]   (bifrost_potential with out_phi == NULL)
     double* wpart = nullptr;         // [ceil(max_n / 4096)] block partials of the W reduction
     unsigned long long* smin = nullptr;   // [max_n] per-subsystem minima (bifrost_subsys_min)
+    int small_m = 128;               // FSI cycles / level splits of at most this many particles run as ONE single-CTA launch
+                                     // (env BIFROST_SMALL_M = 0..256 overrides; 0 disables; tuning / test aid)
     int64_t fused_max_sinks = 4096;  // below: one fused launch per call (env BIFROST_FUSED_MAX_SINKS overrides; tuning aid)
     unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel (zero between launches)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
@@ -1276,7 +123,7 @@ inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // Source-range split: enough CTAs for ~16 per resident slot (tail < a few %), bounded by the
 // number of source tiles, MAX_SPLIT and the partial workspace.
 Geom make_geom(const bifrost_ctx* ctx, int64_t n_sink, int64_t n_src, int sinks_per_cta, int resident_per_sm,
-               size_t partial_bytes_per_sink) {
+               size_t partial_bytes_per_sink, double* model_time = nullptr) {
     Geom g;
     g.n_sink = (int)n_sink;
     g.n_src = (int)n_src;
@@ -1306,6 +153,8 @@ Geom make_geom(const bifrost_ctx* ctx, int64_t n_sink, int64_t n_src, int sinks_
     }
     g.tiles_per_split = n_tiles > 0 ? ceil_div(n_tiles, split) : 1;
     g.n_split = n_tiles > 0 ? ceil_div(n_tiles, g.tiles_per_split) : 1;
+    // modelled SM time of the launch in (sink x tile) units: waves x tiles per CTA x the CTA's share of an SM
+    if (model_time) *model_time = best_t * (double)sinks_per_cta * (double)resident_per_sm;
     return g;
 }
 
@@ -1334,7 +183,19 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
 //   below: ONE fused launch with 128 threads and S = 4, 2 or 1 sinks per thread - the largest S
 //   that still yields >= 4 CTAs per SM (sink blocks x source-range splits), because a small set
 //   is short of parallelism, not of registers.
-template <class P, class Big, class F4, class F2, class F1>
+template <class P, class Sh>
+int launch_big(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
+    dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
+    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    ctx->launches++;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+// Huge = the shape that is fastest per pair (more sinks per thread; measured gain HUGE_GAIN_PERMILLE),
+// Big = a smaller CTA that quantises better over the SMs when there are few sink blocks.  The launch
+// model of make_geom (waves x tiles per CTA x sinks per CTA) picks between them per call.
+template <class P, class Huge, int HUGE_GAIN_PERMILLE, class Big, class F4, class F2, class F1>
 int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src,
              size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
     Geom g;
@@ -1353,12 +214,19 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     }
-    g = make_geom(ctx, n_sink, n_src, Big::T * Big::S, Big::MINB, partial_bytes_per_sink);
-    g.compact = compact;
-    dim3 grid(ceil_div(g.n_sink, Big::T * Big::S), g.n_split);
-    pair_kernel<P, Big::S, Big::T, Big::MINB, Big::UNR><<<grid, Big::T, 0, st>>>(a, g, ctx->src_rec);
-    ctx->launches++;
-    CU_TRY(ctx, cudaGetLastError());
+    double t_big = 0.0, t_huge = 0.0;
+    g = make_geom(ctx, n_sink, n_src, Big::T * Big::S, Big::MINB, partial_bytes_per_sink, &t_big);
+    const Geom gh = make_geom(ctx, n_sink, n_src, Huge::T * Huge::S, Huge::MINB, partial_bytes_per_sink, &t_huge);
+    int rc;
+    if (t_huge * (1000 - HUGE_GAIN_PERMILLE) < t_big * 1000) {
+        g = gh;
+        g.compact = compact;
+        rc = launch_big<P, Huge>(ctx, a, g, st);
+    } else {
+        g.compact = compact;
+        rc = launch_big<P, Big>(ctx, a, g, st);
+    }
+    if (rc) return rc;
     if (g.n_split > 1 || P::ALWAYS_FINISH) {
         finish_kernel<P><<<ceil_div(n_sink, 256), 256, 0, st>>>(a, g);
         ctx->launches++;
@@ -1378,8 +246,8 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     using F4 = Shape<4, 128, 4, 2>;
     using F2 = Shape<2, 128, 6, 2>;
     using F1 = Shape<1, 128, 8, 4>;
-    return sub ? run_pass<AccPassT<true>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-               : run_pass<AccPassT<false>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return sub ? run_pass<AccPassT<true>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<AccPassT<false>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
@@ -1389,12 +257,13 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     if (n_sink == 0) return BIFROST_OK;
     const SrcArrays src{pos, acc, mass, sub, src_idx};
     const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    using Huge = Shape<5, 256, 1, 2>;     // phase-major (GradPassT::pairs), 1.4 % faster per pair than Big
     using Big = Shape<4, 256, 1, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    return sub ? run_pass<GradPassT<true>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-               : run_pass<GradPassT<false>, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return sub ? run_pass<GradPassT<true>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<GradPassT<false>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
@@ -1409,13 +278,15 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
     const SrcArrays src{pos, vel, mass, sub, src_idx};
     const DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb};
+    using Huge = Shape<6, 128, 2, 1>;     // 2.9 % faster per pair than Big
     using Big = Shape<4, 128, 3, 2>;
+    using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                            : run_pass<DtPassT<true, true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
-    return src_idx ? run_pass<DtPass, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                   : run_pass<DtPassAsc, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                            : run_pass<DtPassT<true, true>, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return src_idx ? run_pass<DtPass, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                   : run_pass<DtPassAsc, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
@@ -1433,8 +304,8 @@ int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     using Big = Shape<4, 128, 4, 2>;
     using F2 = Shape<2, 128, 6, 2>;
     using F1 = Shape<1, 128, 8, 4>;
-    int rc = sub ? run_pass<PotPassT<true>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st)
-                 : run_pass<PotPassT<false>, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st);
+    int rc = sub ? run_pass<PotPassT<true>, Big, 0, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st)
+                 : run_pass<PotPassT<false>, Big, 0, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st);
     if (rc) return rc;
     if (out_W) {
         const int nb = ceil_div(n_sink, WSUM_PER_BLOCK);
@@ -1558,6 +429,13 @@ int drift_impl(bifrost_ctx* ctx, const int32_t* idx, int64_t m, const double* ve
 int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, const int32_t* idx, int64_t m,
              double G, double eps_soft, double eps, cudaStream_t st) {
     if (m == 0) return BIFROST_OK;
+    const bool excl = ctx->subsys && ctx->subsys_n == n;
+    if (m <= ctx->small_m && !excl) {                      // one launch for the whole cycle
+        fsi_small_kernel<<<1, SMALL_M, 0, st>>>((int)m, idx, pos, vel, mass, G, soft2(eps_soft), eps);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+        return BIFROST_OK;
+    }
     double* a = ctx->w_acc;
     double* g = ctx->w_grad;
     RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
@@ -1589,15 +467,22 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     if (!all_slow)   // time-steps of the level's particles among themselves (Eq. 21-22)
         RC_TRY(dtmin_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eta_ff, h.eta_fb, ctx->w_dtff, ctx->w_dtfb,
                           nullptr, nullptr, 0, st));
-    const int nb = ceil_div(m, PART_T);
-    unsigned char* fast = ctx->is_bh;                      // scratch shared with bifrost_pn1 (one call at a time per ctx)
-    level_flag_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow, fast);
-    part_count_kernel<<<nb, PART_T, 0, st>>>((int)m, fast, ctx->w_bcount);
-    part_scan_kernel<<<1, 32, 0, st>>>(nb, ctx->w_bcount, ctx->w_nslow);
-    part_scatter_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, fast, ctx->w_bcount, ctx->w_nslow, ctx->w_tmp);
-    ctx->launches += 4;
-    CU_TRY(ctx, cudaGetLastError());
-    CU_TRY(ctx, cudaMemcpyAsync(seg, ctx->w_tmp, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
+    if (m <= ctx->small_m) {
+        level_split_small_kernel<<<1, SMALL_M, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow,
+                                                        ctx->w_nslow);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    } else {
+        const int nb = ceil_div(m, PART_T);
+        unsigned char* fast = ctx->is_bh;                  // scratch shared with bifrost_pn1 (one call at a time per ctx)
+        level_flag_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow, fast);
+        part_count_kernel<<<nb, PART_T, 0, st>>>((int)m, fast, ctx->w_bcount);
+        part_scan_kernel<<<1, 32, 0, st>>>(nb, ctx->w_bcount, ctx->w_nslow);
+        part_scatter_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, fast, ctx->w_bcount, ctx->w_nslow, ctx->w_tmp);
+        ctx->launches += 4;
+        CU_TRY(ctx, cudaGetLastError());
+        CU_TRY(ctx, cudaMemcpyAsync(seg, ctx->w_tmp, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
+    }
     CU_TRY(ctx, cudaMemcpyAsync(ctx->h_nslow, ctx->w_nslow, 4, cudaMemcpyDeviceToHost, st));
     CU_TRY(ctx, cudaStreamSynchronize(st));                // the host decides the recursion (as in the paper)
     const int64_t ns = *ctx->h_nslow, nf = m - ns;
@@ -1677,6 +562,10 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     if (const char* e = getenv("BIFROST_FUSED_MAX_SINKS")) {
         const long long v = atoll(e);
         if (v >= 0 && v <= (long long)TICKETS * 128) ctx->fused_max_sinks = v;
+    }
+    if (const char* e = getenv("BIFROST_SMALL_M")) {
+        const int v = atoi(e);
+        if (v >= 0 && v <= SMALL_M) ctx->small_m = v;
     }
     const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
     ctx->partial_bytes = 24 * (size_t)max_n * 16;   // up to 16 source-range splits at n_sink = max_n

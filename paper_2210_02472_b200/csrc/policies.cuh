@@ -1,0 +1,423 @@
+// policies.cuh - the pass policies (acc, grad / jerk, dtmin, potential): packed source record, per-sink state, the pair update (the FP64 inner loop), store and split-j finish of each pass.
+// Part of the single translation unit bifrost.cu (see its header and DESIGN.md); not a public header.
+#pragma once
+
+namespace {
+
+// ----------------------------------------------------------------------------------------
+// Pass policies.  Each defines the packed source record, the per-sink state, the pair update
+// and how a thread's result is stored.
+// ----------------------------------------------------------------------------------------
+
+// NEXT-2: with EXCL = true every record carries the subsystem code of
+// its source (-1 for a single particle) and every sink its own (-2 for a single particle, so that it
+// never matches); a pair with equal codes gets the seed y0 = 0, hence the weight 0 - one integer
+// compare and one 32-bit select per pair, nothing on the FP64 pipe.
+__device__ __forceinline__ double mask_seed(double y0, bool same) {
+    return __hiloint2double(same ? 0 : __double2hiint(y0), 0);
+}
+__device__ __forceinline__ int sink_code(const int32_t* subsys, int id) {
+    const int c = subsys[id];
+    return c < 0 ? -2 : c;
+}
+
+// source-side subsystem code: -1 for a single particle (never equal to a sink's code, which is
+// -2 for a single particle), the subsystem id otherwise
+__device__ __forceinline__ int src_code(const int32_t* subsys, int j) {
+    if (!subsys) return -1;
+    const int c = subsys[j];
+    return c < 0 ? -1 : c;
+}
+
+// a5 + a7: reduction of one sink's partials in a FIXED order, then scatter.  A group of L lanes
+// (L = 1, 2, .. 32, a power of two; lane = index in the group) shares one sink: lane l adds the
+// partials of splits l, l+L, ... in that order and a butterfly adds the lanes - an order that
+// depends only on (n_split, L), never on which CTA runs it.  All 32 lanes of a warp must call
+// (write = false for a group that shadows a sink).  The partials come from other CTAs: L2 loads.
+__device__ __forceinline__ double group_add(double v, int L) {
+    for (int off = L >> 1; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v;
+}
+__device__ __forceinline__ void finish_vec3(const double* partial, double* out, double G, const Geom& g, int k, int id,
+                                            int lane, int L, bool write) {
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int s = lane; s < g.n_split; s += L) {
+        const double* p = partial + 3 * ((size_t)s * g.n_sink + k);
+        sx += __ldcg(p); sy += __ldcg(p + 1); sz += __ldcg(p + 2);
+    }
+    if (L > 1) { sx = group_add(sx, L); sy = group_add(sy, L); sz = group_add(sz, L); }
+    if (write && lane == 0) {
+        double* o = out + 3 * (size_t)(g.compact ? k : id);
+        o[0] = G * sx; o[1] = G * sy; o[2] = G * sz;
+    }
+}
+
+struct AccArgs {
+    const double* pos;
+    const int32_t* subsys;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;        // final output [.][3]
+    double* partial;    // [split][n_sink][3]
+};
+
+template <bool EXCL>
+struct AccPassT {
+    static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
+    static constexpr int PHASED_MIN_S = 0;
+    using Args = AccArgs;
+    struct Sink { double x, y, z; int sub; };
+    struct Acc { double x, y, z; };
+    struct Raw { double x, y, z, m; int code; };
+    // a1: gather one source (j < 0: padding record) and write its packed record
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
+            w.m = s.mass[j]; w.code = EXCL ? src_code(s.subsys, j) : 0;
+        } else { w.x = w.y = w.z = w.m = 0.0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(1.5 * w.m, 1.875 * w.m);
+        if (EXCL) o[3] = make_double2(__hiloint2double(0, w.code), 0.0);
+    }
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2];
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
+    }
+    __device__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
+    // 15 FP64-pipe instructions: 3 DADD, 3 DFMA (r2), DMUL t, DFMA e, 2 DFMA poly, 2 DMUL, 3 DFMA.
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        double y0 = rsqrt_seed(r2);
+        if (EXCL) y0 = mask_seed(y0, __double2loint(r[6]) == s.sub);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 3/2 e + 15/8 e^2)
+        const double w = (y0 * t) * pm;                       // m / s^3
+        c.x = fma(w, dx, c.x); c.y = fma(w, dy, c.y); c.z = fma(w, dz, c.z);
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        if (g.n_split == 1) {
+            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
+            o[0] = a.G * c.x; o[1] = a.G * c.y; o[2] = a.G * c.z;
+        } else {
+            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
+            o[0] = c.x; o[1] = c.y; o[2] = c.z;
+        }
+    }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
+    }
+};
+
+using AccPass = AccPassT<false>;
+
+struct GradArgs {
+    const double* pos;
+    const double* acc;
+    const int32_t* subsys;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;
+    double* partial;
+};
+
+template <bool EXCL>
+struct GradPassT {
+    static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
+    static constexpr int PHASED_MIN_S = 5;   // measured: phase-major helps at S = 5 (+1.4 %), hurts at S = 4
+    using Args = GradArgs;
+    struct Sink { double x, y, z, ax, ay, az; int sub; };
+    struct Acc { double ux, uy, uz, wx, wy, wz; };   // U = sum w a_ji,  W = sum w (a_ji.r_ji)/s^2 r_ji
+    struct Raw { double x, y, z, ax, ay, az, m; int code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            const size_t b = 3 * (size_t)j;
+            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
+            w.ax = s.aux[b]; w.ay = s.aux[b + 1]; w.az = s.aux[b + 2];
+            w.m = s.mass[j]; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.ax = w.ay = w.az = w.m = 0.0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.ax);
+        o[2] = make_double2(w.ay, w.az);
+        o[3] = make_double2(w.m, 1.5 * w.m);
+        o[4] = make_double2(1.875 * w.m, __hiloint2double(0, w.code));
+    }
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        const size_t o = 3 * (size_t)id;
+        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
+        s.ax = a.acc[o]; s.ay = a.acc[o + 1]; s.az = a.acc[o + 2];
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
+    }
+    __device__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
+    // 28 FP64-pipe instructions; C_i = U - 3 W is formed once per sink in store().
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double bx = r[3] - s.ax, by = r[4] - s.ay, bz = r[5] - s.az;       // a_ji
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        const double q = fma(bx, dx, fma(by, dy, bz * dz));                       // a_ji . r_ji
+        double y0 = rsqrt_seed(r2);
+        if (EXCL) y0 = mask_seed(y0, __double2loint(r[9]) == s.sub);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[8], r[7]), e, r[6]);
+        const double w = (y0 * t) * pm;                                           // m / s^3
+        const double y2 = fma(t, fma(e, e, e), t);                                // 1 / s^2
+        const double v = (w * y2) * q;                                            // m (a_ji.r_ji) / s^5
+        c.ux = fma(w, bx, c.ux); c.uy = fma(w, by, c.uy); c.uz = fma(w, bz, c.uz);
+        c.wx = fma(v, dx, c.wx); c.wy = fma(v, dy, c.wy); c.wz = fma(v, dz, c.wz);
+    }
+    // the same 28 instructions per pair, stage by stage over the S sinks of a thread
+    template <int S>
+    __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        double dx[S], dy[S], dz[S], bx[S], by[S], bz[S], r2[S], q[S], y0[S], w[S], v[S];
+#pragma unroll
+        for (int s = 0; s < S; ++s) { dx[s] = r[0] - sk[s].x; dy[s] = r[1] - sk[s].y; dz[s] = r[2] - sk[s].z; }
+#pragma unroll
+        for (int s = 0; s < S; ++s) r2[s] = fma(dx[s], dx[s], fma(dy[s], dy[s], fma(dz[s], dz[s], a.eps2)));
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            y0[s] = rsqrt_seed(r2[s]);
+            if (EXCL) y0[s] = mask_seed(y0[s], __double2loint(r[9]) == sk[s].sub);
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s) { bx[s] = r[3] - sk[s].ax; by[s] = r[4] - sk[s].ay; bz[s] = r[5] - sk[s].az; }
+#pragma unroll
+        for (int s = 0; s < S; ++s) q[s] = fma(bx[s], dx[s], fma(by[s], dy[s], bz[s] * dz[s]));
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const double t = y0[s] * y0[s];
+            const double e = fma(-r2[s], t, 1.0);
+            const double pm = fma(fma(e, r[8], r[7]), e, r[6]);
+            w[s] = (y0[s] * t) * pm;
+            const double y2 = fma(t, fma(e, e, e), t);
+            v[s] = (w[s] * y2) * q[s];
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            c[s].ux = fma(w[s], bx[s], c[s].ux); c[s].uy = fma(w[s], by[s], c[s].uy); c[s].uz = fma(w[s], bz[s], c[s].uz);
+            c[s].wx = fma(v[s], dx[s], c[s].wx); c[s].wy = fma(v[s], dy[s], c[s].wy); c[s].wz = fma(v[s], dz[s], c[s].wz);
+        }
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        const double cx = fma(-3.0, c.wx, c.ux), cy = fma(-3.0, c.wy, c.uy), cz = fma(-3.0, c.wz, c.uz);
+        if (g.n_split == 1) {
+            double* o = a.out + 3 * (size_t)(g.compact ? k : id);
+            o[0] = a.G * cx; o[1] = a.G * cy; o[2] = a.G * cz;
+        } else {
+            double* o = a.partial + 3 * ((size_t)split * g.n_sink + k);
+            o[0] = cx; o[1] = cy; o[2] = cz;
+        }
+    }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
+    }
+};
+
+using GradPass = GradPassT<false>;
+
+struct DtArgs {
+    const double* pos;
+    const double* vel;
+    const double* mass;
+    const int32_t* subsys;
+    const int32_t* sink_idx;
+    double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
+    int32_t* pid;      // [split][2][n_sink]  their source ids
+    double G, eta_ff, eta_fb;
+    double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
+};
+
+// ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
+// the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
+template <bool ASC, bool EXCL>
+struct DtPassT {
+    static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
+    static constexpr int PHASED_MIN_S = 0;
+    using Args = DtArgs;
+    struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
+    // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
+    struct Acc { double kff, kfb; int jff, jfb; };
+    struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            const size_t b = 3 * (size_t)j;
+            w.x = s.pos[b]; w.y = s.pos[b + 1]; w.z = s.pos[b + 2];
+            w.vx = s.aux[b]; w.vy = s.aux[b + 1]; w.vz = s.aux[b + 2];
+            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.vx = w.vy = w.vz = w.m = 0.0; w.j = 0; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(w.vx, w.vy);
+        o[3] = make_double2(w.vz, __hiloint2double(w.code, w.j));
+    }
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        const size_t o = 3 * (size_t)id;
+        s.x = a.pos[o]; s.y = a.pos[o + 1]; s.z = a.pos[o + 2];
+        s.vx = a.vel[o]; s.vy = a.vel[o + 1]; s.vz = a.vel[o + 2];
+        s.m = a.mass[id]; s.id = id;
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
+    }
+    __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
+    // FP64-pipe instructions: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
+    // 2 DMUL keys = 23, plus 2 (ASC) or 4 DSETP.
+    __device__ __forceinline__ static void pair(const Args&, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
+        const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
+        const int jid = __double2loint(r[7]);
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
+        const double y3 = (y0 * t) * p3;
+        const double y2 = fma(t, fma(e, e, e), t);
+        double kff = (s.m + r[3]) * y3;
+        double kfb = v2 * y2;
+        // j != i (Eq. 21, 22) and, with EXCL, not in the sink's subsystem
+        const bool other = EXCL ? ((jid != s.id) & (__double2hiint(r[7]) != s.sub)) : (jid != s.id);
+        if (ASC) {
+            const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
+            c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
+            c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
+        } else {
+            if (!other) { kff = -1.0; kfb = -1.0; }
+            if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
+            if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+        }
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
+        const size_t o = (size_t)split * 2 * g.n_sink + k;
+        a.pkey[o] = c.kff; a.pkey[o + g.n_sink] = c.kfb;
+        a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
+    }
+    // dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
+    // Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
+    static constexpr bool ALWAYS_FINISH = true;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int i, int lane, int L, bool write) {
+        double kb[2] = {0.0, 0.0};
+        int jb[2] = {-1, -1};
+        for (int s = lane; s < g.n_split; s += L) {
+            for (int w = 0; w < 2; ++w) {
+                const size_t o = ((size_t)s * 2 + w) * g.n_sink + k;
+                const double key = __ldcg(a.pkey + o);
+                const int j = __ldcg(a.pid + o);
+                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+            }
+        }
+        for (int off = L >> 1; off > 0; off >>= 1) {      // (max key, then min id) is order-independent
+            for (int w = 0; w < 2; ++w) {
+                const double key = __shfl_xor_sync(0xffffffffu, kb[w], off);
+                const int j = __shfl_xor_sync(0xffffffffu, jb[w], off);
+                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+            }
+        }
+        if (!write || lane != 0) return;
+        const double* pos = a.pos; const double* vel = a.vel;
+        const int row = g.compact ? k : i;
+        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+        double tff = inf, tfb = inf;
+        if (jb[0] >= 0) {
+            const int j = jb[0];
+            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            const double r = sqrt(r2);
+            tff = a.eta_ff * sqrt(__dmul_rn(r2, r) / (a.G * (a.mass[i] + a.mass[j])));
+        }
+        if (jb[1] >= 0) {
+            const int j = jb[1];
+            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
+                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
+            const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
+                         uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+            tfb = __dmul_rn(a.eta_fb, sqrt(r2)) / sqrt(v2);
+        }
+        if (a.dt_ff) a.dt_ff[row] = tff;
+        if (a.dt_fb) a.dt_fb[row] = tfb;
+        if (a.j_ff) a.j_ff[row] = jb[0];
+        if (a.j_fb) a.j_fb[row] = jb[1];
+    }
+};
+
+using DtPass = DtPassT<false, false>;
+using DtPassAsc = DtPassT<true, false>;
+
+struct PotArgs {
+    const double* pos;
+    const int32_t* subsys;
+    const int32_t* sink_idx;
+    double eps2, G;
+    double* out;        // phi at [.]
+    double* partial;    // [split][n_sink]
+};
+
+// Potential (Eq. 4 second term, Eq. 68): p_i = sum_j m_j / s_ij; phi_i = -G p_i.
+// 1/s = y0 (1 + e/2 + 3/8 e^2); the record carries m, m/2, 3m/8 and the source id, because here
+// the self pair does not multiply a zero separation and must be dropped by id (integer select).
+template <bool EXCL>
+struct PotPassT {
+    static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
+    static constexpr int PHASED_MIN_S = 0;
+    using Args = PotArgs;
+    struct Sink { double x, y, z; int id, sub; };
+    struct Acc { double p; };
+    struct Raw { double x, y, z, m; int j, code; };
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
+        if (j >= 0) {
+            w.x = s.pos[3 * (size_t)j]; w.y = s.pos[3 * (size_t)j + 1]; w.z = s.pos[3 * (size_t)j + 2];
+            w.m = s.mass[j]; w.j = j; w.code = src_code(s.subsys, j);
+        } else { w.x = w.y = w.z = w.m = 0.0; w.j = -1; w.code = 0; }
+    }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) {
+        o[0] = make_double2(w.x, w.y);
+        o[1] = make_double2(w.z, w.m);
+        o[2] = make_double2(0.5 * w.m, 0.375 * w.m);
+        o[3] = make_double2(__hiloint2double(w.code, w.j), 0.0);
+    }
+    __device__ static void load_sink(const Args& a, int id, Sink& s) {
+        s.x = a.pos[3 * (size_t)id]; s.y = a.pos[3 * (size_t)id + 1]; s.z = a.pos[3 * (size_t)id + 2]; s.id = id;
+        s.sub = EXCL ? sink_code(a.subsys, id) : 0;
+    }
+    __device__ static void init(Acc& c) { c.p = 0.0; }
+    // 12 FP64-pipe instructions: 3 DADD, 3 DFMA, DMUL, DFMA, 2 DFMA, DMUL, DADD.
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 1/2 e + 3/8 e^2)
+        double w = y0 * pm;                                   // m / s
+        if (__double2loint(r[6]) == s.id) w = 0.0;            // j != i
+        if (EXCL && __double2hiint(r[6]) == s.sub) w = 0.0;   // same subsystem
+        c.p += w;
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        if (g.n_split == 1) a.out[g.compact ? k : id] = -a.G * c.p;
+        else a.partial[(size_t)split * g.n_sink + k] = c.p;
+    }
+    static constexpr bool ALWAYS_FINISH = false;
+    __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
+        double s = 0.0;
+        for (int q = lane; q < g.n_split; q += L) s += __ldcg(a.partial + (size_t)q * g.n_sink + k);     // fixed order
+        if (L > 1) s = group_add(s, L);
+        if (write && lane == 0) a.out[g.compact ? k : id] = -a.G * s;
+    }
+};
+
+using PotPass = PotPassT<false>;
+
+}  // namespace

@@ -713,3 +713,39 @@ def test_hhs_fsi_config2_full_size(torch, ctx):
     assert np.array_equal(log, ref_levels), (log, ref_levels)
     assert ref_levels[0, 2] > 0 and ref_levels[0, 1] > 0
     assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
+
+
+@pytest.mark.parametrize("m", [1, 2, 5, 64, 128])
+def test_small_level_single_launch_equals_the_general_path_bit_for_bit(torch, ctx, m, monkeypatch):
+    """FSI cycles / level splits of <= 128 particles run as ONE single-CTA launch (fsi_small_kernel,
+    level_split_small_kernel); same pair arithmetic, same summation order as the multi-launch path."""
+    from paper_2210_02472_b200.binding import Context
+    w = workload(2)
+    rng = np.random.default_rng(100 + m)
+    idx = rng.permutation(w.n)[:m].astype(np.int32)          # unsorted on purpose
+    monkeypatch.setenv("BIFROST_SMALL_M", "0")
+    general = Context(w.n)
+    monkeypatch.delenv("BIFROST_SMALL_M")
+    try:
+        out = []
+        for c in (ctx, general):
+            pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+            l0 = c.launch_count
+            for _ in range(2):
+                c.fsi_step(pos, vel, mass, w.G, w.eps, 1e-4, dev(torch, idx))
+            torch.cuda.synchronize()
+            out.append((pos, vel, c.launch_count - l0))
+        assert out[0][2] == 2 and out[1][2] == 18              # 1 launch per cycle instead of 9
+        assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+        # the hierarchy over a small system: identical level log and state on both paths
+        sub = rng.permutation(w.n)[:96]
+        p0, v0, m0 = w.pos[sub].copy(), w.vel[sub].copy(), w.mass[sub].copy()
+        res = []
+        for c in (ctx, general):
+            pos, vel, mass = dev(torch, p0), dev(torch, v0), dev(torch, m0)
+            summ, log = c.hhs_fsi(pos, vel, mass, w.G, w.eps, 0.05, 0.05, 2.0 ** -6, max_depth=6, log_cap=256)
+            res.append((pos, vel, summ, log))
+        assert res[0][2] == res[1][2] and np.array_equal(res[0][3], res[1][3]) and res[0][2]["levels"] > 1
+        assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
+    finally:
+        general.close()
