@@ -414,6 +414,19 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
         if name == "fsi_step":
             out[name]["interactions_per_s"] = 4.0 * n * n / (ms * 1e-3)     # four O(N^2) sums
     out["neighbours"]["pairs_found"] = int(cnt.sum().item())
+    # one HHS-FSI integration interval (Eq. 11) on config 2 (N = 16384, Kroupa masses): the hierarchy the
+    # active-subset sweep stands for; host-steered recursion, so wall time is what counts
+    from paper_2210_02472_b200 import workloads as W
+    w2 = W.config2()
+    p, v, m = (torch.from_numpy(x).to(pos.device) for x in (w2.pos, w2.vel, w2.mass))
+    ctx.hhs_fsi(p.clone(), v.clone(), m, w2.G, w2.eps, 0.1, 0.1, 2.0 ** -9, max_depth=12)      # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    l0 = ctx.launch_count
+    summ, _ = ctx.hhs_fsi(p, v, m, w2.G, w2.eps, 0.1, 0.1, 2.0 ** -9, max_depth=12)
+    torch.cuda.synchronize()
+    out["hhs_fsi_config2"] = {"ms": 1e3 * (time.perf_counter() - t0), "tau": 2.0 ** -9, "eta": 0.1, "max_depth": 12,
+                              "launches": ctx.launch_count - l0, **summ}
     return out
 
 
