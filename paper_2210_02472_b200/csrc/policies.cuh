@@ -286,19 +286,14 @@ struct DtPassT {
         double kfb = v2 * y2;
         // j != i (Eq. 21, 22) and, with EXCL, not in the sink's subsystem
         const bool other = EXCL ? ((jid != s.id) & (__double2hiint(r[7]) != s.sub)) : (jid != s.id);
-        // The keys are non-negative (or the -1 sentinel), so they order like their bit patterns read as
-        // signed 64-bit integers: the comparisons run on the integer pipe, not as DSETP on the FP64 pipe.
         if (ASC) {
-            const bool uf = other & (__double_as_longlong(kff) > __double_as_longlong(c.kff));
-            const bool ub = other & (__double_as_longlong(kfb) > __double_as_longlong(c.kfb));
+            const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
             c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
             c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
         } else {
             if (!other) { kff = -1.0; kfb = -1.0; }
-            const long long iff = __double_as_longlong(kff), cff = __double_as_longlong(c.kff);
-            const long long ifb = __double_as_longlong(kfb), cfb = __double_as_longlong(c.kfb);
-            if (iff >= cff) { if (iff > cff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
-            if (ifb >= cfb) { if (ifb > cfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+            if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
+            if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
         }
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
