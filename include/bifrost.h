@@ -231,11 +231,14 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
  * over S and H_F = this procedure over F with tau/2.  A level without fast particles (or at depth max_depth,
  * 0 <= max_depth <= 62) is one FSI cycle of length tau.  Every sum and update runs on the device; the host
  * reads one integer (|S|) per level to steer the recursion, so the call is SYNCHRONOUS.
+ *   dt_cap : DEVICE double[n] or NULL - further per-particle time-steps taken at the start of the interval
+ *            (e.g. bifrost_timestep_criteria's Eq. 24-29 minimum): eps_i^{level 0} = min(eps_ff, eps_fb, dt_cap[i]),
+ *            "the final time-step of a particle is the minimum of the set of its different time-steps" (L293);
  *   out_level_log : HOST int64[log_cap][3] or NULL - (depth, |S|, |F|) of the first log_cap levels, in the
  *                   order they are entered;   out_summary : HOST int64[3] or NULL - levels entered, deepest
  *                   depth, FSI cycles run.  pos, vel : DEVICE double[n][3], updated in place. */
 int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G,
-                    double eps_soft, double eta_ff, double eta_fb, double tau, int max_depth,
+                    double eps_soft, double eta_ff, double eta_fb, const double* dt_cap, double tau, int max_depth,
                     int64_t* out_level_log, int64_t log_cap, int64_t* out_summary, void* stream);
 
 /* bifrost_kinetic_energy - first term of Eq. 4: *out_T = 1/2 sum_{i in idx} m_i |v_i|^2

@@ -87,12 +87,13 @@ def level_timesteps(pos, vel, mass, idx, G, eta_ff, eta_fb):
     return np.minimum(d["dt_ff"], d["dt_fb"])
 
 
-def hhs_fsi(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, stats=None):
+def hhs_fsi(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, stats=None, dt_cap=None):
     """One HHS-FSI integration interval of length tau (Eq. 11), in place.  stats (a dict, optional)
-    receives 'levels' (list of (depth, n_slow, n_fast, tau)) in the order the levels are entered."""
+    receives 'levels' (list of (depth, n_slow, n_fast, tau)) in the order the levels are entered.
+    dt_cap (optional, [n]): further per-particle time-steps (e.g. Eq. 24-29) min'd into the level-0 value."""
     n = mass.shape[0]
     order = np.arange(n, dtype=np.int32)
-    dt0 = np.full(n, np.inf)
+    dt0 = np.full(n, np.inf) if dt_cap is None else np.array(dt_cap, dtype=np.float64)   # further criteria (L293)
     if stats is not None:
         stats["levels"] = []
     _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, 0, n, tau, 0, max_depth, dt0, stats)
@@ -105,7 +106,7 @@ def _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, lo, hi, tau, 
     if depth < max_depth:
         dt = level_timesteps(pos, vel, mass, idx, G, eta_ff, eta_fb)
         if depth == 0:
-            dt0[idx] = dt
+            dt0[idx] = np.minimum(dt, dt0[idx])             # level-0 value = minimum of all criteria
         dt = np.minimum(dt, dt0[idx])
         fast = dt < tau
     else:

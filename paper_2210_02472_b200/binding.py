@@ -78,7 +78,7 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_kick.argtypes = [_P, _I64, _P, _I64, _P, _P, _D, _D, _P, _P]
     lib.bifrost_drift.argtypes = [_P, _I64, _P, _I64, _P, _D, _P, _P]
     lib.bifrost_fsi_step.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _D, _P]
-    lib.bifrost_hhs_fsi.argtypes = [_P, _I64, _P, _P, _P, _D, _D, _D, _D, _D, _I, _P, _I64, _P, _P]
+    lib.bifrost_hhs_fsi.argtypes = [_P, _I64, _P, _P, _P, _D, _D, _D, _D, _P, _D, _I, _P, _I64, _P, _P]
     lib.bifrost_kinetic_energy.argtypes = [_P, _I64, _P, _P, _P, _I64, _P, _P]
     lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
     _lib = lib
@@ -420,14 +420,15 @@ class Context:
                                         self._stream())
         self._check(rc, "bifrost_fsi_step")
 
-    def hhs_fsi(self, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, log_cap=0):
+    def hhs_fsi(self, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, log_cap=0, dt_cap=None):
         """One HHS-FSI interval (Eq. 11) in place.  Returns (summary dict, level log as an int64 array [k, 3])."""
         pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
         n = mass.shape[0]
         log = np.zeros((max(int(log_cap), 1), 3), dtype=np.int64)
         summ = np.zeros(3, dtype=np.int64)
         rc = self._lib.bifrost_hhs_fsi(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), float(G),
-                                       float(eps_soft), float(eta_ff), float(eta_fb), float(tau), int(max_depth),
+                                       float(eps_soft), float(eta_ff), float(eta_fb),
+                                       None if dt_cap is None else _dev_f64(dt_cap, (), "dt_cap").data_ptr(), float(tau), int(max_depth),
                                        log.ctypes.data if log_cap else None, int(log_cap), summ.ctypes.data, self._stream())
         self._check(rc, "bifrost_hhs_fsi")
         k = min(int(summ[0]), int(log_cap))

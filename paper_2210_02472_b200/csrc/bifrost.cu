@@ -452,7 +452,7 @@ int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double
 
 struct Hhs {
     bifrost_ctx* ctx; int64_t n; double* pos; double* vel; const double* mass;
-    double G, eps_soft, eta_ff, eta_fb; int max_depth; cudaStream_t st;
+    double G, eps_soft, eta_ff, eta_fb; const double* dt_cap; int max_depth; cudaStream_t st;
     int64_t* log; int64_t log_cap; int64_t n_levels; int64_t deepest; int64_t fsi_steps;
 };
 
@@ -468,14 +468,14 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
         RC_TRY(dtmin_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eta_ff, h.eta_fb, ctx->w_dtff, ctx->w_dtfb,
                           nullptr, nullptr, 0, st));
     if (m <= ctx->small_m) {
-        level_split_small_kernel<<<1, SMALL_M, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow,
+        level_split_small_kernel<<<1, SMALL_M, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, h.dt_cap, depth, tau, all_slow,
                                                         ctx->w_nslow);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());
     } else {
         const int nb = ceil_div(m, PART_T);
         unsigned char* fast = ctx->is_bh;                  // scratch shared with bifrost_pn1 (one call at a time per ctx)
-        level_flag_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, depth, tau, all_slow, fast);
+        level_flag_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, h.dt_cap, depth, tau, all_slow, fast);
         part_count_kernel<<<nb, PART_T, 0, st>>>((int)m, fast, ctx->w_bcount);
         part_scan_kernel<<<1, 32, 0, st>>>(nb, ctx->w_bcount, ctx->w_nslow);
         part_scatter_kernel<<<nb, PART_T, 0, st>>>((int)m, seg, fast, ctx->w_bcount, ctx->w_nslow, ctx->w_tmp);
@@ -907,8 +907,8 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
 }
 
 int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G, double eps_soft,
-                    double eta_ff, double eta_fb, double tau, int max_depth, int64_t* out_level_log, int64_t log_cap,
-                    int64_t* out_summary, void* stream) {
+                    double eta_ff, double eta_fb, const double* dt_cap, double tau, int max_depth, int64_t* out_level_log,
+                    int64_t log_cap, int64_t* out_summary, void* stream) {
     if (!ctx) return BIFROST_EINVAL;
     ctx->err[0] = 0;
     if (n < 0 || n > ctx->max_n || max_depth < 0 || max_depth > 62 || log_cap < 0 || !(tau > 0.0)) return BIFROST_EINVAL;
@@ -924,7 +924,7 @@ int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const
     fill_f64_kernel<<<ceil_div(n, 256), 256, 0, st>>>((int)n, HUGE_VAL, ctx->w_dt0);
     ctx->launches += 2;
     CU_TRY(ctx, cudaGetLastError());
-    Hhs h{ctx, n, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, max_depth, st, out_level_log, log_cap, 0, 0, 0};
+    Hhs h{ctx, n, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, dt_cap, max_depth, st, out_level_log, log_cap, 0, 0, 0};
     rc = hhs_level(h, 0, n, tau, 0);
     if (out_summary) { out_summary[0] = h.n_levels; out_summary[1] = h.deepest; out_summary[2] = h.fsi_steps; }
     if (rc) return rc;

@@ -31,14 +31,15 @@ __global__ void drift_kernel(int m, const int32_t* __restrict__ idx, const doubl
 
 // eps_i = min(eps_ff, eps_fb), never above the level-0 value; fast iff eps_i < tau
 __global__ void level_flag_kernel(int m, const int32_t* __restrict__ seg, const double* __restrict__ dt_ff,
-                                  const double* __restrict__ dt_fb, double* __restrict__ dt0, int depth, double tau,
+                                  const double* __restrict__ dt_fb, double* __restrict__ dt0,
+                                  const double* __restrict__ dt_cap, int depth, double tau,
                                   int all_slow, unsigned char* __restrict__ fast) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= m) return;
     if (all_slow) { fast[k] = 0; return; }
     const int i = seg[k];
     double dt = fmin(dt_ff[i], dt_fb[i]);
-    if (depth == 0) dt0[i] = dt;
+    if (depth == 0) { if (dt_cap) dt = fmin(dt, dt_cap[i]); dt0[i] = dt; }
     dt = fmin(dt, dt0[i]);
     fast[k] = dt < tau ? 1 : 0;
 }
@@ -153,7 +154,8 @@ fsi_small_kernel(int m, const int32_t* __restrict__ idx, double* __restrict__ po
 // Small levels: flag + stable S|F partition + write-back of the level's segment in one CTA.
 __global__ void __launch_bounds__(SMALL_M)
 level_split_small_kernel(int m, int32_t* __restrict__ seg, const double* __restrict__ dt_ff, const double* __restrict__ dt_fb,
-                         double* __restrict__ dt0, int depth, double tau, int all_slow, int* __restrict__ n_slow) {
+                         double* __restrict__ dt0, const double* __restrict__ dt_cap, int depth, double tau, int all_slow,
+                         int* __restrict__ n_slow) {
     __shared__ int warp_slow[SMALL_M / 32];
     const int k = threadIdx.x;
     const bool live = k < m;
@@ -162,7 +164,7 @@ level_split_small_kernel(int m, int32_t* __restrict__ seg, const double* __restr
         i = seg[k];
         if (!all_slow) {
             double dt = fmin(dt_ff[i], dt_fb[i]);
-            if (depth == 0) dt0[i] = dt;
+            if (depth == 0) { if (dt_cap) dt = fmin(dt, dt_cap[i]); dt0[i] = dt; }
             dt = fmin(dt, dt0[i]);
             fast = dt < tau ? 1 : 0;
         }

@@ -689,6 +689,20 @@ def test_hhs_fsi_parity_level_structure_and_energy(torch, ctx):
     assert abs(e1 / e0 - 1) < 1e-7
     assert abs(e1 / I.total_energy(rp, rv, mass, G, eps_soft) - 1) < 1e-12
     assert np.abs((mass[:, None] * vg).sum(0) - (mass[:, None] * vel0).sum(0)).max() < 1e-15
+    # further criteria handed in as dt_cap (here Eq. 24-29 from the oracle's acc, grad, jerk): same hierarchy, same state
+    a0 = oracle.acc(pos0, mass, G, eps_soft)
+    crit = oracle.criteria(vel0, a0, oracle.grad(pos0, mass, a0, G, eps_soft), oracle.jerk(pos0, vel0, mass, G, eps_soft),
+                           eta, eta, eta)
+    cap = np.minimum.reduce([np.asarray(v, dtype=np.float64) for v in crit.values()])
+    rp2, rv2 = pos0.copy(), vel0.copy()
+    stats2 = {}
+    I.hhs_fsi(rp2, rv2, mass, G, eps_soft, eta, eta, tau, max_depth=4, stats=stats2, dt_cap=cap)
+    ref2 = np.array([(d, s, f) for d, s, f, _ in stats2["levels"]], dtype=np.int64)
+    assert not np.array_equal(ref2[0], ref_levels[0])             # the cap does change the level-0 split
+    pos, vel = dev(torch, pos0), dev(torch, vel0)
+    summ, log = ctx.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=4, log_cap=len(ref2) + 4, dt_cap=dev(torch, cap))
+    assert np.array_equal(log, ref2)
+    assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp2, rv2) < 1e-12
     # max_depth = 0: the interval is one FSI cycle over everything
     pos, vel = dev(torch, pos0), dev(torch, vel0)
     summ, log = ctx.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=0, log_cap=4)

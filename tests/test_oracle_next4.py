@@ -185,3 +185,23 @@ def test_hhs_max_depth_bounds_the_recursion():
     I.hhs_fsi(pos, vel, mass, G, 0.0, 0.02, 0.02, 2e-3, max_depth=2, stats=stats)
     assert max(d for d, *_ in stats["levels"]) == 2
     assert all(f == 0 for d, s, f, _ in stats["levels"] if d == 2)
+
+
+def test_hhs_dt_cap_is_minned_into_the_level0_timestep():
+    """"The final time-step of a particle is the minimum of the set of its different time-steps" (L293):
+    a further criterion handed in as dt_cap sends exactly the capped particles to the fast levels."""
+    pos, vel, mass = small_cluster(24, 2)
+    tau = 1e-4                                              # all slow by the pairwise criteria (see above)
+    cap = np.full(24, np.inf)
+    cap[[5, 17]] = 0.3 * tau                                # tau/4 <= cap < tau/2: fast at depths 0 and 1, slow at 2
+    stats = {}
+    I.hhs_fsi(pos, vel, mass, G, 0.05, 0.5, 0.5, tau, stats=stats, dt_cap=cap)
+    lv = [(d, s, f) for d, s, f, _ in stats["levels"]]
+    assert lv[0] == (0, 22, 2) and lv[1] == (1, 0, 2) and lv[2] == (2, 2, 0)
+    assert sorted(lv) == sorted([(0, 22, 2), (1, 0, 2), (1, 0, 2), (2, 2, 0), (2, 2, 0), (2, 2, 0), (2, 2, 0)])
+    # an infinite cap changes nothing
+    p1, v1 = small_cluster(24, 2)[:2]
+    p2, v2 = p1.copy(), v1.copy()
+    I.hhs_fsi(p1, v1, mass, G, 0.05, 0.5, 0.5, tau)
+    I.hhs_fsi(p2, v2, mass, G, 0.05, 0.5, 0.5, tau, dt_cap=np.full(24, np.inf))
+    assert np.array_equal(p1, p2) and np.array_equal(v1, v2)
