@@ -390,9 +390,11 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
     cnt = torch.zeros(n, dtype=torch.int32, device=pos.device)
     lst = torch.full((n, 16), -1, dtype=torch.int32, device=pos.device)
     jerk = torch.zeros_like(acc)
+    acc2 = torch.zeros_like(acc)
     p2, v2 = pos.clone(), vel.clone()
     calls = {
         "jerk": lambda: ctx.jerk(pos, vel, mass, w.G, w.eps, out=jerk),
+        "acc_jerk": lambda: ctx.acc_jerk(pos, vel, mass, w.G, w.eps, out=(acc2, jerk)),
         "potential": lambda: ctx.potential(pos, mass, w.G, w.eps, want_phi=False),
         "neighbours": lambda: ctx.neighbours(pos, vel, mass, w.G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"],
                                              cap=16, out=(cnt, lst)),
@@ -409,7 +411,7 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / 2
         out[name] = {"ms": ms}
-        if name in ("jerk", "potential", "neighbours"):
+        if name in ("jerk", "acc_jerk", "potential", "neighbours"):
             out[name]["interactions_per_s"] = float(n) * n / (ms * 1e-3)
         if name == "fsi_step":
             out[name]["interactions_per_s"] = 4.0 * n * n / (ms * 1e-3)     # four O(N^2) sums

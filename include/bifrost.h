@@ -123,6 +123,15 @@ int bifrost_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* v
                  const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
                  double G, double eps, double* out_jerk, void* stream);
 
+/* bifrost_acc_jerk - NEXT-1 ("can be fused into the acc pass"): bifrost_acc's acceleration
+ * (Eq. 6) and bifrost_jerk's jerk (Eq. 28) of the sinks in ONE pass over the
+ * sources - the pair's separation, softened distance and reciprocal square root are shared, 31 FP64
+ * instructions per pair instead of 15 + 28.  Arguments, layout and index semantics as bifrost_acc /
+ * bifrost_jerk; out_acc and out_jerk (double[n][3], distinct, written at sink rows) must not alias inputs. */
+int bifrost_acc_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                     const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                     double G, double eps, double* out_acc, double* out_jerk, void* stream);
+
 /* bifrost_potential - the potential term of PAPER.md:L63 Eq. 4 (and the first two terms' potential
  * part of the energy book-keeping, L724 Eq. 68), softened like bifrost_acc:
  *     out_phi[i] = -G * sum_{j in src, j != i} mass[j] / sqrt(|r_ji|^2 + eps^2)      (i in sinks; double[n])

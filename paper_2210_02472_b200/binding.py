@@ -30,7 +30,7 @@ SYMBOLS = [
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
     "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
     "bifrost_neighbours", "bifrost_components",
-    "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
+    "bifrost_acc_jerk", "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
 ]
 
 
@@ -75,6 +75,7 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
     lib.bifrost_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _I64, _P, _P, _P]
     lib.bifrost_components.argtypes = [_P, _I64, _P, _P, _I64, _P, _P]
+    lib.bifrost_acc_jerk.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P, _P]
     lib.bifrost_kick.argtypes = [_P, _I64, _P, _I64, _P, _P, _D, _D, _P, _P]
     lib.bifrost_drift.argtypes = [_P, _I64, _P, _I64, _P, _D, _P, _P]
     lib.bifrost_fsi_step.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _D, _P]
@@ -443,4 +444,20 @@ class Context:
         rc = self._lib.bifrost_kinetic_energy(self._h, n, vel.data_ptr(), mass.data_ptr(), ixp or None,
                                               n if ix is None else ix.shape[0], out.data_ptr(), self._stream())
         self._check(rc, "bifrost_kinetic_energy")
+        return out
+
+    def acc_jerk(self, pos, vel, mass, G, eps, sink_idx=None, src_idx=None, out=None):
+        """Acceleration (Eq. 6) and jerk (Eq. 28) in one pass; returns (acc, jerk), each [n, 3]."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        if out is None:
+            out = (torch.zeros((n, 3), dtype=torch.float64, device=pos.device),
+                   torch.zeros((n, 3), dtype=torch.float64, device=pos.device))
+        _dev_f64(out[0], (3,), "out_acc"); _dev_f64(out[1], (3,), "out_jerk")
+        rc = self._lib.bifrost_acc_jerk(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
+                                        n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
+                                        float(G), float(eps), out[0].data_ptr(), out[1].data_ptr(), self._stream())
+        self._check(rc, "bifrost_acc_jerk")
         return out

@@ -256,7 +256,7 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     const SrcArrays src{pos, acc, mass, sub, src_idx};
-    const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial, nullptr, nullptr};
     using Huge = Shape<5, 256, 1, 2>;     // phase-major (GradPassT::pairs), 1.4 % faster per pair than Big
     using Big = Shape<4, 256, 1, 2>;
     using F4 = Shape<4, 128, 3, 2>;
@@ -264,6 +264,24 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     using F1 = Shape<1, 128, 5, 2>;
     return sub ? run_pass<GradPassT<true>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
                : run_pass<GradPassT<false>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+}
+
+// acceleration (Eq. 6) and jerk (Eq. 28) in one pass: GradPassT<EXCL, true> over (x, v, m) records
+int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                  const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                  double* out_acc, double* out_jerk, cudaStream_t st) {
+    const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;
+    if (n_sink == 0) return BIFROST_OK;
+    const SrcArrays src{pos, vel, mass, sub, src_idx};
+    double* p1 = (double*)ctx->partial;
+    double* p2 = (double*)((char*)ctx->partial + ctx->partial_bytes / 2);
+    const GradArgs a{pos, vel, sub, sink_idx, soft2(eps), G, out_jerk, p1, out_acc, p2};
+    using Big = Shape<4, 256, 1, 2>;
+    using F4 = Shape<4, 128, 2, 2>;       // 9 accumulators per sink: two CTAs per SM keep it out of local memory
+    using F2 = Shape<2, 128, 4, 2>;
+    using F1 = Shape<1, 128, 5, 2>;
+    return sub ? run_pass<GradPassT<true, true>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st)
+               : run_pass<GradPassT<false, true>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st);
 }
 
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
@@ -658,6 +676,17 @@ int bifrost_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* v
     DeviceGuard guard(ctx->device);
     // Eq. 28 is Eq. 9's tensor contraction with v_ji in place of a_ji: the same kernel.
     return grad_impl(ctx, n, pos, mass, vel, sink_idx, n_sink, src_idx, n_src, G, eps, out_jerk, 0, (cudaStream_t)stream);
+}
+
+int bifrost_acc_jerk(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                     const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps,
+                     double* out_acc, double* out_jerk, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (n_sink > 0 && (!pos || !vel || !mass || !out_acc || !out_jerk)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return acc_jerk_impl(ctx, n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eps, out_acc, out_jerk,
+                         (cudaStream_t)stream);
 }
 
 int bifrost_potential(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,

@@ -763,3 +763,23 @@ def test_small_level_single_launch_equals_the_general_path_bit_for_bit(torch, ct
         assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
     finally:
         general.close()
+
+
+@pytest.mark.parametrize("cfg,k", [(1, None), (2, 0), (2, 9), (2, 13), (3, 3)])
+def test_acc_jerk_single_pass(torch, ctx, cfg, k):
+    """bifrost_acc_jerk: Eq. 6 and Eq. 28 from one pass over the sources, against the oracle's acc and jerk;
+    all-active, small (fused single-launch) and large (pack -> pair -> finish, split-j) sink sets."""
+    w = workload(cfg)
+    sinks = None if k is None else (W.config2_sink_list(k) if cfg == 2 else W.config3_sink_list(k))
+    if cfg == 3:
+        sinks = sinks[:4096 + 37]                              # config 3: a sample of the 16384-sink list
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    si = None if sinks is None else dev(torch, sinks)
+    a, j = ctx.acc_jerk(pos, vel, mass, w.G, w.eps, si, None)
+    torch.cuda.synchronize()
+    rows = np.arange(w.n) if sinks is None else sinks
+    check_vec(a.cpu().numpy()[rows], oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, None), f"acc_jerk acc cfg{cfg} k={k}")
+    check_vec(j.cpu().numpy()[rows], oracle.jerk(w.pos, w.vel, w.mass, w.G, w.eps, sinks, None), f"acc_jerk jerk cfg{cfg} k={k}")
+    if sinks is not None:
+        rest = np.ones(w.n, bool); rest[sinks] = False
+        assert (a.cpu().numpy()[rest] == 0).all() and (j.cpu().numpy()[rest] == 0).all()
