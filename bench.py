@@ -42,7 +42,7 @@ UNIT = "interactions/s"
 
 # FP64-pipe instruction / flop counts per pair of the kernels' inner loops (
 # cross-checked against the SASS and ncu's smsp__sass_thread_inst_executed_op_d*_pred_on).
-FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 25}     # dtmin: 23 arithmetic + 2 DSETP (ascending source ids)
+FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 23}     # dtmin: 23 arithmetic; the running-maximum test runs on the integer pipe
 FP64_FLOPS = {"acc": 24, "grad": 44, "dtmin": 33}     # FMA = 2, ADD/MUL = 1
 # B200 FP64 ALU peak derived from unit counts and clocks (no fp64 entry in MEASURED_PEAKS.json):
 # 148 SMs x 64 FP64 lanes/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.

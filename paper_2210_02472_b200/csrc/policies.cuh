@@ -253,10 +253,12 @@ struct DtArgs {
 
 // ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
 // the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
+constexpr bool DT_RARE_UPDATE = true;   // dtmin: branch around the running-maximum update (see DtPassT::pairs)
+
 template <bool ASC, bool EXCL>
 struct DtPassT {
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
-    static constexpr int PHASED_MIN_S = 0;
+    static constexpr int PHASED_MIN_S = DT_RARE_UPDATE ? 2 : 0;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
     // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
@@ -310,6 +312,47 @@ struct DtPassT {
             if (!other) { kff = -1.0; kfb = -1.0; }
             if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
             if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
+        }
+    }
+    // The same keys for the S sinks of a thread, but the running (key, id) maxima are touched only when some
+    // key of this source beats one of them - after the first sources that is rare (~1/j for the j-th source), so
+    // the four FSEL and two SEL per pair of pair() become one branch per source that is almost never taken.
+    template <int S>
+    __device__ __forceinline__ static void pairs(const Args&, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        double kff[S], kfb[S];
+        const int jid = __double2loint(r[7]);
+        bool any = false;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const double dx = r[0] - sk[s].x, dy = r[1] - sk[s].y, dz = r[2] - sk[s].z;
+            const double ux = r[4] - sk[s].vx, uy = r[5] - sk[s].vy, uz = r[6] - sk[s].vz;
+            const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
+            const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
+            const double y0 = rsqrt_seed(r2);
+            const double t = y0 * y0;
+            const double e = fma(-r2, t, 1.0);
+            const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
+            const double y3 = (y0 * t) * p3;
+            const double y2 = fma(t, fma(e, e, e), t);
+            kff[s] = (sk[s].m + r[3]) * y3;
+            kfb[s] = v2 * y2;
+            // (the self pair and same-subsystem pairs are filtered in the rare path only)
+            // necessary condition on the integer pipe: the keys are >= 0, so key >= best implies hi(key) >= hi(best)
+            any |= (__double2hiint(kff[s]) >= __double2hiint(c[s].kff)) | (__double2hiint(kfb[s]) >= __double2hiint(c[s].kfb));
+        }
+        if (any) {
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const bool other = EXCL ? ((jid != sk[s].id) & (__double2hiint(r[7]) != sk[s].sub)) : (jid != sk[s].id);
+                if (!other) continue;
+                if (ASC) {
+                    if (kff[s] > c[s].kff) { c[s].kff = kff[s]; c[s].jff = jid; }
+                    if (kfb[s] > c[s].kfb) { c[s].kfb = kfb[s]; c[s].jfb = jid; }
+                } else {
+                    if (kff[s] > c[s].kff || (kff[s] == c[s].kff && jid < c[s].jff)) { c[s].kff = kff[s]; c[s].jff = jid; }
+                    if (kfb[s] > c[s].kfb || (kfb[s] == c[s].kfb && jid < c[s].jfb)) { c[s].kfb = kfb[s]; c[s].jfb = jid; }
+                }
+            }
         }
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
