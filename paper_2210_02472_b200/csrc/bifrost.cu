@@ -296,15 +296,15 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
     const SrcArrays src{pos, vel, mass, sub, src_idx};
     const DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb};
-    using Huge = Shape<6, 128, 2, 1>;     // 2.9 % faster per pair than Big
+    using Huge = Shape<6, 128, 2, 1>;     // 0.7 % faster per pair than Big (after the rarely-taken update branch)
     using Big = Shape<4, 128, 3, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                            : run_pass<DtPassT<true, true>, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
-    return src_idx ? run_pass<DtPass, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                   : run_pass<DtPassAsc, Huge, 28, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                            : run_pass<DtPassT<true, true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return src_idx ? run_pass<DtPass, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+                   : run_pass<DtPassAsc, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,

@@ -89,6 +89,7 @@ ngb_kernel(const NgbArgs a, const Geom g, const double* __restrict__ src_rec) {
         else if (g.n_split == 1) lst[s] = a.out_list + (size_t)(g.compact ? k : ids[s]) * a.cap;
         else lst[s] = a.plist + ((size_t)blockIdx.y * g.n_sink + k) * a.cap;
     }
+    const int guard_hi = __double2hiint(a.r2_guard);
     const int n_tiles = (g.n_src + TILE - 1) / TILE;
     const int tile0 = blockIdx.y * g.tiles_per_split;
     const int tile1 = min(tile0 + g.tiles_per_split, n_tiles);
@@ -109,20 +110,27 @@ ngb_kernel(const NgbArgs a, const Geom g, const double* __restrict__ src_rec) {
         for (int jj = 0; jj < cnt_t; ++jj) {
             const double2 p0 = *reinterpret_cast<const double2*>(tb + jj * REC);
             const double pz = tb[jj * REC + 2];
+            // fast path: the S distances and ONE rarely taken branch.  r^2 >= 0 and the guard >= 0, so
+            // r^2 < guard implies hi(r^2) <= hi(guard): a necessary condition on the integer pipe.
+            double dx[S], dy[S], dz[S], r2[S];
+            bool any = false;
 #pragma unroll
             for (int s = 0; s < S; ++s) {
-                const double dx = p0.x - sx[s], dy = p0.y - sy[s], dz = pz - sz[s];
-                const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-                if (r2 < a.r2_guard) {                      // rare: candidate pair, exact evaluation
-                    const int j = __double2loint(tb[jj * REC + 7]);
-                    if (j != ids[s]) {
-                        const size_t o = 3 * (size_t)ids[s];
-                        const double ux = tb[jj * REC + 4] - a.vel[o], uy = tb[jj * REC + 5] - a.vel[o + 1],
-                                     uz = tb[jj * REC + 6] - a.vel[o + 2];
-                        if (ngb_exact(a, dx, dy, dz, ux, uy, uz, a.mass[ids[s]], tb[jj * REC + 3])) {
-                            if (lst[s] && cnt[s] < a.cap) lst[s][cnt[s]] = j;
-                            ++cnt[s];
-                        }
+                dx[s] = p0.x - sx[s]; dy[s] = p0.y - sy[s]; dz[s] = pz - sz[s];
+                r2[s] = fma(dx[s], dx[s], fma(dy[s], dy[s], dz[s] * dz[s]));
+                any |= __double2hiint(r2[s]) <= guard_hi;
+            }
+            if (any) {                                      // rare: candidate pairs, exact evaluation
+                const int j = __double2loint(tb[jj * REC + 7]);
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    if (!(r2[s] < a.r2_guard) || j == ids[s]) continue;
+                    const size_t o = 3 * (size_t)ids[s];
+                    const double ux = tb[jj * REC + 4] - a.vel[o], uy = tb[jj * REC + 5] - a.vel[o + 1],
+                                 uz = tb[jj * REC + 6] - a.vel[o + 2];
+                    if (ngb_exact(a, dx[s], dy[s], dz[s], ux, uy, uz, a.mass[ids[s]], tb[jj * REC + 3])) {
+                        if (lst[s] && cnt[s] < a.cap) lst[s][cnt[s]] = j;
+                        ++cnt[s];
                     }
                 }
             }
