@@ -172,7 +172,10 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     Geom g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
     g.compact = compact;
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+    if (g.tiles_per_split < RARE_MIN_TILES)     // short source range per CTA: the policy's variant for it (dtmin)
+        pair_fused_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+    else
+        pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -186,7 +189,10 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
 template <class P, class Sh>
 int launch_big(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    if (g.tiles_per_split < RARE_MIN_TILES)
+        pair_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    else
+        pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;

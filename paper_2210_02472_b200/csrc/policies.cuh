@@ -63,6 +63,7 @@ struct AccArgs {
 
 template <bool EXCL>
 struct AccPassT {
+    using Short = AccPassT;
     static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
     static constexpr int PHASED_MIN_S = 0;
     using Args = AccArgs;
@@ -132,6 +133,7 @@ struct GradArgs {
 // Eq. 6's w * r_ji - acceleration and jerk in 31 FP64 instructions instead of 15 + 28.
 template <bool EXCL, bool WITH_ACC = false>
 struct GradPassT {
+    using Short = GradPassT;
     static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
     static constexpr int PHASED_MIN_S = 5;   // measured: phase-major helps at S = 5 (+1.4 %), hurts at S = 4
     using Args = GradArgs;
@@ -253,12 +255,17 @@ struct DtArgs {
 
 // ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
 // the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
-constexpr bool DT_RARE_UPDATE = true;   // dtmin: branch around the running-maximum update (see DtPassT::pairs)
+// RARE = true: the running maxima are updated in a rarely taken branch (DtPassT::pairs) - right when a CTA
+// walks a long source range (an update every ~1/j sources); RARE = false: branch-free selects (pair()) - right
+// when the range is a few tiles, where the maxima still change every few sources.  `Short` names the variant
+// the launcher uses for short ranges (other policies: themselves).
+constexpr int RARE_MIN_TILES = 24;   // measured crossover: ~2500 sources per CTA (profiles/r1_shape_tuning.md)
 
-template <bool ASC, bool EXCL>
+template <bool ASC, bool EXCL, bool RARE = true>
 struct DtPassT {
+    using Short = DtPassT<ASC, EXCL, false>;
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
-    static constexpr int PHASED_MIN_S = DT_RARE_UPDATE ? 2 : 0;
+    static constexpr int PHASED_MIN_S = RARE ? 2 : 0;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
     // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
@@ -428,6 +435,7 @@ struct PotArgs {
 // the self pair does not multiply a zero separation and must be dropped by id (integer select).
 template <bool EXCL>
 struct PotPassT {
+    using Short = PotPassT;
     static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
     static constexpr int PHASED_MIN_S = 0;
     using Args = PotArgs;
