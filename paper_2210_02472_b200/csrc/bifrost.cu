@@ -74,6 +74,7 @@ struct bifrost_ctx {
     // NEXT-4 integrator scratch (allocated on first use of bifrost_fsi_step / bifrost_hhs_fsi)
     bool integ_ready = false;
     double *w_acc = nullptr, *w_grad = nullptr, *w_dtff = nullptr, *w_dtfb = nullptr, *w_dt0 = nullptr;
+    double* w_acc_s = nullptr;       // accelerations of the FSI cycles (rows of a level's slow set), kept between the two H_S of a level
     int32_t *w_order = nullptr, *w_tmp = nullptr;
     int *w_bcount = nullptr, *w_nslow = nullptr;
     int* h_nslow = nullptr;          // pinned
@@ -419,6 +420,7 @@ int ensure_integrator(bifrost_ctx* ctx) {
     const size_t n = (size_t)ctx->max_n;
     CU_TRY(ctx, cudaMalloc(&ctx->w_acc, 24 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_grad, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_acc_s, 24 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dtff, 8 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dtfb, 8 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dt0, 8 * n));
@@ -450,8 +452,11 @@ int drift_impl(bifrost_ctx* ctx, const int32_t* idx, int64_t m, const double* ve
 #define RC_TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
 
 // Eq. 10 over the particles idx[0..m) interacting among themselves (idx == NULL: all n).
+// first_acc_valid: w_acc_s already holds the accelerations of this set at the current positions (left there by the
+// previous cycle over the same set, no drift of its particles since) - the opening sum is then skipped.  Eq. 11 has
+// exactly this situation: between the two H_S of a level only the fast particles move and the slow ones are kicked.
 int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, const int32_t* idx, int64_t m,
-             double G, double eps_soft, double eps, cudaStream_t st) {
+             double G, double eps_soft, double eps, cudaStream_t st, bool first_acc_valid = false) {
     if (m == 0) return BIFROST_OK;
     const bool excl = ctx->subsys && ctx->subsys_n == n;
     if (m <= ctx->small_m && !excl) {                      // one launch for the whole cycle
@@ -460,9 +465,9 @@ int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double
         CU_TRY(ctx, cudaGetLastError());
         return BIFROST_OK;
     }
-    double* a = ctx->w_acc;
+    double* a = ctx->w_acc_s;
     double* g = ctx->w_grad;
-    RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
+    if (!first_acc_valid) RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
     RC_TRY(kick_impl(ctx, idx, m, a, nullptr, eps / 6.0, 0.0, vel, st));
     RC_TRY(drift_impl(ctx, idx, m, vel, eps / 2.0, pos, st));
     RC_TRY(acc_impl(ctx, n, pos, mass, idx, m, idx, m, G, eps_soft, a, 0, st));
@@ -530,16 +535,16 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
         RC_TRY(acc_impl(ctx, h.n, h.pos, h.mass, F, nf, S, ns, h.G, h.eps_soft, a, 0, st));
         return BIFROST_OK;
     };
-    auto H_S = [&]() -> int {
+    auto H_S = [&](bool second) -> int {
         if (ns == 0) return BIFROST_OK;
         h.fsi_steps++;
-        return fsi_impl(ctx, h.n, h.pos, h.vel, h.mass, S, ns, h.G, h.eps_soft, tau / 2.0, st);
+        return fsi_impl(ctx, h.n, h.pos, h.vel, h.mass, S, ns, h.G, h.eps_soft, tau / 2.0, st, second);
     };
     auto H_F = [&]() -> int { return hhs_level(h, lo + ns, hi, tau / 2.0, depth + 1); };
 
     RC_TRY(inter_level_acc());
     if (ns) RC_TRY(kick_impl(ctx, seg, m, a, nullptr, tau / 6.0, 0.0, h.vel, st));
-    RC_TRY(H_S());
+    RC_TRY(H_S(false));
     RC_TRY(H_F());
     RC_TRY(inter_level_acc());
     if (ns) {                                              // Eq. 13
@@ -548,7 +553,7 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
         RC_TRY(kick_impl(ctx, seg, m, a, g, 2.0 * tau / 3.0, tau * tau / 24.0, h.vel, st));
     }
     RC_TRY(H_F());
-    RC_TRY(H_S());
+    RC_TRY(H_S(true));
     RC_TRY(inter_level_acc());
     if (ns) RC_TRY(kick_impl(ctx, seg, m, a, nullptr, tau / 6.0, 0.0, h.vel, st));
     return BIFROST_OK;
@@ -616,7 +621,7 @@ int bifrost_destroy(bifrost_ctx* ctx) {
     cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
-    cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
+    cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_acc_s); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
     cudaFree(ctx->w_order); cudaFree(ctx->w_tmp); cudaFree(ctx->w_bcount); cudaFree(ctx->w_nslow);
     if (ctx->h_nslow) cudaFreeHost(ctx->h_nslow);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
