@@ -783,3 +783,21 @@ def test_acc_jerk_single_pass(torch, ctx, cfg, k):
     if sinks is not None:
         rest = np.ones(w.n, bool); rest[sinks] = False
         assert (a.cpu().numpy()[rest] == 0).all() and (j.cpu().numpy()[rest] == 0).all()
+
+
+@pytest.mark.parametrize("n_sink,n_src", [(5000, 1), (5000, 130), (4096, 3000), (20000, 20000), (4100, 20000),
+                                          (700, 20000), (300, 257), (20000, 4000)])
+def test_launch_paths_matrix(torch, ctx, n_sink, n_src):
+    """Every launch path against the oracle: large sink sets with one or a few source tiles (pack -> pair -> finish,
+    the select variant of dtmin), long source ranges (the update-branch variant, the large grad / dtmin shapes chosen by
+    the launch model), and fused single-launch sets with S = 1, 2, 4."""
+    w = workload(3, n=20000)
+    rng = np.random.default_rng(n_sink * 7 + n_src)
+    sinks = np.sort(rng.choice(w.n, n_sink, replace=False)).astype(np.int32) if n_sink < w.n else None
+    srcs = rng.permutation(w.n)[:n_src].astype(np.int32) if n_src < w.n else None        # unsorted: general tie-break path
+    if srcs is not None and n_src > 200:
+        srcs = np.sort(srcs)                                                             # ascending ids, but through a list
+    a, c, d, acc_in = run_all(torch, ctx, w, sinks=sinks, srcs=srcs)
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), "acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps, sinks, srcs), "grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs), "dtmin")
