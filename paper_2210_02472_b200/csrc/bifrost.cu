@@ -329,8 +329,9 @@ int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     using Big = Shape<4, 128, 4, 2>;
     using F2 = Shape<2, 128, 6, 2>;
     using F1 = Shape<1, 128, 8, 4>;
-    int rc = sub ? run_pass<PotPassT<true>, Big, 0, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st)
-                 : run_pass<PotPassT<false>, Big, 0, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st);
+    using Huge = Shape<8, 128, 2, 1>;     // 5 % faster per pair than Big (profiles/r1_shape_tuning.md)
+    int rc = sub ? run_pass<PotPassT<true>, Huge, 50, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st)
+                 : run_pass<PotPassT<false>, Huge, 50, Big, Big, F2, F1>(ctx, a, src, n_sink, n_src, 8, compact, st);
     if (rc) return rc;
     if (out_W) {
         const int nb = ceil_div(n_sink, WSUM_PER_BLOCK);

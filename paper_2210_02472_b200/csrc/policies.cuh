@@ -437,7 +437,7 @@ template <bool EXCL>
 struct PotPassT {
     using Short = PotPassT;
     static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
-    static constexpr int PHASED_MIN_S = 0;
+    static constexpr int PHASED_MIN_S = 2;
     using Args = PotArgs;
     struct Sink { double x, y, z; int id, sub; };
     struct Acc { double p; };
@@ -471,6 +471,32 @@ struct PotPassT {
         if (__double2loint(r[6]) == s.id) w = 0.0;            // j != i
         if (EXCL && __double2hiint(r[6]) == s.sub) w = 0.0;   // same subsystem
         c.p += w;
+    }
+    // the same sums for the S sinks of a thread; the self pair (and a same-subsystem pair) is zeroed in a branch
+    // that is taken once per sink and source list, instead of two selects per pair
+    template <int S>
+    __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        double w[S];
+        const int jid = __double2loint(r[6]), jcode = __double2hiint(r[6]);
+        bool any = false;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const double dx = r[0] - sk[s].x, dy = r[1] - sk[s].y, dz = r[2] - sk[s].z;
+            const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, a.eps2)));
+            const double y0 = rsqrt_seed(r2);
+            const double t = y0 * y0;
+            const double e = fma(-r2, t, 1.0);
+            const double pm = fma(fma(e, r[5], r[4]), e, r[3]);
+            w[s] = y0 * pm;
+            any |= (jid == sk[s].id) | (EXCL && jcode == sk[s].sub);
+        }
+        if (any) {
+#pragma unroll
+            for (int s = 0; s < S; ++s)
+                if ((jid == sk[s].id) | (EXCL && jcode == sk[s].sub)) w[s] = 0.0;
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s) c[s].p += w[s];
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         if (g.n_split == 1) a.out[g.compact ? k : id] = -a.G * c.p;
