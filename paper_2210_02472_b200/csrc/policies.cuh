@@ -65,7 +65,7 @@ template <bool EXCL>
 struct AccPassT {
     using Short = AccPassT;
     static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
-    static constexpr int PHASED_MIN_S = 0;
+    static constexpr int PHASED_MIN_S = EXCL ? 2 : 0;
     using Args = AccArgs;
     struct Sink { double x, y, z; int sub; };
     struct Acc { double x, y, z; };
@@ -99,6 +99,35 @@ struct AccPassT {
         const double pm = fma(fma(e, r[5], r[4]), e, r[3]);   // m (1 + 3/2 e + 15/8 e^2)
         const double w = (y0 * t) * pm;                       // m / s^3
         c.x = fma(w, dx, c.x); c.y = fma(w, dy, c.y); c.z = fma(w, dz, c.z);
+    }
+    // EXCL only: the same 15 instructions per pair for the S sinks of a thread; a same-subsystem pair is rare, so its
+    // weight is zeroed in a branch taken only when the source shares a subsystem with one of the thread's sinks,
+    // instead of an integer compare and a select per pair (N = 2^20: 1063 -> 1042 ms; plain acc 995 ms).
+    template <int S>
+    __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        double dx[S], dy[S], dz[S], w[S];
+        const int jcode = __double2loint(r[6]);
+        bool any = false;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            dx[s] = r[0] - sk[s].x; dy[s] = r[1] - sk[s].y; dz[s] = r[2] - sk[s].z;
+            const double r2 = fma(dx[s], dx[s], fma(dy[s], dy[s], fma(dz[s], dz[s], a.eps2)));
+            const double y0 = rsqrt_seed(r2);
+            const double t = y0 * y0;
+            const double e = fma(-r2, t, 1.0);
+            const double pm = fma(fma(e, r[5], r[4]), e, r[3]);
+            w[s] = (y0 * t) * pm;
+            any |= jcode == sk[s].sub;
+        }
+        if (any) {
+#pragma unroll
+            for (int s = 0; s < S; ++s)
+                if (jcode == sk[s].sub) w[s] = 0.0;
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            c[s].x = fma(w[s], dx[s], c[s].x); c[s].y = fma(w[s], dy[s], c[s].y); c[s].z = fma(w[s], dz[s], c[s].z);
+        }
     }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         if (g.n_split == 1) {
