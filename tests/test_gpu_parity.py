@@ -544,7 +544,7 @@ def test_neighbours_dense_cluster_every_branch(torch, ctx):
     _check_ngb(got, ref, None, n, 2)
 
 
-@pytest.mark.parametrize("n,sel", [(20000, None), (20000, "subset"), (131072, "subset")])
+@pytest.mark.parametrize("n,sel", [(20000, None), (20000, "subset"), (131072, "subset"), (131072, None)])
 def test_neighbours_config3_binaries(torch, ctx, n, sel):
     """Config 3's binaries (a log-uniform in 1e-4..1e-2 r_h, thermal e): all-active (split-j partial
     lists, concatenated in split order), and random sink subsets against a permuted source list."""
