@@ -37,6 +37,11 @@
  *  - One context per stream; concurrent calls on one context are not allowed.
  *  - Results are bit-identical for identical inputs on the same GPU model: tiling is fixed by
  *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
+ *  - Launch shapes are chosen from the argument sizes alone: below 4096 sinks a call is one
+ *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish.
+ *    Two environment variables, read once in bifrost_create, exist as tuning / test aids and never change
+ *    results beyond the summation order: BIFROST_FUSED_MAX_SINKS (default 4096) and BIFROST_SMALL_M
+ *    (default 128, 0..256: largest particle set whose FSI cycle / level split runs as one single-CTA launch).
  *  - Return value: BIFROST_OK (0) or a negative BIFROST_E* code.  Nothing is printed, nothing
  *    aborts.  On BIFROST_ECUDA, bifrost_last_cuda_error(ctx) holds the CUDA error string.
  */

@@ -6,6 +6,9 @@ paper_2210_02472_b200.  It shares no code with the CUDA path and does not
 import it.  See the header of bifrost_oracle.cpp for what each routine computes,
 the passages of /root/reference/PAPER.md it follows and how it is pinned.
 
+oracle/integrator.py (plain numpy over these routines) is the oracle of the FSI / HHS-FSI integrator
+(NEXT-4).
+
 All routines take host numpy arrays (float64 / int32, C-contiguous) and return
 new numpy arrays; per-sink outputs are compact (row k belongs to sink_idx[k]).
 """
