@@ -264,13 +264,13 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     if (n_sink == 0) return BIFROST_OK;
     const SrcArrays src{pos, acc, mass, sub, src_idx};
     const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial, nullptr, nullptr};
-    using Huge = Shape<5, 256, 1, 2>;     // phase-major (GradPassT::pairs), 1.4 % faster per pair than Big
+    using Huge = Shape<5, 128, 2, 2>;     // phase-major (GradPassT::pairs), 1.6 % faster per pair than Big
     using Big = Shape<4, 256, 1, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    return sub ? run_pass<GradPassT<true>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-               : run_pass<GradPassT<false>, Huge, 14, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return sub ? run_pass<GradPassT<true>, Huge, 8, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<GradPassT<false>, Huge, 8, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 // acceleration (Eq. 6) and jerk (Eq. 28) in one pass: GradPassT<EXCL, true> over (x, v, m) records
