@@ -801,3 +801,20 @@ def test_launch_paths_matrix(torch, ctx, n_sink, n_src):
     check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), "acc")
     check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps, sinks, srcs), "grad")
     check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs), "dtmin")
+
+
+def test_large_set_paths_are_bit_reproducible(torch, ctx):
+    """pack -> pair -> finish with split-j (fixed-order finish), the rarely-taken update branch of dtmin and the
+    model-chosen shapes give bit-identical results run after run (config 3 at full size, all active)."""
+    w = workload(3)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    runs = []
+    for _ in range(2):
+        a = ctx.acc(pos, mass, w.G, w.eps)
+        c = ctx.grad(pos, mass, a, w.G, w.eps)
+        d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+        aj = ctx.acc_jerk(pos, vel, mass, w.G, w.eps)
+        torch.cuda.synchronize()
+        runs.append((a, c, *d, *aj))
+    assert all(torch.equal(x, y) for x, y in zip(*runs))
+    assert torch.isfinite(runs[0][0]).all() and torch.isfinite(runs[0][1]).all()
