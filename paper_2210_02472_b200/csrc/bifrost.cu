@@ -287,8 +287,9 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
     using F4 = Shape<4, 128, 2, 2>;       // 9 accumulators per sink: two CTAs per SM keep it out of local memory
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    return sub ? run_pass<GradPassT<true, true>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st)
-               : run_pass<GradPassT<false, true>, Big, 0, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st);
+    using Huge = Shape<5, 128, 1, 2>;     // phase-major, 4 % faster per pair than Big (2100 vs 2188 ms at N = 2^20)
+    return sub ? run_pass<GradPassT<true, true>, Huge, 40, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st)
+               : run_pass<GradPassT<false, true>, Huge, 40, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st);
 }
 
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
