@@ -37,10 +37,13 @@
 // fly-bys built from chosen (a, e, true anomaly) so that every branch of Eq. 18-19 is hit with a known
 // answer; Fig. 1's chain F-G (shared neighbour) for the components; numpy re-derivation of a, e from
 // the vis-viva and Laplace-Runge-Lenz vector; brute-force union-find.
-// Parity status: acc, grad, dtmin, potential, jerk, phi, criteria pinned.  pn1: the relative two-body
-// dynamics are pinned; the paper prints no PN1.0 formula (PAPER.md:L439, L476 cite
-// Thorne & Hartle 1985 / Einstein et al. 1938), so parity with the paper's own
-// implementation of the per-body split is "parity unpinned" (reading P1).
+// Parity status: acc, grad, dtmin, potential, jerk, phi, criteria, pn1 pinned.  pn1: the paper prints
+// no PN1.0 formula (PAPER.md:L439, L476 cite Thorne & Hartle 1985 / Einstein et al. 1938); reading P1
+// takes the two-body EIH term.  Its relative dynamics are pinned by the test-particle
+// limit, the centre-of-mass identity and the periapsis advance of Eq. 46; the split
+// of the velocity terms between the two bodies, which those cannot see, is pinned in a BOOSTED
+// frame: the 1PN total momentum and energy (Landau & Lifshitz §106) drift as c^-4 along an orbit
+// integrated with acc + pn1, and as c^-2 for any other split (tests/test_oracle_dtmin_pn1.py).
 //
 // Conventions: r_ji = r_j - r_i, the force on
 // sink i points towards source j; a source whose particle id equals the sink's id

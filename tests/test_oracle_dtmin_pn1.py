@@ -243,3 +243,112 @@ def test_pn1_periapsis_advance(q):
     advance = (peri_angles[1] - peri_angles[0]) % (2 * np.pi)
     want = 6 * np.pi * G * M / (c * c * a_sma * (1 - ecc * ecc))
     assert abs(advance / want - 1) < 0.01
+
+
+# --- the per-body split of the PN1.0 pair term (reading P1) --------
+# In the centre-of-mass frame `+4 v_i.v_j` and `-2 v_j.v_j` enter the relative acceleration only
+# through their difference, so the pins above cannot tell (4, -2) from (6, 0).  A BOOSTED frame can:
+# the 1PN (EIH) equations of motion conserve the 1PN total momentum and energy (Landau & Lifshitz,
+# Classical Theory of Fields, §106)
+#   P = sum_a m_a v_a [1 + v_a^2/2c^2 - sum_b G m_b/(2 c^2 r_ab)] - sum_a sum_b G m_a m_b/(2 c^2 r_ab) (n_ab.v_a) n_ab
+#   E = sum_a m_a v_a^2/2 + 3/(8c^2) sum_a m_a v_a^4 - 1/2 sum_ab G m_a m_b/r_ab
+#       + sum_ab G m_a m_b/(4 c^2 r_ab) [6 v_a^2 - 7 v_a.v_b - (n_ab.v_a)(n_ab.v_b)] + sum_abc G^2 m_a m_b m_c/(2 c^2 r_ab r_ac)
+# up to O(c^-4): along an orbit integrated with acc + pn1, their drift must fall 16-fold when c doubles.
+# Any other split of the velocity terms between the two bodies leaves an O(c^-2) drift (ratio 4).
+
+def _eih_momentum(pos, vel, m, G, c):
+    P = np.zeros(3)
+    for a in range(len(m)):
+        s = 1 + vel[a] @ vel[a] / (2 * c * c)
+        for b in range(len(m)):
+            if b == a:
+                continue
+            d = pos[a] - pos[b]
+            r = np.linalg.norm(d)
+            s -= G * m[b] / (2 * c * c * r)
+            P -= G * m[a] * m[b] / (2 * c * c * r) * ((d / r) @ vel[a]) * (d / r)
+        P += m[a] * vel[a] * s
+    return P
+
+
+def _eih_energy(pos, vel, m, G, c):
+    E = 0.0
+    for a in range(len(m)):
+        va2 = vel[a] @ vel[a]
+        E += 0.5 * m[a] * va2 + 3.0 / (8 * c * c) * m[a] * va2 * va2
+        for b in range(len(m)):
+            if b == a:
+                continue
+            d = pos[a] - pos[b]
+            r = np.linalg.norm(d)
+            nab = d / r
+            E -= 0.5 * G * m[a] * m[b] / r
+            E += G * m[a] * m[b] / (4 * c * c * r) * (6 * va2 - 7 * (vel[a] @ vel[b]) - (nab @ vel[a]) * (nab @ vel[b]))
+            for k in range(len(m)):
+                if k != a:
+                    E += G * G * m[a] * m[b] * m[k] / (2 * c * c * r * np.linalg.norm(pos[a] - pos[k]))
+    return E
+
+
+def _pn1_split(ca, cb):
+    """numpy restatement of the pair term with the coefficients of v_i.v_j and v_j.v_j left free
+    (negative control only: (4, -2) is reading P1)."""
+    def f(pos, vel, m, G, c):
+        out = np.zeros_like(pos)
+        for i in range(len(m)):
+            for j in range(len(m)):
+                if i == j:
+                    continue
+                d = pos[i] - pos[j]
+                r = np.linalg.norm(d)
+                n = d / r
+                vi, vj = vel[i], vel[j]
+                A = 5 * G * m[i] / r + 4 * G * m[j] / r + 1.5 * (n @ vj) ** 2 - vi @ vi + ca * (vi @ vj) + cb * (vj @ vj)
+                out[i] += G * m[j] / (c * c * r * r) * (n * A + (4 * (n @ vi) - 3 * (n @ vj)) * (vi - vj))
+        return out
+    return f
+
+
+def _boosted_drift(pn, c, invariant):
+    G = 1.0
+    m = np.array([1.0, 0.4])
+    pos = np.array([[0.6, 0.1, -0.2], [-0.5, 0.3, 0.4]])
+    vel = np.array([[0.3, 0.5, 0.1], [0.2, -0.6, 0.35]])       # total momentum far from zero
+
+    def rhs(p, v):
+        return oracle.acc(p, m, G, 0.0) + pn(p, v, m, G, c)
+
+    q0 = invariant(pos, vel, m, G, c)
+    steps = 400
+    h = 1.0 / steps
+    for _ in range(steps):                                      # RK4, test-only
+        k1p, k1v = vel, rhs(pos, vel)
+        k2p, k2v = vel + 0.5 * h * k1v, rhs(pos + 0.5 * h * k1p, vel + 0.5 * h * k1v)
+        k3p, k3v = vel + 0.5 * h * k2v, rhs(pos + 0.5 * h * k2p, vel + 0.5 * h * k2v)
+        k4p, k4v = vel + h * k3v, rhs(pos + h * k3p, vel + h * k3v)
+        pos = pos + h / 6 * (k1p + 2 * k2p + 2 * k3p + k4p)
+        vel = vel + h / 6 * (k1v + 2 * k2v + 2 * k3v + k4v)
+    return float(np.linalg.norm(np.atleast_1d(invariant(pos, vel, m, G, c) - q0)))
+
+
+def _oracle_pn(pos, vel, m, G, c):
+    return oracle.pn1(pos, vel, m, [0, 1], G, c)
+
+
+@pytest.mark.parametrize("invariant", [_eih_momentum, _eih_energy], ids=["momentum", "energy"])
+def test_pn1_per_body_split_conserves_eih_invariants_in_a_boosted_frame(invariant):
+    d = [_boosted_drift(_oracle_pn, c, invariant) for c in (20.0, 40.0, 80.0)]
+    assert d[2] > 1e-10                                         # well above rounding: the ratios mean something
+    assert abs(d[0] / d[1] - 16) < 1 and abs(d[1] / d[2] - 16) < 1
+    # the restatement with reading P1's (4, -2) is the oracle's formula ...
+    pos, vel, mass = _bodies(6, 57)
+    assert np.allclose(_pn1_split(4, -2)(pos, vel, mass, 1.3, 30.0), oracle.pn1(pos, vel, mass, list(range(6)), 1.3, 30.0),
+                       rtol=0, atol=1e-14 * 1e-3)
+
+
+@pytest.mark.parametrize("split", [(6, 0), (2, -4), (5, -1), (4, -2.1)])
+@pytest.mark.parametrize("invariant", [_eih_momentum, _eih_energy], ids=["momentum", "energy"])
+def test_pn1_wrong_split_is_caught(split, invariant):
+    """Negative control: splits that pass every centre-of-mass pin (same -a + b) leave a c^-2 drift."""
+    d = [_boosted_drift(_pn1_split(*split), c, invariant) for c in (20.0, 40.0, 80.0)]
+    assert d[1] / d[2] < 8

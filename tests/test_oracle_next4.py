@@ -205,3 +205,52 @@ def test_hhs_dt_cap_is_minned_into_the_level0_timestep():
     I.hhs_fsi(p1, v1, mass, G, 0.05, 0.5, 0.5, tau)
     I.hhs_fsi(p2, v2, mass, G, 0.05, 0.5, 0.5, tau, dt_cap=np.full(24, np.inf))
     assert np.array_equal(p1, p2) and np.array_equal(v1, v2)
+
+
+# --- the inter-level kicks of Eq. 11-13: fourth order as a whole -------------
+# With the partition held fixed (dt_cap = 0.75 tau sends five chosen particles to level 1 and no
+# further; eta so large that the pairwise criteria never split), HHS-FSI is a composition of FSI
+# operators and must converge with tau^4 to the fine-step solution.  A wrong inter-level
+# gradient coefficient in Eq. 13 (or a missing S<->F gradient kick) leaves an O(tau^2) error.
+
+def _hhs_fixed_partition_error(steps, reference, grad_scale=1.0, monkeypatch=None):
+    pos, vel, mass = small_cluster(12, 21)
+    T, eps_soft = 0.4, 0.3
+    tau = T / steps
+    cap = np.full(12, np.inf)
+    cap[[1, 4, 6, 9, 10]] = 0.75 * tau
+    if monkeypatch is not None:
+        real = oracle.grad
+
+        def scaled(pos_, mass_, acc_, G_, eps_, sink_idx=None, src_idx=None, **kw):
+            out = real(pos_, mass_, acc_, G_, eps_, sink_idx, src_idx, **kw)
+            inter_level = sink_idx is not None and src_idx is not None and not np.array_equal(sink_idx, src_idx)
+            return out * grad_scale if inter_level else out
+        monkeypatch.setattr(oracle, "grad", scaled)
+    stats = {}
+    for _ in range(steps):
+        I.hhs_fsi(pos, vel, mass, G, eps_soft, 1e3, 1e3, tau, dt_cap=cap, stats=stats)
+    assert [(d, s, f) for d, s, f, _ in stats["levels"]] == [(0, 7, 5), (1, 5, 0), (1, 5, 0)]
+    return float(np.abs(pos - reference).max())
+
+
+@pytest.fixture(scope="module")
+def fine_reference():
+    pos, vel, mass = small_cluster(12, 21)
+    idx = np.arange(12, dtype=np.int32)
+    for _ in range(2048):
+        I.fsi_step(pos, vel, mass, idx, G, 0.3, 0.4 / 2048)
+    return pos
+
+
+def test_hhs_two_level_scheme_is_fourth_order(fine_reference):
+    e = [_hhs_fixed_partition_error(s, fine_reference) for s in (4, 8, 16)]
+    assert e[2] < 2e-9
+    assert 15.0 < e[0] / e[1] < 17.0 and 15.0 < e[1] / e[2] < 17.0
+
+
+@pytest.mark.parametrize("scale", [0.0, 0.5, 1.1, 2.0])
+def test_wrong_inter_level_gradient_coefficient_breaks_fourth_order(scale, fine_reference, monkeypatch):
+    """Eq. 13's gradient kick between S and F with 0, 1/2, 1.1 or 2 times its weight: order 2."""
+    e = [_hhs_fixed_partition_error(s, fine_reference, scale, monkeypatch) for s in (8, 16)]
+    assert e[0] / e[1] < 6.0
