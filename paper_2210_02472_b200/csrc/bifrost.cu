@@ -173,10 +173,7 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     Geom g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
     g.compact = compact;
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    if (g.tiles_per_split < RARE_MIN_TILES)     // short source range per CTA: the policy's variant for it (dtmin)
-        pair_fused_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
-    else
-        pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -190,10 +187,7 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
 template <class P, class Sh>
 int launch_big(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    if (g.tiles_per_split < RARE_MIN_TILES)
-        pair_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
-    else
-        pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -309,10 +303,8 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
-    if (sub) return src_idx ? run_pass<DtPassT<false, true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                            : run_pass<DtPassT<true, true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
-    return src_idx ? run_pass<DtPass, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
-                   : run_pass<DtPassAsc, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+    return sub ? run_pass<DtPassT<true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
+               : run_pass<DtPassT<false>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
 
 int pot_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,

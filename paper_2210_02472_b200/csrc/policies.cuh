@@ -63,7 +63,6 @@ struct AccArgs {
 
 template <bool EXCL>
 struct AccPassT {
-    using Short = AccPassT;
     static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
     static constexpr int PHASED_MIN_S = EXCL ? 2 : 0;
     using Args = AccArgs;
@@ -162,7 +161,6 @@ struct GradArgs {
 // Eq. 6's w * r_ji - acceleration and jerk in 31 FP64 instructions instead of 15 + 28.
 template <bool EXCL, bool WITH_ACC = false>
 struct GradPassT {
-    using Short = GradPassT;
     static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
     static constexpr int PHASED_MIN_S = 5;   // measured: phase-major helps at S = 5 (+1.4 %), hurts at S = 4
     using Args = GradArgs;
@@ -276,29 +274,58 @@ struct DtArgs {
     const double* mass;
     const int32_t* subsys;
     const int32_t* sink_idx;
-    double* pkey;      // [split][2][n_sink]  best keys (ff, fb)
+    double* pkey;      // [split][2][n_sink]  best time-steps (ff, fb) of a split, exact (Eq. 21 / 22 in IEEE operations)
     int32_t* pid;      // [split][2][n_sink]  their source ids
     double G, eta_ff, eta_fb;
     double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
 };
 
-// ASC = true: the source list is in ascending id order (src_idx == NULL), so a strict '>' keeps
-// the first, i.e. the smallest, id among exactly equal keys and the tie-break costs nothing.
-// RARE = true: the running maxima are updated in a rarely taken branch (DtPassT::pairs) - right when a CTA
-// walks a long source range (an update every ~1/j sources); RARE = false: branch-free selects (pair()) - right
-// when the range is a few tiles, where the maxima still change every few sources.  `Short` names the variant
-// the launcher uses for short ranges (other policies: themselves).
-constexpr int RARE_MIN_TILES = 24;   // measured crossover: ~2500 sources per CTA (profiles/r1_shape_tuning.md)
+// Eq. 21 / Eq. 22 for ONE pair in plain IEEE operations (no contraction, correctly rounded sqrt and division),
+// term by term in the oracle's order: the value a time-step is reported with, and the value near-ties are decided
+// on.  Never on the hot path, so they stay out of line.
+__device__ __noinline__ double dt_ff_exact(double dx, double dy, double dz, double G, double mi, double mj, double eta) {
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    const double r = sqrt(r2);
+    return __dmul_rn(eta, sqrt(__dmul_rn(r2, r) / __dmul_rn(G, __dadd_rn(mi, mj))));
+}
+__device__ __noinline__ double dt_fb_exact(double dx, double dy, double dz, double ux, double uy, double uz, double eta) {
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+    if (v2 == 0.0) return __longlong_as_double(0x7ff0000000000000LL);    // reading T3
+    return __dmul_rn(eta, sqrt(r2)) / sqrt(v2);
+}
+// exact time-step of sink i against source j, both read from the caller's arrays (w = 0: Eq. 21, w = 1: Eq. 22)
+__device__ __noinline__ double dt_exact_ids(const DtArgs& a, int w, int i, int j) {
+    const size_t oi = 3 * (size_t)i, oj = 3 * (size_t)j;
+    const double dx = a.pos[oj] - a.pos[oi], dy = a.pos[oj + 1] - a.pos[oi + 1], dz = a.pos[oj + 2] - a.pos[oi + 2];
+    if (w == 0) return dt_ff_exact(dx, dy, dz, a.G, a.mass[i], a.mass[j], a.eta_ff);
+    return dt_fb_exact(dx, dy, dz, a.vel[oj] - a.vel[oi], a.vel[oj + 1] - a.vel[oi + 1], a.vel[oj + 2] - a.vel[oi + 2], a.eta_fb);
+}
+// near-tie between the running best jb and the contender jc of sink i: the oracle's rule on the exact values
+// (smaller time-step; equal time-steps -> smaller particle id, reading T4)
+__device__ __noinline__ bool dt_contender_wins(const DtArgs& a, int w, int i, int jb, int jc) {
+    if (jb < 0) return true;
+    const double tb = dt_exact_ids(a, w, i, jb), tc = dt_exact_ids(a, w, i, jc);
+    return tc < tb || (tc == tb && jc < jb);
+}
 
-template <bool ASC, bool EXCL, bool RARE = true>
+// The fast path MAXIMISES the monotone keys kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)) and kfb = v^2/r^2
+// (= eta^2/dt_fb^2): no sqrt or division per pair.  The keys carry a few ulp of rounding error (<~ 1e-15
+// relative), so a key decides only when it is clear of the running maximum by KEY_SLACK = 1e-12 relative; inside
+// that band (a near-tie) the contender and the running best are both evaluated with dt_*_exact and the
+// oracle's rule decides.  The running best is thus always the exact (time-step, id) minimum of the sources seen,
+// whatever the order of the source list, and the argmin is the oracle's bit for bit.
+constexpr double KEY_SLACK = 1.0 - 1e-12;
+constexpr double KEY_SLACK2 = KEY_SLACK * KEY_SLACK;
+
+template <bool EXCL>
 struct DtPassT {
-    using Short = DtPassT<ASC, EXCL, false>;
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
-    static constexpr int PHASED_MIN_S = RARE ? 2 : 0;
+    static constexpr int PHASED_MIN_S = 1;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
-    // Keys are maximised: kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)), kfb = v^2/r^2 (= eta^2/dt_fb^2).
-    struct Acc { double kff, kfb; int jff, jfb; };
+    // thr = (key of the running best) * KEY_SLACK; j = its source id (-1: none yet)
+    struct Acc { double thr_ff, thr_fb; int jff, jfb; };
     struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
     __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
         if (j >= 0) {
@@ -321,134 +348,95 @@ struct DtPassT {
         s.m = a.mass[id]; s.id = id;
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
-    __device__ static void init(Acc& c) { c.kff = 0.0; c.kfb = 0.0; c.jff = -1; c.jfb = -1; }
-    // FP64-pipe instructions: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
-    // 2 DMUL keys = 23, plus 2 (ASC) or 4 DSETP.
-    __device__ __forceinline__ static void pair(const Args&, const Sink& s, Acc& c, const double* __restrict__ r) {
+    __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; }
+    // one key of one sink against the running best (rare path)
+    __device__ __forceinline__ static void contend(const Args& a, int w, int i, double key, int jid, double& thr, int& jbest) {
+        if (!(key >= thr)) return;
+        const double ks = key * KEY_SLACK;
+        if (key * KEY_SLACK2 > thr || dt_contender_wins(a, w, i, jbest, jid)) { thr = ks; jbest = jid; }
+    }
+    // FP64-pipe instructions of the keys: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
+    // 2 DMUL keys = 23.
+    __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb) {
         const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
         const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
         const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
         const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
-        const int jid = __double2loint(r[7]);
         const double y0 = rsqrt_seed(r2);
         const double t = y0 * y0;
         const double e = fma(-r2, t, 1.0);
         const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
         const double y3 = (y0 * t) * p3;
         const double y2 = fma(t, fma(e, e, e), t);
-        double kff = (s.m + r[3]) * y3;
-        double kfb = v2 * y2;
-        // j != i (Eq. 21, 22) and, with EXCL, not in the sink's subsystem
-        const bool other = EXCL ? ((jid != s.id) & (__double2hiint(r[7]) != s.sub)) : (jid != s.id);
-        if (ASC) {
-            const bool uf = other & (kff > c.kff), ub = other & (kfb > c.kfb);
-            c.kff = uf ? kff : c.kff; c.jff = uf ? jid : c.jff;   // selects, no branches
-            c.kfb = ub ? kfb : c.kfb; c.jfb = ub ? jid : c.jfb;
-        } else {
-            if (!other) { kff = -1.0; kfb = -1.0; }
-            if (kff >= c.kff) { if (kff > c.kff || jid < c.jff) { c.kff = kff; c.jff = jid; } }
-            if (kfb >= c.kfb) { if (kfb > c.kfb || jid < c.jfb) { c.kfb = kfb; c.jfb = jid; } }
-        }
+        kff = (s.m + r[3]) * y3;
+        kfb = v2 * y2;
     }
-    // The same keys for the S sinks of a thread, but the running (key, id) maxima are touched only when some
-    // key of this source beats one of them - after the first sources that is rare (~1/j for the j-th source), so
-    // the four FSEL and two SEL per pair of pair() become one branch per source that is almost never taken.
+    // The keys of the S sinks of a thread and ONE branch per source that is almost never taken (after the first
+    // sources a key comes near the running maximum ~1/j of the time for the j-th source).  The pre-test is a
+    // necessary condition on the integer pipe: keys and thresholds are >= 0, so key >= thr implies
+    // hi(key) >= hi(thr).  (The self pair and same-subsystem pairs are filtered in the rare path only.)
     template <int S>
-    __device__ __forceinline__ static void pairs(const Args&, const Sink* sk, Acc* c, const double* __restrict__ r) {
+    __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
         double kff[S], kfb[S];
-        const int jid = __double2loint(r[7]);
         bool any = false;
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            const double dx = r[0] - sk[s].x, dy = r[1] - sk[s].y, dz = r[2] - sk[s].z;
-            const double ux = r[4] - sk[s].vx, uy = r[5] - sk[s].vy, uz = r[6] - sk[s].vz;
-            const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
-            const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
-            const double y0 = rsqrt_seed(r2);
-            const double t = y0 * y0;
-            const double e = fma(-r2, t, 1.0);
-            const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
-            const double y3 = (y0 * t) * p3;
-            const double y2 = fma(t, fma(e, e, e), t);
-            kff[s] = (sk[s].m + r[3]) * y3;
-            kfb[s] = v2 * y2;
-            // (the self pair and same-subsystem pairs are filtered in the rare path only)
-            // necessary condition on the integer pipe: the keys are >= 0, so key >= best implies hi(key) >= hi(best)
-            any |= (__double2hiint(kff[s]) >= __double2hiint(c[s].kff)) | (__double2hiint(kfb[s]) >= __double2hiint(c[s].kfb));
+            keys(sk[s], r, kff[s], kfb[s]);
+            any |= (__double2hiint(kff[s]) >= __double2hiint(c[s].thr_ff)) | (__double2hiint(kfb[s]) >= __double2hiint(c[s].thr_fb));
         }
         if (any) {
+            const int jid = __double2loint(r[7]);
 #pragma unroll
             for (int s = 0; s < S; ++s) {
                 const bool other = EXCL ? ((jid != sk[s].id) & (__double2hiint(r[7]) != sk[s].sub)) : (jid != sk[s].id);
                 if (!other) continue;
-                if (ASC) {
-                    if (kff[s] > c[s].kff) { c[s].kff = kff[s]; c[s].jff = jid; }
-                    if (kfb[s] > c[s].kfb) { c[s].kfb = kfb[s]; c[s].jfb = jid; }
-                } else {
-                    if (kff[s] > c[s].kff || (kff[s] == c[s].kff && jid < c[s].jff)) { c[s].kff = kff[s]; c[s].jff = jid; }
-                    if (kfb[s] > c[s].kfb || (kfb[s] == c[s].kfb && jid < c[s].jfb)) { c[s].kfb = kfb[s]; c[s].jfb = jid; }
-                }
+                contend(a, 0, sk[s].id, kff[s], jid, c[s].thr_ff, c[s].jff);
+                if (kfb[s] > 0.0) contend(a, 1, sk[s].id, kfb[s], jid, c[s].thr_fb, c[s].jfb);   // v_ij = 0: dt_fb = +inf, never a minimum (T3)
             }
         }
     }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int, const Sink&, const Acc& c) {
+    // the split's winners with their exact time-steps (Eq. 21 / 22 evaluated once per sink and split)
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         const size_t o = (size_t)split * 2 * g.n_sink + k;
-        a.pkey[o] = c.kff; a.pkey[o + g.n_sink] = c.kfb;
+        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+        a.pkey[o] = c.jff >= 0 ? dt_exact_ids(a, 0, id, c.jff) : inf;
+        a.pkey[o + g.n_sink] = c.jfb >= 0 ? dt_exact_ids(a, 1, id, c.jfb) : inf;
         a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
     }
-    // dtmin epilogue: pick the winner over splits (larger key; ties -> smaller id), then evaluate
-    // Eq. 21 / Eq. 22 for the winning pair with IEEE sqrt and division, term by term.
+    // dtmin epilogue: the minimum over the splits' exact time-steps (ties -> smaller id): order-independent.
     static constexpr bool ALWAYS_FINISH = true;
     __device__ static void finish(const Args& a, const Geom& g, int k, int i, int lane, int L, bool write) {
-        double kb[2] = {0.0, 0.0};
+        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+        double tb[2] = {inf, inf};
         int jb[2] = {-1, -1};
+        auto better = [](double t, int j, double tbest, int jbest) {
+            return j >= 0 && (jbest < 0 || t < tbest || (t == tbest && j < jbest));
+        };
         for (int s = lane; s < g.n_split; s += L) {
             for (int w = 0; w < 2; ++w) {
                 const size_t o = ((size_t)s * 2 + w) * g.n_sink + k;
-                const double key = __ldcg(a.pkey + o);
+                const double t = __ldcg(a.pkey + o);
                 const int j = __ldcg(a.pid + o);
-                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+                if (better(t, j, tb[w], jb[w])) { tb[w] = t; jb[w] = j; }
             }
         }
-        for (int off = L >> 1; off > 0; off >>= 1) {      // (max key, then min id) is order-independent
+        for (int off = L >> 1; off > 0; off >>= 1) {      // (min t, then min id) is order-independent
             for (int w = 0; w < 2; ++w) {
-                const double key = __shfl_xor_sync(0xffffffffu, kb[w], off);
+                const double t = __shfl_xor_sync(0xffffffffu, tb[w], off);
                 const int j = __shfl_xor_sync(0xffffffffu, jb[w], off);
-                if (key > kb[w] || (key == kb[w] && j < jb[w])) { kb[w] = key; jb[w] = j; }
+                if (better(t, j, tb[w], jb[w])) { tb[w] = t; jb[w] = j; }
             }
         }
         if (!write || lane != 0) return;
-        const double* pos = a.pos; const double* vel = a.vel;
         const int row = g.compact ? k : i;
-        const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        double tff = inf, tfb = inf;
-        if (jb[0] >= 0) {
-            const int j = jb[0];
-            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            const double r = sqrt(r2);
-            tff = a.eta_ff * sqrt(__dmul_rn(r2, r) / (a.G * (a.mass[i] + a.mass[j])));
-        }
-        if (jb[1] >= 0) {
-            const int j = jb[1];
-            const double dx = pos[3 * (size_t)j] - pos[3 * (size_t)i], dy = pos[3 * (size_t)j + 1] - pos[3 * (size_t)i + 1],
-                         dz = pos[3 * (size_t)j + 2] - pos[3 * (size_t)i + 2];
-            const double ux = vel[3 * (size_t)j] - vel[3 * (size_t)i], uy = vel[3 * (size_t)j + 1] - vel[3 * (size_t)i + 1],
-                         uz = vel[3 * (size_t)j + 2] - vel[3 * (size_t)i + 2];
-            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
-            tfb = __dmul_rn(a.eta_fb, sqrt(r2)) / sqrt(v2);
-        }
-        if (a.dt_ff) a.dt_ff[row] = tff;
-        if (a.dt_fb) a.dt_fb[row] = tfb;
+        if (a.dt_ff) a.dt_ff[row] = jb[0] >= 0 ? tb[0] : inf;
+        if (a.dt_fb) a.dt_fb[row] = jb[1] >= 0 ? tb[1] : inf;
         if (a.j_ff) a.j_ff[row] = jb[0];
         if (a.j_fb) a.j_fb[row] = jb[1];
     }
 };
 
-using DtPass = DtPassT<false, false>;
-using DtPassAsc = DtPassT<true, false>;
+using DtPass = DtPassT<false>;
 
 struct PotArgs {
     const double* pos;
@@ -464,7 +452,6 @@ struct PotArgs {
 // the self pair does not multiply a zero separation and must be dropped by id (integer select).
 template <bool EXCL>
 struct PotPassT {
-    using Short = PotPassT;
     static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
     static constexpr int PHASED_MIN_S = 2;
     using Args = PotArgs;

@@ -4,7 +4,7 @@ element by element on the same seeded inputs.  All tests here need a B200 (`-m g
 Gates (BASELINE.json north_star):
   acc, grad, acc_pn : per-component normwise relative error over the sink set <= 1e-12
   dt_ff, dt_fb      : max relative error <= 1e-13
-  j_ff, j_fb        : identical (where the oracle's runner-up margin exceeds 1e-12; see reading T4)
+  j_ff, j_fb        : identical, bit for bit, ties included (reading T4)
 """
 import numpy as np
 import pytest
@@ -57,12 +57,15 @@ def check_dt(got, ref, what):
         assert np.array_equal(np.isfinite(g), fin), f"{what}: {name} finiteness"
         rel = np.abs(g[fin] / r[fin] - 1.0)
         assert rel.size == 0 or rel.max() <= TOL_DT, f"{what}: {name} rel err {rel.max()}"
-    for name, g, marg in (("j_ff", got[2], ref["margin_ff"]), ("j_fb", got[3], ref["margin_fb"])):
-        r = ref[name]
-        bad = g != r
-        # a mismatch is only admissible when best and runner-up agree to rounding (reading T4)
-        assert not (bad & ~(marg < 1e-12)).any(), f"{what}: {name} argmin mismatch at {np.flatnonzero(bad)[:8]}"
-        assert bad.mean() <= 1e-4, f"{what}: {name} too many near-tie mismatches"
+        # stronger than the gate: the winning pair is evaluated in the oracle's IEEE operation order, so the
+        # values are the oracle's bit for bit
+        assert np.array_equal(g, r), f"{what}: {name} not bit-identical (max rel {rel.max() if rel.size else 0})"
+    for name, g in (("j_ff", got[2]), ("j_fb", got[3])):
+        bad = g != ref[name]
+        near = int((ref["margin" + name[1:]] < 1e-12).sum())
+        print(f"{what}: {name} mismatches {int(bad.sum())} of {bad.size} (near-ties below 1e-12 in the oracle: {near})")
+        # north_star: bit-exact argmin indices - no admissible mismatch, near-ties included (reading T4)
+        assert not bad.any(), f"{what}: {name} argmin mismatch at {np.flatnonzero(bad)[:8]}"
 
 
 def run_all(torch, ctx, w, sinks=None, srcs=None, acc_full=None):
@@ -273,18 +276,16 @@ def test_exact_ties_pick_smaller_id(torch, ctx):
     assert (ref["margin_ff"] == 0).any()
     assert np.array_equal(d[2], ref["j_ff"])
     assert np.array_equal(d[0], ref["dt_ff"])
-    ok = ref["margin_fb"] > 1e-12                       # unequal-r ties are not exact on the GPU's key
-    tie = ref["margin_fb"] == 0
-    assert np.array_equal(d[3][ok], ref["j_fb"][ok])
-    assert np.abs(d[1] / ref["dt_fb"] - 1).max() <= TOL_DT
-    assert tie.sum() >= 0
+    assert (ref["margin_fb"] == 0).any()               # exact fly-by ties, also between pairs of unequal r
+    assert np.array_equal(d[3], ref["j_fb"])
+    assert np.array_equal(d[1], ref["dt_fb"])
     # the same lattice through an UNSORTED source list (the general tie-break path of the kernel)
     srcs = np.random.default_rng(6).permutation(n).astype(np.int32)
     _, _, d2, _ = run_all(torch, ctx, w, srcs=srcs)
     ref2 = oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, src_idx=srcs)
     assert np.array_equal(ref2["j_ff"], ref["j_ff"])          # the minimum does not depend on the list order
     assert np.array_equal(d2[2], ref2["j_ff"]) and np.array_equal(d2[0], ref2["dt_ff"])
-    assert np.array_equal(d2[3][ok], ref2["j_fb"][ok])
+    assert np.array_equal(d2[3], ref2["j_fb"]) and np.array_equal(d2[1], ref2["dt_fb"])
 
 
 def test_determinism_and_host_variants(torch, ctx):
