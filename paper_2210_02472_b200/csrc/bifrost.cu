@@ -42,6 +42,7 @@
 #include "common.cuh"
 #include "policies.cuh"
 #include "pair_kernels.cuh"
+#include "sym_kernels.cuh"
 #include "epilogues.cuh"
 #include "pn1.cuh"
 #include "subsystems.cuh"
@@ -67,6 +68,9 @@ struct bifrost_ctx {
                                      // (env BIFROST_SMALL_M = 0..256 overrides; 0 disables; tuning / test aid)
     int64_t fused_max_sinks = 4096;  // below: one fused launch per call (env BIFROST_FUSED_MAX_SINKS overrides; tuning aid)
     unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel (zero between launches)
+    double* sym_ws = nullptr;        // source-side rows of the symmetric (every pair once) kernels, [block][source][3]
+    size_t sym_ws_bytes = 0;
+    int64_t sym_min_n = 32768;       // shortest list the symmetric kernels are used for
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
     int64_t subsys_n = 0;
     int64_t launches = 0;
@@ -236,11 +240,49 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
     return BIFROST_OK;
 }
 
+// acc / grad over one list that is both sink and source set, every pair once (sym_kernels.cuh).
+// Returns 1 when the call does not qualify (list too short, workspace too small): the caller then takes the plain path.
+template <class P, int S, int T, int MINB>
+int sym_impl(bifrost_ctx* ctx, const double* pos, const double* mass, const double* aux, const int32_t* idx, int64_t m,
+             double G, double eps, double* out, int compact, cudaStream_t st) {
+    if (m < ctx->sym_min_n || !ctx->sym_ws) return 1;
+    SymGeom g;
+    g.m = (int)m;
+    g.n_tiles = ceil_div(m, TILE);
+    g.bs = T * S;
+    g.tb = g.bs / TILE;
+    g.n_blocks = ceil_div(m, g.bs);
+    g.compact = compact;
+    int64_t total = 0;
+    for (int b = 0; b < g.n_blocks; ++b) total += sym_range(g, b);
+    const int64_t slots = (int64_t)ctx->num_sms * MINB;
+    g.unit_tiles = (int)std::max<int64_t>(g.tb, (total + 24 * slots - 1) / (24 * slots));
+    // the sink-side pieces must fit the split-j workspace, the source-side rows the symmetric workspace
+    const int64_t max_pieces_ws = (int64_t)(ctx->partial_bytes / (24 * (size_t)m));
+    if (max_pieces_ws < 1) return 1;
+    while (sym_pieces(g, 0) > max_pieces_ws) g.unit_tiles *= 2;
+    if (24 * (sym_joff(g, g.n_blocks - 1) + (size_t)sym_range(g, g.n_blocks - 1) * TILE) > ctx->sym_ws_bytes) return 1;
+    const int m_pad = g.n_tiles * TILE;
+    sym_pack_kernel<P><<<ceil_div(m_pad, 256), 256, 0, st>>>((int)m, m_pad, idx, pos, mass, aux, ctx->src_rec);
+    const SymArgs a{soft2(eps), G, idx, out, (double*)ctx->partial, ctx->sym_ws};
+    const size_t smem = (2 * TILE * P::REC + (T / 32) * TILE * 3) * sizeof(double);
+    dim3 grid(sym_pieces(g, 0), g.n_blocks);
+    sym_pair_kernel<P, S, T, MINB><<<grid, T, smem, st>>>(a, g, ctx->src_rec);
+    sym_finish_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);
+    ctx->launches += 3;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
 int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* sink_idx,
              int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G, double eps, double* out, int compact,
              cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
+    if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
+        const int rc = sym_impl<SymAcc, 8, 256, 1>(ctx, pos, mass, nullptr, sink_idx, n_sink, G, eps, out, compact, st);
+        if (rc <= 0) return rc;
+    }
     const SrcArrays src{pos, nullptr, mass, sub, src_idx};
     const AccArgs a{pos, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
     using Big = Shape<8, 256, 1, 1>;
@@ -256,6 +298,10 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
               double* out, int compact, cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
+    if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
+        const int rc = sym_impl<SymGrad, 4, 256, 1>(ctx, pos, mass, acc, sink_idx, n_sink, G, eps, out, compact, st);
+        if (rc <= 0) return rc;
+    }
     const SrcArrays src{pos, acc, mass, sub, src_idx};
     const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial, nullptr, nullptr};
     using Huge = Shape<5, 128, 2, 2>;     // phase-major (GradPassT::pairs), 1.6 % faster per pair than Big
@@ -605,6 +651,16 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
         bifrost_destroy(ctx);
         return BIFROST_ENOMEM;
     }
+    // symmetric kernels: 12 max_n^2 / (sinks per CTA) bytes of source-side rows (sized for the smaller block of the two
+    // passes); skipped when that exceeds a quarter of the free device memory (those calls then take the plain path)
+    {
+        const size_t need = 24 * ((size_t)max_n + 2048) * ((size_t)max_n / 2048 + 2);
+        size_t free_b = 0, total_b = 0;
+        if (max_n >= ctx->sym_min_n && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need < free_b / 4 &&
+            cudaMalloc(&ctx->sym_ws, need) == cudaSuccess)
+            ctx->sym_ws_bytes = need;
+        else { cudaGetLastError(); ctx->sym_ws = nullptr; }
+    }
     *out = ctx;
     return BIFROST_OK;
 }
@@ -612,7 +668,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
 int bifrost_destroy(bifrost_ctx* ctx) {
     if (!ctx) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets);
+    cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets); cudaFree(ctx->sym_ws);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
     cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_acc_s); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);

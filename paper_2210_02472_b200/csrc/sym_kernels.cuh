@@ -1,0 +1,328 @@
+// sym_kernels.cuh - acc (Eq. 6) and grad (Eq. 9) over ONE list that is both the sink and the source set, every
+// unordered pair evaluated ONCE (Newton's third law: "pairwise kicks").
+// Part of the single translation unit bifrost.cu (see its header and DESIGN.md); not a public header.
+//
+// 12 of acc's 15 and 22 of grad's 28 FP64 instructions per ordered pair are pair geometry that is identical for
+// (i <- j) and (j <- i); here they are issued once and both members get their term:
+//     acc : a_i += m_j s^-3 r_ji              a_j -= m_i s^-3 r_ji                         20 instructions per unordered pair
+//     grad: U_i += m_j s^-3 a_ji,  W_i += m_j q s^-5 r_ji     U_j -= m_i s^-3 a_ji,  W_j -= m_i q s^-5 r_ji   38
+// The list is cut into blocks of BS = T*S positions.  A CTA owns one block as SINKS (S per thread, in registers)
+// and a range of source tiles strictly beyond its block; for every source it also forms the source-side sum
+// over its own sinks: per thread over its S sinks in registers, over the 32 lanes of a warp with a fixed
+// reduce-scatter + butterfly of shuffles (4 sources at a time: 4.5 DADD per source and warp instead of 15), over
+// the warps of the CTA through shared memory in warp order.  That sum goes to a [block][source] workspace; the
+// tiles of the block itself (the diagonal) are evaluated the plain way (both orders, sink side only).  A finish
+// kernel adds, for list position k in block b, the sink-side pieces of block b and the source-side rows written by
+// blocks 0..b-1, all in a fixed order: bit-identical run to run, no floating-point atomics.
+#pragma once
+
+namespace {
+
+struct SymGeom {
+    int m;            // list length (sinks = sources)
+    int n_tiles;      // ceil(m / TILE); records are zero-padded to n_tiles * TILE
+    int bs;           // list positions per block = T * S
+    int tb;           // tiles per block = bs / TILE
+    int n_blocks;     // ceil(m / bs)
+    int unit_tiles;   // target number of source tiles per CTA
+    int compact;      // 1: output row = list position, 0: output row = particle id
+};
+// source tiles strictly beyond block b
+__host__ __device__ inline int sym_range(const SymGeom& g, int b) {
+    const int r = g.n_tiles - (b + 1) * g.tb;
+    return r > 0 ? r : 0;
+}
+// CTAs (pieces) that share block b: piece 0 also does the diagonal
+__host__ __device__ inline int sym_pieces(const SymGeom& g, int b) {
+    const int r = sym_range(g, b);
+    return r > 0 ? (r + g.unit_tiles - 1) / g.unit_tiles : 1;
+}
+// first row of block b in the source-side workspace: rows of blocks b' < b, each (n_tiles - (b'+1) tb) * TILE long
+__host__ __device__ inline size_t sym_joff(const SymGeom& g, int b) {
+    return ((size_t)b * g.n_tiles - (size_t)g.tb * ((size_t)b * (b + 1) / 2)) * TILE;
+}
+
+struct SymArgs {
+    double eps2, G;
+    const int32_t* idx;     // the list (NULL: particles 0..m-1)
+    double* out;            // [.][3]
+    double* pi;             // sink-side pieces   [piece][m][3]
+    double* pj;             // source-side rows   [sym_joff(b) + j - (b+1) bs][3]
+};
+
+// ---- policies ---------------------------------------------------------------------------------------
+
+struct SymAcc {
+    static constexpr int REC = 4;            // x y z m
+    struct Sink { double x, y, z, m; };
+    struct Acc { double x, y, z; };
+    __device__ __forceinline__ static void load_sink(const double* __restrict__ r, bool live, Sink& s) {
+        s.x = r[0]; s.y = r[1]; s.z = r[2]; s.m = live ? r[3] : 0.0;
+    }
+    __device__ __forceinline__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
+    // s^-3 of one pair: 3 DADD, 3 DFMA, DMUL, DFMA, 2 DFMA, 2 DMUL = 12 FP64-pipe instructions
+    __device__ __forceinline__ static double inv_s3(double eps2, const Sink& s, const double* __restrict__ r, double& dx,
+                                                    double& dy, double& dz) {
+        dx = r[0] - s.x; dy = r[1] - s.y; dz = r[2] - s.z;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double p = fma(fma(e, 1.875, 1.5), e, 1.0);
+        return (y0 * t) * p;
+    }
+    // diagonal tiles: ordered pairs, sink side only (15 instructions)
+    __device__ __forceinline__ static void pair(const SymArgs& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        double dx, dy, dz;
+        const double w = inv_s3(a.eps2, s, r, dx, dy, dz) * r[3];
+        c.x = fma(w, dx, c.x); c.y = fma(w, dy, c.y); c.z = fma(w, dz, c.z);
+    }
+    // S sinks of a thread against one source, both sides (20 instructions per pair); J[0..3) = the thread's
+    // source-side sum  sum_s m_s s^-3 r_js  (the finish kernel subtracts it: the force on j points to i)
+    template <int S>
+    __device__ __forceinline__ static void pairs(const SymArgs& a, const Sink* sk, Acc* c, const double* __restrict__ r,
+                                                 double* J) {
+        double jx = 0.0, jy = 0.0, jz = 0.0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            double dx, dy, dz;
+            const double s3 = inv_s3(a.eps2, sk[s], r, dx, dy, dz);
+            const double wi = s3 * r[3], wj = s3 * sk[s].m;
+            c[s].x = fma(wi, dx, c[s].x); c[s].y = fma(wi, dy, c[s].y); c[s].z = fma(wi, dz, c[s].z);
+            jx = fma(wj, dx, jx); jy = fma(wj, dy, jy); jz = fma(wj, dz, jz);
+        }
+        J[0] = jx; J[1] = jy; J[2] = jz;
+    }
+    __device__ __forceinline__ static void result(const Acc& c, double* o) { o[0] = c.x; o[1] = c.y; o[2] = c.z; }
+};
+
+struct SymGrad {
+    static constexpr int REC = 8;            // x y z m ax ay az -
+    struct Sink { double x, y, z, m, ax, ay, az; };
+    struct Acc { double ux, uy, uz, wx, wy, wz; };
+    __device__ __forceinline__ static void load_sink(const double* __restrict__ r, bool live, Sink& s) {
+        s.x = r[0]; s.y = r[1]; s.z = r[2]; s.m = live ? r[3] : 0.0; s.ax = r[4]; s.ay = r[5]; s.az = r[6];
+    }
+    __device__ __forceinline__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
+    // common part of one pair (22 instructions): s3 = s^-3, v = (a_ji . r_ji) s^-5
+    __device__ __forceinline__ static void geom(double eps2, const Sink& s, const double* __restrict__ r, double& dx, double& dy,
+                                                double& dz, double& bx, double& by, double& bz, double& s3, double& v) {
+        dx = r[0] - s.x; dy = r[1] - s.y; dz = r[2] - s.z;
+        bx = r[4] - s.ax; by = r[5] - s.ay; bz = r[6] - s.az;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+        const double q = fma(bx, dx, fma(by, dy, bz * dz));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double p = fma(fma(e, 1.875, 1.5), e, 1.0);
+        s3 = (y0 * t) * p;
+        const double y2 = fma(t, fma(e, e, e), t);
+        v = (s3 * y2) * q;
+    }
+    __device__ __forceinline__ static void pair(const SymArgs& a, const Sink& s, Acc& c, const double* __restrict__ r) {
+        double dx, dy, dz, bx, by, bz, s3, v;
+        geom(a.eps2, s, r, dx, dy, dz, bx, by, bz, s3, v);
+        const double wi = s3 * r[3], vi = v * r[3];
+        c.ux = fma(wi, bx, c.ux); c.uy = fma(wi, by, c.uy); c.uz = fma(wi, bz, c.uz);
+        c.wx = fma(vi, dx, c.wx); c.wy = fma(vi, dy, c.wy); c.wz = fma(vi, dz, c.wz);
+    }
+    // both sides (38 instructions per pair): the source's term is -(m_i / m_j) times the sink's
+    template <int S>
+    __device__ __forceinline__ static void pairs(const SymArgs& a, const Sink* sk, Acc* c, const double* __restrict__ r,
+                                                 double* J) {
+        double ux = 0.0, uy = 0.0, uz = 0.0, wx = 0.0, wy = 0.0, wz = 0.0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            double dx, dy, dz, bx, by, bz, s3, v;
+            geom(a.eps2, sk[s], r, dx, dy, dz, bx, by, bz, s3, v);
+            const double wi = s3 * r[3], vi = v * r[3], wj = s3 * sk[s].m, vj = v * sk[s].m;
+            c[s].ux = fma(wi, bx, c[s].ux); c[s].uy = fma(wi, by, c[s].uy); c[s].uz = fma(wi, bz, c[s].uz);
+            c[s].wx = fma(vi, dx, c[s].wx); c[s].wy = fma(vi, dy, c[s].wy); c[s].wz = fma(vi, dz, c[s].wz);
+            ux = fma(wj, bx, ux); uy = fma(wj, by, uy); uz = fma(wj, bz, uz);
+            wx = fma(vj, dx, wx); wy = fma(vj, dy, wy); wz = fma(vj, dz, wz);
+        }
+        J[0] = fma(-3.0, wx, ux); J[1] = fma(-3.0, wy, uy); J[2] = fma(-3.0, wz, uz);
+    }
+    __device__ __forceinline__ static void result(const Acc& c, double* o) {
+        o[0] = fma(-3.0, c.wx, c.ux); o[1] = fma(-3.0, c.wy, c.uy); o[2] = fma(-3.0, c.wz, c.uz);
+    }
+};
+
+// ---- pack: the list's records in list order, zero-padded to a whole number of tiles -------------------
+template <class P>
+__global__ void sym_pack_kernel(int m, int m_pad, const int32_t* __restrict__ idx, const double* __restrict__ pos,
+                                const double* __restrict__ mass, const double* __restrict__ aux, double* __restrict__ rec) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= m_pad) return;
+    double2* o = reinterpret_cast<double2*>(rec + (size_t)l * P::REC);
+    if (l >= m) {
+#pragma unroll
+        for (int q = 0; q < P::REC / 2; ++q) o[q] = make_double2(0.0, 0.0);
+        return;
+    }
+    const size_t j = idx ? idx[l] : l;
+    o[0] = make_double2(pos[3 * j], pos[3 * j + 1]);
+    o[1] = make_double2(pos[3 * j + 2], mass[j]);
+    if (P::REC == 8) {
+        o[2] = make_double2(aux[3 * j], aux[3 * j + 1]);
+        o[3] = make_double2(aux[3 * j + 2], 0.0);
+    }
+}
+
+// Sum over the 32 lanes of a warp of 4 sources x 3 components held per lane (L[q][c]): two reduce-scatter steps
+// (lane bit 0 keeps sources {0,1} or {2,3}, lane bit 1 one of the two) and a butterfly over lane bits 2-4.
+// Afterwards every lane holds, in R[0..3), the warp's sum for source q = 2 (lane & 1) + ((lane >> 1) & 1).
+// 18 DADD per 4 sources; the order of the additions is fixed by the lane numbers (a + b is commutative bit for
+// bit, so all lanes of a residue class agree).
+__device__ __forceinline__ void warp_sum_4x3(const double (*L)[3], int lane, double* R) {
+    const bool b0 = lane & 1, b1 = lane & 2;
+    double M[2][3];
+#pragma unroll
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double keep = b0 ? L[q + 2][c] : L[q][c];
+            const double send = b0 ? L[q][c] : L[q + 2][c];
+            M[q][c] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+        }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double keep = b1 ? M[1][c] : M[0][c];
+        const double send = b1 ? M[0][c] : M[1][c];
+        double v = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        v += __shfl_xor_sync(0xffffffffu, v, 8);
+        v += __shfl_xor_sync(0xffffffffu, v, 16);
+        R[c] = v;
+    }
+}
+
+// ---- the pair kernel: grid = (max pieces, blocks) ---------------------------------------------------
+template <class P, int S, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB)
+sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec) {
+    constexpr int REC = P::REC;
+    constexpr int NW = T / 32;
+    constexpr int CHUNKS = TILE * REC * 8 / 16;
+    extern __shared__ __align__(16) double sym_sm[];
+    double* tile_sm = sym_sm;                       // [2][TILE * REC]
+    double* wbuf = sym_sm + 2 * TILE * REC;         // [NW][TILE][3] source-side sums per warp
+
+    const int b = blockIdx.y, piece = blockIdx.x;
+    const int range = sym_range(g, b), np = sym_pieces(g, b);
+    if (piece >= np) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    typename P::Sink sink[S];
+    typename P::Acc accu[S];
+    const int kbase = b * g.bs + threadIdx.x;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * T;
+        const bool live = k < g.m;                  // tail threads shadow the last list entry with mass 0
+        P::load_sink(rec + (size_t)(live ? k : g.m - 1) * REC, live, sink[s]);
+        P::init(accu[s]);
+    }
+
+    auto load_tile = [&](int tile, int buf) {
+        const double* gsrc = rec + (size_t)tile * TILE * REC;
+        double* dst = tile_sm + buf * TILE * REC;
+        for (int ch = threadIdx.x; ch < CHUNKS; ch += T) cp_async16(dst + 2 * ch, gsrc + 2 * ch);
+        cp_async_commit();
+    };
+
+    // this piece's tiles: [d0, d1) diagonal (piece 0 only), then [t0, t1) beyond the block
+    const int jb = (b + 1) * g.tb;
+    const int len = range > 0 ? (range + np - 1) / np : 0;
+    const int t0 = jb + piece * len, t1 = min(t0 + len, g.n_tiles);
+    const int d0 = b * g.tb, d1 = piece == 0 ? min(jb, g.n_tiles) : d0;
+    const int n_my = (d1 - d0) + max(t1 - t0, 0);
+    auto tile_of = [&](int q) { return q < d1 - d0 ? d0 + q : t0 + (q - (d1 - d0)); };
+
+    if (n_my > 0) load_tile(tile_of(0), 0);
+    for (int q = 0; q < n_my; ++q) {
+        const int buf = q & 1;
+        const int tile = tile_of(q);
+        if (q + 1 < n_my) { load_tile(tile_of(q + 1), buf ^ 1); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        const double* __restrict__ tb = tile_sm + buf * TILE * REC;
+        if (tile < jb) {                            // diagonal: ordered pairs, sink side only
+            const int cnt = min(TILE, g.m - tile * TILE);
+            for (int jj = 0; jj < cnt; ++jj) {
+                double r[REC];
+#pragma unroll
+                for (int w = 0; w < REC; w += 2) {
+                    const double2 v = *reinterpret_cast<const double2*>(tb + jj * REC + w);
+                    r[w] = v.x; r[w + 1] = v.y;
+                }
+#pragma unroll
+                for (int s = 0; s < S; ++s) P::pair(a, sink[s], accu[s], r);
+            }
+            __syncthreads();
+            continue;
+        }
+        // beyond the block: every pair once, both sides (padding records have mass 0 and get a sum nobody reads)
+        for (int j4 = 0; j4 < TILE; j4 += 4) {
+            double L[4][3];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                double r[REC];
+#pragma unroll
+                for (int w = 0; w < REC; w += 2) {
+                    const double2 v = *reinterpret_cast<const double2*>(tb + (j4 + u) * REC + w);
+                    r[w] = v.x; r[w + 1] = v.y;
+                }
+                P::template pairs<S>(a, sink, accu, r, L[u]);
+            }
+            double R[3];
+            warp_sum_4x3(L, lane, R);
+            if (lane < 4) {
+                double* o = wbuf + ((size_t)warp * TILE + j4 + 2 * (lane & 1) + (lane >> 1)) * 3;
+                o[0] = R[0]; o[1] = R[1]; o[2] = R[2];
+            }
+        }
+        __syncthreads();
+        // the CTA's source-side sum of this tile: warps added in warp order, rows to the workspace
+        {
+            double* dst = a.pj + (sym_joff(g, b) + (size_t)(tile - jb) * TILE) * 3;
+            for (int e = threadIdx.x; e < TILE * 3; e += T) {
+                double v = wbuf[e];
+#pragma unroll
+                for (int w = 1; w < NW; ++w) v += wbuf[w * TILE * 3 + e];
+                dst[e] = v;
+            }
+        }
+        __syncthreads();
+    }
+
+    // sink-side piece
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const int k = kbase + s * T;
+        if (k < g.m) P::result(accu[s], a.pi + 3 * ((size_t)piece * g.m + k));
+    }
+}
+
+// ---- finish: fixed-order sum of the sink-side pieces of the own block and the source-side rows of the earlier blocks
+__global__ void sym_finish_kernel(const SymArgs a, const SymGeom g) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= g.m) return;
+    const int b = k / g.bs;
+    const int np = sym_pieces(g, b);
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int p = 0; p < np; ++p) {
+        const double* q = a.pi + 3 * ((size_t)p * g.m + k);
+        sx += __ldcg(q); sy += __ldcg(q + 1); sz += __ldcg(q + 2);
+    }
+    double jx = 0.0, jy = 0.0, jz = 0.0;
+    for (int bb = 0; bb < b; ++bb) {
+        const double* q = a.pj + 3 * (sym_joff(g, bb) + (size_t)(k - (bb + 1) * g.bs));
+        jx += __ldcg(q); jy += __ldcg(q + 1); jz += __ldcg(q + 2);
+    }
+    const size_t row = g.compact ? (size_t)k : (size_t)(a.idx ? a.idx[k] : k);
+    double* o = a.out + 3 * row;
+    o[0] = a.G * (sx - jx); o[1] = a.G * (sy - jy); o[2] = a.G * (sz - jz);
+}
+
+}  // namespace
