@@ -20,17 +20,27 @@
  *  - sink_idx / src_idx / bh_idx : int32 particle ids in [0, n) (not range-checked).
  *    NULL means "all n particles in id order" and then the matching count must equal n.
  *  - r_ji = r_j - r_i (L65): the force on sink i points towards source j.
- *  - A source whose id equals the sink's id is skipped ("j != i", Eq. 6).  Distinct particles
- *    at exactly the same position with eps = 0 are outside the contract (the pair is dropped
- *    from acc/grad instead of producing inf/NaN).
+ *  - A source whose id equals the sink's id is skipped ("j != i", Eq. 6).
+ *  - Coincident DISTINCT particles (r_ji = 0 exactly, j != i) at eps = 0 (reading A3b), where the
+ *    literal formulas have 0/0: r^2 carries a floor of 2^-300, so the pair's weight is finite (m 2^450) and
+ *    nothing becomes inf or NaN.  In bifrost_acc it multiplies a zero separation: the pair contributes
+ *    exactly 0.  In bifrost_grad / bifrost_jerk it multiplies a_ji (v_ji): the two coincident sinks get a
+ *    finite value WITHOUT meaning (0 if a_ji = 0 exactly, else rounding noise times 2^450); every OTHER
+ *    sink is unaffected in all calls.
+ *    bifrost_dtmin reports dt_ff = 0 (and dt_fb = 0 unless v_ij = 0 too) with that source as argmin, as
+ *    Eq. 21-22 give; bifrost_potential a large finite value.  With eps > 0 such a pair is regular.
  *  - Duplicate ids in src_idx are summed twice; duplicates in sink_idx are harmless.
  *  - n_sink == 0 is a no-op.  n_src == 0 gives zeros (acc, grad) or +inf with id -1 (dtmin).
  *  - Results are written only at out[sink id]; other rows are untouched (bifrost_pn1 overwrites
  *    all n rows).  Outputs must not alias inputs.
  *  - Device entry points: every pointer is a DEVICE pointer owned by the caller; the call is
  *    asynchronous on `stream` (a cudaStream_t passed as void*, NULL = legacy default stream) and
- *    never synchronises the host.  The library owns only the scratch inside bifrost_ctx, which
- *    is allocated once in bifrost_create (no allocation afterwards).
+ *    never synchronises the host.  The library owns only the scratch inside bifrost_ctx.  The scratch of
+ *    the pair calls (packed records, split-j partials, the symmetric kernels' rows) is allocated in
+ *    bifrost_create.  Two groups are allocated on FIRST USE - an implicit device synchronisation and a
+ *    possible BIFROST_ECUDA in the middle of a run: the device mirrors + pinned staging of the *_host
+ *    calls, and the integrator scratch of bifrost_fsi_step / bifrost_hhs_fsi.  bifrost_reserve
+ *    allocates them ahead of time; after it no call allocates.
  *  - *_host entry points: every pointer is a HOST pointer (pinned or pageable); the call copies
  *    the inputs to device scratch owned by the context, runs the same kernels, copies the
  *    results back and returns after the stream has drained.
@@ -38,10 +48,10 @@
  *  - Results are bit-identical for identical inputs on the same GPU model: tiling is fixed by
  *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
  *  - Launch shapes are chosen from the argument sizes alone: below 4096 sinks a call is one
- *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish.
- *    Two environment variables, read once in bifrost_create, exist as tuning / test aids and never change
- *    results beyond the summation order: BIFROST_FUSED_MAX_SINKS (default 4096) and BIFROST_SMALL_M
- *    (default 128, 0..256: largest particle set whose FSI cycle / level split runs as one single-CTA launch).
+ *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish;
+ *    bifrost_acc / bifrost_grad whose sink and source lists are the SAME list (same pointer, or both
+ *    NULL) of >= 16384 / 12288 entries evaluate every unordered pair once (symmetric kernels).  The
+ *    thresholds are bifrost_set_tuning knobs; no environment variable or file is read.
  *  - Return value: BIFROST_OK (0) or a negative BIFROST_E* code.  Nothing is printed, nothing
  *    aborts.  On BIFROST_ECUDA, bifrost_last_cuda_error(ctx) holds the CUDA error string.
  */
@@ -63,11 +73,32 @@ extern "C" {
 typedef struct bifrost_ctx bifrost_ctx;
 
 /* Create a context on CUDA device `device` able to handle up to max_n particles (ids < max_n,
- * list lengths <= max_n).  Allocates all scratch: packed source records (80 B x max_n),
- * split-j partials, BH flags, and device mirrors for the *_host entry points (lazily, on the
- * first *_host call).  *ctx is set to NULL on failure. */
+ * list lengths <= max_n).  Allocates the scratch of the pair calls: packed source records (80 B x max_n),
+ * split-j partials (1536 B x max_n), BH flags, and - when max_n >= 12288 and it fits in a quarter of the
+ * free device memory - the source-side rows of the symmetric kernels (12 max_n^2 / 1536 bytes: 8.6 GB at
+ * max_n = 2^20, 34 GB at 2^21; without them those calls take the plain kernels).  *ctx is set to NULL on failure. */
 int bifrost_create(bifrost_ctx** ctx, int device, int64_t max_n);
 int bifrost_destroy(bifrost_ctx* ctx);
+
+/* Allocate now what would otherwise be allocated on first use (see "Device entry points" above):
+ * what = BIFROST_RESERVE_HOST (mirrors of the *_host calls, ~30 x 8 B x max_n device + 32 B x max_n pinned)
+ * and/or BIFROST_RESERVE_INTEGRATOR (scratch of bifrost_fsi_step / bifrost_hhs_fsi, ~110 B x max_n).
+ * Synchronous.  BIFROST_ECUDA if an allocation fails (the context stays usable for the other calls). */
+#define BIFROST_RESERVE_HOST        1
+#define BIFROST_RESERVE_INTEGRATOR  2
+int bifrost_reserve(bifrost_ctx* ctx, int what);
+
+/* Launch-shape knobs.  They never change a result beyond its summation order; they exist for tuning and so
+ * that tests can drive every launch path at small sizes.
+ *   BIFROST_TUNE_FUSED_MAX_SINKS  calls with fewer sinks run as one fused launch (default 4096, 0..131072)
+ *   BIFROST_TUNE_SMALL_M          largest particle set whose FSI cycle / level split is one single-CTA launch
+ *                                 (default 128, 0..256; 0 disables)
+ *   BIFROST_TUNE_SYM_MIN_N        shortest same-list call that takes the symmetric kernels (default 16384 for
+ *                                 acc, 12288 for grad; this knob sets both; a value above max_n disables them) */
+#define BIFROST_TUNE_FUSED_MAX_SINKS 0
+#define BIFROST_TUNE_SMALL_M         1
+#define BIFROST_TUNE_SYM_MIN_N       2
+int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value);
 
 const char* bifrost_strerror(int code);                 /* static string */
 const char* bifrost_last_cuda_error(bifrost_ctx* ctx);  /* "" if none; valid until the next call */
@@ -232,7 +263,10 @@ int bifrost_drift(bifrost_ctx* ctx, int64_t n, const int32_t* idx, int64_t n_idx
  * drift(eps/2) kick(eps/6) over the particles idx interacting ONLY among themselves (sinks = sources = idx;
  * idx == NULL: all n): four O(N^2) sums (acc, acc, grad, acc) and five O(N) updates, all on
  * stream, no host synchronisation.  pos and vel (double[n][3]) are updated in place at the rows in idx.
- * eps_soft is the Plummer softening of the sums, eps the time-step. */
+ * eps_soft is the Plummer softening of the sums, eps the time-step.  BIFROST_EINVAL while
+ * bifrost_set_subsystems is active: Alg. 1 drifts single particles only and hands subsystem
+ * members to the regularised integrator, which is outside this library (reading H5) - integrating
+ * them here would move them without their mutual force. */
 int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass,
                      const int32_t* idx, int64_t n_idx, double G, double eps_soft, double eps, void* stream);
 
@@ -250,7 +284,8 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
  *            "the final time-step of a particle is the minimum of the set of its different time-steps" (L293);
  *   out_level_log : HOST int64[log_cap][3] or NULL - (depth, |S|, |F|) of the first log_cap levels, in the
  *                   order they are entered;   out_summary : HOST int64[3] or NULL - levels entered, deepest
- *                   depth, FSI cycles run.  pos, vel : DEVICE double[n][3], updated in place. */
+ *                   depth, FSI cycles run.  pos, vel : DEVICE double[n][3], updated in place.
+ * BIFROST_EINVAL while bifrost_set_subsystems is active (as bifrost_fsi_step). */
 int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G,
                     double eps_soft, double eta_ff, double eta_fb, const double* dt_cap, double tau, int max_depth,
                     int64_t* out_level_log, int64_t log_cap, int64_t* out_summary, void* stream);

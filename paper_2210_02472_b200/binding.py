@@ -30,6 +30,7 @@ SYMBOLS = [
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
     "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
     "bifrost_neighbours", "bifrost_components",
+    "bifrost_reserve", "bifrost_set_tuning",
     "bifrost_acc_jerk", "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
 ]
 
@@ -71,6 +72,8 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_grad_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P]
     lib.bifrost_dtmin_host.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _P, _P, _P, _P]
     lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
+    lib.bifrost_reserve.argtypes = [_P, _I]
+    lib.bifrost_set_tuning.argtypes = [_P, _I, _I64]
     lib.bifrost_set_subsystems.argtypes = [_P, _P, _I64]
     lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
     lib.bifrost_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _I64, _P, _P, _P]
@@ -159,6 +162,15 @@ class Context:
             msg = self._lib.bifrost_strerror(rc).decode()
             cu = self._lib.bifrost_last_cuda_error(self._h).decode()
             raise BifrostError(f"{what}: {msg}" + (f" [{cu}]" if cu else ""))
+
+    RESERVE_HOST, RESERVE_INTEGRATOR = 1, 2
+    TUNE_FUSED_MAX_SINKS, TUNE_SMALL_M, TUNE_SYM_MIN_N = 0, 1, 2
+
+    def reserve(self, what: int):
+        self._check(self._lib.bifrost_reserve(self._h, int(what)), "bifrost_reserve")
+
+    def set_tuning(self, knob: int, value: int):
+        self._check(self._lib.bifrost_set_tuning(self._h, int(knob), int(value)), "bifrost_set_tuning")
 
     @property
     def launch_count(self) -> int:

@@ -65,12 +65,14 @@ struct bifrost_ctx {
     double* wpart = nullptr;         // [ceil(max_n / 4096)] block partials of the W reduction
     unsigned long long* smin = nullptr;   // [max_n] per-subsystem minima (bifrost_subsys_min)
     int small_m = 128;               // FSI cycles / level splits of at most this many particles run as ONE single-CTA launch
-                                     // (env BIFROST_SMALL_M = 0..256 overrides; 0 disables; tuning / test aid)
-    int64_t fused_max_sinks = 4096;  // below: one fused launch per call (env BIFROST_FUSED_MAX_SINKS overrides; tuning aid)
-    unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel (zero between launches)
+                                     // (bifrost_set_tuning BIFROST_TUNE_SMALL_M: 0..256; 0 disables)
+    int64_t fused_max_sinks = 4096;  // below: one fused launch per call (BIFROST_TUNE_FUSED_MAX_SINKS)
+    unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel, tagged with the launch epoch
+    unsigned epoch = 0;              // one per fused launch (22 bits): a stale count of an aborted launch never matches
     double* sym_ws = nullptr;        // source-side rows of the symmetric (every pair once) kernels, [block][source][3]
     size_t sym_ws_bytes = 0;
-    int64_t sym_min_n = 32768;       // shortest list the symmetric kernels are used for
+    int64_t sym_min_acc = 16384, sym_min_grad = 12288;   // shortest list the symmetric kernels are used for (measured
+                                     // crossover, profiles/r2_symmetric.md; BIFROST_TUNE_SYM_MIN_N sets both)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
     int64_t subsys_n = 0;
     int64_t launches = 0;
@@ -177,7 +179,12 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     Geom g = make_geom(ctx, n_sink, n_src, Sh::T * Sh::S, Sh::MINB, partial_bytes_per_sink);
     g.compact = compact;
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+    if (grid.x > (unsigned)TICKETS) {            // one ticket per sink block (cannot happen below fused_max_sinks <= TICKETS * 128)
+        snprintf(ctx->err, sizeof(ctx->err), "fused launch: %u sink blocks exceed the %d tickets", grid.x, TICKETS);
+        return BIFROST_EINVAL;
+    }
+    ctx->epoch = ctx->epoch % 0x3ffffeu + 1u;      // 1 .. 2^22 - 2, never 0
+    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets, ctx->epoch);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -242,10 +249,11 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
 
 // acc / grad over one list that is both sink and source set, every pair once (sym_kernels.cuh).
 // Returns 1 when the call does not qualify (list too short, workspace too small): the caller then takes the plain path.
+constexpr int SYM_ACC_BS = 8 * 256, SYM_GRAD_BS = 6 * 256;   // sinks per CTA of the two symmetric shapes (sym_impl callers)
 template <class P, int S, int T, int MINB>
-int sym_impl(bifrost_ctx* ctx, const double* pos, const double* mass, const double* aux, const int32_t* idx, int64_t m,
-             double G, double eps, double* out, int compact, cudaStream_t st) {
-    if (m < ctx->sym_min_n || !ctx->sym_ws) return 1;
+int sym_impl(bifrost_ctx* ctx, int64_t min_n, const double* pos, const double* mass, const double* aux, const int32_t* idx,
+             int64_t m, double G, double eps, double* out, int compact, cudaStream_t st) {
+    if (m < min_n || m < 2 || !ctx->sym_ws) return 1;
     SymGeom g;
     g.m = (int)m;
     g.n_tiles = ceil_div(m, TILE);
@@ -256,7 +264,8 @@ int sym_impl(bifrost_ctx* ctx, const double* pos, const double* mass, const doub
     int64_t total = 0;
     for (int b = 0; b < g.n_blocks; ++b) total += sym_range(g, b);
     const int64_t slots = (int64_t)ctx->num_sms * MINB;
-    g.unit_tiles = (int)std::max<int64_t>(g.tb, (total + 24 * slots - 1) / (24 * slots));
+    // ~64 CTAs per SM slot keep the tail of the last wave below ~1 % (measured: 24 -> 64 gains 1.5 %)
+    g.unit_tiles = (int)std::max<int64_t>(2, (total + 64 * slots - 1) / (64 * slots));
     // the sink-side pieces must fit the split-j workspace, the source-side rows the symmetric workspace
     const int64_t max_pieces_ws = (int64_t)(ctx->partial_bytes / (24 * (size_t)m));
     if (max_pieces_ws < 1) return 1;
@@ -280,7 +289,7 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
-        const int rc = sym_impl<SymAcc, 8, 256, 1>(ctx, pos, mass, nullptr, sink_idx, n_sink, G, eps, out, compact, st);
+        const int rc = sym_impl<SymAcc, 8, 256, 1>(ctx, ctx->sym_min_acc, pos, mass, nullptr, sink_idx, n_sink, G, eps, out, compact, st);
         if (rc <= 0) return rc;
     }
     const SrcArrays src{pos, nullptr, mass, sub, src_idx};
@@ -299,7 +308,7 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
     if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
-        const int rc = sym_impl<SymGrad, 4, 256, 1>(ctx, pos, mass, acc, sink_idx, n_sink, G, eps, out, compact, st);
+        const int rc = sym_impl<SymGrad, 6, 256, 1>(ctx, ctx->sym_min_grad, pos, mass, acc, sink_idx, n_sink, G, eps, out, compact, st);
         if (rc <= 0) return rc;
     }
     const SrcArrays src{pos, acc, mass, sub, src_idx};
@@ -628,16 +637,8 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     ctx->device = device;
     ctx->max_n = max_n;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
-    if (const char* e = getenv("BIFROST_FUSED_MAX_SINKS")) {
-        const long long v = atoll(e);
-        if (v >= 0 && v <= (long long)TICKETS * 128) ctx->fused_max_sinks = v;
-    }
-    if (const char* e = getenv("BIFROST_SMALL_M")) {
-        const int v = atoi(e);
-        if (v >= 0 && v <= SMALL_M) ctx->small_m = v;
-    }
     const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
-    ctx->partial_bytes = 24 * (size_t)max_n * 16;   // up to 16 source-range splits at n_sink = max_n
+    ctx->partial_bytes = 24 * (size_t)max_n * 64;   // up to 16 source-range splits at n_sink = max_n
     if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
     if (cudaMalloc(&ctx->src_rec, n_pad * 10 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
@@ -654,14 +655,45 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     // symmetric kernels: 12 max_n^2 / (sinks per CTA) bytes of source-side rows (sized for the smaller block of the two
     // passes); skipped when that exceeds a quarter of the free device memory (those calls then take the plain path)
     {
-        const size_t need = 24 * ((size_t)max_n + 2048) * ((size_t)max_n / 2048 + 2);
+        auto rows = [&](int bs) {       // source-side rows of a list of max_n entries cut into blocks of bs
+            SymGeom g{};
+            g.n_tiles = ceil_div(max_n, TILE); g.bs = bs; g.tb = bs / TILE; g.n_blocks = ceil_div(max_n, bs);
+            return sym_joff(g, g.n_blocks - 1) + (size_t)sym_range(g, g.n_blocks - 1) * TILE;
+        };
+        const size_t need = 24 * std::max(rows(SYM_ACC_BS), rows(SYM_GRAD_BS)) + 4096;
         size_t free_b = 0, total_b = 0;
-        if (max_n >= ctx->sym_min_n && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need < free_b / 4 &&
+        if (max_n >= std::min(ctx->sym_min_acc, ctx->sym_min_grad) && cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need < free_b / 4 &&
             cudaMalloc(&ctx->sym_ws, need) == cudaSuccess)
             ctx->sym_ws_bytes = need;
         else { cudaGetLastError(); ctx->sym_ws = nullptr; }
     }
     *out = ctx;
+    return BIFROST_OK;
+}
+
+int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
+    if (!ctx || value < 0) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    switch (knob) {
+        case BIFROST_TUNE_FUSED_MAX_SINKS:
+            if (value > (int64_t)TICKETS * 128) return BIFROST_EINVAL;
+            ctx->fused_max_sinks = value; return BIFROST_OK;
+        case BIFROST_TUNE_SMALL_M:
+            if (value > SMALL_M) return BIFROST_EINVAL;
+            ctx->small_m = (int)value; return BIFROST_OK;
+        case BIFROST_TUNE_SYM_MIN_N:
+            ctx->sym_min_acc = ctx->sym_min_grad = value; return BIFROST_OK;
+        default: return BIFROST_EINVAL;
+    }
+}
+
+int bifrost_reserve(bifrost_ctx* ctx, int what) {
+    if (!ctx || (what & ~(BIFROST_RESERVE_HOST | BIFROST_RESERVE_INTEGRATOR))) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    DeviceGuard guard(ctx->device);
+    int rc;
+    if ((what & BIFROST_RESERVE_HOST) && (rc = ensure_host_mirrors(ctx))) return rc;
+    if ((what & BIFROST_RESERVE_INTEGRATOR) && (rc = ensure_integrator(ctx))) return rc;
     return BIFROST_OK;
 }
 
@@ -994,6 +1026,7 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
                      int64_t n_idx, double G, double eps_soft, double eps, void* stream) {
     int rc = check_lists(ctx, n, idx, n_idx, idx, n_idx);
     if (rc) return rc;
+    if (ctx->subsys) return BIFROST_EINVAL;    // no subsystem integrator here (reading H5): members would move without their mutual force
     if (n_idx == 0) return BIFROST_OK;
     if (!pos || !vel || !mass) return BIFROST_EINVAL;
     DeviceGuard guard(ctx->device);
@@ -1007,7 +1040,7 @@ int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const
     if (!ctx) return BIFROST_EINVAL;
     ctx->err[0] = 0;
     if (n < 0 || n > ctx->max_n || max_depth < 0 || max_depth > 62 || log_cap < 0 || !(tau > 0.0)) return BIFROST_EINVAL;
-    if (ctx->subsys && ctx->subsys_n != n) return BIFROST_EINVAL;
+    if (ctx->subsys) return BIFROST_EINVAL;    // as bifrost_fsi_step (reading H5)
     if (out_summary) out_summary[0] = out_summary[1] = out_summary[2] = 0;
     if (n == 0) return BIFROST_OK;
     if (!pos || !vel || !mass) return BIFROST_EINVAL;
@@ -1053,9 +1086,13 @@ int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm
         return BIFROST_EINVAL;
     ctx->err[0] = 0;
     DeviceGuard guard(ctx->device);
-    cudaEvent_t e0, e1;
-    CU_TRY(ctx, cudaEventCreate(&e0));
-    CU_TRY(ctx, cudaEventCreate(&e1));
+    struct Events {                            // destroyed on every return path
+        cudaEvent_t a = nullptr, b = nullptr;
+        ~Events() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    } ev;
+    CU_TRY(ctx, cudaEventCreate(&ev.a));
+    CU_TRY(ctx, cudaEventCreate(&ev.b));
+    cudaEvent_t e0 = ev.a, e1 = ev.b;
     const int grid = ctx->num_sms * ctas_per_sm;
     const double b = 0.999999999, c = 1e-9;
     double* sink = (double*)ctx->partial;      // never written (see kernel); >= 64 MiB
@@ -1077,7 +1114,6 @@ int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm
     }
     float ms = 0.f;
     CU_TRY(ctx, cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     *out_ms = ms;
     const double per_thread = (double)iters * (mix == 0 ? 32.0 : mix == 1 ? 120.0 : 12.0);
     *out_lane_instr = per_thread * (double)grid * PROBE_THREADS;

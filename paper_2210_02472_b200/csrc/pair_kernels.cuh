@@ -121,11 +121,11 @@ __global__ void finish_kernel(const typename P::Args a, const Geom g) {
 // tile's loads are in flight while the current one is evaluated), and when the source range is
 // split across blockIdx.y the CTA that arrives last at a ticket (one per blockIdx.x) reduces all
 // partials in split order - so the result does not depend on which CTA that is (deterministic) and
-// no second or third launch is needed.  The ticket resets itself (CUDA-graph replay safe).
+// no second or third launch is needed.
 // ----------------------------------------------------------------------------------------
 template <class P, int S, int T, int MINB, int UNR>
 __global__ void __launch_bounds__(T, MINB)
-pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, unsigned* __restrict__ ticket) {
+pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, unsigned* __restrict__ ticket, unsigned epoch) {
     static_assert(T >= TILE, "one gathering thread per source of a tile");
     constexpr int REC = P::REC;
     __shared__ __align__(16) double sm[2][TILE * REC];
@@ -195,7 +195,19 @@ pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, u
     }
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(&ticket[blockIdx.x], 1u) == gridDim.y - 1);
+    if (threadIdx.x == 0) {
+        // arrival count tagged with this launch's epoch (never 0): a count left behind by an aborted launch (another
+        // epoch) is overwritten, not continued; the last CTA still zeroes the ticket, so a CUDA graph that replays
+        // this launch with the same epoch starts from a clean ticket
+        unsigned seen = ticket[blockIdx.x], now;
+        while (true) {
+            now = (seen >> 10) == epoch ? seen + 1u : (epoch << 10) | 1u;
+            const unsigned old = atomicCAS(&ticket[blockIdx.x], seen, now);
+            if (old == seen) break;
+            seen = old;
+        }
+        s_last = (now & 1023u) == gridDim.y;
+    }
     __syncthreads();
     if (!s_last) return;
     __threadfence();

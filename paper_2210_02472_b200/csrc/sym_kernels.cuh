@@ -5,7 +5,7 @@
 // 12 of acc's 15 and 22 of grad's 28 FP64 instructions per ordered pair are pair geometry that is identical for
 // (i <- j) and (j <- i); here they are issued once and both members get their term:
 //     acc : a_i += m_j s^-3 r_ji              a_j -= m_i s^-3 r_ji                         20 instructions per unordered pair
-//     grad: U_i += m_j s^-3 a_ji,  W_i += m_j q s^-5 r_ji     U_j -= m_i s^-3 a_ji,  W_j -= m_i q s^-5 r_ji   38
+//     grad: C_i += m_j s^-3 t                 C_j -= m_i s^-3 t,   t = a_ji - 3 (a_ji.r_ji) r_ji / s^2   33
 // The list is cut into blocks of BS = T*S positions.  A CTA owns one block as SINKS (S per thread, in registers)
 // and a range of source tiles strictly beyond its block; for every source it also forms the source-side sum
 // over its own sinks: per thread over its S sinks in registers, over the 32 lanes of a warp with a fixed
@@ -32,10 +32,17 @@ __host__ __device__ inline int sym_range(const SymGeom& g, int b) {
     const int r = g.n_tiles - (b + 1) * g.tb;
     return r > 0 ? r : 0;
 }
-// CTAs (pieces) that share block b: piece 0 also does the diagonal
+// CTAs (pieces) that share block b: the first sym_diag_pieces do the block's own tiles (the diagonal), the others
+// the tiles beyond the block, at most unit_tiles each
+__host__ __device__ inline int sym_diag_tiles(const SymGeom& g, int b) {
+    const int r = g.n_tiles - b * g.tb;
+    return r < g.tb ? r : g.tb;
+}
+__host__ __device__ inline int sym_diag_pieces(const SymGeom& g, int b) {
+    return (sym_diag_tiles(g, b) + g.unit_tiles - 1) / g.unit_tiles;
+}
 __host__ __device__ inline int sym_pieces(const SymGeom& g, int b) {
-    const int r = sym_range(g, b);
-    return r > 0 ? (r + g.unit_tiles - 1) / g.unit_tiles : 1;
+    return sym_diag_pieces(g, b) + (sym_range(g, b) + g.unit_tiles - 1) / g.unit_tiles;
 }
 // first row of block b in the source-side workspace: rows of blocks b' < b, each (n_tiles - (b'+1) tb) * TILE long
 __host__ __device__ inline size_t sym_joff(const SymGeom& g, int b) {
@@ -88,8 +95,9 @@ struct SymAcc {
             double dx, dy, dz;
             const double s3 = inv_s3(a.eps2, sk[s], r, dx, dy, dz);
             const double wi = s3 * r[3], wj = s3 * sk[s].m;
-            c[s].x = fma(wi, dx, c[s].x); c[s].y = fma(wi, dy, c[s].y); c[s].z = fma(wi, dz, c[s].z);
-            jx = fma(wj, dx, jx); jy = fma(wj, dy, jy); jz = fma(wj, dz, jz);
+            c[s].x = fma(wi, dx, c[s].x); jx = fma(wj, dx, jx);        // neighbours share an operand (reuse cache)
+            jy = fma(wj, dy, jy); c[s].y = fma(wi, dy, c[s].y);
+            c[s].z = fma(wi, dz, c[s].z); jz = fma(wj, dz, jz);
         }
         J[0] = jx; J[1] = jy; J[2] = jz;
     }
@@ -99,16 +107,19 @@ struct SymAcc {
 struct SymGrad {
     static constexpr int REC = 8;            // x y z m ax ay az -
     struct Sink { double x, y, z, m, ax, ay, az; };
-    struct Acc { double ux, uy, uz, wx, wy, wz; };
+    struct Acc { double x, y, z; };
     __device__ __forceinline__ static void load_sink(const double* __restrict__ r, bool live, Sink& s) {
         s.x = r[0]; s.y = r[1]; s.z = r[2]; s.m = live ? r[3] : 0.0; s.ax = r[4]; s.ay = r[5]; s.az = r[6];
     }
-    __device__ __forceinline__ static void init(Acc& c) { c.ux = c.uy = c.uz = c.wx = c.wy = c.wz = 0.0; }
-    // common part of one pair (22 instructions): s3 = s^-3, v = (a_ji . r_ji) s^-5
-    __device__ __forceinline__ static void geom(double eps2, const Sink& s, const double* __restrict__ r, double& dx, double& dy,
-                                                double& dz, double& bx, double& by, double& bz, double& s3, double& v) {
-        dx = r[0] - s.x; dy = r[1] - s.y; dz = r[2] - s.z;
-        bx = r[4] - s.ax; by = r[5] - s.ay; bz = r[6] - s.az;
+    __device__ __forceinline__ static void init(Acc& c) { c.x = c.y = c.z = 0.0; }
+    // One pair, mass-free (25 instructions): s3 = s^-3 and the bracket of Eq. 9 times s^3,
+    //     t = a_ji - 3 (a_ji . r_ji) r_ji / s^2,
+    // so that the sink's term is (m_j s3) t and the source's -(m_i s3) t: one weight and three accumulate DFMAs per
+    // side (the plain kernel keeps two running sums U, W per sink instead, which is cheaper for ONE side only).
+    __device__ __forceinline__ static void geom(double eps2, const Sink& s, const double* __restrict__ r, double& s3, double& tx,
+                                                double& ty, double& tz) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double bx = r[4] - s.ax, by = r[5] - s.ay, bz = r[6] - s.az;
         const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
         const double q = fma(bx, dx, fma(by, dy, bz * dz));
         const double y0 = rsqrt_seed(r2);
@@ -116,36 +127,33 @@ struct SymGrad {
         const double e = fma(-r2, t, 1.0);
         const double p = fma(fma(e, 1.875, 1.5), e, 1.0);
         s3 = (y0 * t) * p;
-        const double y2 = fma(t, fma(e, e, e), t);
-        v = (s3 * y2) * q;
+        const double tn = -3.0 * t;
+        const double qq = q * fma(tn, fma(e, e, e), tn);      // -3 (a_ji . r_ji) / s^2
+        tx = fma(qq, dx, bx); ty = fma(qq, dy, by); tz = fma(qq, dz, bz);
     }
     __device__ __forceinline__ static void pair(const SymArgs& a, const Sink& s, Acc& c, const double* __restrict__ r) {
-        double dx, dy, dz, bx, by, bz, s3, v;
-        geom(a.eps2, s, r, dx, dy, dz, bx, by, bz, s3, v);
-        const double wi = s3 * r[3], vi = v * r[3];
-        c.ux = fma(wi, bx, c.ux); c.uy = fma(wi, by, c.uy); c.uz = fma(wi, bz, c.uz);
-        c.wx = fma(vi, dx, c.wx); c.wy = fma(vi, dy, c.wy); c.wz = fma(vi, dz, c.wz);
+        double s3, tx, ty, tz;
+        geom(a.eps2, s, r, s3, tx, ty, tz);
+        const double wi = s3 * r[3];
+        c.x = fma(wi, tx, c.x); c.y = fma(wi, ty, c.y); c.z = fma(wi, tz, c.z);
     }
-    // both sides (38 instructions per pair): the source's term is -(m_i / m_j) times the sink's
+    // both sides: 33 instructions per pair
     template <int S>
     __device__ __forceinline__ static void pairs(const SymArgs& a, const Sink* sk, Acc* c, const double* __restrict__ r,
                                                  double* J) {
-        double ux = 0.0, uy = 0.0, uz = 0.0, wx = 0.0, wy = 0.0, wz = 0.0;
+        double jx = 0.0, jy = 0.0, jz = 0.0;
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            double dx, dy, dz, bx, by, bz, s3, v;
-            geom(a.eps2, sk[s], r, dx, dy, dz, bx, by, bz, s3, v);
-            const double wi = s3 * r[3], vi = v * r[3], wj = s3 * sk[s].m, vj = v * sk[s].m;
-            c[s].ux = fma(wi, bx, c[s].ux); c[s].uy = fma(wi, by, c[s].uy); c[s].uz = fma(wi, bz, c[s].uz);
-            c[s].wx = fma(vi, dx, c[s].wx); c[s].wy = fma(vi, dy, c[s].wy); c[s].wz = fma(vi, dz, c[s].wz);
-            ux = fma(wj, bx, ux); uy = fma(wj, by, uy); uz = fma(wj, bz, uz);
-            wx = fma(vj, dx, wx); wy = fma(vj, dy, wy); wz = fma(vj, dz, wz);
+            double s3, tx, ty, tz;
+            geom(a.eps2, sk[s], r, s3, tx, ty, tz);
+            const double wi = s3 * r[3], wj = s3 * sk[s].m;
+            c[s].x = fma(wi, tx, c[s].x); jx = fma(wj, tx, jx);
+            jy = fma(wj, ty, jy); c[s].y = fma(wi, ty, c[s].y);
+            c[s].z = fma(wi, tz, c[s].z); jz = fma(wj, tz, jz);
         }
-        J[0] = fma(-3.0, wx, ux); J[1] = fma(-3.0, wy, uy); J[2] = fma(-3.0, wz, uz);
+        J[0] = jx; J[1] = jy; J[2] = jz;
     }
-    __device__ __forceinline__ static void result(const Acc& c, double* o) {
-        o[0] = fma(-3.0, c.wx, c.ux); o[1] = fma(-3.0, c.wy, c.uy); o[2] = fma(-3.0, c.wz, c.uz);
-    }
+    __device__ __forceinline__ static void result(const Acc& c, double* o) { o[0] = c.x; o[1] = c.y; o[2] = c.z; }
 };
 
 // ---- pack: the list's records in list order, zero-padded to a whole number of tiles -------------------
@@ -231,13 +239,15 @@ sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec
         cp_async_commit();
     };
 
-    // this piece's tiles: [d0, d1) diagonal (piece 0 only), then [t0, t1) beyond the block
+    // this piece's tiles: an equal share of the diagonal [b tb, (b+1) tb) or of the tiles beyond the block
     const int jb = (b + 1) * g.tb;
-    const int len = range > 0 ? (range + np - 1) / np : 0;
-    const int t0 = jb + piece * len, t1 = min(t0 + len, g.n_tiles);
-    const int d0 = b * g.tb, d1 = piece == 0 ? min(jb, g.n_tiles) : d0;
-    const int n_my = (d1 - d0) + max(t1 - t0, 0);
-    auto tile_of = [&](int q) { return q < d1 - d0 ? d0 + q : t0 + (q - (d1 - d0)); };
+    const int nd = sym_diag_pieces(g, b), dt = sym_diag_tiles(g, b);
+    const bool diag = piece < nd;
+    const int len = diag ? (dt + nd - 1) / nd : (range + (np - nd) - 1) / (np - nd);
+    const int t0 = diag ? b * g.tb + piece * len : jb + (piece - nd) * len;
+    const int t1 = min(t0 + len, diag ? b * g.tb + dt : g.n_tiles);
+    const int n_my = max(t1 - t0, 0);
+    auto tile_of = [&](int q) { return t0 + q; };
 
     if (n_my > 0) load_tile(tile_of(0), 0);
     for (int q = 0; q < n_my; ++q) {

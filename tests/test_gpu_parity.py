@@ -141,9 +141,13 @@ def test_config4_full_size_sampled(torch, ctx):
     a, c, d, acc_in = run_all(torch, ctx, w)
     pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
     apn = ctx.pn1(pos, vel, mass, dev(torch, w.bh_idx), w.G, w.c).cpu().numpy()
+    # 8192 sinks: the first and the last 256 (first / last sink block, the tail CTA), all 101 BHs,
+    # the sinks either side of every 2048- and 1536-block boundary near the middle, and a seeded random rest
     rng = np.random.default_rng(44)
-    pick = np.sort(np.concatenate([w.bh_idx[:8].astype(np.int64), rng.choice(n, 760, replace=False)]))
-    pick = np.unique(pick).astype(np.int32)
+    edges = np.concatenate([np.arange(b - 2, b + 2) for b in (2048 * 255, 2048 * 256, 1536 * 341, 1536 * 342)])
+    forced = np.concatenate([np.arange(256), np.arange(n - 256, n), w.bh_idx.astype(np.int64), edges])
+    pick = np.unique(np.concatenate([forced, rng.choice(n, 8192 - forced.size, replace=False)])).astype(np.int32)
+    assert pick.size >= 8000 and np.isin(w.bh_idx, pick).all()
     check_vec(a[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=pick), "acc")
     check_vec(c[pick], oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps, sink_idx=pick), "grad")
     check_dt(tuple(x[pick] for x in d), oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sink_idx=pick), "dtmin")
@@ -165,7 +169,12 @@ def test_config5_full_size_sampled(torch, ctx):
     c_t = ctx.grad(pos, mass, a_t, w.G, w.eps)
     torch.cuda.synchronize()
     a, c = a_t.cpu().numpy(), c_t.cpu().numpy()
-    pick = np.sort(np.random.default_rng(55).choice(w.n, 384, replace=False)).astype(np.int32)
+    # 4096 sinks: first / last 256, block boundaries of both symmetric shapes, a seeded random rest
+    edges = np.concatenate([np.arange(b - 2, b + 2) for b in (2048 * 511, 2048 * 512, 1536 * 682, 1536 * 683)])
+    forced = np.concatenate([np.arange(256), np.arange(w.n - 256, w.n), edges])
+    pick = np.unique(np.concatenate([forced, np.random.default_rng(55).choice(w.n, 4096 - forced.size, replace=False)]))
+    pick = pick.astype(np.int32)
+    assert pick.size >= 4000
     check_vec(a[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=pick), "acc")
     check_vec(c[pick], oracle.grad(w.pos, w.mass, a, w.G, w.eps, sink_idx=pick), "grad")
     for x, name in ((a, "acc"), (c, "grad")):
@@ -731,16 +740,15 @@ def test_hhs_fsi_config2_full_size(torch, ctx):
 
 
 @pytest.mark.parametrize("m", [1, 2, 5, 64, 128])
-def test_small_level_single_launch_equals_the_general_path_bit_for_bit(torch, ctx, m, monkeypatch):
+def test_small_level_single_launch_equals_the_general_path_bit_for_bit(torch, ctx, m):
     """FSI cycles / level splits of <= 128 particles run as ONE single-CTA launch (fsi_small_kernel,
     level_split_small_kernel); same pair arithmetic, same summation order as the multi-launch path."""
     from paper_2210_02472_b200.binding import Context
     w = workload(2)
     rng = np.random.default_rng(100 + m)
     idx = rng.permutation(w.n)[:m].astype(np.int32)          # unsorted on purpose
-    monkeypatch.setenv("BIFROST_SMALL_M", "0")
     general = Context(w.n)
-    monkeypatch.delenv("BIFROST_SMALL_M")
+    general.set_tuning(Context.TUNE_SMALL_M, 0)
     try:
         out = []
         for c in (ctx, general):
@@ -819,3 +827,175 @@ def test_large_set_paths_are_bit_reproducible(torch, ctx):
         runs.append((a, c, *d, *aj))
     assert all(torch.equal(x, y) for x, y in zip(*runs))
     assert torch.isfinite(runs[0][0]).all() and torch.isfinite(runs[0][1]).all()
+
+
+# ---- round 2: symmetric (every pair once) kernels, switch points, edge cases -------------------------
+
+@pytest.fixture(scope="module")
+def ctx_sym(torch):
+    """A context whose same-list acc / grad calls ALWAYS take the symmetric kernels (threshold 0)."""
+    from paper_2210_02472_b200.binding import Context
+    c = Context(1 << 17)
+    c.set_tuning(Context.TUNE_SYM_MIN_N, 0)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("m", [2, 3, 127, 129, 1535, 1537, 2047, 2049, 4097, 6144, 10000])
+def test_symmetric_kernels_ragged_sizes(torch, ctx, ctx_sym, m):
+    """acc / grad over one list, every unordered pair once: list lengths around the tile (128) and block
+    (1536 / 2048) sizes, against the oracle and against the plain kernels; bit-identical repeats."""
+    w = _small(m, 500 + m)
+    pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+    l0 = ctx_sym.launch_count
+    a = ctx_sym.acc(pos, mass, w.G, 1e-4)
+    assert ctx_sym.launch_count - l0 == 3            # sym_pack, sym_pair, sym_finish
+    c = ctx_sym.grad(pos, mass, a, w.G, 1e-4)
+    a2 = ctx_sym.acc(pos, mass, w.G, 1e-4)
+    c2 = ctx_sym.grad(pos, mass, a, w.G, 1e-4)
+    assert torch.equal(a, a2) and torch.equal(c, c2)
+    a_np = a.cpu().numpy()
+    check_vec(a_np, oracle.acc(w.pos, w.mass, w.G, 1e-4), "sym acc")
+    check_vec(c.cpu().numpy(), oracle.grad(w.pos, w.mass, a_np, w.G, 1e-4), "sym grad")
+    check_vec(a_np, ctx.acc(pos, mass, w.G, 1e-4).cpu().numpy(), "sym vs plain acc", tol=1e-13)
+    check_vec(c.cpu().numpy(), ctx.grad(pos, mass, a, w.G, 1e-4).cpu().numpy(), "sym vs plain grad", tol=1e-13)
+
+
+def test_symmetric_kernels_through_an_index_list(torch, ctx_sym):
+    """The same list (one tensor) as sinks and sources: an unsorted subset of the particles; rows of the others
+    stay untouched; eps = 0 with the self pair inside the list; momentum of the subset is conserved."""
+    w = _small(9000, 77)
+    ids = np.random.default_rng(78).permutation(w.n)[:5000].astype(np.int32)
+    pos, mass, li = dev(torch, w.pos), dev(torch, w.mass), dev(torch, ids)
+    out = torch.full((w.n, 3), 7.25, dtype=torch.float64, device="cuda")
+    l0 = ctx_sym.launch_count
+    ctx_sym.acc(pos, mass, w.G, 0.0, li, li, out=out)
+    assert ctx_sym.launch_count - l0 == 3
+    got = out.cpu().numpy()
+    rest = np.ones(w.n, bool); rest[ids] = False
+    assert np.all(got[rest] == 7.25)
+    check_vec(got[ids], oracle.acc(w.pos, w.mass, w.G, 0.0, ids, ids), "sym acc list")
+    a_full = torch.from_numpy(np.where(rest[:, None], 0.0, got)).cuda()
+    c = ctx_sym.grad(pos, mass, a_full, w.G, 0.0, li, li).cpu().numpy()
+    check_vec(c[ids], oracle.grad(w.pos, w.mass, a_full.cpu().numpy(), w.G, 0.0, ids, ids), "sym grad list")
+    for x in (got[ids], c[ids]):
+        tot = np.abs((w.mass[ids, None] * x).sum(0)); scale = (w.mass[ids, None] * np.abs(x)).sum(0)
+        assert (tot <= 1e-13 * scale).all()
+
+
+@pytest.mark.parametrize("m", [12287, 12288, 16383, 16384])
+def test_symmetric_switch_points(torch, ctx, m):
+    """Default thresholds: grad switches to the symmetric kernel at 12288 entries, acc at 16384."""
+    w = workload(3, n=20000)
+    pos, mass = dev(torch, w.pos[:m].copy()), dev(torch, w.mass[:m].copy())
+    a = ctx.acc(pos, mass, w.G, w.eps)
+    c = ctx.grad(pos, mass, a, w.G, w.eps)
+    a_np = a.cpu().numpy()
+    pick = np.sort(np.random.default_rng(m).choice(m, 2048, replace=False)).astype(np.int32)
+    check_vec(a_np[pick], oracle.acc(w.pos[:m], w.mass[:m], w.G, w.eps, sink_idx=pick), "acc")
+    check_vec(c.cpu().numpy()[pick], oracle.grad(w.pos[:m], w.mass[:m], a_np, w.G, w.eps, sink_idx=pick), "grad")
+
+
+@pytest.mark.parametrize("n_sink", [4095, 4096, 4097])
+def test_fused_to_packed_switch(torch, ctx, n_sink):
+    """n_sink = 4095 is one fused launch, 4096 and 4097 are pack -> pair -> finish."""
+    w = workload(3, n=20000)
+    sinks = np.sort(np.random.default_rng(n_sink).choice(w.n, n_sink, replace=False)).astype(np.int32)
+    a, c, d, acc_in = run_all(torch, ctx, w, sinks=sinks)
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks), "acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_in, w.G, w.eps, sinks), "grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks), "dtmin")
+
+
+def test_coincident_distinct_particles_at_eps0(torch, ctx, ctx_sym):
+    """include/bifrost.h, reading A3b: two distinct particles at exactly the same position with eps = 0.
+    Nothing becomes inf / NaN; every OTHER sink agrees with the oracle in acc, grad and dtmin; in acc the
+    coincident pair contributes exactly 0 (the two sinks agree with the oracle evaluated WITHOUT their partner);
+    in grad the two sinks hold a finite value without meaning (the weight m 2^450 times a_ji, which is 0 or
+    rounding noise); dtmin gives dt_ff = 0
+    with the partner as argmin, as Eq. 21 does."""
+    w = _small(3000, 91)
+    p, q = 17, 2500
+    w.pos[q] = w.pos[p]
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    others = np.array([k for k in range(w.n) if k not in (p, q)], dtype=np.int32)
+    for c_ in (ctx, ctx_sym):
+        a = c_.acc(pos, mass, w.G, 0.0)
+        c = c_.grad(pos, mass, a, w.G, 0.0)
+        a_np, c_np = a.cpu().numpy(), c.cpu().numpy()
+        assert np.isfinite(a_np).all() and np.isfinite(c_np).all()
+        # the oracle divides by r = 0 for the coincident pair itself: compare all other sinks ...
+        with np.errstate(all="ignore"):
+            a_ref = oracle.acc(w.pos, w.mass, w.G, 0.0, sink_idx=others)
+        check_vec(a_np[others], a_ref, "acc, other sinks")
+        check_vec(c_np[others], oracle.grad(w.pos, w.mass, a_np, w.G, 0.0, sink_idx=others), "grad, other sinks")
+        # ... and the coincident sinks against the sums without their partner (the pair's term is 0)
+        for i, j in ((p, q), (q, p)):
+            src = np.array([k for k in range(w.n) if k != j], dtype=np.int32)
+            one = np.array([i], dtype=np.int32)
+            ref = oracle.acc(w.pos, w.mass, w.G, 0.0, sink_idx=one, src_idx=src)
+            assert np.abs(a_np[i] - ref[0]).max() <= 1e-12 * np.abs(ref[0]).max()
+    d = ctx.dtmin(pos, vel, mass, w.G, 0.02, 0.03)
+    dff, dfb, jff, jfb = (t.cpu().numpy() for t in d)
+    assert dff[p] == 0.0 and dff[q] == 0.0 and jff[p] == q and jff[q] == p
+    assert dfb[p] == 0.0 and jfb[p] == q
+    ref = oracle.dtmin(w.pos, w.vel, w.mass, w.G, 0.02, 0.03, sink_idx=others)
+    check_dt(tuple(x[others] for x in (dff, dfb, jff, jfb)), ref, "dtmin, other sinks")
+
+
+def test_dtmin_sources_sorted_by_distance(torch, ctx):
+    """Worst case of dtmin's rarely taken branch: a source list sorted by DECREASING distance
+    from a sink, so that this sink's free-fall key grows at every source.  Correctness only (its time is in
+    profiles/): indices and values bit-identical to the oracle."""
+    w = workload(3, n=20000)
+    i0 = 1234
+    order = np.argsort(-np.linalg.norm(w.pos - w.pos[i0], axis=1), kind="stable").astype(np.int32)
+    sinks = np.sort(np.random.default_rng(5).choice(w.n, 5000, replace=False)).astype(np.int32)
+    sinks[0] = min(i0, sinks[1] - 1) if i0 < sinks[1] else sinks[0]
+    sinks = np.unique(np.append(sinks, i0)).astype(np.int32)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    for sk in (sinks, np.array([i0], dtype=np.int32)):
+        d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, dev(torch, sk), dev(torch, order))
+        check_dt(tuple(t.cpu().numpy()[sk] for t in d),
+                 oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sk, order), "dtmin sorted sources")
+
+
+def test_integrator_refuses_subsystems(torch, ctx):
+    """bifrost_fsi_step / bifrost_hhs_fsi return BIFROST_EINVAL while subsystems are set (Alg. 1 hands
+    members to the subsystem integrator, which this library does not have - reading H5)."""
+    from paper_2210_02472_b200.binding import BifrostError
+    w = _small(600, 12)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    sub = np.full(w.n, -1, dtype=np.int32); sub[[3, 9]] = 3
+    sub_t = dev(torch, sub)
+    ctx.set_subsystems(sub_t)
+    try:
+        p0, v0 = pos.clone(), vel.clone()
+        with pytest.raises(BifrostError):
+            ctx.fsi_step(pos, vel, mass, w.G, 0.0, 1e-4)
+        with pytest.raises(BifrostError):
+            ctx.hhs_fsi(pos, vel, mass, w.G, 0.0, 0.02, 0.02, 1e-3)
+        assert torch.equal(pos, p0) and torch.equal(vel, v0)
+    finally:
+        ctx.set_subsystems(None)
+    ctx.fsi_step(pos, vel, mass, w.G, 0.0, 1e-4)      # fine again without subsystems
+
+
+def test_reserve_and_tuning_api(torch):
+    from paper_2210_02472_b200.binding import BifrostError, Context
+    c = Context(5000)
+    c.reserve(Context.RESERVE_HOST | Context.RESERVE_INTEGRATOR)
+    c.reserve(Context.RESERVE_HOST)                    # idempotent
+    with pytest.raises(BifrostError):
+        c.reserve(64)
+    with pytest.raises(BifrostError):
+        c.set_tuning(99, 1)
+    with pytest.raises(BifrostError):
+        c.set_tuning(Context.TUNE_SMALL_M, 257)
+    w = _small(3000, 3)
+    a1 = c.acc_host(w.pos, w.mass, w.G, 1e-3)
+    c.set_tuning(Context.TUNE_FUSED_MAX_SINKS, 0)      # the same call through pack -> pair -> finish
+    a2 = c.acc_host(w.pos, w.mass, w.G, 1e-3)
+    check_vec(a1, a2, "fused vs packed", tol=1e-13)
+    check_vec(a1, oracle.acc(w.pos, w.mass, w.G, 1e-3), "acc_host")
+    c.close()
