@@ -40,10 +40,17 @@ if ROOT not in sys.path:
 METRIC = "fp64 pair interactions/s (acc+FSI grad) at N=1e6; % of B200 FP64 peak"
 UNIT = "interactions/s"
 
-# FP64-pipe instruction / flop counts per pair of the kernels' inner loops (
-# cross-checked against the SASS and ncu's smsp__sass_thread_inst_executed_op_d*_pred_on).
-FP64_INSTR = {"acc": 15, "grad": 28, "dtmin": 23}     # dtmin: 23 arithmetic; the running-maximum test runs on the integer pipe
-FP64_FLOPS = {"acc": 24, "grad": 44, "dtmin": 33}     # FMA = 2, ADD/MUL = 1
+# EXECUTED FP64-pipe instructions / flops (FMA = 2, ADD/MUL = 1) per INTERACTION (= one ordered (sink, source) pair
+# delivered) of the kernels' inner loops (cross-checked against ncu's source page, profiles/).
+#   plain kernels (sinks != sources, or a sharded sink range): every ordered pair is evaluated.
+#   symmetric kernels (one list on both sides, all-active): every UNORDERED pair is evaluated once - acc 20 + 4.5/8
+#   (source-side warp reduction, 8 sinks per thread) = 20.56 instructions / 32.6 flops per unordered pair,
+#   grad 33 + 4.5/6 = 33.75 / 52.75 - i.e. half of that per interaction.
+FP64_INSTR = {"plain": {"acc": 15, "grad": 28, "dtmin": 23}, "sym": {"acc": 20.5625 / 2, "grad": 33.75 / 2, "dtmin": 23}}
+FP64_FLOPS = {"plain": {"acc": 24, "grad": 44, "dtmin": 33}, "sym": {"acc": 32.5625 / 2, "grad": 52.75 / 2, "dtmin": 33}}
+# SURVEY.md 8(d)'s budget for the minimal ONE-SIDED sequence: flops per ordered pair.  Against it the symmetric
+# kernels deliver more interactions than the executed flops alone would ("work-equivalent" fraction, may exceed 1).
+SURVEY_8D_FLOPS = {"acc": 26, "grad": 42}
 # B200 FP64 ALU peak derived from unit counts and clocks (no fp64 entry in MEASURED_PEAKS.json):
 # 148 SMs x 64 FP64 lanes/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.
 FP64_LANES_PER_SM = 64
@@ -142,6 +149,28 @@ def cpu_baseline(w, n_sample_sinks: int):
     return {"value": s["pairs"] / (s["t_acc"] + s["t_grad"]), "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
             "sample": f"{s['n_sinks']} seeded sinks x all {w.n} sources, acc then grad "
                       f"({s['pairs']:.3g} pairs per pass; acc {s['t_acc']:.2f} s, grad {s['t_grad']:.2f} s)"}
+
+
+def cpu_fast_baseline(w, n_sample_sinks: int):
+    """the oracle is deliberately slow (compensated sums, -O2, IEEE sqrt + division per pair), so the
+    GPU/oracle ratio flatters the GPU.  This times a plain restatement (oracle/cpu_fast.c: uncompensated sums,
+    -O3 -mavx2 -mfma, vectorised over sources, OpenMP over sinks; pinned to the oracle at 1e-12 in
+    tests/test_oracle_cpu_fast.py) on the same seeded sample.  Context only - neither the parity oracle nor a target."""
+    import oracle
+    from oracle import cpu_fast
+    cpu_fast.build()
+    rng = np.random.default_rng(777)
+    sinks = np.sort(rng.choice(w.n, size=min(n_sample_sinks, w.n), replace=False)).astype(np.int32)
+    fake_acc = np.ascontiguousarray(w.vel)
+    cpu_fast.acc(w.pos, w.mass, w.G, w.eps, sinks[:64])            # warm-up (thread pool, page faults)
+    t0 = time.perf_counter()
+    cpu_fast.acc(w.pos, w.mass, w.G, w.eps, sinks)
+    t1 = time.perf_counter()
+    cpu_fast.grad(w.pos, w.mass, fake_acc, w.G, w.eps, sinks)
+    t2 = time.perf_counter()
+    pairs = float(sinks.shape[0]) * w.n
+    return {"value": pairs / (t2 - t0), "unit": UNIT, "cores": oracle.n_threads(), "kind": "plain restatement, -O3 AVX2+FMA",
+            "sample": f"{sinks.shape[0]} seeded sinks x all {w.n} sources, acc then grad (acc {t1 - t0:.2f} s, grad {t2 - t1:.2f} s)"}
 
 
 def run_reference(args):
@@ -284,14 +313,25 @@ def run_cuda(args):
         hgrad = pinned(np.zeros((n, 3)))
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
         t_ag, t_all = 0.0, 0.0
+        if world > 1:
+            d_pos, d_mass = torch.empty_like(pos), torch.empty_like(mass)
+            t_pos, t_mass = torch.from_numpy(hpos), torch.from_numpy(hmass)
+            t_acc_rows, t_grad_rows = torch.from_numpy(hacc[b:e]), torch.from_numpy(hgrad[b:e])
         for it in range(1 + e2e_steps):                   # first iteration = warm-up (allocates the mirrors)
             barrier()
             t0 = time.perf_counter()
-            ctx.acc_host(hpos, hmass, w.G, w.eps, hsinks, None, out=hacc)
-            if world > 1:
-                g = sharding.allgather_rows(torch.from_numpy(hacc[b:e]).to(dev), n)
-                hacc[:] = g.cpu().numpy()
-            ctx.grad_host(hpos, hmass, hacc, w.G, w.eps, hsinks, None, out=hgrad)
+            if world == 1:
+                ctx.acc_host(hpos, hmass, w.G, w.eps, None, None, out=hacc)
+                ctx.grad_host(hpos, hmass, hacc, w.G, w.eps, None, None, out=hgrad)
+            else:
+                # sharded: inputs from pinned host memory, the acc all-gather stays on the device (NCCL), this rank's
+                # result rows back to the host - no device -> host -> device bounce around the collective
+                d_pos.copy_(t_pos, non_blocking=True); d_mass.copy_(t_mass, non_blocking=True)
+                ctx.acc(d_pos, d_mass, w.G, w.eps, sinks, None, out=acc)
+                acc.copy_(sharding.allgather_rows(acc[b:e], n))
+                ctx.grad(d_pos, d_mass, acc, w.G, w.eps, sinks, None, out=grad)
+                t_acc_rows.copy_(acc[b:e], non_blocking=True); t_grad_rows.copy_(grad[b:e], non_blocking=True)
+                torch.cuda.synchronize()
             t1 = time.perf_counter()
             if full_path:
                 ctx.dtmin_host(hpos, hvel, hmass, w.G, w.eta_ff, w.eta_fb, hsinks, None)
@@ -305,12 +345,15 @@ def run_cuda(args):
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         tt = tt.cpu().tolist()
         idx_b = 0 if world == 1 else 4 * n_loc
-        h2d = (32 * n + idx_b) + (56 * n + idx_b) + ((56 * n + idx_b) + (56 * n + 4 * len(w.bh_idx)) if full_path else 0)
+        h2d = ((32 * n) + (56 * n) if world == 1 else 32 * n) + ((56 * n + idx_b) + (56 * n + 4 * len(w.bh_idx)) if full_path else 0)
         d2h = 24 * n_loc * 2 + ((24 * n_loc) + 24 * n if full_path else 0)
         e2e = {"value": float(n) * n / tt[0], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * tt[1], "steps": e2e_steps,
-               "how": "bifrost_*_host entry points on pinned host arrays: H2D copies, kernels, D2H copies per call; "
-                      "value = N^2 / host wall time of acc_host + grad_host"}
+               "how": ("bifrost_*_host entry points on pinned host arrays: H2D copies, kernels, D2H copies per call; "
+                       "value = N^2 / host wall time of acc_host + grad_host") if world == 1 else
+                      ("per rank: pinned-host -> device copies of pos / mass, bifrost_acc on the rank's sinks, NCCL all-gather "
+                       "of acc on the device, bifrost_grad, the rank's acc / grad rows back to pinned host memory; "
+                       "value = N^2 / max over ranks of that wall time")}
 
     if rank == 0:
         num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -322,40 +365,40 @@ def run_cuda(args):
                 ms, rate = ctx.fp64_probe(mix=mix, iters=(1 << 15) if mix < 2 else (1 << 16), ctas_per_sm=32)
                 probe[name] = {"ms": ms, "lane_instr_per_s": rate, "frac_of_derived_pipe_peak": rate / (peak * 1e12 / 2)}
         pairs_rank = float(max(sharding.slice_counts(n, world))) * n     # the slowest rank's share
+        path = "sym" if world == 1 and n >= 16384 else "plain"          # which acc / grad kernels these sizes select
+        kernel_name = {"acc": {"sym": "sym_pair_kernel<SymAcc, 8, 256, 1>", "plain": "pair_kernel<AccPass, 8, 256, 1, 1>"},
+                       "grad": {"sym": "sym_pair_kernel<SymGrad, 6, 256, 1>", "plain": "pair_kernel<GradPass, 5, 128, 2, 2>"},
+                       "dtmin": {"sym": "pair_kernel<DtPass, 6, 128, 2, 1>", "plain": "pair_kernel<DtPass, 6, 128, 2, 1>"}}
 
         def kern(name):
             ms = mean_ms[name]
-            tf = pairs_rank * FP64_FLOPS[name] / (ms * 1e-3) / 1e12
-            pipe = pairs_rank * FP64_INSTR[name] / (ms * 1e-3) / (peak * 1e12 / 2)
-            return {"ms": ms, "interactions_per_s": pairs_rank / (ms * 1e-3), "tflops": tf, "frac_of_flop_peak": tf / peak,
-                    "fp64_pipe_issue_util": pipe}
+            tf = pairs_rank * FP64_FLOPS[path][name] / (ms * 1e-3) / 1e12
+            pipe = pairs_rank * FP64_INSTR[path][name] / (ms * 1e-3) / (peak * 1e12 / 2)
+            out = {"ms": ms, "kernel": kernel_name[name][path], "interactions_per_s": pairs_rank / (ms * 1e-3),
+                   "executed_flops_per_interaction": FP64_FLOPS[path][name],
+                   "executed_fp64_instr_per_interaction": FP64_INSTR[path][name],
+                   "tflops": tf, "frac_of_flop_peak": tf / peak, "fp64_pipe_issue_util": pipe}
+            if name in SURVEY_8D_FLOPS:
+                out["frac_survey_8d"] = pairs_rank * SURVEY_8D_FLOPS[name] / (ms * 1e-3) / 1e12 / peak
+            return out
         passes = {k: kern(k) for k in ("acc", "grad", "dtmin") if k in mean_ms}
         if "pn1" in mean_ms:
             passes["pn1"] = {"ms": mean_ms["pn1"], "interactions_per_s": 2.0 * len(w.bh_idx) * n / (mean_ms["pn1"] * 1e-3)}
         if "allgather" in mean_ms:
             passes["allgather"] = {"ms": mean_ms["allgather"], "bytes": 24 * n}
-        dom = passes["grad"]
-        traffic = None
-        prof = os.path.join(ROOT, "profiles", "r1_traffic_per_launch.csv")   # ncu dram__bytes_* of the bench launch
-        if os.path.exists(prof):
-            for row in open(prof).read().splitlines()[1:]:
-                f = row.split(",")
-                if len(f) >= 4 and f[0] == str(args.config) and f[1] == "grad_pair_kernel" and n == {4: 1 << 20, 5: 1 << 21}[args.config]:
-                    traffic = int(f[2]) + int(f[3])
-        roofline = {"bound": "alu", "kernel": "pair_kernel<GradPass> (bifrost_grad: pack + pair [+ reduce] timed together; "
-                                              "the pair kernel is > 99.9 % of it)",
-                    "achieved": dom["tflops"], "peak": peak, "unit": "TFLOP/s", "frac": dom["tflops"] / peak,
-                    "peak_source": f"derived: {num_sms} SMs x 64 FP64 lanes x 2 flop x clocks.max.sm "
-                                   f"(no FP64 figure in MEASURED_PEAKS.json)",
-                    "flops_per_interaction": FP64_FLOPS["grad"], "fp64_instr_per_interaction": FP64_INSTR["grad"],
-                    "fp64_pipe_issue_util": dom["fp64_pipe_issue_util"],
-                    "acc_grad_combined_frac": (FP64_FLOPS["acc"] + FP64_FLOPS["grad"]) * pairs_rank
-                    / (1e-3 * (mean_ms["acc"] + mean_ms["grad"])) / 1e12 / peak,
-                    "traffic": traffic}
+        dom_name = max((k for k in ("acc", "grad", "dtmin") if k in passes), key=lambda k: passes[k]["ms"])
+        dom = passes[dom_name]
+        roofline = roofline_of(args.config, n, dom_name, dom, passes, peak, num_sms, mean_ms, step_ms, path)
         if probe:
             roofline["measured_fp64_pipe"] = probe
             roofline["pipe_util_vs_measured_dfma"] = (
                 dom["fp64_pipe_issue_util"] / probe["dfma"]["frac_of_derived_pipe_peak"])
+        config5 = None
+        if world == 1 and args.config == 4 and not args.no_config5 and not args.n:
+            ctx.close()
+            del pos, vel, mass, acc, grad, dts, apn
+            torch.cuda.empty_cache()
+            config5 = run_config5(torch, dev, peak, num_sms)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
@@ -365,17 +408,98 @@ def run_cuda(args):
                            "timing": "CUDA events per C-ABI call on the launching stream, mean over steps, max over ranks"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "wall_s_timed_region": t_wall,
                 "passes": passes, "roofline": roofline}
+        if config5 is not None:
+            line["config5"] = config5
         if world == 1 and args.extras:
             line["extras"] = run_extras(torch, ctx, w, pos, vel, mass, acc)
         if world == 1 and not args.no_cpu_baseline:
             import oracle
             oracle.build()
             line["cpu_baseline"] = cpu_baseline(w, args.cpu_sinks)
+            line["cpu_fast"] = cpu_fast_baseline(w, 4 * args.cpu_sinks)
         print(json.dumps(line), flush=True)
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def static_traffic(cfg: int, n: int, kernel: str):
+    """dram__bytes_read + dram__bytes_write per launch of `kernel` from the committed ncu capture of this workload
+    (profiles/r2_traffic_per_launch.csv): a STATIC figure of an earlier run of the same source, not measured now."""
+    prof = os.path.join(ROOT, "profiles", "r2_traffic_per_launch.csv")
+    if not os.path.exists(prof) or n != {4: 1 << 20, 5: 1 << 21}.get(cfg):
+        return None, None
+    for row in open(prof).read().splitlines()[1:]:
+        f = row.split(",")
+        if len(f) >= 4 and f[0] == str(cfg) and f[1] == kernel:
+            return int(f[2]) + int(f[3]), f"static: profiles/r2_traffic_per_launch.csv ({f[4] if len(f) > 4 else 'ncu'})"
+    return None, None
+
+
+def roofline_of(cfg, n, dom_name, dom, passes, peak, num_sms, mean_ms, step_ms, path):
+    traffic, src = static_traffic(cfg, n, dom["kernel"].split("<")[0] + "_" + dom_name)
+    r = {"bound": "alu", "kernel": f"{dom['kernel']} (bifrost_{dom_name}: pack + pair + finish timed together; the pair "
+                                   "kernel is > 99.8 % of it)",
+         "share_of_step": dom["ms"] / step_ms,
+         "achieved": dom["tflops"], "peak": peak, "unit": "TFLOP/s", "frac": dom["tflops"] / peak,
+         "frac_is": "EXECUTED flops (2 DFMA + DADD + DMUL, SURVEY.md 8d's convention) / derived FP64 peak",
+         "peak_source": f"derived: {num_sms} SMs x 64 FP64 lanes x 2 flop x clocks.max.sm "
+                        f"(no FP64 figure in MEASURED_PEAKS.json); a register-only DFMA stream measures 0.997 of it",
+         "flops_per_interaction": dom["executed_flops_per_interaction"],
+         "fp64_instr_per_interaction": dom["executed_fp64_instr_per_interaction"],
+         "fp64_pipe_issue_util": dom["fp64_pipe_issue_util"],
+         "traffic": traffic, "traffic_source": src}
+    ag = mean_ms["acc"] + mean_ms["grad"]
+    pairs = passes["acc"]["interactions_per_s"] * passes["acc"]["ms"] * 1e-3
+    r["acc_grad"] = {
+        "ms": ag,
+        "frac_executed": (FP64_FLOPS[path]["acc"] + FP64_FLOPS[path]["grad"]) * pairs / (1e-3 * ag) / 1e12 / peak,
+        "frac_survey_8d": (SURVEY_8D_FLOPS["acc"] + SURVEY_8D_FLOPS["grad"]) * pairs / (1e-3 * ag) / 1e12 / peak,
+        "note": "frac_executed counts the flops the kernels execute; frac_survey_8d charges SURVEY.md 8(d)'s one-sided "
+                "26 + 42 flops to every ordered interaction delivered - it exceeds frac_executed (and may exceed 1) "
+                "because the symmetric kernels evaluate each unordered pair once"}
+    return r
+
+
+def run_config5(torch, dev, peak, num_sms):
+    """north_star's peak-throughput case (BASELINE.json configs[4]: N = 2^21, all active, acc + grad), timed in the
+    same run: 1 warm-up + 2 timed steps, CUDA events per call, L2 flushed between steps."""
+    from paper_2210_02472_b200.binding import Context
+    w = make_workload(5)
+    n = w.n
+    ctx = Context(n)
+    pos, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.mass))
+    acc = torch.zeros((n, 3), dtype=torch.float64, device=dev)
+    grad = torch.zeros_like(acc)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t_acc, t_grad, steps = 0.0, 0.0, 2
+    l0 = 0
+    for it in range(1 + steps):
+        flush.fill_(1)
+        if it == 1:
+            l0 = ctx.launch_count
+        ev[0].record()
+        ctx.acc(pos, mass, w.G, w.eps, out=acc)
+        ev[1].record()
+        ctx.grad(pos, mass, acc, w.G, w.eps, out=grad)
+        ev[2].record()
+        torch.cuda.synchronize()
+        if it > 0:
+            t_acc += ev[0].elapsed_time(ev[1]) / steps
+            t_grad += ev[1].elapsed_time(ev[2]) / steps
+    launches = ctx.launch_count - l0
+    ctx.close()
+    pairs = float(n) * n
+    fl = FP64_FLOPS["sym"]
+    return {"workload": workload_name(5, n), "steps": steps, "warmup": 1, "gpu_launches": int(launches),
+            "value": pairs / (1e-3 * (t_acc + t_grad)), "unit": UNIT, "acc_ms": t_acc, "grad_ms": t_grad,
+            "frac_executed": (fl["acc"] + fl["grad"]) * pairs / (1e-3 * (t_acc + t_grad)) / 1e12 / peak,
+            "frac_executed_acc": fl["acc"] * pairs / (1e-3 * t_acc) / 1e12 / peak,
+            "frac_executed_grad": fl["grad"] * pairs / (1e-3 * t_grad) / 1e12 / peak,
+            "frac_survey_8d": (SURVEY_8D_FLOPS["acc"] + SURVEY_8D_FLOPS["grad"]) * pairs / (1e-3 * (t_acc + t_grad)) / 1e12 / peak,
+            "target": "north_star: >= 0.60 of FP64 peak on this case (executed-flop convention)"}
 
 
 def run_extras(torch, ctx, w, pos, vel, mass, acc):
@@ -513,6 +637,7 @@ def main():
     ap.add_argument("--extras", action="store_true", help="also time the NEXT rows (jerk, potential, neighbours, components, one FSI cycle) once, outside the timed step")
     ap.add_argument("--sweep", action="store_true", help="small-active-set sweep of configs 2 and 3 (us per call); prints one JSON line")
     ap.add_argument("--no-fp64-probe", action="store_true", help="skip the register-only FP64-pipe peak probe")
+    ap.add_argument("--no-config5", action="store_true", help="skip the N = 2^21 acc + grad block of the default line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
