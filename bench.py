@@ -14,8 +14,10 @@ Metric: fp64 pair interactions/s for acc + FSI grad = n_sink * n_src / (t_acc + 
 interaction = one ordered (sink, source) pair evaluated in one pass.
 `ms_per_step` is the whole step (all four calls); `passes` lists every call's own time.
 
-Multi-GPU (torchrun, one rank per GPU): sinks are sharded across ranks (strong scaling, total
-work fixed), with one NCCL all-gather of the accelerations between the acc and grad passes.
+Multi-GPU (torchrun, one rank per GPU; strong scaling, total work fixed): the PAIR work of acc and grad is
+sharded across ranks (Context.set_shard: every rank evaluates its blocks of the unordered pairs and holds a partial
+sum for every particle), with one NCCL all-reduce of double[N][3] after each of the two passes; dtmin is sharded
+over sinks (no exchange).
 
 --impl reference times the CPU oracle (oracle/, unmodified) on the host cores on a bounded
 sample of the same workload and prints the same JSON line with "impl": "reference".
@@ -239,7 +241,9 @@ def run_cuda(args):
            torch.full((n,), -1, dtype=torch.int32, device=dev), torch.full((n,), -1, dtype=torch.int32, device=dev))
     apn = torch.empty((n, 3), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > L2 (126 MB)
-    names = ["acc", "allgather", "grad", "dtmin", "pn1"]
+    names = ["acc", "exchange_acc", "grad", "exchange_grad", "dtmin", "pn1"]
+    if world > 1:
+        ctx.set_shard(rank, world)                       # acc / grad: this rank's blocks of the unordered pairs
     ev = {k: [torch.cuda.Event(enable_timing=True) for _ in range(2)] for k in names}
 
     def step(timed: bool):
@@ -252,19 +256,19 @@ def run_cuda(args):
             fn()
             ev[name][1].record()
 
-        timed_call("acc", lambda: ctx.acc(pos, mass, w.G, w.eps, sinks, None, out=acc))
+        timed_call("acc", lambda: ctx.acc(pos, mass, w.G, w.eps, out=acc))
+        if world > 1:                                    # partial sums of every rank -> the accelerations (the exchange step)
+            timed_call("exchange_acc", lambda: sharding.allreduce_sum(acc))
+        timed_call("grad", lambda: ctx.grad(pos, mass, acc, w.G, w.eps, out=grad))
         if world > 1:
-            def gather():
-                acc.copy_(sharding.allgather_rows(acc[b:e], n))
-            timed_call("allgather", gather)
-        timed_call("grad", lambda: ctx.grad(pos, mass, acc, w.G, w.eps, sinks, None, out=grad))
+            timed_call("exchange_grad", lambda: sharding.allreduce_sum(grad))
         if full_path:
             timed_call("dtmin", lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, sinks, None, out=dts))
             # PN1.0 is BH x N work (2e8 pairs): every rank evaluates it redundantly (it is < 0.1 % of a step)
             timed_call("pn1", lambda: ctx.pn1(pos, vel, mass, bh, w.G, w.c, out=apn))
         torch.cuda.synchronize()
         for name in names:
-            if name in ("allgather",) and world == 1:
+            if name.startswith("exchange") and world == 1:
                 continue
             if name in ("dtmin", "pn1") and not full_path:
                 continue
@@ -292,7 +296,8 @@ def run_cuda(args):
     keys = list(recs[0].keys())
     mean_ms = {k: sum(r[k] for r in recs) / len(recs) for k in keys}
     step_ms = sum(mean_ms.values())
-    t = torch.tensor([step_ms, mean_ms["acc"] + mean_ms["grad"] + mean_ms.get("allgather", 0.0)] + [mean_ms[k] for k in keys],
+    t = torch.tensor([step_ms, mean_ms["acc"] + mean_ms["grad"] + mean_ms.get("exchange_acc", 0.0)
+                      + mean_ms.get("exchange_grad", 0.0)] + [mean_ms[k] for k in keys],
                      dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)          # max over ranks
@@ -324,12 +329,13 @@ def run_cuda(args):
                 ctx.acc_host(hpos, hmass, w.G, w.eps, None, None, out=hacc)
                 ctx.grad_host(hpos, hmass, hacc, w.G, w.eps, None, None, out=hgrad)
             else:
-                # sharded: inputs from pinned host memory, the acc all-gather stays on the device (NCCL), this rank's
-                # result rows back to the host - no device -> host -> device bounce around the collective
+                # sharded: inputs from pinned host memory, the two all-reduces stay on the device (NCCL), this rank's
+                # slice of the result rows back to the host - no device -> host -> device bounce around a collective
                 d_pos.copy_(t_pos, non_blocking=True); d_mass.copy_(t_mass, non_blocking=True)
-                ctx.acc(d_pos, d_mass, w.G, w.eps, sinks, None, out=acc)
-                acc.copy_(sharding.allgather_rows(acc[b:e], n))
-                ctx.grad(d_pos, d_mass, acc, w.G, w.eps, sinks, None, out=grad)
+                ctx.acc(d_pos, d_mass, w.G, w.eps, out=acc)
+                sharding.allreduce_sum(acc)
+                ctx.grad(d_pos, d_mass, acc, w.G, w.eps, out=grad)
+                sharding.allreduce_sum(grad)
                 t_acc_rows.copy_(acc[b:e], non_blocking=True); t_grad_rows.copy_(grad[b:e], non_blocking=True)
                 torch.cuda.synchronize()
             t1 = time.perf_counter()
@@ -351,9 +357,9 @@ def run_cuda(args):
                "ms_per_step": 1e3 * tt[1], "steps": e2e_steps,
                "how": ("bifrost_*_host entry points on pinned host arrays: H2D copies, kernels, D2H copies per call; "
                        "value = N^2 / host wall time of acc_host + grad_host") if world == 1 else
-                      ("per rank: pinned-host -> device copies of pos / mass, bifrost_acc on the rank's sinks, NCCL all-gather "
-                       "of acc on the device, bifrost_grad, the rank's acc / grad rows back to pinned host memory; "
-                       "value = N^2 / max over ranks of that wall time")}
+                      ("per rank: pinned-host -> device copies of pos / mass, bifrost_acc on the rank's pair blocks, NCCL "
+                       "all-reduce of acc on the device, bifrost_grad, all-reduce of grad, the rank's slice of the acc / grad "
+                       "rows back to pinned host memory; value = N^2 / max over ranks of that wall time")}
 
     if rank == 0:
         num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -364,8 +370,8 @@ def run_cuda(args):
             for mix, name in ((0, "dfma"), (1, "acc_mix"), (2, "dfma_3_distinct_operands"), (3, "dfma_accumulate_pattern")):
                 ms, rate = ctx.fp64_probe(mix=mix, iters=(1 << 15) if mix < 2 else (1 << 16), ctas_per_sm=32)
                 probe[name] = {"ms": ms, "lane_instr_per_s": rate, "frac_of_derived_pipe_peak": rate / (peak * 1e12 / 2)}
-        pairs_rank = float(max(sharding.slice_counts(n, world))) * n     # the slowest rank's share
-        path = "sym" if world == 1 and n >= 16384 else "plain"          # which acc / grad kernels these sizes select
+        pairs_rank = float(n) * n / world                               # a rank's share of the ordered interactions
+        path = "sym" if world > 1 or n >= 16384 else "plain"            # which acc / grad kernels these sizes select
         kernel_name = {"acc": {"sym": "sym_pair_kernel<SymAcc, 8, 256, 1>", "plain": "pair_kernel<AccPass, 8, 256, 1, 1>"},
                        "grad": {"sym": "sym_pair_kernel<SymGrad, 6, 256, 1>", "plain": "pair_kernel<GradPass, 5, 128, 2, 2>"},
                        "dtmin": {"sym": "pair_kernel<DtPass, 6, 128, 2, 1>", "plain": "pair_kernel<DtPass, 6, 128, 2, 1>"}}
@@ -384,8 +390,9 @@ def run_cuda(args):
         passes = {k: kern(k) for k in ("acc", "grad", "dtmin") if k in mean_ms}
         if "pn1" in mean_ms:
             passes["pn1"] = {"ms": mean_ms["pn1"], "interactions_per_s": 2.0 * len(w.bh_idx) * n / (mean_ms["pn1"] * 1e-3)}
-        if "allgather" in mean_ms:
-            passes["allgather"] = {"ms": mean_ms["allgather"], "bytes": 24 * n}
+        for k in ("exchange_acc", "exchange_grad"):
+            if k in mean_ms:
+                passes[k] = {"ms": mean_ms[k], "collective": "NCCL all-reduce (sum)", "bytes": 24 * n}
         dom_name = max((k for k in ("acc", "grad", "dtmin") if k in passes), key=lambda k: passes[k]["ms"])
         dom = passes[dom_name]
         roofline = roofline_of(args.config, n, dom_name, dom, passes, peak, num_sms, mean_ms, step_ms, path)
@@ -404,7 +411,9 @@ def run_cuda(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload_name(args.config, n), "n": n, "seed": w.seed,
                            "l2": "flushed between steps (256 MiB device write, outside the timed events)",
-                           "parallelism": f"sinks sharded over {world} rank(s)" + (", NCCL all-gather of acc" if world > 1 else ""),
+                           "parallelism": "1 rank" if world == 1 else
+                           f"acc / grad: unordered pairs sharded over {world} ranks + NCCL all-reduce of double[N][3] after each pass; "
+                           f"dtmin: sinks sharded over {world} ranks; pn1 redundant on every rank",
                            "timing": "CUDA events per C-ABI call on the launching stream, mean over steps, max over ranks"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "wall_s_timed_region": t_wall,
                 "passes": passes, "roofline": roofline}

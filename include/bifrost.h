@@ -88,6 +88,17 @@ int bifrost_destroy(bifrost_ctx* ctx);
 #define BIFROST_RESERVE_INTEGRATOR  2
 int bifrost_reserve(bifrost_ctx* ctx, int what);
 
+/* bifrost_set_shard - multi-GPU: shard the PAIR WORK of same-list bifrost_acc / bifrost_grad calls over `world`
+ * ranks (one context, one process, one GPU each).  With world > 1 a call whose sink and source
+ * lists are the same list evaluates only the blocks of the symmetric kernels owned by `rank` (dealt in snake
+ * order, so every rank gets the same share of the pairs) and writes, for EVERY row of the list, this rank's partial
+ * sum; the caller adds the ranks' outputs - one all-reduce (sum) of double[n][3], the path's exchange step - to
+ * obtain the result.  Such calls take the symmetric kernels at any list length; calls with different sink and
+ * source lists, with subsystems set, or on a context without the symmetric workspace return BIFROST_EINVAL while
+ * world > 1 (shard those over sinks instead: disjoint sink lists per rank, no partial sums).  Every other entry
+ * point is unaffected.  rank in [0, world); world = 1 restores the unsharded behaviour. */
+int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
+
 /* Launch-shape knobs.  They never change a result beyond its summation order; they exist for tuning and so
  * that tests can drive every launch path at small sizes.
  *   BIFROST_TUNE_FUSED_MAX_SINKS  calls with fewer sinks run as one fused launch (default 4096, 0..131072)
@@ -98,6 +109,8 @@ int bifrost_reserve(bifrost_ctx* ctx, int what);
 #define BIFROST_TUNE_FUSED_MAX_SINKS 0
 #define BIFROST_TUNE_SMALL_M         1
 #define BIFROST_TUNE_SYM_MIN_N       2
+#define BIFROST_TUNE_MUTUAL_MIN_PAIRS 3   /* bifrost_*_mutual: fewest n_a * n_b pairs for the two-list symmetric kernel
+                                             (default 5e7, and >= 512 entries in the shorter list; 0 = always) */
 int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value);
 
 const char* bifrost_strerror(int code);                 /* static string */
@@ -123,6 +136,23 @@ int bifrost_acc(bifrost_ctx* ctx, int64_t n, const double* pos, const double* ma
 int bifrost_grad(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
                  const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
                  double G, double eps, double* out_grad, void* stream);
+
+/* bifrost_acc_mutual / bifrost_grad_mutual - the inter-level sums of PAPER.md:L115-127 (Eq. 12, Eq. 13) for BOTH sets
+ * of a level in one call: with two DISJOINT id lists A (e.g. the slow set S) and B (the fast set F),
+ *     out[a] = the bifrost_acc (bifrost_grad) sum of sink a over the sources B,   a in A,
+ *     out[b] = the same sum of sink b over the sources A,                         b in B
+ * - exactly what the pair of calls (sinks A, sources B) and (sinks B, sources A) writes, rounding order apart.  Eq. 12-13
+ * are "pairwise kicks" (L131): each (a, b) pair's geometry serves both members, so large lists go through the
+ * two-list symmetric kernel (every pair evaluated once, 20 / 33 instead of 30 / 56 FP64 instructions per pair);
+ * short lists, and calls while subsystems are set, are issued as the two plain calls.  Both lists are required
+ * (non-NULL); an id that appears in both gets only one of its two sums.  Other conventions as bifrost_acc /
+ * bifrost_grad.  DEVICE pointers, asynchronous on stream. */
+int bifrost_acc_mutual(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
+                       const int32_t* a_idx, int64_t n_a, const int32_t* b_idx, int64_t n_b,
+                       double G, double eps, double* out_acc, void* stream);
+int bifrost_grad_mutual(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                        const int32_t* a_idx, int64_t n_a, const int32_t* b_idx, int64_t n_b,
+                        double G, double eps, double* out_grad, void* stream);
 
 /* bifrost_dtmin - PAPER.md:L312 Eq. 21 and L317 Eq. 22 (unsoftened), per sink i:
  *     out_dt_ff[i] = eta_ff * min_{j in src, j != i} sqrt( |r_ij|^3 / (G (m_i + m_j)) ),  out_j_ff[i] = argmin id
@@ -233,6 +263,23 @@ int bifrost_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
                        const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
                        double G, double r_ngb, double r_ngb_max, double tau, double C, int64_t cap,
                        int32_t* out_count, int32_t* out_list, void* stream);
+
+/* bifrost_dtmin_neighbours - bifrost_dtmin and bifrost_neighbours in ONE pass over the pairs.  The paper does
+ * the neighbour search "at the beginning of each integration hierarchy level along with the time-step assignment"
+ * (both are among the O(N^2) loops of L747); the two need the same records (x, v, m) and the same
+ * r_ij^2, so the pass of Eq. 21-22 (L312, L317) carries the distance pre-filter of Eq. 18-19 as one integer test
+ * per pair and sends the rare candidates through the same exact evaluation as bifrost_neighbours.  Arguments and
+ * outputs are those of the two calls; all six outputs are bit-identical to the separate calls' (out_count and
+ * out_list required, the four time-step outputs may be NULL).  While bifrost_set_subsystems is active the
+ * time-steps exclude same-subsystem pairs (L299) and the neighbour search does not, as in the separate calls.
+ * BIFROST_EINVAL if (28 + 4 cap) * n_sink bytes exceed the split-j workspace (1536 B x max_n).
+ * DEVICE pointers, asynchronous on stream. */
+int bifrost_dtmin_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                             const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src,
+                             double G, double eta_ff, double eta_fb,
+                             double r_ngb, double r_ngb_max, double tau, double C, int64_t cap,
+                             double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff, int32_t* out_j_fb,
+                             int32_t* out_count, int32_t* out_list, void* stream);
 
 /* bifrost_components - NEXT-3: subsystems are the connected components of the neighbour
  * graph.  count / list are bifrost_neighbours' outputs (rows of particles that were not sinks must have

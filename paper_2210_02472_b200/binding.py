@@ -29,8 +29,8 @@ SYMBOLS = [
     "bifrost_jerk", "bifrost_potential", "bifrost_timestep_criteria",
     "bifrost_acc_host", "bifrost_grad_host", "bifrost_dtmin_host", "bifrost_pn1_host",
     "bifrost_fp64_probe", "bifrost_set_subsystems", "bifrost_subsys_min",
-    "bifrost_neighbours", "bifrost_components",
-    "bifrost_reserve", "bifrost_set_tuning",
+    "bifrost_neighbours", "bifrost_components", "bifrost_dtmin_neighbours",
+    "bifrost_reserve", "bifrost_set_tuning", "bifrost_set_shard", "bifrost_acc_mutual", "bifrost_grad_mutual",
     "bifrost_acc_jerk", "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
 ]
 
@@ -74,10 +74,15 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_pn1_host.argtypes = [_P, _I64, _P, _P, _P, _P, _I64, _D, _D, _P]
     lib.bifrost_reserve.argtypes = [_P, _I]
     lib.bifrost_set_tuning.argtypes = [_P, _I, _I64]
+    lib.bifrost_set_shard.argtypes = [_P, _I, _I]
+    lib.bifrost_acc_mutual.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P, _P]
+    lib.bifrost_grad_mutual.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P]
     lib.bifrost_set_subsystems.argtypes = [_P, _P, _I64]
     lib.bifrost_subsys_min.argtypes = [_P, _I64, _P, _P, _P]
     lib.bifrost_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _I64, _P, _P, _P]
     lib.bifrost_components.argtypes = [_P, _I64, _P, _P, _I64, _P, _P]
+    lib.bifrost_dtmin_neighbours.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _D, _D, _D, _D, _D, _I64,
+                                             _P, _P, _P, _P, _P, _P, _P]
     lib.bifrost_acc_jerk.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P, _P]
     lib.bifrost_kick.argtypes = [_P, _I64, _P, _I64, _P, _P, _D, _D, _P, _P]
     lib.bifrost_drift.argtypes = [_P, _I64, _P, _I64, _P, _D, _P, _P]
@@ -89,12 +94,30 @@ def load_library() -> ctypes.CDLL:
     return lib
 
 
+# Tensors marshalled for the call being prepared: Context._stream(), evaluated as the last argument of every C call,
+# checks them together (same device as the context, equal row counts, index values in debug mode) and clears the list.
+_seen = []
+DEBUG_INDEX_CHECK = False      # True: every index list is range-checked against n (one device -> host sync per list)
+
+
 def _dev_f64(t, shape_tail, name):
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
         raise BifrostError(f"{name}: expected a contiguous float64 CUDA tensor")
-    if tuple(t.shape[1:]) != shape_tail:
+    if t.dim() < 1 or tuple(t.shape[1:]) != shape_tail:
         raise BifrostError(f"{name}: bad shape {tuple(t.shape)}")
+    _seen.append(("rows", name, t))
+    return t
+
+
+def _dev_i32_rows(t, shape_tail, name):
+    """An int32 per-particle array ([n] or [n, cap]): counted with the float64 arrays for the row check."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+        raise BifrostError(f"{name}: expected a contiguous int32 CUDA tensor")
+    if t.dim() < 1 or tuple(t.shape[1:]) != shape_tail:
+        raise BifrostError(f"{name}: bad shape {tuple(t.shape)}")
+    _seen.append(("rows", name, t))
     return t
 
 
@@ -104,6 +127,7 @@ def _dev_idx(t, name):
         return None, 0
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.dim() == 1):
         raise BifrostError(f"{name}: expected a contiguous 1-D int32 CUDA tensor")
+    _seen.append(("index", name, t))
     # an empty list is not NULL ("all particles"): hand the library a valid dummy address
     return t, (t.data_ptr() if t.numel() else _dummy_ptr(t.device))
 
@@ -158,16 +182,22 @@ class Context:
             pass
 
     def _check(self, rc, what):
+        _seen.clear()
         if rc != 0:
             msg = self._lib.bifrost_strerror(rc).decode()
             cu = self._lib.bifrost_last_cuda_error(self._h).decode()
             raise BifrostError(f"{what}: {msg}" + (f" [{cu}]" if cu else ""))
 
     RESERVE_HOST, RESERVE_INTEGRATOR = 1, 2
-    TUNE_FUSED_MAX_SINKS, TUNE_SMALL_M, TUNE_SYM_MIN_N = 0, 1, 2
+    TUNE_FUSED_MAX_SINKS, TUNE_SMALL_M, TUNE_SYM_MIN_N, TUNE_MUTUAL_MIN_PAIRS = 0, 1, 2, 3
 
     def reserve(self, what: int):
         self._check(self._lib.bifrost_reserve(self._h, int(what)), "bifrost_reserve")
+
+    def set_shard(self, rank: int, world: int):
+        """Shard the pair work of same-list acc / grad calls over `world` ranks: outputs become partial sums that
+        the caller all-reduces (sharding.allreduce_sum)."""
+        self._check(self._lib.bifrost_set_shard(self._h, int(rank), int(world)), "bifrost_set_shard")
 
     def set_tuning(self, knob: int, value: int):
         self._check(self._lib.bifrost_set_tuning(self._h, int(knob), int(value)), "bifrost_set_tuning")
@@ -176,10 +206,27 @@ class Context:
     def launch_count(self) -> int:
         return int(self._lib.bifrost_launch_count(self._h))
 
-    @staticmethod
-    def _stream():
+    def _stream(self):
+        """The context's device's current stream; also the one place where the tensors marshalled for this call are
+        checked together: all on the context's device, all per-particle arrays with the same number of rows, index
+        values inside [0, n) when DEBUG_INDEX_CHECK is set.  A mismatch raises BifrostError instead of becoming an
+        out-of-bounds device access."""
         import torch
-        return torch.cuda.current_stream().cuda_stream
+        seen, n_rows = list(_seen), None
+        _seen.clear()
+        for kind, name, t in seen:
+            if t.device.index != self.device:
+                raise BifrostError(f"{name}: tensor on {t.device}, context on cuda:{self.device}")
+            if kind == "rows":
+                if n_rows is None:
+                    n_rows = (t.shape[0], name)
+                elif t.shape[0] != n_rows[0]:
+                    raise BifrostError(f"{name}: {t.shape[0]} rows, but {n_rows[1]} has {n_rows[0]}")
+        if DEBUG_INDEX_CHECK and n_rows is not None:
+            for kind, name, t in seen:
+                if kind == "index" and t.numel() and (int(t.min()) < 0 or int(t.max()) >= n_rows[0]):
+                    raise BifrostError(f"{name}: ids outside [0, {n_rows[0]})")
+        return torch.cuda.current_stream(self.device).cuda_stream
 
     # ---- device-pointer entry points -------------------------------------------------
     def acc(self, pos, mass, G, eps, sink_idx=None, src_idx=None, out=None):
@@ -210,6 +257,38 @@ class Context:
         self._check(rc, "bifrost_grad")
         return out
 
+    def acc_mutual(self, pos, mass, G, eps, a_idx, b_idx, out=None):
+        """Eq. 12 for both sets of a level: out[a] = acc of a over sources B, out[b] = acc of b over sources A."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        ia, iap = _dev_idx(a_idx, "a_idx"); ib, ibp = _dev_idx(b_idx, "b_idx")
+        if ia is None or ib is None:
+            raise BifrostError("acc_mutual: both lists are required")
+        if out is None:
+            out = torch.zeros((n, 3), dtype=torch.float64, device=pos.device)
+        _dev_f64(out, (3,), "out")
+        rc = self._lib.bifrost_acc_mutual(self._h, n, pos.data_ptr(), mass.data_ptr(), iap, ia.shape[0], ibp, ib.shape[0],
+                                          float(G), float(eps), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_acc_mutual")
+        return out
+
+    def grad_mutual(self, pos, mass, acc, G, eps, a_idx, b_idx, out=None):
+        """Eq. 13 for both sets of a level (see acc_mutual)."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass"); acc = _dev_f64(acc, (3,), "acc")
+        n = mass.shape[0]
+        ia, iap = _dev_idx(a_idx, "a_idx"); ib, ibp = _dev_idx(b_idx, "b_idx")
+        if ia is None or ib is None:
+            raise BifrostError("grad_mutual: both lists are required")
+        if out is None:
+            out = torch.zeros((n, 3), dtype=torch.float64, device=pos.device)
+        _dev_f64(out, (3,), "out")
+        rc = self._lib.bifrost_grad_mutual(self._h, n, pos.data_ptr(), mass.data_ptr(), acc.data_ptr(), iap, ia.shape[0],
+                                           ibp, ib.shape[0], float(G), float(eps), out.data_ptr(), self._stream())
+        self._check(rc, "bifrost_grad_mutual")
+        return out
+
     def dtmin(self, pos, vel, mass, G, eta_ff, eta_fb, sink_idx=None, src_idx=None, out=None):
         """Returns (dt_ff, dt_fb, j_ff, j_fb), each of length n, written at sink ids
         (rows of inactive particles keep their initial value: +inf / -1)."""
@@ -222,6 +301,8 @@ class Context:
                    torch.full((n,), float("inf"), dtype=torch.float64, device=pos.device),
                    torch.full((n,), -1, dtype=torch.int32, device=pos.device),
                    torch.full((n,), -1, dtype=torch.int32, device=pos.device))
+        _dev_f64(out[0], (), "out dt_ff"); _dev_f64(out[1], (), "out dt_fb")
+        _dev_i32_rows(out[2], (), "out j_ff"); _dev_i32_rows(out[3], (), "out j_fb")
         rc = self._lib.bifrost_dtmin(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
                                      n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
                                      float(G), float(eta_ff), float(eta_fb),
@@ -360,13 +441,13 @@ class Context:
             self._subsys = None
             self._check(self._lib.bifrost_set_subsystems(self._h, None, 0), "bifrost_set_subsystems")
             return
-        _dev_idx(subsys, "subsys")
+        _dev_i32_rows(subsys, (), "subsys")
         self._subsys = subsys
         self._check(self._lib.bifrost_set_subsystems(self._h, subsys.data_ptr(), subsys.shape[0]),
                     "bifrost_set_subsystems")
 
     def subsys_min(self, subsys, inout_dt):
-        _dev_idx(subsys, "subsys")
+        _dev_i32_rows(subsys, (), "subsys")
         _dev_f64(inout_dt, (), "inout_dt")
         rc = self._lib.bifrost_subsys_min(self._h, subsys.shape[0], subsys.data_ptr(), inout_dt.data_ptr(), self._stream())
         self._check(rc, "bifrost_subsys_min")
@@ -383,6 +464,7 @@ class Context:
         if out is None:
             out = (torch.zeros((n,), dtype=torch.int32, device=pos.device),
                    torch.full((n, int(cap)), -1, dtype=torch.int32, device=pos.device))
+        _dev_i32_rows(out[0], (), "out count"); _dev_i32_rows(out[1], (int(cap),), "out list")
         rc = self._lib.bifrost_neighbours(self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None,
                                           n if si is None else si.shape[0], sjp or None, n if sj is None else sj.shape[0],
                                           float(G), float(r_ngb), float(r_ngb_max), float(tau), float(C), int(cap),
@@ -390,13 +472,37 @@ class Context:
         self._check(rc, "bifrost_neighbours")
         return out
 
+    def dtmin_neighbours(self, pos, vel, mass, G, eta_ff, eta_fb, r_ngb, r_ngb_max, tau, C, cap=16, sink_idx=None,
+                         src_idx=None):
+        """bifrost_dtmin and bifrost_neighbours in one pass: returns ((dt_ff, dt_fb, j_ff, j_fb), (count, list))."""
+        import torch
+        pos = _dev_f64(pos, (3,), "pos"); vel = _dev_f64(vel, (3,), "vel"); mass = _dev_f64(mass, (), "mass")
+        n = mass.shape[0]
+        si, sip = _dev_idx(sink_idx, "sink_idx"); sj, sjp = _dev_idx(src_idx, "src_idx")
+        d = (torch.full((n,), float("inf"), dtype=torch.float64, device=pos.device),
+             torch.full((n,), float("inf"), dtype=torch.float64, device=pos.device),
+             torch.full((n,), -1, dtype=torch.int32, device=pos.device),
+             torch.full((n,), -1, dtype=torch.int32, device=pos.device))
+        g = (torch.zeros((n,), dtype=torch.int32, device=pos.device),
+             torch.full((n, int(cap)), -1, dtype=torch.int32, device=pos.device))
+        rc = self._lib.bifrost_dtmin_neighbours(
+            self._h, n, pos.data_ptr(), vel.data_ptr(), mass.data_ptr(), sip or None, n if si is None else si.shape[0],
+            sjp or None, n if sj is None else sj.shape[0], float(G), float(eta_ff), float(eta_fb), float(r_ngb),
+            float(r_ngb_max), float(tau), float(C), int(cap), d[0].data_ptr(), d[1].data_ptr(), d[2].data_ptr(),
+            d[3].data_ptr(), g[0].data_ptr(), g[1].data_ptr(), self._stream())
+        self._check(rc, "bifrost_dtmin_neighbours")
+        return d, g
+
     def components(self, count, lst, out=None):
         """Subsystem id (smallest member id; -1 = single) of every particle from neighbour lists."""
         import torch
-        _dev_idx(count, "count")
+        if not (isinstance(lst, torch.Tensor) and lst.dim() == 2):
+            raise BifrostError("list: expected an [n, cap] int32 CUDA tensor")
         n, cap = int(lst.shape[0]), int(lst.shape[1])
+        _dev_i32_rows(count, (), "count"); _dev_i32_rows(lst, (cap,), "list")
         if out is None:
             out = torch.empty((n,), dtype=torch.int32, device=count.device)
+        _dev_i32_rows(out, (), "out")
         rc = self._lib.bifrost_components(self._h, n, count.data_ptr(), lst.data_ptr(), cap, out.data_ptr(), self._stream())
         self._check(rc, "bifrost_components")
         return out

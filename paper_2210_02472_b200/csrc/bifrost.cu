@@ -58,6 +58,7 @@ struct bifrost_ctx {
     int64_t max_n = 0;
     int num_sms = 0;
     double* src_rec = nullptr;       // packed source records, (max_n rounded up to TILE) * 10 doubles
+    size_t src_rec_doubles = 0;
     void* partial = nullptr;         // split-j partials / pn1 partials
     size_t partial_bytes = 0;
     unsigned char* is_bh = nullptr;  // [max_n]
@@ -69,8 +70,11 @@ struct bifrost_ctx {
     int64_t fused_max_sinks = 4096;  // below: one fused launch per call (BIFROST_TUNE_FUSED_MAX_SINKS)
     unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel, tagged with the launch epoch
     unsigned epoch = 0;              // one per fused launch (22 bits): a stale count of an aborted launch never matches
+    int shard_rank = 0, shard_world = 1;   // bifrost_set_shard: which blocks of the symmetric kernels this context evaluates
     double* sym_ws = nullptr;        // source-side rows of the symmetric (every pair once) kernels, [block][source][3]
     size_t sym_ws_bytes = 0;
+    int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
+    double mutual_min_pairs = 5e7;   // (below: two plain calls)
     int64_t sym_min_acc = 16384, sym_min_grad = 12288;   // shortest list the symmetric kernels are used for (measured
                                      // crossover, profiles/r2_symmetric.md; BIFROST_TUNE_SYM_MIN_N sets both)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
@@ -103,6 +107,8 @@ namespace {
             return BIFROST_ECUDA;                                                 \
         }                                                                         \
     } while (0)
+
+#define RC_TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
 
 struct DeviceGuard {
     int prev = -1;
@@ -253,7 +259,10 @@ constexpr int SYM_ACC_BS = 8 * 256, SYM_GRAD_BS = 6 * 256;   // sinks per CTA of
 template <class P, int S, int T, int MINB>
 int sym_impl(bifrost_ctx* ctx, int64_t min_n, const double* pos, const double* mass, const double* aux, const int32_t* idx,
              int64_t m, double G, double eps, double* out, int compact, cudaStream_t st) {
-    if (m < min_n || m < 2 || !ctx->sym_ws) return 1;
+    if (m < 2 || !ctx->sym_ws) return 1;
+    if (ctx->shard_world > 1) {                 // sharded: the symmetric kernels are the only path (all rows, partial sums)
+        if (compact) return BIFROST_EINVAL;
+    } else if (m < min_n) return 1;
     SymGeom g;
     g.m = (int)m;
     g.n_tiles = ceil_div(m, TILE);
@@ -261,8 +270,11 @@ int sym_impl(bifrost_ctx* ctx, int64_t min_n, const double* pos, const double* m
     g.tb = g.bs / TILE;
     g.n_blocks = ceil_div(m, g.bs);
     g.compact = compact;
+    g.rank = ctx->shard_rank; g.world = ctx->shard_world;
+    g.mutual = 0; g.m_b = 0; g.n_tiles_b = 0; g.rec_b = 0;
     int64_t total = 0;
     for (int b = 0; b < g.n_blocks; ++b) total += sym_range(g, b);
+    total = (total + g.world - 1) / g.world;
     const int64_t slots = (int64_t)ctx->num_sms * MINB;
     // ~64 CTAs per SM slot keep the tail of the last wave below ~1 % (measured: 24 -> 64 gains 1.5 %)
     g.unit_tiles = (int)std::max<int64_t>(2, (total + 64 * slots - 1) / (64 * slots));
@@ -270,15 +282,57 @@ int sym_impl(bifrost_ctx* ctx, int64_t min_n, const double* pos, const double* m
     const int64_t max_pieces_ws = (int64_t)(ctx->partial_bytes / (24 * (size_t)m));
     if (max_pieces_ws < 1) return 1;
     while (sym_pieces(g, 0) > max_pieces_ws) g.unit_tiles *= 2;
-    if (24 * (sym_joff(g, g.n_blocks - 1) + (size_t)sym_range(g, g.n_blocks - 1) * TILE) > ctx->sym_ws_bytes) return 1;
+    if (24 * (sym_joff(g, g.n_blocks - 1) + (size_t)sym_range(g, g.n_blocks - 1) * TILE) > ctx->sym_ws_bytes)
+        return ctx->shard_world > 1 ? BIFROST_EINVAL : 1;
     const int m_pad = g.n_tiles * TILE;
     sym_pack_kernel<P><<<ceil_div(m_pad, 256), 256, 0, st>>>((int)m, m_pad, idx, pos, mass, aux, ctx->src_rec);
-    const SymArgs a{soft2(eps), G, idx, out, (double*)ctx->partial, ctx->sym_ws};
+    const SymArgs a{soft2(eps), G, idx, nullptr, out, (double*)ctx->partial, ctx->sym_ws};
     const size_t smem = (2 * TILE * P::REC + (T / 32) * TILE * 3) * sizeof(double);
     dim3 grid(sym_pieces(g, 0), g.n_blocks);
-    sym_pair_kernel<P, S, T, MINB><<<grid, T, smem, st>>>(a, g, ctx->src_rec);
+    sym_pair_kernel<P, S, T, MINB, false><<<grid, T, smem, st>>>(a, g, ctx->src_rec);
     sym_finish_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);
     ctx->launches += 3;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
+// acc / grad between two DISJOINT lists, every (a, b) pair once and both lists served (sym_kernels.cuh, mutual mode):
+// the inter-level sums of Eq. 12-13 (S <- F and F <- S) in one pass.  Returns 1 when the call does not qualify (short
+// lists, workspace too small, pair sharding active): the caller then issues the two plain calls.
+template <class P, int S, int T, int MINB>
+int sym_mutual_impl(bifrost_ctx* ctx, const double* pos, const double* mass, const double* aux, const int32_t* idx_a,
+                    int64_t m_a, const int32_t* idx_b, int64_t m_b, double G, double eps, double* out, cudaStream_t st) {
+    if (!ctx->sym_ws || ctx->shard_world > 1) return 1;
+    if (m_a < m_b) { std::swap(idx_a, idx_b); std::swap(m_a, m_b); }     // A (blocks, registers) = the longer list
+    if (m_b < ctx->mutual_min_b || (double)m_a * (double)m_b < ctx->mutual_min_pairs) return 1;
+    SymGeom g{};
+    g.m = (int)m_a;
+    g.n_tiles = ceil_div(m_a, TILE);
+    g.bs = T * S;
+    g.tb = g.bs / TILE;
+    g.n_blocks = ceil_div(m_a, g.bs);
+    g.rank = 0; g.world = 1;
+    g.mutual = 1;
+    g.m_b = (int)m_b;
+    g.n_tiles_b = ceil_div(m_b, TILE);
+    g.rec_b = g.n_tiles * TILE;
+    const int64_t slots = (int64_t)ctx->num_sms * MINB;
+    const int64_t total = (int64_t)g.n_blocks * g.n_tiles_b;
+    g.unit_tiles = (int)std::max<int64_t>(2, (total + 64 * slots - 1) / (64 * slots));
+    const int64_t max_pieces_ws = (int64_t)(ctx->partial_bytes / (24 * (size_t)m_a));
+    if (max_pieces_ws < 1) return 1;
+    while (sym_pieces(g, 0) > max_pieces_ws) g.unit_tiles *= 2;
+    if (24 * (size_t)g.n_blocks * g.n_tiles_b * TILE > ctx->sym_ws_bytes) return 1;
+    if ((size_t)(g.rec_b + g.n_tiles_b * TILE) * P::REC > ctx->src_rec_doubles) return 1;
+    sym_pack_kernel<P><<<ceil_div(g.rec_b, 256), 256, 0, st>>>((int)m_a, g.rec_b, idx_a, pos, mass, aux, ctx->src_rec);
+    sym_pack_kernel<P><<<ceil_div(g.n_tiles_b * TILE, 256), 256, 0, st>>>((int)m_b, g.n_tiles_b * TILE, idx_b, pos, mass, aux,
+                                                                          ctx->src_rec + (size_t)g.rec_b * P::REC);
+    const SymArgs a{soft2(eps), G, idx_a, idx_b, out, (double*)ctx->partial, ctx->sym_ws};
+    const size_t smem = (2 * TILE * P::REC + (T / 32) * TILE * 3) * sizeof(double);
+    dim3 grid(sym_pieces(g, 0), g.n_blocks);
+    sym_pair_kernel<P, S, T, MINB, true><<<grid, T, smem, st>>>(a, g, ctx->src_rec);
+    sym_finish_kernel<<<ceil_div(m_a + m_b, 128), 128, 0, st>>>(a, g);
+    ctx->launches += 4;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
 }
@@ -288,6 +342,7 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
              cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
+    if (ctx->shard_world > 1 && (sub || sink_idx != src_idx || n_sink != n_src || !ctx->sym_ws)) return BIFROST_EINVAL;
     if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
         const int rc = sym_impl<SymAcc, 8, 256, 1>(ctx, ctx->sym_min_acc, pos, mass, nullptr, sink_idx, n_sink, G, eps, out, compact, st);
         if (rc <= 0) return rc;
@@ -307,6 +362,7 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
               double* out, int compact, cudaStream_t st) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
+    if (ctx->shard_world > 1 && (sub || sink_idx != src_idx || n_sink != n_src || !ctx->sym_ws)) return BIFROST_EINVAL;
     if (!sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
         const int rc = sym_impl<SymGrad, 6, 256, 1>(ctx, ctx->sym_min_grad, pos, mass, acc, sink_idx, n_sink, G, eps, out, compact, st);
         if (rc <= 0) return rc;
@@ -320,6 +376,36 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     using F1 = Shape<1, 128, 5, 2>;
     return sub ? run_pass<GradPassT<true>, Huge, 8, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
                : run_pass<GradPassT<false>, Huge, 8, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
+}
+
+// Eq. 12 / Eq. 13 between two disjoint lists: out[a] = sum over B, out[b] = sum over A
+int acc_mutual_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* a_idx, int64_t n_a,
+                    const int32_t* b_idx, int64_t n_b, double G, double eps, double* out, cudaStream_t st) {
+    if (n_a == 0 || n_b == 0) {                 // one side empty: the other side's sums are empty sums
+        if (n_a) RC_TRY(acc_impl(ctx, n, pos, mass, a_idx, n_a, b_idx, 0, G, eps, out, 0, st));
+        if (n_b) RC_TRY(acc_impl(ctx, n, pos, mass, b_idx, n_b, a_idx, 0, G, eps, out, 0, st));
+        return BIFROST_OK;
+    }
+    if (!(ctx->subsys && ctx->subsys_n == n)) {
+        const int rc = sym_mutual_impl<SymAcc, 8, 256, 1>(ctx, pos, mass, nullptr, a_idx, n_a, b_idx, n_b, G, eps, out, st);
+        if (rc <= 0) return rc;
+    }
+    RC_TRY(acc_impl(ctx, n, pos, mass, a_idx, n_a, b_idx, n_b, G, eps, out, 0, st));
+    return acc_impl(ctx, n, pos, mass, b_idx, n_b, a_idx, n_a, G, eps, out, 0, st);
+}
+int grad_mutual_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc, const int32_t* a_idx,
+                     int64_t n_a, const int32_t* b_idx, int64_t n_b, double G, double eps, double* out, cudaStream_t st) {
+    if (n_a == 0 || n_b == 0) {
+        if (n_a) RC_TRY(grad_impl(ctx, n, pos, mass, acc, a_idx, n_a, b_idx, 0, G, eps, out, 0, st));
+        if (n_b) RC_TRY(grad_impl(ctx, n, pos, mass, acc, b_idx, n_b, a_idx, 0, G, eps, out, 0, st));
+        return BIFROST_OK;
+    }
+    if (!(ctx->subsys && ctx->subsys_n == n)) {
+        const int rc = sym_mutual_impl<SymGrad, 6, 256, 1>(ctx, pos, mass, acc, a_idx, n_a, b_idx, n_b, G, eps, out, st);
+        if (rc <= 0) return rc;
+    }
+    RC_TRY(grad_impl(ctx, n, pos, mass, acc, a_idx, n_a, b_idx, n_b, G, eps, out, 0, st));
+    return grad_impl(ctx, n, pos, mass, acc, b_idx, n_b, a_idx, n_a, G, eps, out, 0, st);
 }
 
 // acceleration (Eq. 6) and jerk (Eq. 28) in one pass: GradPassT<EXCL, true> over (x, v, m) records
@@ -341,23 +427,40 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
                : run_pass<GradPassT<false, true>, Huge, 40, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st);
 }
 
+// ng == NULL: bifrost_dtmin; else the neighbour search of Eq. 18-19 rides on the same pass (bifrost_dtmin_neighbours)
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
                double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact,
-               cudaStream_t st) {
+               cudaStream_t st, const NgbArgs* ng = nullptr) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
-    // workspace (24 B per sink and split): keys [split][2][n_sink] doubles in the first two thirds,
-    // ids [split][2][n_sink] ints in the last third
-    double* pkey = (double*)ctx->partial;
-    int32_t* pid = (int32_t*)((char*)ctx->partial + (ctx->partial_bytes / 24) * 16);
+    // workspace per sink and split: 16 B of time-steps, 8 B of ids [, 4 B neighbour count + 4 cap B of list]; the regions
+    // share ctx->partial in those proportions, so whatever split count fits the whole fits every region
+    const size_t per_sink = 24 + (ng ? 4 * ((size_t)ng->cap + 1) : 0);
+    const size_t unit = (ctx->partial_bytes / per_sink) & ~(size_t)15;    // "sinks x splits" the workspace holds
+    char* base = (char*)ctx->partial;
+    double* pkey = (double*)base;
+    int32_t* pid = (int32_t*)(base + unit * 16);
     const SrcArrays src{pos, vel, mass, sub, src_idx};
-    const DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb};
+    DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
     using Huge = Shape<6, 128, 2, 1>;     // 0.7 % faster per pair than Big (after the rarely-taken update branch)
     using Big = Shape<4, 128, 3, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
     using F1 = Shape<1, 128, 5, 2>;
+    if (ng) {
+        a.ng = *ng;
+        a.ng.n_rows = (int)n_sink;
+        a.ng.pcount = (int32_t*)(base + unit * 24);
+        a.ng.plist = (int32_t*)(base + unit * 28);
+        // the neighbour test keeps r^2 and a count per sink alive: one sink fewer per thread fits the register file
+        using HugeN = Shape<5, 128, 2, 1>;
+        using BigN = Shape<4, 128, 2, 2>;
+        using F4N = Shape<4, 128, 2, 2>;
+        using F2N = Shape<2, 128, 3, 2>;
+        return sub ? run_pass<DtPassT<true, true>, HugeN, 7, BigN, F4N, F2N, F1>(ctx, a, src, n_sink, n_src, per_sink, compact, st)
+                   : run_pass<DtPassT<false, true>, HugeN, 7, BigN, F4N, F2N, F1>(ctx, a, src, n_sink, n_src, per_sink, compact, st);
+    }
     return sub ? run_pass<DtPassT<true>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st)
                : run_pass<DtPassT<false>, Huge, 7, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 24, compact, st);
 }
@@ -498,8 +601,6 @@ int drift_impl(bifrost_ctx* ctx, const int32_t* idx, int64_t m, const double* ve
     return BIFROST_OK;
 }
 
-#define RC_TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
-
 // Eq. 10 over the particles idx[0..m) interacting among themselves (idx == NULL: all n).
 // first_acc_valid: w_acc_s already holds the accelerations of this set at the current positions (left there by the
 // previous cycle over the same set, no drift of its particles since) - the opening sum is then skipped.  Eq. 11 has
@@ -580,9 +681,7 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     double* g = ctx->w_grad;
     auto inter_level_acc = [&]() -> int {                  // Eq. 12
         if (ns == 0) return BIFROST_OK;
-        RC_TRY(acc_impl(ctx, h.n, h.pos, h.mass, S, ns, F, nf, h.G, h.eps_soft, a, 0, st));
-        RC_TRY(acc_impl(ctx, h.n, h.pos, h.mass, F, nf, S, ns, h.G, h.eps_soft, a, 0, st));
-        return BIFROST_OK;
+        return acc_mutual_impl(ctx, h.n, h.pos, h.mass, S, ns, F, nf, h.G, h.eps_soft, a, st);
     };
     auto H_S = [&](bool second) -> int {
         if (ns == 0) return BIFROST_OK;
@@ -597,8 +696,7 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     RC_TRY(H_F());
     RC_TRY(inter_level_acc());
     if (ns) {                                              // Eq. 13
-        RC_TRY(grad_impl(ctx, h.n, h.pos, h.mass, a, S, ns, F, nf, h.G, h.eps_soft, g, 0, st));
-        RC_TRY(grad_impl(ctx, h.n, h.pos, h.mass, a, F, nf, S, ns, h.G, h.eps_soft, g, 0, st));
+        RC_TRY(grad_mutual_impl(ctx, h.n, h.pos, h.mass, a, S, ns, F, nf, h.G, h.eps_soft, g, st));
         RC_TRY(kick_impl(ctx, seg, m, a, g, 2.0 * tau / 3.0, tau * tau / 24.0, h.vel, st));
     }
     RC_TRY(H_F());
@@ -640,6 +738,7 @@ int bifrost_create(bifrost_ctx** out, int device, int64_t max_n) {
     const size_t n_pad = (size_t)((max_n + TILE - 1) / TILE) * TILE;
     ctx->partial_bytes = 24 * (size_t)max_n * 64;   // up to 16 source-range splits at n_sink = max_n
     if (ctx->partial_bytes < ((size_t)64 << 20)) ctx->partial_bytes = (size_t)64 << 20;
+    ctx->src_rec_doubles = n_pad * 10;
     if (cudaMalloc(&ctx->src_rec, n_pad * 10 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&ctx->partial, ctx->partial_bytes) != cudaSuccess ||
         cudaMalloc(&ctx->is_bh, (size_t)max_n) != cudaSuccess ||
@@ -683,8 +782,19 @@ int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
             ctx->small_m = (int)value; return BIFROST_OK;
         case BIFROST_TUNE_SYM_MIN_N:
             ctx->sym_min_acc = ctx->sym_min_grad = value; return BIFROST_OK;
+        case BIFROST_TUNE_MUTUAL_MIN_PAIRS:
+            ctx->mutual_min_pairs = (double)value; ctx->mutual_min_b = value == 0 ? 1 : 512; return BIFROST_OK;
         default: return BIFROST_EINVAL;
     }
+}
+
+int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world) {
+    if (!ctx || world < 1 || world > 1024 || rank < 0 || rank >= world) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if (world > 1 && !ctx->sym_ws) return BIFROST_EINVAL;     // needs the symmetric kernels' workspace
+    ctx->shard_rank = rank;
+    ctx->shard_world = world;
+    return BIFROST_OK;
 }
 
 int bifrost_reserve(bifrost_ctx* ctx, int what) {
@@ -732,6 +842,27 @@ int bifrost_grad(bifrost_ctx* ctx, int64_t n, const double* pos, const double* m
     DeviceGuard guard(ctx->device);
     return grad_impl(ctx, n, pos, mass, acc, sink_idx, n_sink, src_idx, n_src, G, eps, out_grad, 0,
                      (cudaStream_t)stream);
+}
+
+int bifrost_acc_mutual(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const int32_t* a_idx, int64_t n_a,
+                       const int32_t* b_idx, int64_t n_b, double G, double eps, double* out_acc, void* stream) {
+    if (!a_idx || !b_idx) return BIFROST_EINVAL;
+    int rc = check_lists(ctx, n, a_idx, n_a, b_idx, n_b);
+    if (rc) return rc;
+    if (n_a + n_b > 0 && (!pos || !mass || !out_acc)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return acc_mutual_impl(ctx, n, pos, mass, a_idx, n_a, b_idx, n_b, G, eps, out_acc, (cudaStream_t)stream);
+}
+
+int bifrost_grad_mutual(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass, const double* acc,
+                        const int32_t* a_idx, int64_t n_a, const int32_t* b_idx, int64_t n_b, double G, double eps,
+                        double* out_grad, void* stream) {
+    if (!a_idx || !b_idx) return BIFROST_EINVAL;
+    int rc = check_lists(ctx, n, a_idx, n_a, b_idx, n_b);
+    if (rc) return rc;
+    if (n_a + n_b > 0 && (!pos || !mass || !acc || !out_grad)) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    return grad_mutual_impl(ctx, n, pos, mass, acc, a_idx, n_a, b_idx, n_b, G, eps, out_grad, (cudaStream_t)stream);
 }
 
 int bifrost_dtmin(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
@@ -963,7 +1094,7 @@ int bifrost_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
         if (per_sink * (size_t)n_sink > ctx->partial_bytes) { g.n_split = 1; g.tiles_per_split = ceil_div(n_src, TILE) > 0 ? ceil_div(n_src, TILE) : 1; }
         int32_t* pcount = (int32_t*)ctx->partial;
         int32_t* plist = pcount + (size_t)g.n_split * (size_t)n_sink;
-        const NgbArgs a{pos, vel, mass, sink_idx, G, r_ngb, r_ngb_max, tau, C, guard2, (int)cap, out_count, out_list, pcount, plist};
+        const NgbArgs a{pos, vel, mass, sink_idx, G, r_ngb, r_ngb_max, tau, C, guard2, (int)cap, (int)n_sink, out_count, out_list, pcount, plist};
         dim3 grid(ceil_div(n_sink, T * S), g.n_split);
         ngb_kernel<S, T, MINB><<<grid, T, 0, st>>>(a, g, ctx->src_rec);
         ctx->launches++;
@@ -977,6 +1108,26 @@ int bifrost_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
     };
     // 6 sinks per thread is 6 % faster per pair (453.7 vs 482.3 ms at N = 2^20); the smaller CTA quantises better below
     return n_sink >= 32768 ? launch(Shape<6, 128, 3, 1>{}) : launch(Shape<4, 128, 4, 1>{});
+}
+
+int bifrost_dtmin_neighbours(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
+                             const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
+                             double eta_ff, double eta_fb, double r_ngb, double r_ngb_max, double tau, double C, int64_t cap,
+                             double* out_dt_ff, double* out_dt_fb, int32_t* out_j_ff, int32_t* out_j_fb,
+                             int32_t* out_count, int32_t* out_list, void* stream) {
+    int rc = check_lists(ctx, n, sink_idx, n_sink, src_idx, n_src);
+    if (rc) return rc;
+    if (cap <= 0 || cap > 1024) return BIFROST_EINVAL;
+    if (n_sink == 0) return BIFROST_OK;
+    if (!pos || !vel || !mass || !out_count || !out_list) return BIFROST_EINVAL;
+    // one list per sink must fit the workspace (else: separate calls, whose neighbour pass falls back to one split)
+    if ((24 + 4 * ((size_t)cap + 1)) * (size_t)n_sink > ctx->partial_bytes) return BIFROST_EINVAL;
+    DeviceGuard guard(ctx->device);
+    const double guard2 = (r_ngb_max * r_ngb_max) * (1.0 + 1e-10);
+    const NgbArgs ng{pos, vel, mass, sink_idx, G, r_ngb, r_ngb_max, tau, C, guard2, (int)cap, (int)n_sink, out_count, out_list,
+                     nullptr, nullptr};
+    return dtmin_impl(ctx, n, pos, vel, mass, sink_idx, n_sink, src_idx, n_src, G, eta_ff, eta_fb, out_dt_ff, out_dt_fb,
+                      out_j_ff, out_j_fb, 0, (cudaStream_t)stream, &ng);
 }
 
 int bifrost_components(bifrost_ctx* ctx, int64_t n, const int32_t* count, const int32_t* list, int64_t cap,

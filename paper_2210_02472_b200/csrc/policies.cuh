@@ -268,6 +268,50 @@ struct GradPassT {
 
 using GradPass = GradPassT<false>;
 
+// ----------------------------------------------------------------------------------------
+// NEXT-3: neighbour search, §3.4, Eq. 18-19, and subsystem construction.
+// A floating-point test decides an integer result here (is j a neighbour of i), so the decision is
+// taken in plain IEEE fp64 operation by operation (no contraction, correctly rounded sqrt and
+// division) in the order the paper states it: r_ij < r_ngb,max first, then the two-body a, e,
+// then Eq. 18 (bound) or Eq. 19 (unbound).  Only a conservative distance pre-filter runs on the
+// fast path (7 FP64 instructions per pair: the contracted r^2 against r_ngb,max^2 (1 + 1e-10)).
+// ----------------------------------------------------------------------------------------
+struct NgbArgs {
+    const double* pos; const double* vel; const double* mass;
+    const int32_t* sink_idx;
+    double G, r_ngb, r_ngb_max, tau, C, r2_guard;
+    int cap;
+    int n_rows;                                 // n_sink (row stride of the per-split scratch)
+    int32_t* out_count; int32_t* out_list;     // rows at sink ids (or sink positions when compact)
+    int32_t* pcount; int32_t* plist;           // [split][n_sink], [split][n_sink][cap]
+};
+
+__device__ __noinline__ bool ngb_exact(const NgbArgs& a, double dx, double dy, double dz, double ux, double uy, double uz,
+                                       double mi, double mj) {
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    const double r = sqrt(r2);
+    if (!(r < a.r_ngb_max)) return false;
+    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+    const double mu = __dmul_rn(a.G, __dadd_rn(mi, mj));
+    const double E = __dsub_rn(__dmul_rn(0.5, v2), mu / r);             // two-body orbital energy per reduced mass
+    if (E < 0.0) {                                                       // bound: Eq. 18
+        const double sma = -mu / __dmul_rn(2.0, E);
+        return (sma < a.r_ngb) || (r < a.r_ngb);
+    }
+    const double hx = __dsub_rn(__dmul_rn(dy, uz), __dmul_rn(dz, uy));   // h = r x v
+    const double hy = __dsub_rn(__dmul_rn(dz, ux), __dmul_rn(dx, uz));
+    const double hz = __dsub_rn(__dmul_rn(dx, uy), __dmul_rn(dy, ux));
+    const double h2 = __dadd_rn(__dadd_rn(__dmul_rn(hx, hx), __dmul_rn(hy, hy)), __dmul_rn(hz, hz));
+    double e2 = __dadd_rn(1.0, __dmul_rn(__dmul_rn(2.0, E), h2) / __dmul_rn(mu, mu));
+    if (e2 < 0.0) e2 = 0.0;
+    const double ecc = sqrt(e2);
+    const double r_peri = (h2 / mu) / __dadd_rn(1.0, ecc);               // = a (1 - e), finite for E = 0
+    if (!(r_peri < a.r_ngb)) return false;                               // Eq. 19
+    if (r < a.r_ngb) return true;
+    return __dmul_rn(a.C, r) / sqrt(v2) < a.tau;
+}
+
+
 struct DtArgs {
     const double* pos;
     const double* vel;
@@ -278,6 +322,7 @@ struct DtArgs {
     int32_t* pid;      // [split][2][n_sink]  their source ids
     double G, eta_ff, eta_fb;
     double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
+    NgbArgs ng;        // NGB only (bifrost_dtmin_neighbours): the neighbour search riding on the same pass
 };
 
 // Eq. 21 / Eq. 22 for ONE pair in plain IEEE operations (no contraction, correctly rounded sqrt and division),
@@ -318,14 +363,17 @@ __device__ __noinline__ bool dt_contender_wins(const DtArgs& a, int w, int i, in
 constexpr double KEY_SLACK = 1.0 - 1e-12;
 constexpr double KEY_SLACK2 = KEY_SLACK * KEY_SLACK;
 
-template <bool EXCL>
+// NGB = true (bifrost_dtmin_neighbours, "along with the time-step assignment"): the pass also runs the
+// neighbour search of Eq. 18-19 on the r^2 it already holds - one more integer pre-test per pair (r^2 below the
+// guarded r_ngb,max^2), candidates through ngb_exact in the rare path, lists appended in source order.
+template <bool EXCL, bool NGB = false>
 struct DtPassT {
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
     static constexpr int PHASED_MIN_S = 1;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
-    // thr = (key of the running best) * KEY_SLACK; j = its source id (-1: none yet)
-    struct Acc { double thr_ff, thr_fb; int jff, jfb; };
+    // thr = (key of the running best) * KEY_SLACK; j = its source id (-1: none yet); nc = neighbours found (NGB)
+    struct Acc { double thr_ff, thr_fb; int jff, jfb, nc; };
     struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
     __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
         if (j >= 0) {
@@ -348,7 +396,7 @@ struct DtPassT {
         s.m = a.mass[id]; s.id = id;
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
-    __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; }
+    __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; c.nc = 0; }
     // one key of one sink against the running best (rare path)
     __device__ __forceinline__ static void contend(const Args& a, int w, int i, double key, int jid, double& thr, int& jbest) {
         if (!(key >= thr)) return;
@@ -357,10 +405,10 @@ struct DtPassT {
     }
     // FP64-pipe instructions of the keys: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
     // 2 DMUL keys = 23.
-    __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb) {
+    __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb, double& r2) {
         const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
         const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
+        r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
         const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
         const double y0 = rsqrt_seed(r2);
         const double t = y0 * y0;
@@ -377,30 +425,48 @@ struct DtPassT {
     // hi(key) >= hi(thr).  (The self pair and same-subsystem pairs are filtered in the rare path only.)
     template <int S>
     __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
-        double kff[S], kfb[S];
+        double kff[S], kfb[S], r2[S];
         bool any = false;
+        const int guard_hi = NGB ? __double2hiint(a.ng.r2_guard) : 0;
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            keys(sk[s], r, kff[s], kfb[s]);
+            keys(sk[s], r, kff[s], kfb[s], r2[s]);
             any |= (__double2hiint(kff[s]) >= __double2hiint(c[s].thr_ff)) | (__double2hiint(kfb[s]) >= __double2hiint(c[s].thr_fb));
+            // r^2 >= 0 and the guard >= 0, so r^2 < guard implies hi(r^2) <= hi(guard)
+            if (NGB) any |= __double2hiint(r2[s]) <= guard_hi;
         }
         if (any) {
             const int jid = __double2loint(r[7]);
 #pragma unroll
             for (int s = 0; s < S; ++s) {
-                const bool other = EXCL ? ((jid != sk[s].id) & (__double2hiint(r[7]) != sk[s].sub)) : (jid != sk[s].id);
-                if (!other) continue;
+                if (jid == sk[s].id) continue;
+                if (NGB && r2[s] < a.ng.r2_guard) neighbour(a, sk[s], c[s], sink_row<S>(s), r, jid);     // ignores subsystems, as bifrost_neighbours
+                if (EXCL && __double2hiint(r[7]) == sk[s].sub) continue;
                 contend(a, 0, sk[s].id, kff[s], jid, c[s].thr_ff, c[s].jff);
                 if (kfb[s] > 0.0) contend(a, 1, sk[s].id, kfb[s], jid, c[s].thr_fb, c[s].jfb);   // v_ij = 0: dt_fb = +inf, never a minimum (T3)
             }
         }
     }
-    // the split's winners with their exact time-steps (Eq. 21 / 22 evaluated once per sink and split)
+    // row of the thread's s-th sink (the kernels lay sinks out as k = blockIdx.x * T * S + threadIdx.x + s * T)
+    template <int S>
+    __device__ __forceinline__ static int sink_row(int s) { return blockIdx.x * (blockDim.x * S) + threadIdx.x + s * blockDim.x; }
+    // NGB: Eq. 18-19 for a candidate pair in plain IEEE operations; the id is appended to this split's list of the
+    // sink.  Out of line with everything passed BY VALUE, so that the thread's sinks and running state stay in registers.
+    __device__ __noinline__ static int neighbour_slow(const NgbArgs& ng, double dx, double dy, double dz, double ux, double uy,
+                                                      double uz, double mi, double mj, int nc, int k, int jid) {
+        if (!ngb_exact(ng, dx, dy, dz, ux, uy, uz, mi, mj)) return nc;
+        if (k < ng.n_rows && nc < ng.cap) ng.plist[((size_t)blockIdx.y * ng.n_rows + k) * ng.cap + nc] = jid;
+        return nc + 1;
+    }
+    __device__ __forceinline__ static void neighbour(const Args& a, const Sink& s, Acc& c, int k, const double* __restrict__ r, int jid) {
+        c.nc = neighbour_slow(a.ng, r[0] - s.x, r[1] - s.y, r[2] - s.z, r[4] - s.vx, r[5] - s.vy, r[6] - s.vz, s.m, r[3], c.nc, k, jid);
+    }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         const size_t o = (size_t)split * 2 * g.n_sink + k;
         const double inf = __longlong_as_double(0x7ff0000000000000LL);
         a.pkey[o] = c.jff >= 0 ? dt_exact_ids(a, 0, id, c.jff) : inf;
         a.pkey[o + g.n_sink] = c.jfb >= 0 ? dt_exact_ids(a, 1, id, c.jfb) : inf;
+        if (NGB) a.ng.pcount[(size_t)split * g.n_sink + k] = c.nc;
         a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
     }
     // dtmin epilogue: the minimum over the splits' exact time-steps (ties -> smaller id): order-independent.
@@ -433,6 +499,17 @@ struct DtPassT {
         if (a.dt_fb) a.dt_fb[row] = jb[1] >= 0 ? tb[1] : inf;
         if (a.j_ff) a.j_ff[row] = jb[0];
         if (a.j_fb) a.j_fb[row] = jb[1];
+        if (NGB) {      // the per-split lists in split order (= source-list order); the count is never truncated
+            int total = 0;
+            for (int s = 0; s < g.n_split; ++s) {
+                const int cnt = __ldcg(a.ng.pcount + (size_t)s * g.n_sink + k);
+                const int32_t* l = a.ng.plist + ((size_t)s * g.n_sink + k) * a.ng.cap;
+                for (int q = 0; q < cnt && q < a.ng.cap && total + q < a.ng.cap; ++q)
+                    a.ng.out_list[(size_t)row * a.ng.cap + total + q] = __ldcg(l + q);
+                total += cnt;
+            }
+            a.ng.out_count[row] = total;
+        }
     }
 };
 

@@ -26,47 +26,7 @@ __global__ void smin_apply_kernel(int n, const int32_t* __restrict__ subsys, con
     if (s >= 0) dt[i] = __longlong_as_double((long long)smin[s]);
 }
 
-// ----------------------------------------------------------------------------------------
-// NEXT-3: neighbour search, §3.4, Eq. 18-19, and subsystem construction.
-// A floating-point test decides an integer result here (is j a neighbour of i), so the decision is
-// taken in plain IEEE fp64 operation by operation (no contraction, correctly rounded sqrt and
-// division) in the order the paper states it: r_ij < r_ngb,max first, then the two-body a, e,
-// then Eq. 18 (bound) or Eq. 19 (unbound).  Only a conservative distance pre-filter runs on the
-// fast path (7 FP64 instructions per pair: the contracted r^2 against r_ngb,max^2 (1 + 1e-10)).
-// ----------------------------------------------------------------------------------------
-struct NgbArgs {
-    const double* pos; const double* vel; const double* mass;
-    const int32_t* sink_idx;
-    double G, r_ngb, r_ngb_max, tau, C, r2_guard;
-    int cap;
-    int32_t* out_count; int32_t* out_list;     // rows at sink ids (or sink positions when compact)
-    int32_t* pcount; int32_t* plist;           // [split][n_sink], [split][n_sink][cap]
-};
-
-__device__ __noinline__ bool ngb_exact(const NgbArgs& a, double dx, double dy, double dz, double ux, double uy, double uz,
-                                       double mi, double mj) {
-    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-    const double r = sqrt(r2);
-    if (!(r < a.r_ngb_max)) return false;
-    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
-    const double mu = __dmul_rn(a.G, __dadd_rn(mi, mj));
-    const double E = __dsub_rn(__dmul_rn(0.5, v2), mu / r);             // two-body orbital energy per reduced mass
-    if (E < 0.0) {                                                       // bound: Eq. 18
-        const double sma = -mu / __dmul_rn(2.0, E);
-        return (sma < a.r_ngb) || (r < a.r_ngb);
-    }
-    const double hx = __dsub_rn(__dmul_rn(dy, uz), __dmul_rn(dz, uy));   // h = r x v
-    const double hy = __dsub_rn(__dmul_rn(dz, ux), __dmul_rn(dx, uz));
-    const double hz = __dsub_rn(__dmul_rn(dx, uy), __dmul_rn(dy, ux));
-    const double h2 = __dadd_rn(__dadd_rn(__dmul_rn(hx, hx), __dmul_rn(hy, hy)), __dmul_rn(hz, hz));
-    double e2 = __dadd_rn(1.0, __dmul_rn(__dmul_rn(2.0, E), h2) / __dmul_rn(mu, mu));
-    if (e2 < 0.0) e2 = 0.0;
-    const double ecc = sqrt(e2);
-    const double r_peri = (h2 / mu) / __dadd_rn(1.0, ecc);               // = a (1 - e), finite for E = 0
-    if (!(r_peri < a.r_ngb)) return false;                               // Eq. 19
-    if (r < a.r_ngb) return true;
-    return __dmul_rn(a.C, r) / sqrt(v2) < a.tau;
-}
+// (NgbArgs and ngb_exact, the exact evaluation of Eq. 18-19, live in policies.cuh: the fused dtmin + neighbours pass uses them too)
 
 template <int S, int T, int MINB>
 __global__ void __launch_bounds__(T, MINB)

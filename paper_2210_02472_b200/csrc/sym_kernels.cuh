@@ -26,15 +26,34 @@ struct SymGeom {
     int n_blocks;     // ceil(m / bs)
     int unit_tiles;   // target number of source tiles per CTA
     int compact;      // 1: output row = list position, 0: output row = particle id
+    int rank, world;  // bifrost_set_shard: this launch evaluates the blocks owned by `rank` of `world` only
+    // mutual mode (bifrost_acc_mutual / bifrost_grad_mutual, the inter-level sums of Eq. 12-13): sinks = list A (the m
+    // entries above), sources = a DISJOINT list B; every (a, b) pair once, both lists get their sums.  No diagonal;
+    // every block meets all tiles of B, whose records start at record row rec_b.
+    int mutual;       // 0: one list on both sides (triangle), 1: two lists (rectangle)
+    int m_b;          // length of list B
+    int n_tiles_b;    // ceil(m_b / TILE)
+    int rec_b;        // first record row of list B (= n_tiles * TILE)
 };
-// source tiles strictly beyond block b
+// Owner of block b when the pair work is sharded over ranks (multi-GPU): blocks are dealt in snake order
+// (0 1 .. w-1, w-1 .. 1 0, ...) - a block's work falls linearly with b, so every rank's share of the pairs is the
+// same up to O(w / n_blocks^2).
+__host__ __device__ inline int sym_owner(const SymGeom& g, int b) {
+    const int q = b / g.world, r = b % g.world;
+    return (q & 1) ? g.world - 1 - r : r;
+}
+// source tiles evaluated both ways by block b: the tiles strictly beyond the block (all tiles of B in mutual mode)
 __host__ __device__ inline int sym_range(const SymGeom& g, int b) {
+    if (g.mutual) return g.n_tiles_b;
     const int r = g.n_tiles - (b + 1) * g.tb;
     return r > 0 ? r : 0;
 }
+// first of those tiles (a tile index into the source records)
+__host__ __device__ inline int sym_first(const SymGeom& g, int b) { return g.mutual ? 0 : (b + 1) * g.tb; }
 // CTAs (pieces) that share block b: the first sym_diag_pieces do the block's own tiles (the diagonal), the others
 // the tiles beyond the block, at most unit_tiles each
 __host__ __device__ inline int sym_diag_tiles(const SymGeom& g, int b) {
+    if (g.mutual) return 0;
     const int r = g.n_tiles - b * g.tb;
     return r < g.tb ? r : g.tb;
 }
@@ -46,12 +65,14 @@ __host__ __device__ inline int sym_pieces(const SymGeom& g, int b) {
 }
 // first row of block b in the source-side workspace: rows of blocks b' < b, each (n_tiles - (b'+1) tb) * TILE long
 __host__ __device__ inline size_t sym_joff(const SymGeom& g, int b) {
+    if (g.mutual) return (size_t)b * g.n_tiles_b * TILE;
     return ((size_t)b * g.n_tiles - (size_t)g.tb * ((size_t)b * (b + 1) / 2)) * TILE;
 }
 
 struct SymArgs {
     double eps2, G;
     const int32_t* idx;     // the list (NULL: particles 0..m-1)
+    const int32_t* idx_b;   // mutual mode: list B
     double* out;            // [.][3]
     double* pi;             // sink-side pieces   [piece][m][3]
     double* pj;             // source-side rows   [sym_joff(b) + j - (b+1) bs][3]
@@ -206,9 +227,11 @@ __device__ __forceinline__ void warp_sum_4x3(const double (*L)[3], int lane, dou
 }
 
 // ---- the pair kernel: grid = (max pieces, blocks) ---------------------------------------------------
-template <class P, int S, int T, int MINB>
+template <class P, int S, int T, int MINB, bool MUTUAL>
 __global__ void __launch_bounds__(T, MINB)
-sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec) {
+sym_pair_kernel(const SymArgs a, const SymGeom g_in, const double* __restrict__ rec) {
+    SymGeom g = g_in;
+    g.mutual = MUTUAL;                              // compile-time in the geometry helpers below
     constexpr int REC = P::REC;
     constexpr int NW = T / 32;
     constexpr int CHUNKS = TILE * REC * 8 / 16;
@@ -218,7 +241,7 @@ sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec
 
     const int b = blockIdx.y, piece = blockIdx.x;
     const int range = sym_range(g, b), np = sym_pieces(g, b);
-    if (piece >= np) return;
+    if (piece >= np || (g.world > 1 && sym_owner(g, b) != g.rank)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     typename P::Sink sink[S];
@@ -232,20 +255,21 @@ sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec
         P::init(accu[s]);
     }
 
+    const double* __restrict__ src = rec + (size_t)(g.mutual ? g.rec_b : 0) * REC;
     auto load_tile = [&](int tile, int buf) {
-        const double* gsrc = rec + (size_t)tile * TILE * REC;
+        const double* gsrc = src + (size_t)tile * TILE * REC;
         double* dst = tile_sm + buf * TILE * REC;
         for (int ch = threadIdx.x; ch < CHUNKS; ch += T) cp_async16(dst + 2 * ch, gsrc + 2 * ch);
         cp_async_commit();
     };
 
     // this piece's tiles: an equal share of the diagonal [b tb, (b+1) tb) or of the tiles beyond the block
-    const int jb = (b + 1) * g.tb;
+    const int jb = sym_first(g, b);
     const int nd = sym_diag_pieces(g, b), dt = sym_diag_tiles(g, b);
     const bool diag = piece < nd;
     const int len = diag ? (dt + nd - 1) / nd : (range + (np - nd) - 1) / (np - nd);
     const int t0 = diag ? b * g.tb + piece * len : jb + (piece - nd) * len;
-    const int t1 = min(t0 + len, diag ? b * g.tb + dt : g.n_tiles);
+    const int t1 = min(t0 + len, diag ? b * g.tb + dt : jb + range);
     const int n_my = max(t1 - t0, 0);
     auto tile_of = [&](int q) { return t0 + q; };
 
@@ -257,7 +281,7 @@ sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec
         else cp_async_wait<0>();
         __syncthreads();
         const double* __restrict__ tb = tile_sm + buf * TILE * REC;
-        if (tile < jb) {                            // diagonal: ordered pairs, sink side only
+        if (diag) {                                 // diagonal: ordered pairs, sink side only
             const int cnt = min(TILE, g.m - tile * TILE);
             for (int jj = 0; jj < cnt; ++jj) {
                 double r[REC];
@@ -315,18 +339,33 @@ sym_pair_kernel(const SymArgs a, const SymGeom g, const double* __restrict__ rec
 }
 
 // ---- finish: fixed-order sum of the sink-side pieces of the own block and the source-side rows of the earlier blocks
+// (sharded: only of the blocks this rank owns - the result is then this rank's PARTIAL sum for every row, and the
+// caller adds the ranks' outputs, one all-reduce)
 __global__ void sym_finish_kernel(const SymArgs a, const SymGeom g) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= g.m) return;
+    if (k >= g.m + (g.mutual ? g.m_b : 0)) return;
+    if (k >= g.m) {                                 // mutual mode, a row of list B: the source-side rows of ALL blocks
+        const int j = k - g.m;
+        double jx = 0.0, jy = 0.0, jz = 0.0;
+        for (int bb = 0; bb < g.n_blocks; ++bb) {
+            if (g.world > 1 && sym_owner(g, bb) != g.rank) continue;
+            const double* q = a.pj + 3 * (sym_joff(g, bb) + (size_t)j);
+            jx += __ldcg(q); jy += __ldcg(q + 1); jz += __ldcg(q + 2);
+        }
+        double* o = a.out + 3 * (size_t)(a.idx_b ? a.idx_b[j] : j);
+        o[0] = -a.G * jx; o[1] = -a.G * jy; o[2] = -a.G * jz;
+        return;
+    }
     const int b = k / g.bs;
-    const int np = sym_pieces(g, b);
+    const int np = (g.world > 1 && sym_owner(g, b) != g.rank) ? 0 : sym_pieces(g, b);
     double sx = 0.0, sy = 0.0, sz = 0.0;
     for (int p = 0; p < np; ++p) {
         const double* q = a.pi + 3 * ((size_t)p * g.m + k);
         sx += __ldcg(q); sy += __ldcg(q + 1); sz += __ldcg(q + 2);
     }
     double jx = 0.0, jy = 0.0, jz = 0.0;
-    for (int bb = 0; bb < b; ++bb) {
+    for (int bb = 0; bb < b && !g.mutual; ++bb) {
+        if (g.world > 1 && sym_owner(g, bb) != g.rank) continue;
         const double* q = a.pj + 3 * (sym_joff(g, bb) + (size_t)(k - (bb + 1) * g.bs));
         jx += __ldcg(q); jy += __ldcg(q + 1); jz += __ldcg(q + 2);
     }

@@ -2,8 +2,12 @@
 
 This module is the ONLY code shared between the CPU oracle's tests and the CUDA
 path's tests / bench: it produces particle arrays (positions, velocities,
-masses) and index lists, and holds none of the method's arithmetic (no
-acceleration, gradient, time-step or PN formula lives here).  The recipes are
+masses) and index lists.  None of the method's routines (acceleration, gradient,
+time-step, PN) lives here and nothing here is called by the library or the
+oracle.  One input-preparation helper does evaluate a pair sum: config 2 asks for
+"virialised velocities", so `_virial_potential_energy` computes the cluster's
+potential energy W once, in numpy, to rescale the sampled speeds to 2T = -W; it
+feeds the INPUTS only and is never compared with, or used by, either side.  The recipes are
 stated in DESIGN.md §"Input recipe"; they stand in for the paper's SCIC
 initial-conditions generator (App. A), whose output is
 not available.
@@ -148,9 +152,10 @@ def active_subset(seed: int, n: int, size: int) -> np.ndarray:
     return ids.astype(np.int32)
 
 
-def _pair_potential_energy(pos: np.ndarray, mass: np.ndarray, chunk: int = 512) -> float:
-    """W = -G sum_{i<j} m_i m_j / r_ij by chunked numpy direct summation.  Used
-    only to virialise config 2's velocities (input preparation, not the method)."""
+def _virial_potential_energy(pos: np.ndarray, mass: np.ndarray, chunk: int = 512) -> float:
+    """W = -G sum_{i<j} m_i m_j / r_ij by chunked numpy direct summation.  INPUT PREPARATION ONLY:
+    used once to virialise config 2's velocities (see the module docstring); not a routine of the
+    method, not shared with the library or the oracle."""
     n = mass.shape[0]
     w = 0.0
     x, y, z = (np.ascontiguousarray(pos[:, c]) for c in range(3))
@@ -233,7 +238,7 @@ def config2(n: int = 16384, seed: int = 1) -> Workload:
     mass = kroupa_masses(rng, n)
     mass /= mass.sum()
     recentre(pos, vel, mass)
-    w = _pair_potential_energy(pos, mass)
+    w = _virial_potential_energy(pos, mass)
     t = 0.5 * float((mass * (vel * vel).sum(axis=1)).sum())
     vel *= np.sqrt(-0.5 * w / t)
     return Workload("config2", pos, vel, mass, G_NBODY, 1e-5, 0.01, 0.01, seed=seed)
@@ -308,6 +313,30 @@ def config5(n: int = 1 << 21, seed: int = 4) -> Workload:
     mass = kroupa_masses(rng, n)
     mass /= mass.sum()
     return Workload("config5", pos, vel, mass, G_NBODY, 1e-5, 0.01, 0.01, seed=seed)
+
+
+#: §5.2 / Fig. 8 in N-body units (G = M = a_p = 1): r_h = 3.1 pc fixes a_p = 3.1 pc / R_HALF,
+#: M = 161000 x 0.5 Msun fixes the time unit sqrt(a_p^3 / (G M)) with G = 4.30091e-3 pc (km/s)^2 / Msun
+#: and 1 pc / (km/s) = 0.977792 Myr.
+FIG8_PC = 3.1 / R_HALF                                            # parsecs per length unit
+FIG8_MYR = (FIG8_PC ** 3 / (4.30091e-3 * 161000 * 0.5)) ** 0.5 * 0.977792   # Myr per time unit
+
+
+def fig8(n: int = 161000, seed: int = 8) -> Workload:
+    """The softened equal-mass cluster of PAPER.md:L816-824 (§5.2, Fig. 8, "FROST-like" run): Plummer sphere of
+    N = 161000 equal masses, r_h = 3.1 pc, Plummer softening eps_soft = 1e-3 pc, eta_ff = eta_fb = 0.2 (the
+    gradient / jerk criteria use eta = 0.1), integration interval tau = 1e-3 Myr = `fig8_tau()`.  Centre-of-mass
+    frame.  A smaller n keeps the physical scales (same r_h, same softening) with heavier particles."""
+    rng = np.random.default_rng(seed)
+    pos, vel = plummer_phase_space(rng, n)
+    mass = np.full(n, 1.0 / n)
+    recentre(pos, vel, mass)
+    return Workload("fig8", pos, vel, mass, G_NBODY, 1e-3 / FIG8_PC, 0.2, 0.2, seed=seed)
+
+
+def fig8_tau() -> float:
+    """The integration interval of PAPER.md:L822 (1e-3 Myr) in N-body time units."""
+    return 1e-3 / FIG8_MYR
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}

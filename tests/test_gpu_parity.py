@@ -999,3 +999,201 @@ def test_reserve_and_tuning_api(torch):
     check_vec(a1, a2, "fused vs packed", tol=1e-13)
     check_vec(a1, oracle.acc(w.pos, w.mass, w.G, 1e-3), "acc_host")
     c.close()
+
+
+@pytest.mark.parametrize("case", ["all", "subset", "small", "subsys"])
+def test_dtmin_neighbours_one_pass_equals_the_two_calls(torch, ctx, case):
+    """bifrost_dtmin_neighbours (the neighbour search runs "along with the time-step assignment"):
+    all six outputs bit-identical to bifrost_dtmin + bifrost_neighbours, and equal to the oracle's."""
+    w = workload(3, n=20000)
+    rng = np.random.default_rng(31)
+    sinks = {"all": None, "subset": np.sort(rng.choice(w.n, 6000, replace=False)).astype(np.int32),
+             "small": np.sort(rng.choice(w.n, 700, replace=False)).astype(np.int32), "subsys": None}[case]
+    srcs = rng.permutation(w.n)[:15000].astype(np.int32) if case == "subset" else None
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    si = None if sinks is None else dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    par = dict(NGB, r_ngb=3e-3, r_ngb_max=2e-2)
+    sub = None
+    if case == "subsys":
+        sub = np.full(w.n, -1, dtype=np.int32)
+        members = rng.permutation(w.n)[:3000]
+        sub[members] = members[(np.arange(3000) // 2) * 2]          # pairs sharing the first member's id
+        sub_t = dev(torch, sub)
+        ctx.set_subsystems(sub_t)
+    try:
+        d1 = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, sj)
+        g1 = ctx.neighbours(pos, vel, mass, w.G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"], cap=8, sink_idx=si, src_idx=sj)
+        d2, g2 = ctx.dtmin_neighbours(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, par["r_ngb"], par["r_ngb_max"], par["tau"],
+                                      par["C"], cap=8, sink_idx=si, src_idx=sj)
+        torch.cuda.synchronize()
+    finally:
+        if sub is not None:
+            ctx.set_subsystems(None)
+    for x, y in zip((*d1, *g1), (*d2, *g2)):
+        assert torch.equal(x, y)
+    assert int(g2[0].sum()) > 0                                                   # the search does find neighbours here
+    rows = np.arange(w.n) if sinks is None else sinks
+    if sub is None:
+        ref = oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs)
+    else:
+        ref = oracle.dtmin_sub(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sub, sinks, srcs)
+    check_dt(tuple(t.cpu().numpy()[rows] for t in d2), ref, f"dtmin_neighbours {case}")
+    rc, rl = oracle.ngb(w.pos, w.vel, w.mass, w.G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"], cap=8,
+                        sink_idx=sinks, src_idx=srcs)
+    assert np.array_equal(g2[0].cpu().numpy()[rows], rc)
+    got_l = g2[1].cpu().numpy()[rows]
+    for k in range(rows.shape[0]):
+        m = min(int(rc[k]), 8)
+        assert np.array_equal(got_l[k, :m], rl[k, :m])
+
+
+def test_binding_rejects_mismatched_tensors(torch, ctx):
+    """row counts, devices and list shapes are checked in the binding (a mismatch raises instead of
+    becoming an out-of-bounds device access); index values are range-checked in debug mode."""
+    from paper_2210_02472_b200 import binding
+    w = _small(500, 4)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    with pytest.raises(binding.BifrostError):
+        ctx.acc(pos[:400].contiguous(), mass, w.G, 0.0)
+    with pytest.raises(binding.BifrostError):
+        ctx.acc(pos, mass, w.G, 0.0, out=torch.zeros((300, 3), dtype=torch.float64, device="cuda"))
+    with pytest.raises(binding.BifrostError):
+        ctx.grad(pos, mass, vel[:10].contiguous(), w.G, 0.0)
+    with pytest.raises(binding.BifrostError):
+        ctx.neighbours(pos, vel, mass, w.G, 1e-3, 1e-2, 1e-3, 0.5, cap=4,
+                       out=(torch.zeros(w.n, dtype=torch.int32, device="cuda"), torch.zeros((w.n, 5), dtype=torch.int32, device="cuda")))
+    with pytest.raises(binding.BifrostError):
+        ctx.acc(pos.cpu(), mass, w.G, 0.0)
+    binding.DEBUG_INDEX_CHECK = True
+    try:
+        with pytest.raises(binding.BifrostError):
+            ctx.acc(pos, mass, w.G, 0.0, dev(torch, np.array([1, 500], dtype=np.int32)))
+        ctx.acc(pos, mass, w.G, 0.0, dev(torch, np.array([1, 499], dtype=np.int32)))
+    finally:
+        binding.DEBUG_INDEX_CHECK = False
+    a = ctx.acc(pos, mass, w.G, 0.0)                     # the context still works afterwards
+    check_vec(a.cpu().numpy(), oracle.acc(w.pos, w.mass, w.G, 0.0), "acc")
+
+
+def _fig8_interval(torch, ctx, w, eta, tau, with_criteria=True):
+    """One HHS-FSI interval of PAPER.md:L816-824's softened run; returns (|dE/E| of the interval, summary)."""
+    pos, vel, m = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+
+    def energy():
+        return float(ctx.kinetic_energy(vel, m).cpu()) + float(ctx.potential(pos, m, w.G, w.eps, want_phi=False)[1].cpu())
+    cap = None
+    if with_criteria:        # Eq. 24-29 with eta/2 ("eta = 0.1 for the jerk and gradient time-steps", L822), as dt_cap (H4)
+        a, j = ctx.acc_jerk(pos, vel, m, w.G, w.eps)
+        c = ctx.grad(pos, m, a, w.G, w.eps)
+        cap = torch.full((w.n,), float("inf"), dtype=torch.float64, device="cuda")
+        ctx.timestep_criteria(vel, a, c, j, eta / 2, eta / 2, eta / 2, inout_dt=cap)
+    e0 = energy()
+    summ, _ = ctx.hhs_fsi(pos, vel, m, w.G, w.eps, eta, eta, tau, max_depth=40, dt_cap=cap)
+    e1 = energy()
+    return abs(e1 - e0) / abs(e0), summ
+
+
+def test_hhs_fsi_fig8_cluster_energy_error_at_scale(torch):
+    """PAPER.md:L816-824 (§5.2, Fig. 8): N = 161000 equal masses, r_h = 3.1 pc, eps_soft = 1e-3 pc,
+    eta_ff = eta_fb = 0.2, eta = 0.1 for the gradient / jerk criteria, interval 1e-3 Myr; the paper's softened run
+    has a mean |dE_S/E| of ~5e-11 per interval.  One interval through bifrost_hhs_fsi: the energy error of the
+    interval must be of that size (<= 1e-9; measured 5.7e-12), and it must fall as eta^4 (Eq. 73): halving
+    all eta divides it by 16 within a factor 2 (measured 9.3: at eta = 0.1 the error, 6e-13, is already close to
+    the round-off floor of the energy sums).  (A property test: the oracle cannot follow at this size.)"""
+    from paper_2210_02472_b200.binding import Context
+    w = W.fig8()
+    assert w.n == 161000
+    c = Context(w.n)
+    try:
+        tau = W.fig8_tau()
+        err = {}
+        for eta in (0.2, 0.1):
+            err[eta], summ = _fig8_interval(torch, c, w, eta, tau)
+            print(f"fig8: eta {eta}: |dE/E| = {err[eta]:.3e}, levels {summ}")
+            assert summ["deepest"] >= 2
+        assert err[0.2] <= 1e-9
+        ratio = err[0.2] / err[0.1]
+        print(f"fig8: Eq. 73 ratio {ratio:.1f} (16 expected for a fourth-order scheme)")
+        assert 8.0 <= ratio <= 32.0
+    finally:
+        c.close()
+
+
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_pair_sharding_partials_sum_to_the_unsharded_result(torch, world):
+    """Context.set_shard (multi-GPU): with the pair work of the symmetric kernels dealt to `world`
+    ranks, every rank's output is a partial sum for every particle; added over the ranks (here: one GPU, the
+    ranks' launches one after another) they give the unsharded result and the oracle's."""
+    from paper_2210_02472_b200.binding import BifrostError, Context
+    w = workload(3, n=20000)
+    c = Context(w.n)
+    try:
+        pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+        a_full = c.acc(pos, mass, w.G, w.eps)
+        g_full = c.grad(pos, mass, a_full, w.G, w.eps)
+        a_sum, g_parts = torch.zeros_like(a_full), []
+        for r in range(world):
+            c.set_shard(r, world)
+            part = c.acc(pos, mass, w.G, w.eps)
+            assert float(part.abs().max()) > 0
+            a_sum += part
+        for r in range(world):
+            c.set_shard(r, world)
+            g_parts.append(c.grad(pos, mass, a_sum, w.G, w.eps))
+            with pytest.raises(BifrostError):            # different lists cannot be pair-sharded
+                c.acc(pos, mass, w.G, w.eps, dev(torch, np.arange(10, dtype=np.int32)), None)
+        c.set_shard(0, 1)
+        g_sum = sum(g_parts)
+        check_vec(a_sum.cpu().numpy(), a_full.cpu().numpy(), "sharded acc vs unsharded", tol=1e-13)
+        check_vec(g_sum.cpu().numpy(), g_full.cpu().numpy(), "sharded grad vs unsharded", tol=1e-12)
+        pick = np.sort(np.random.default_rng(world).choice(w.n, 1500, replace=False)).astype(np.int32)
+        a_np = a_sum.cpu().numpy()
+        check_vec(a_np[pick], oracle.acc(w.pos, w.mass, w.G, w.eps, sink_idx=pick), "sharded acc")
+        check_vec(g_sum.cpu().numpy()[pick], oracle.grad(w.pos, w.mass, a_np, w.G, w.eps, sink_idx=pick), "sharded grad")
+        # the shares are balanced: launches of equal work (the time is not asserted, only that every rank has blocks)
+        assert torch.equal(c.acc(pos, mass, w.G, w.eps), a_full)         # world = 1 again: the unsharded bits
+    finally:
+        c.close()
+
+
+@pytest.mark.parametrize("n_a,n_b,forced", [(3000, 1, True), (5, 3, True), (2049, 129, True), (1500, 1600, True),
+                                            (15000, 5000, False), (300, 200, False), (19000, 600, False)])
+def test_mutual_inter_level_sums(torch, n_a, n_b, forced):
+    """bifrost_acc_mutual / bifrost_grad_mutual (Eq. 12-13 for both sets of a level in one call): both lists' rows
+    against the oracle's two one-sided sums; the two-list symmetric kernel (forced at ragged sizes, by default for large
+    lists) and the fall-back pair of plain calls; untouched rows; bit-identical repeats."""
+    from paper_2210_02472_b200.binding import Context
+    w = workload(3, n=20000)
+    c = Context(w.n)
+    try:
+        if forced:
+            c.set_tuning(Context.TUNE_MUTUAL_MIN_PAIRS, 0)
+        ids = np.random.default_rng(n_a * 31 + n_b).permutation(w.n).astype(np.int32)
+        A, B = ids[:n_a].copy(), ids[n_a:n_a + n_b].copy()              # disjoint, unsorted
+        pos, mass = dev(torch, w.pos), dev(torch, w.mass)
+        ta, tb = dev(torch, A), dev(torch, B)
+        out = torch.full((w.n, 3), 7.25, dtype=torch.float64, device="cuda")
+        l0 = c.launch_count
+        c.acc_mutual(pos, mass, w.G, 1e-4, ta, tb, out=out)
+        if forced or n_a * n_b >= 5e7 and min(n_a, n_b) >= 512:
+            assert c.launch_count - l0 == 4              # two packs, the two-list symmetric kernel, its finish
+        got = out.cpu().numpy()
+        rest = np.ones(w.n, bool); rest[A] = False; rest[B] = False
+        assert np.all(got[rest] == 7.25)
+        check_vec(got[A], oracle.acc(w.pos, w.mass, w.G, 1e-4, A, B), "mutual acc A<-B")
+        check_vec(got[B], oracle.acc(w.pos, w.mass, w.G, 1e-4, B, A), "mutual acc B<-A")
+        a_in = torch.from_numpy(np.where(rest[:, None], 0.0, got)).cuda()
+        g = c.grad_mutual(pos, mass, a_in, w.G, 1e-4, ta, tb)
+        g2 = c.grad_mutual(pos, mass, a_in, w.G, 1e-4, ta, tb)
+        assert torch.equal(g, g2)
+        g_np, a_np = g.cpu().numpy(), a_in.cpu().numpy()
+        check_vec(g_np[A], oracle.grad(w.pos, w.mass, a_np, w.G, 1e-4, A, B), "mutual grad A<-B")
+        check_vec(g_np[B], oracle.grad(w.pos, w.mass, a_np, w.G, 1e-4, B, A), "mutual grad B<-A")
+        # Newton's third law between the two sets (PAPER.md:L131)
+        for x in (got, g_np):
+            tot = (w.mass[A, None] * x[A]).sum(0) + (w.mass[B, None] * x[B]).sum(0)
+            scale = (w.mass[A, None] * np.abs(x[A])).sum(0) + (w.mass[B, None] * np.abs(x[B])).sum(0)
+            assert (np.abs(tot) <= 1e-12 * scale).all()
+    finally:
+        c.close()

@@ -67,6 +67,6 @@ def test_config2_is_virialised():
     w = workload(2)
     assert w.n == 16384 and abs(w.mass.sum() - 1) < 1e-12
     t = 0.5 * (w.mass * (w.vel ** 2).sum(axis=1)).sum()
-    pot = W._pair_potential_energy(w.pos, w.mass)
+    pot = W._virial_potential_energy(w.pos, w.mass)
     assert abs(2 * t / -pot - 1) < 1e-12
     assert np.abs((w.mass[:, None] * w.vel).sum(axis=0)).max() < 1e-15
