@@ -48,8 +48,10 @@ UNIT = "interactions/s"
 #   symmetric kernels (one list on both sides, all-active): every UNORDERED pair is evaluated once - acc 20 + 4.5/8
 #   (source-side warp reduction, 8 sinks per thread) = 20.56 instructions / 32.6 flops per unordered pair,
 #   grad 33 + 4.5/6 = 33.75 / 52.75 - i.e. half of that per interaction.
-FP64_INSTR = {"plain": {"acc": 15, "grad": 28, "dtmin": 23}, "sym": {"acc": 20.5625 / 2, "grad": 33.75 / 2, "dtmin": 23}}
-FP64_FLOPS = {"plain": {"acc": 24, "grad": 44, "dtmin": 33}, "sym": {"acc": 32.5625 / 2, "grad": 52.75 / 2, "dtmin": 33}}
+#   dtmin: 17 instructions in the hot path (7 DADD + 6 DFMA + 4 DMUL = 23 flops: keys from the unrefined rsqrt seed; the
+#   refinement and the exact time-steps run in the rarely taken branch only).
+FP64_INSTR = {"plain": {"acc": 15, "grad": 28, "dtmin": 17}, "sym": {"acc": 20.5625 / 2, "grad": 33.75 / 2, "dtmin": 17}}
+FP64_FLOPS = {"plain": {"acc": 24, "grad": 44, "dtmin": 23}, "sym": {"acc": 32.5625 / 2, "grad": 52.75 / 2, "dtmin": 23}}
 # SURVEY.md 8(d)'s budget for the minimal ONE-SIDED sequence: flops per ordered pair.  Against it the symmetric
 # kernels deliver more interactions than the executed flops alone would ("work-equivalent" fraction, may exceed 1).
 SURVEY_8D_FLOPS = {"acc": 26, "grad": 42}
@@ -374,7 +376,7 @@ def run_cuda(args):
         path = "sym" if world > 1 or n >= 16384 else "plain"            # which acc / grad kernels these sizes select
         kernel_name = {"acc": {"sym": "sym_pair_kernel<SymAcc, 8, 256, 1>", "plain": "pair_kernel<AccPass, 8, 256, 1, 1>"},
                        "grad": {"sym": "sym_pair_kernel<SymGrad, 6, 256, 1>", "plain": "pair_kernel<GradPass, 5, 128, 2, 2>"},
-                       "dtmin": {"sym": "pair_kernel<DtPass, 6, 128, 2, 1>", "plain": "pair_kernel<DtPass, 6, 128, 2, 1>"}}
+                       "dtmin": {"sym": "pair_kernel<DtPass, 4, 128, 3, 2>", "plain": "pair_kernel<DtPass, 4, 128, 3, 2>"}}
 
         def kern(name):
             ms = mean_ms[name]
@@ -400,6 +402,7 @@ def run_cuda(args):
             roofline["measured_fp64_pipe"] = probe
             roofline["pipe_util_vs_measured_dfma"] = (
                 dom["fp64_pipe_issue_util"] / probe["dfma"]["frac_of_derived_pipe_peak"])
+        extras = run_extras(torch, ctx, w, pos, vel, mass, acc) if world == 1 and args.extras else None
         config5 = None
         if world == 1 and args.config == 4 and not args.no_config5 and not args.n:
             ctx.close()
@@ -419,8 +422,8 @@ def run_cuda(args):
                 "passes": passes, "roofline": roofline}
         if config5 is not None:
             line["config5"] = config5
-        if world == 1 and args.extras:
-            line["extras"] = run_extras(torch, ctx, w, pos, vel, mass, acc)
+        if extras is not None:
+            line["extras"] = extras
         if world == 1 and not args.no_cpu_baseline:
             import oracle
             oracle.build()
@@ -512,6 +515,7 @@ def run_config5(torch, dev, peak, num_sms):
 
 
 def run_extras(torch, ctx, w, pos, vel, mass, acc):
+    from paper_2210_02472_b200.binding import Context
     """Device times of the NEXT rows (SURVEY.md §8f) on the same workload, outside the timed step:
     jerk, potential, neighbour search + components, one FSI cycle.  ms per call, 2 calls each after
     one warm-up, CUDA events on the launching stream."""
@@ -531,6 +535,9 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
         "potential": lambda: ctx.potential(pos, mass, w.G, w.eps, want_phi=False),
         "neighbours": lambda: ctx.neighbours(pos, vel, mass, w.G, par["r_ngb"], par["r_ngb_max"], par["tau"], par["C"],
                                              cap=16, out=(cnt, lst)),
+        "dtmin": lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb),
+        "dtmin_neighbours": lambda: ctx.dtmin_neighbours(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, par["r_ngb"], par["r_ngb_max"],
+                                                         par["tau"], par["C"], cap=16),
         "components": lambda: ctx.components(cnt, lst),
         "fsi_step": lambda: ctx.fsi_step(p2, v2, mass, w.G, max(w.eps, 1e-4), 2.0 ** -12),
     }
@@ -544,7 +551,7 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / 2
         out[name] = {"ms": ms}
-        if name in ("jerk", "acc_jerk", "potential", "neighbours"):
+        if name in ("jerk", "acc_jerk", "potential", "neighbours", "dtmin", "dtmin_neighbours"):
             out[name]["interactions_per_s"] = float(n) * n / (ms * 1e-3)
         if name == "fsi_step":
             out[name]["interactions_per_s"] = 4.0 * n * n / (ms * 1e-3)     # four O(N^2) sums
@@ -562,6 +569,49 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
     torch.cuda.synchronize()
     out["hhs_fsi_config2"] = {"ms": 1e3 * (time.perf_counter() - t0), "tau": 2.0 ** -9, "eta": 0.1, "max_depth": 12,
                               "launches": ctx.launch_count - l0, **summ}
+    # the inter-level sums of Eq. 12-13 between a slow and a fast set (S = 7/8 of the particles, F = 1/8): one mutual call
+    # against the pair of one-sided calls
+    ids = torch.randperm(n, device=pos.device, generator=torch.Generator(device=pos.device).manual_seed(5)).to(torch.int32)
+    S_, F_ = ids[: n - n // 8].contiguous(), ids[n - n // 8:].contiguous()
+    a_m = torch.zeros_like(acc)
+    for name, fn in (("acc_mutual", lambda: ctx.acc_mutual(pos, mass, w.G, w.eps, S_, F_, out=a_m)),
+                     ("acc_two_calls", lambda: (ctx.acc(pos, mass, w.G, w.eps, S_, F_, out=a_m),
+                                                ctx.acc(pos, mass, w.G, w.eps, F_, S_, out=a_m))),
+                     ("grad_mutual", lambda: ctx.grad_mutual(pos, mass, acc, w.G, w.eps, S_, F_, out=a_m)),
+                     ("grad_two_calls", lambda: (ctx.grad(pos, mass, acc, w.G, w.eps, S_, F_, out=a_m),
+                                                 ctx.grad(pos, mass, acc, w.G, w.eps, F_, S_, out=a_m)))):
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(); fn(); fn(); e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 2
+        out[name] = {"ms": ms, "n_slow": int(S_.numel()), "n_fast": int(F_.numel()),
+                     "interactions_per_s": 2.0 * S_.numel() * F_.numel() / (ms * 1e-3)}
+    # one HHS-FSI interval of the paper's softened equal-mass cluster (Fig. 8): N = 161000,
+    # eta_ff = eta_fb = 0.2, Eq. 24-29 with eta = 0.1 as dt_cap, tau = 1e-3 Myr; energy error of the interval
+    w8 = W.fig8()
+    ctx8 = Context(w8.n)
+    p, v, m = (torch.from_numpy(x).to(pos.device) for x in (w8.pos, w8.vel, w8.mass))
+
+    def energy():
+        return float(ctx8.kinetic_energy(v, m).cpu()) + float(ctx8.potential(p, m, w8.G, w8.eps, want_phi=False)[1].cpu())
+    rec8 = {"n": w8.n, "tau": W.fig8_tau(), "eta": 0.2, "eta_criteria": 0.1}
+    for it in range(2):                                   # first interval = warm-up (allocates the integrator scratch)
+        a8, j8 = ctx8.acc_jerk(p, v, m, w8.G, w8.eps)
+        c8 = ctx8.grad(p, m, a8, w8.G, w8.eps)
+        cap = torch.full((w8.n,), float("inf"), dtype=torch.float64, device=pos.device)
+        ctx8.timestep_criteria(v, a8, c8, j8, 0.1, 0.1, 0.1, inout_dt=cap)
+        e_before = energy()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        l0 = ctx8.launch_count
+        summ, _ = ctx8.hhs_fsi(p, v, m, w8.G, w8.eps, 0.2, 0.2, W.fig8_tau(), max_depth=40, dt_cap=cap)
+        torch.cuda.synchronize()
+        rec8.update({"ms": 1e3 * (time.perf_counter() - t0), "launches": ctx8.launch_count - l0, **summ,
+                     "rel_energy_error_of_the_interval": abs(energy() - e_before) / abs(e_before)})
+    out["hhs_fsi_fig8"] = rec8
+    ctx8.close()
     return out
 
 
@@ -627,6 +677,31 @@ def run_sweep(args):
             rec["acc_source_bytes"] = 80 * w.n
             out["cases"].append(rec)
         ctx.close()
+    # same-list (all-active) acc / grad over the list length m: the symmetric kernels (every unordered pair once)
+    # against the plain ones, switched with bifrost_set_tuning; config 4's recipe at reduced N
+    out["same_list"] = []
+    ctx = Context(1 << 18)
+    for m in (4096, 8192, 12288, 16384, 24576, 32768, 65536, 131072, 262144):
+        w = W.config4(n=m, n_sbh=10)
+        pos, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.mass))
+        rec = {"m": m}
+        for mode, thr in (("sym", 0), ("plain", 1 << 40)):
+            ctx.set_tuning(Context.TUNE_SYM_MIN_N, thr)
+            a = ctx.acc(pos, mass, w.G, w.eps)
+            for name, fn in (("acc", lambda: ctx.acc(pos, mass, w.G, w.eps)), ("grad", lambda: ctx.grad(pos, mass, a, w.G, w.eps))):
+                reps = 20 if m <= 65536 else 4
+                for _ in range(reps):
+                    fn()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                for _ in range(reps):
+                    fn()
+                e1.record()
+                torch.cuda.synchronize()
+                rec[f"{name}_{mode}_us"] = round(1e3 * e0.elapsed_time(e1) / reps, 1)
+        out["same_list"].append(rec)
+    ctx.close()
     print(json.dumps(out), flush=True)
     return 0
 

@@ -443,7 +443,9 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     int32_t* pid = (int32_t*)(base + unit * 16);
     const SrcArrays src{pos, vel, mass, sub, src_idx};
     DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
-    using Huge = Shape<6, 128, 2, 1>;     // 0.7 % faster per pair than Big (after the rarely-taken update branch)
+    // 17 FP64 instructions per pair in the hot path: 4 sinks x 128 threads x 3 CTAs/SM, unroll 2 measured best at every size
+    // (N = 2^20: 1193 ms; 6 x 128 x 2 CTAs unroll 2: 1196; unroll 1: 1234 / 1283; 8 x 128 x 2: 1346; profiles/r2_dtmin.md)
+    using Huge = Shape<4, 128, 3, 2>;
     using Big = Shape<4, 128, 3, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
@@ -454,7 +456,7 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
         a.ng.pcount = (int32_t*)(base + unit * 24);
         a.ng.plist = (int32_t*)(base + unit * 28);
         // the neighbour test keeps r^2 and a count per sink alive: one sink fewer per thread fits the register file
-        using HugeN = Shape<5, 128, 2, 1>;
+        using HugeN = Shape<4, 128, 2, 2>;
         using BigN = Shape<4, 128, 2, 2>;
         using F4N = Shape<4, 128, 2, 2>;
         using F2N = Shape<2, 128, 3, 2>;

@@ -118,7 +118,7 @@ struct AccPassT {
             w[s] = (y0 * t) * pm;
             any |= jcode == sk[s].sub;
         }
-        if (any) {
+        if (__builtin_expect(any, 0)) {
 #pragma unroll
             for (int s = 0; s < S; ++s)
                 if (jcode == sk[s].sub) w[s] = 0.0;
@@ -355,13 +355,20 @@ __device__ __noinline__ bool dt_contender_wins(const DtArgs& a, int w, int i, in
 }
 
 // The fast path MAXIMISES the monotone keys kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)) and kfb = v^2/r^2
-// (= eta^2/dt_fb^2): no sqrt or division per pair.  The keys carry a few ulp of rounding error (<~ 1e-15
-// relative), so a key decides only when it is clear of the running maximum by KEY_SLACK = 1e-12 relative; inside
-// that band (a near-tie) the contender and the running best are both evaluated with dt_*_exact and the
-// oracle's rule decides.  The running best is thus always the exact (time-step, id) minimum of the sources seen,
+// (= eta^2/dt_fb^2): no sqrt or division per pair.  Three tiers:
+//  (1) every pair: the keys from the UNREFINED reciprocal-square-root seed (relative error <= 3 x 2^-20 in y0^3; 17
+//      FP64 instructions) against a threshold kept KEY_PRE = 1 - 1e-5 below the key of the running best - one integer
+//      compare of the high words per key; this only SELECTS, so the seed's accuracy is enough;
+//  (2) a selected pair (rare): the keys again with the polynomial refinement (a few ulp); a refined key decides only
+//      when it is clear of the running best's by KEY_SLACK = 1e-12 relative;
+//  (3) inside that band (a near-tie): the contender and the running best are both evaluated with dt_*_exact and the
+//      oracle's rule decides.
+// Every pair that could win passes (1) and (2): a winner's exact time-step is <= the best's, so its true key is >= the
+// best's up to a few ulp.  The running best is thus always the exact (time-step, id) minimum of the sources seen,
 // whatever the order of the source list, and the argmin is the oracle's bit for bit.
 constexpr double KEY_SLACK = 1.0 - 1e-12;
-constexpr double KEY_SLACK2 = KEY_SLACK * KEY_SLACK;
+constexpr double KEY_PRE = 1.0 - 1e-5;
+constexpr double KEY_PRE_INV = 1.0 / KEY_PRE;
 
 // NGB = true (bifrost_dtmin_neighbours, "along with the time-step assignment"): the pass also runs the
 // neighbour search of Eq. 18-19 on the r^2 it already holds - one more integer pre-test per pair (r^2 below the
@@ -372,7 +379,7 @@ struct DtPassT {
     static constexpr int PHASED_MIN_S = 1;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
-    // thr = (key of the running best) * KEY_SLACK; j = its source id (-1: none yet); nc = neighbours found (NGB)
+    // thr = (refined key of the running best) * KEY_PRE; j = its source id (-1: none yet); nc = neighbours found (NGB)
     struct Acc { double thr_ff, thr_fb; int jff, jfb, nc; };
     struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
     __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
@@ -397,29 +404,37 @@ struct DtPassT {
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
     __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; c.nc = 0; }
-    // one key of one sink against the running best (rare path)
+    // one refined key of one sink against the running best (rare path, tiers 2 and 3)
     __device__ __forceinline__ static void contend(const Args& a, int w, int i, double key, int jid, double& thr, int& jbest) {
-        if (!(key >= thr)) return;
-        const double ks = key * KEY_SLACK;
-        if (key * KEY_SLACK2 > thr || dt_contender_wins(a, w, i, jbest, jid)) { thr = ks; jbest = jid; }
+        const double K = thr * KEY_PRE_INV;               // the running best's key (to ~2 ulp)
+        if (!(key >= K * KEY_SLACK)) return;
+        if (key * KEY_SLACK > K || dt_contender_wins(a, w, i, jbest, jid)) { thr = key * KEY_PRE; jbest = jid; }
     }
-    // FP64-pipe instructions of the keys: 7 DADD, 6 DFMA (r2, v2), DMUL t, DFMA e, 2 DFMA p3, 2 DMUL y3, 2 DFMA y2,
-    // 2 DMUL keys = 23.
-    __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb, double& r2) {
+    // tier 1: 7 DADD, 6 DFMA (r2, v2), DMUL y0^2, DMUL y0^3, 2 DMUL keys = 17 FP64-pipe instructions
+    __device__ __forceinline__ static void keys_fast(const Sink& s, const double* __restrict__ r, double& kff, double& kfb, double& r2) {
         const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
         const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
         r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
         const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
         const double y0 = rsqrt_seed(r2);
         const double t = y0 * y0;
+        kff = (s.m + r[3]) * (y0 * t);
+        kfb = v2 * t;
+    }
+    // tier 2: the same keys with the seed refined (e = 1 - r2 y0^2; y0^3 (1 + 3/2 e + 15/8 e^2), y0^2 (1 + e + e^2))
+    __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        const double ux = r[4] - s.vx, uy = r[5] - s.vy, uz = r[6] - s.vz;
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
+        const double v2 = fma(ux, ux, fma(uy, uy, uz * uz));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
         const double e = fma(-r2, t, 1.0);
         const double p3 = fma(fma(e, 1.875, 1.5), e, 1.0);
-        const double y3 = (y0 * t) * p3;
-        const double y2 = fma(t, fma(e, e, e), t);
-        kff = (s.m + r[3]) * y3;
-        kfb = v2 * y2;
+        kff = (s.m + r[3]) * ((y0 * t) * p3);
+        kfb = v2 * fma(t, fma(e, e, e), t);
     }
-    // The keys of the S sinks of a thread and ONE branch per source that is almost never taken (after the first
+    // The tier-1 keys of the S sinks of a thread and ONE branch per source that is almost never taken (after the first
     // sources a key comes near the running maximum ~1/j of the time for the j-th source).  The pre-test is a
     // necessary condition on the integer pipe: keys and thresholds are >= 0, so key >= thr implies
     // hi(key) >= hi(thr).  (The self pair and same-subsystem pairs are filtered in the rare path only.)
@@ -430,20 +445,25 @@ struct DtPassT {
         const int guard_hi = NGB ? __double2hiint(a.ng.r2_guard) : 0;
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            keys(sk[s], r, kff[s], kfb[s], r2[s]);
+            keys_fast(sk[s], r, kff[s], kfb[s], r2[s]);
             any |= (__double2hiint(kff[s]) >= __double2hiint(c[s].thr_ff)) | (__double2hiint(kfb[s]) >= __double2hiint(c[s].thr_fb));
             // r^2 >= 0 and the guard >= 0, so r^2 < guard implies hi(r^2) <= hi(guard)
             if (NGB) any |= __double2hiint(r2[s]) <= guard_hi;
         }
-        if (any) {
+        if (__builtin_expect(any, 0)) {
             const int jid = __double2loint(r[7]);
 #pragma unroll
             for (int s = 0; s < S; ++s) {
                 if (jid == sk[s].id) continue;
                 if (NGB && r2[s] < a.ng.r2_guard) neighbour(a, sk[s], c[s], sink_row<S>(s), r, jid);     // ignores subsystems, as bifrost_neighbours
                 if (EXCL && __double2hiint(r[7]) == sk[s].sub) continue;
-                contend(a, 0, sk[s].id, kff[s], jid, c[s].thr_ff, c[s].jff);
-                if (kfb[s] > 0.0) contend(a, 1, sk[s].id, kfb[s], jid, c[s].thr_fb, c[s].jfb);   // v_ij = 0: dt_fb = +inf, never a minimum (T3)
+                if (!((kff[s] >= c[s].thr_ff) | (kfb[s] >= c[s].thr_fb))) continue;
+                double rff, rfb;
+                Sink t = sk[s];         // opaque copy: keeps the compiler from holding tier 1's intermediates alive for tier 2
+                asm volatile("" : "+d"(t.x), "+d"(t.y), "+d"(t.z), "+d"(t.vx), "+d"(t.vy), "+d"(t.vz));
+                keys(t, r, rff, rfb);
+                contend(a, 0, sk[s].id, rff, jid, c[s].thr_ff, c[s].jff);
+                if (rfb > 0.0) contend(a, 1, sk[s].id, rfb, jid, c[s].thr_fb, c[s].jfb);   // v_ij = 0: dt_fb = +inf, never a minimum (T3)
             }
         }
     }
@@ -583,7 +603,7 @@ struct PotPassT {
             w[s] = y0 * pm;
             any |= (jid == sk[s].id) | (EXCL && jcode == sk[s].sub);
         }
-        if (any) {
+        if (__builtin_expect(any, 0)) {
 #pragma unroll
             for (int s = 0; s < S; ++s)
                 if ((jid == sk[s].id) | (EXCL && jcode == sk[s].sub)) w[s] = 0.0;
