@@ -706,6 +706,28 @@ def run_sweep(args):
     return 0
 
 
+def run_small(args):
+    """Profiling aid: config 2 (N = 16384 sources), 2^k seeded sinks, acc / grad / dtmin three times each (one fused
+    launch per call) - the command the ncu captures of pair_fused_kernel in profiles/ were taken with."""
+    import torch
+    from paper_2210_02472_b200 import workloads as W
+    from paper_2210_02472_b200.binding import Context
+    torch.cuda.set_device(0)
+    w = W.config2()
+    ctx = Context(w.n)
+    pos, vel, mass = (torch.from_numpy(x).cuda() for x in (w.pos, w.vel, w.mass))
+    acc = ctx.acc(pos, mass, w.G, w.eps)
+    si = torch.from_numpy(W.config2_sink_list(args.small)).cuda()
+    for _ in range(3):
+        ctx.acc(pos, mass, w.G, w.eps, si, None)
+        ctx.grad(pos, mass, acc, w.G, w.eps, si, None)
+        ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb, si, None)
+    torch.cuda.synchronize()
+    print(json.dumps({"small": args.small, "n_sink": int(si.numel()), "launches": ctx.launch_count}))
+    ctx.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -722,7 +744,10 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="small-active-set sweep of configs 2 and 3 (us per call); prints one JSON line")
     ap.add_argument("--no-fp64-probe", action="store_true", help="skip the register-only FP64-pipe peak probe")
     ap.add_argument("--no-config5", action="store_true", help="skip the N = 2^21 acc + grad block of the default line")
+    ap.add_argument("--small", type=int, default=-1, help="profiling aid: config 2 with 2^k sinks, acc / grad / dtmin three times each")
     args = ap.parse_args()
+    if args.small >= 0:
+        return run_small(args)
     if args.impl == "reference":
         return run_reference(args)
     if args.sweep:

@@ -68,8 +68,8 @@ struct bifrost_ctx {
     int small_m = 128;               // FSI cycles / level splits of at most this many particles run as ONE single-CTA launch
                                      // (bifrost_set_tuning BIFROST_TUNE_SMALL_M: 0..256; 0 disables)
     int64_t fused_max_sinks = 4096;  // below: one fused launch per call (BIFROST_TUNE_FUSED_MAX_SINKS)
-    unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel, tagged with the launch epoch
-    unsigned epoch = 0;              // one per fused launch (22 bits): a stale count of an aborted launch never matches
+    unsigned* tickets = nullptr;     // [TICKETS] arrival counters of pair_fused_kernel (zeroed again by the last CTA of a launch)
+    bool tickets_dirty = false;      // a launch failed: counts may be left behind - zero them before the next fused launch
     int shard_rank = 0, shard_world = 1;   // bifrost_set_shard: which blocks of the symmetric kernels this context evaluates
     double* sym_ws = nullptr;        // source-side rows of the symmetric (every pair once) kernels, [block][source][3]
     size_t sym_ws_bytes = 0;
@@ -104,6 +104,7 @@ namespace {
         cudaError_t e_ = (expr);                                                  \
         if (e_ != cudaSuccess) {                                                  \
             snprintf((ctx)->err, sizeof((ctx)->err), "%s: %s", #expr, cudaGetErrorString(e_)); \
+            (ctx)->tickets_dirty = true;                                          \
             return BIFROST_ECUDA;                                                 \
         }                                                                         \
     } while (0)
@@ -189,8 +190,14 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
         snprintf(ctx->err, sizeof(ctx->err), "fused launch: %u sink blocks exceed the %d tickets", grid.x, TICKETS);
         return BIFROST_EINVAL;
     }
-    ctx->epoch = ctx->epoch % 0x3ffffeu + 1u;      // 1 .. 2^22 - 2, never 0
-    pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets, ctx->epoch);
+    if (ctx->tickets_dirty) {
+        CU_TRY(ctx, cudaMemsetAsync(ctx->tickets, 0, TICKETS * sizeof(unsigned), st));
+        ctx->tickets_dirty = false;
+    }
+    if (g.tiles_per_split < DT_SHORT_TILES)      // short source range per CTA: the policy's variant for it (dtmin)
+        pair_fused_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+    else
+        pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -204,7 +211,10 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
 template <class P, class Sh>
 int launch_big(bifrost_ctx* ctx, const typename P::Args& a, const Geom& g, cudaStream_t st) {
     dim3 grid(ceil_div(g.n_sink, Sh::T * Sh::S), g.n_split);
-    pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    if (g.tiles_per_split < DT_SHORT_TILES)
+        pair_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
+    else
+        pair_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, ctx->src_rec);
     ctx->launches++;
     CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
@@ -442,14 +452,14 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     double* pkey = (double*)base;
     int32_t* pid = (int32_t*)(base + unit * 16);
     const SrcArrays src{pos, vel, mass, sub, src_idx};
-    DtArgs a{pos, vel, mass, sub, sink_idx, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
+    DtArgs a{pos, vel, mass, sub, sink_idx, src_idx, (int)n_src, pkey, pid, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
     // 17 FP64 instructions per pair in the hot path: 4 sinks x 128 threads x 3 CTAs/SM, unroll 2 measured best at every size
     // (N = 2^20: 1193 ms; 6 x 128 x 2 CTAs unroll 2: 1196; unroll 1: 1234 / 1283; 8 x 128 x 2: 1346; profiles/r2_dtmin.md)
     using Huge = Shape<4, 128, 3, 2>;
     using Big = Shape<4, 128, 3, 2>;
     using F4 = Shape<4, 128, 3, 2>;
     using F2 = Shape<2, 128, 4, 2>;
-    using F1 = Shape<1, 128, 5, 2>;
+    using F1 = Shape<1, 128, 5, 4>;
     if (ng) {
         a.ng = *ng;
         a.ng.n_rows = (int)n_sink;

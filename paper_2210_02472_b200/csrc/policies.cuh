@@ -63,6 +63,7 @@ struct AccArgs {
 
 template <bool EXCL>
 struct AccPassT {
+    using Short = AccPassT;
     static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
     static constexpr int PHASED_MIN_S = EXCL ? 2 : 0;
     using Args = AccArgs;
@@ -161,6 +162,7 @@ struct GradArgs {
 // Eq. 6's w * r_ji - acceleration and jerk in 31 FP64 instructions instead of 15 + 28.
 template <bool EXCL, bool WITH_ACC = false>
 struct GradPassT {
+    using Short = GradPassT;
     static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
     static constexpr int PHASED_MIN_S = 5;   // measured: phase-major helps at S = 5 (+1.4 %), hurts at S = 4
     using Args = GradArgs;
@@ -318,8 +320,10 @@ struct DtArgs {
     const double* mass;
     const int32_t* subsys;
     const int32_t* sink_idx;
-    double* pkey;      // [split][2][n_sink]  best time-steps (ff, fb) of a split, exact (Eq. 21 / 22 in IEEE operations)
-    int32_t* pid;      // [split][2][n_sink]  their source ids
+    const int32_t* src_idx;   // the source list (NULL: 0..n_src-1), for the exact rescan of an ambiguous sink (SHORT variant)
+    int n_src;
+    double* pkey;      // [split][2][n_sink]  refined key of the best source of a split (ff, fb)
+    int32_t* pid;      // [split][2][n_sink]  its id
     double G, eta_ff, eta_fb;
     double* dt_ff; double* dt_fb; int32_t* j_ff; int32_t* j_fb;   // outputs (any may be NULL)
     NgbArgs ng;        // NGB only (bifrost_dtmin_neighbours): the neighbour search riding on the same pass
@@ -354,6 +358,22 @@ __device__ __noinline__ bool dt_contender_wins(const DtArgs& a, int w, int i, in
     return tc < tb || (tc == tb && jc < jb);
 }
 
+// The exact (time-step, id) minimum of sink i over the sources [l0, l1) of the list, straight from the oracle's
+// definition: used only when a near-tie was seen for this sink in a short source range (DtPassT<.., SHORT>), i.e. for
+// exactly tied inputs such as lattices.  w = 0: Eq. 21, w = 1: Eq. 22.  Returns the id (-1: none).
+__device__ __noinline__ int dt_rescan(const DtArgs& a, int w, int i, int l0, int l1) {
+    double tb = __longlong_as_double(0x7ff0000000000000LL);
+    int jb = -1;
+    const int ci = a.subsys ? a.subsys[i] : -1;
+    for (int l = l0; l < l1; ++l) {
+        const int j = a.src_idx ? a.src_idx[l] : l;
+        if (j == i || (ci >= 0 && a.subsys[j] == ci)) continue;
+        const double t = dt_exact_ids(a, w, i, j);
+        if (t < tb || (t == tb && j < jb)) { tb = t; jb = j; }      // +inf (v_ij = 0) never replaces the initial +inf
+    }
+    return jb;
+}
+
 // The fast path MAXIMISES the monotone keys kff = (m_i+m_j)/r^3 (= eta^2/(G dt_ff^2)) and kfb = v^2/r^2
 // (= eta^2/dt_fb^2): no sqrt or division per pair.  Three tiers:
 //  (1) every pair: the keys from the UNREFINED reciprocal-square-root seed (relative error <= 3 x 2^-20 in y0^3; 17
@@ -373,14 +393,24 @@ constexpr double KEY_PRE_INV = 1.0 / KEY_PRE;
 // NGB = true (bifrost_dtmin_neighbours, "along with the time-step assignment"): the pass also runs the
 // neighbour search of Eq. 18-19 on the r^2 it already holds - one more integer pre-test per pair (r^2 below the
 // guarded r_ngb,max^2), candidates through ngb_exact in the rare path, lists appended in source order.
-template <bool EXCL, bool NGB = false>
+// SHORT = true: the variant for short source ranges per CTA (a few tiles: small sink sets split many ways, the
+// faster levels of the hierarchy).  There the running maxima still change every few sources, so the "rare" branch
+// would be taken at almost every source (measured 3-4x slower than round 1's select variant).  This variant computes
+// the REFINED keys for every pair (23 instructions) and updates the running best with selects when a key is clear of
+// it by the band; only a key INSIDE the band - a near-tie, which is the truly rare event - takes a branch to the
+// exact evaluation.  Same decisions, same results.
+constexpr int DT_SHORT_TILES = 4;      // measured: from ~4 tiles per CTA on the three-tier variant is faster (config 2, 8192 sinks: 347 vs 388 us)
+
+template <bool EXCL, bool NGB = false, bool SHORT = false>
 struct DtPassT {
+    using Short = DtPassT<EXCL, NGB, true>;
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
     static constexpr int PHASED_MIN_S = 1;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
     // thr = (refined key of the running best) * KEY_PRE; j = its source id (-1: none yet); nc = neighbours found (NGB)
-    struct Acc { double thr_ff, thr_fb; int jff, jfb, nc; };
+    // (SHORT: thr = key of the running best * KEY_SLACK; amb = a near-tie was seen: bit 0 ff, bit 1 fb)
+    struct Acc { double thr_ff, thr_fb; int jff, jfb, nc, amb; };
     struct Raw { double x, y, z, m, vx, vy, vz; int j, code; };
     __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) {
         if (j >= 0) {
@@ -403,7 +433,7 @@ struct DtPassT {
         s.m = a.mass[id]; s.id = id;
         s.sub = EXCL ? sink_code(a.subsys, id) : 0;
     }
-    __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; c.nc = 0; }
+    __device__ static void init(Acc& c) { c.thr_ff = 0.0; c.thr_fb = 0.0; c.jff = -1; c.jfb = -1; c.nc = 0; c.amb = 0; }
     // one refined key of one sink against the running best (rare path, tiers 2 and 3)
     __device__ __forceinline__ static void contend(const Args& a, int w, int i, double key, int jid, double& thr, int& jbest) {
         const double K = thr * KEY_PRE_INV;               // the running best's key (to ~2 ulp)
@@ -420,6 +450,10 @@ struct DtPassT {
         const double t = y0 * y0;
         kff = (s.m + r[3]) * (y0 * t);
         kfb = v2 * t;
+    }
+    __device__ __forceinline__ static double dist2(const Sink& s, const double* __restrict__ r) {
+        const double dx = r[0] - s.x, dy = r[1] - s.y, dz = r[2] - s.z;
+        return fma(dx, dx, fma(dy, dy, fma(dz, dz, R2_FLOOR)));
     }
     // tier 2: the same keys with the seed refined (e = 1 - r2 y0^2; y0^3 (1 + 3/2 e + 15/8 e^2), y0^2 (1 + e + e^2))
     __device__ __forceinline__ static void keys(const Sink& s, const double* __restrict__ r, double& kff, double& kfb) {
@@ -440,6 +474,7 @@ struct DtPassT {
     // hi(key) >= hi(thr).  (The self pair and same-subsystem pairs are filtered in the rare path only.)
     template <int S>
     __device__ __forceinline__ static void pairs(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        if (SHORT) { pairs_short<S>(a, sk, c, r); return; }
         double kff[S], kfb[S], r2[S];
         bool any = false;
         const int guard_hi = NGB ? __double2hiint(a.ng.r2_guard) : 0;
@@ -467,6 +502,37 @@ struct DtPassT {
             }
         }
     }
+    // SHORT: refined keys for every pair; a key beyond the band above the running best replaces it by selects; a key
+    // INSIDE the band (a near-tie) only sets a sticky flag - no branch in the loop, so the unrolled sources overlap (a
+    // branch per source, even one never taken, serialised them: 22 us instead of 13 us for one sink) - and store() then
+    // settles that sink by an exact rescan of the CTA's source range.  thr = K * KEY_SLACK, K = the running best's key.
+    template <int S>
+    __device__ __forceinline__ static void pairs_short(const Args& a, const Sink* sk, Acc* c, const double* __restrict__ r) {
+        const int jid = __double2loint(r[7]);
+        const int guard_hi = NGB ? __double2hiint(a.ng.r2_guard) : 0;
+        bool cand = false;
+        double kff[S], kfb[S];
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            keys(sk[s], r, kff[s], kfb[s]);
+            bool other = jid != sk[s].id;
+            if (NGB) cand |= other & (__double2hiint(dist2(sk[s], r)) <= guard_hi);
+            if (EXCL) other &= __double2hiint(r[7]) != sk[s].sub;
+            // ks KEY_SLACK > thr  <=>  key KEY_SLACK > K: beyond the band above the best.  key >= thr: inside or above it.
+            const double ksf = kff[s] * KEY_SLACK, ksb = kfb[s] * KEY_SLACK;
+            const bool wf = other & (ksf * KEY_SLACK > c[s].thr_ff), wb = other & (ksb * KEY_SLACK > c[s].thr_fb);
+            const bool nf = other & !wf & (kff[s] >= c[s].thr_ff) & (jid != c[s].jff);
+            const bool nb = other & !wb & (kfb[s] >= c[s].thr_fb) & (jid != c[s].jfb) & (__double2hiint(kfb[s]) != 0);   // v_ij = 0: never a minimum (T3)
+            c[s].amb |= (nf ? 1 : 0) | (nb ? 2 : 0);
+            c[s].thr_ff = wf ? ksf : c[s].thr_ff; c[s].jff = wf ? jid : c[s].jff;
+            c[s].thr_fb = wb ? ksb : c[s].thr_fb; c[s].jfb = wb ? jid : c[s].jfb;
+        }
+        if (NGB && __builtin_expect(cand, 0)) {
+#pragma unroll
+            for (int s = 0; s < S; ++s)
+                if (jid != sk[s].id && dist2(sk[s], r) < a.ng.r2_guard) neighbour(a, sk[s], c[s], sink_row<S>(s), r, jid);
+        }
+    }
     // row of the thread's s-th sink (the kernels lay sinks out as k = blockIdx.x * T * S + threadIdx.x + s * T)
     template <int S>
     __device__ __forceinline__ static int sink_row(int s) { return blockIdx.x * (blockDim.x * S) + threadIdx.x + s * blockDim.x; }
@@ -481,40 +547,79 @@ struct DtPassT {
     __device__ __forceinline__ static void neighbour(const Args& a, const Sink& s, Acc& c, int k, const double* __restrict__ r, int jid) {
         c.nc = neighbour_slow(a.ng, r[0] - s.x, r[1] - s.y, r[2] - s.z, r[4] - s.vx, r[5] - s.vy, r[6] - s.vz, s.m, r[3], c.nc, k, jid);
     }
+    // the split's winners: refined key of the running best (recovered from the threshold, ~2 ulp) and its id
+    // refined keys of sink s against particle j read from the caller's arrays (rescan only)
+    __device__ __noinline__ static void key_of(const Args& a, const Sink& s, int j, double& kff, double& kfb) {
+        const size_t o = 3 * (size_t)j;
+        const double r[8] = {a.pos[o], a.pos[o + 1], a.pos[o + 2], a.mass[j], a.vel[o], a.vel[o + 1], a.vel[o + 2], 0.0};
+        keys(s, r, kff, kfb);
+    }
     __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
         const size_t o = (size_t)split * 2 * g.n_sink + k;
-        const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        a.pkey[o] = c.jff >= 0 ? dt_exact_ids(a, 0, id, c.jff) : inf;
-        a.pkey[o + g.n_sink] = c.jfb >= 0 ? dt_exact_ids(a, 1, id, c.jfb) : inf;
+        constexpr double UNSCALE = SHORT ? 1.0 / KEY_SLACK : KEY_PRE_INV;
+        double kf = c.thr_ff * UNSCALE, kb = c.thr_fb * UNSCALE;
+        int jf = c.jff, jb = c.jfb;
+        if (SHORT && __builtin_expect(c.amb != 0, 0)) {      // a near-tie in this range: settle it on the exact time-steps
+            const int l0 = min(split * g.tiles_per_split * TILE, g.n_src), l1 = min(l0 + g.tiles_per_split * TILE, g.n_src);
+            Sink t;
+            load_sink(a, id, t);
+            if (c.amb & 1) { jf = dt_rescan(a, 0, id, l0, l1); if (jf >= 0) { double d0, d1; key_of(a, t, jf, d0, d1); kf = d0; } }
+            if (c.amb & 2) { jb = dt_rescan(a, 1, id, l0, l1); if (jb >= 0) { double d0, d1; key_of(a, t, jb, d0, d1); kb = d1; } }
+        }
+        a.pkey[o] = kf; a.pkey[o + g.n_sink] = kb;
+        a.pid[o] = jf;  a.pid[o + g.n_sink] = jb;
         if (NGB) a.ng.pcount[(size_t)split * g.n_sink + k] = c.nc;
-        a.pid[o] = c.jff;  a.pid[o + g.n_sink] = c.jfb;
     }
-    // dtmin epilogue: the minimum over the splits' exact time-steps (ties -> smaller id): order-independent.
+    // dtmin epilogue: the winner over the splits by the same rule as inside a split - a key clear of the best by the band
+    // decides, a near-tie is decided on the exact time-steps - then Eq. 21 / Eq. 22 for the winning pair in IEEE operations
+    // in the oracle's order.  The winner is the exact (time-step, id) minimum, so the order of the splits does not matter.
     static constexpr bool ALWAYS_FINISH = true;
+    __device__ __forceinline__ static void merge(const Args& a, int i, int w, double key, int j, double& kb, int& jb) {
+        const bool clear = (j >= 0) & ((key * KEY_SLACK > kb) | (jb < 0));
+        const bool near = (j >= 0) & !clear & (key >= kb * KEY_SLACK) & (j != jb);
+        if (__builtin_expect(near, 0)) {
+            if (dt_contender_wins(a, w, i, jb, j)) { kb = key; jb = j; }
+        } else {
+            kb = clear ? key : kb; jb = clear ? j : jb;
+        }
+    }
     __device__ static void finish(const Args& a, const Geom& g, int k, int i, int lane, int L, bool write) {
         const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        double tb[2] = {inf, inf};
+        double kb[2] = {0.0, 0.0};
         int jb[2] = {-1, -1};
-        auto better = [](double t, int j, double tbest, int jbest) {
-            return j >= 0 && (jbest < 0 || t < tbest || (t == tbest && j < jbest));
-        };
-        for (int s = lane; s < g.n_split; s += L) {
-            for (int w = 0; w < 2; ++w) {
-                const size_t o = ((size_t)s * 2 + w) * g.n_sink + k;
-                const double t = __ldcg(a.pkey + o);
-                const int j = __ldcg(a.pid + o);
-                if (better(t, j, tb[w], jb[w])) { tb[w] = t; jb[w] = j; }
+        // four splits per trip, all 16 loads issued before the first compare (they come from other CTAs through L2: one
+        // dependent round trip per split made this loop 0.5 us per split - 65 us for 128 sinks x 128 splits)
+        for (int s0 = lane; s0 < g.n_split; s0 += 4 * L) {
+            double t[4][2];
+            int j[4][2];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int s = s0 + q * L;
+                const bool in = s < g.n_split;
+#pragma unroll
+                for (int w = 0; w < 2; ++w) {
+                    const size_t o = ((size_t)(in ? s : s0) * 2 + w) * g.n_sink + k;
+                    t[q][w] = __ldcg(a.pkey + o);
+                    j[q][w] = in ? __ldcg(a.pid + o) : -1;
+                }
             }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int w = 0; w < 2; ++w) merge(a, i, w, t[q][w], j[q][w], kb[w], jb[w]);
         }
-        for (int off = L >> 1; off > 0; off >>= 1) {      // (min t, then min id) is order-independent
+        for (int off = L >> 1; off > 0; off >>= 1) {
             for (int w = 0; w < 2; ++w) {
-                const double t = __shfl_xor_sync(0xffffffffu, tb[w], off);
+                const double key = __shfl_xor_sync(0xffffffffu, kb[w], off);
                 const int j = __shfl_xor_sync(0xffffffffu, jb[w], off);
-                if (better(t, j, tb[w], jb[w])) { tb[w] = t; jb[w] = j; }
+                merge(a, i, w, key, j, kb[w], jb[w]);
             }
         }
         if (!write || lane != 0) return;
         const int row = g.compact ? k : i;
+        double tb[2];
+        tb[0] = jb[0] >= 0 ? dt_exact_ids(a, 0, i, jb[0]) : inf;
+        tb[1] = jb[1] >= 0 ? dt_exact_ids(a, 1, i, jb[1]) : inf;
         if (a.dt_ff) a.dt_ff[row] = jb[0] >= 0 ? tb[0] : inf;
         if (a.dt_fb) a.dt_fb[row] = jb[1] >= 0 ? tb[1] : inf;
         if (a.j_ff) a.j_ff[row] = jb[0];
@@ -549,6 +654,7 @@ struct PotArgs {
 // the self pair does not multiply a zero separation and must be dropped by id (integer select).
 template <bool EXCL>
 struct PotPassT {
+    using Short = PotPassT;
     static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
     static constexpr int PHASED_MIN_S = 2;
     using Args = PotArgs;
