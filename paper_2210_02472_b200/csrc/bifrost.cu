@@ -47,6 +47,7 @@
 #include "pn1.cuh"
 #include "subsystems.cuh"
 #include "integrator.cuh"
+#include "hhs_subtree.cuh"
 #include "fp64_probe.cuh"
 
 // ========================================================================================
@@ -88,6 +89,8 @@ struct bifrost_ctx {
     int32_t *w_order = nullptr, *w_tmp = nullptr;
     int *w_bcount = nullptr, *w_nslow = nullptr;
     int* h_nslow = nullptr;          // pinned
+    long long* w_log = nullptr;      // device level log of bifrost_hhs_fsi, [HHS_LOG_ROWS][3], + 3 counters behind it
+    long long* h_log = nullptr;      // pinned mirror
     // mirrors for the *_host entry points (allocated on first use)
     bool host_ready = false;
     cudaStream_t hstream = nullptr;
@@ -110,6 +113,8 @@ namespace {
     } while (0)
 
 #define RC_TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
+
+constexpr long long HHS_LOG_ROWS = 1 << 16;      // rows of the device level log of bifrost_hhs_fsi (levels beyond it are counted, not logged)
 
 struct DeviceGuard {
     int prev = -1;
@@ -593,6 +598,8 @@ int ensure_integrator(bifrost_ctx* ctx) {
     CU_TRY(ctx, cudaMalloc(&ctx->w_bcount, 4 * (n / PART_T + 1)));
     CU_TRY(ctx, cudaMalloc(&ctx->w_nslow, 4));
     CU_TRY(ctx, cudaMallocHost(&ctx->h_nslow, 4));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_log, sizeof(long long) * (3 * HHS_LOG_ROWS + 3)));
+    CU_TRY(ctx, cudaMallocHost(&ctx->h_log, sizeof(long long) * (3 * HHS_LOG_ROWS + 3)));
     ctx->integ_ready = true;
     return BIFROST_OK;
 }
@@ -641,6 +648,14 @@ int fsi_impl(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double
     return BIFROST_OK;
 }
 
+// a host-steered level appends its row to the device log (the subtree kernel appends its own): one ordered log
+__global__ void hhs_log_kernel(long long* log, long long* counters, long long cap, int depth, const int* n_slow, int m) {
+    const long long row = counters[0];
+    if (row < cap) { log[3 * row] = depth; log[3 * row + 1] = *n_slow; log[3 * row + 2] = m - *n_slow; }
+    counters[0] = row + 1;
+    if (depth > counters[1]) counters[1] = depth;
+}
+
 struct Hhs {
     bifrost_ctx* ctx; int64_t n; double* pos; double* vel; const double* mass;
     double G, eps_soft, eta_ff, eta_fb; const double* dt_cap; int max_depth; cudaStream_t st;
@@ -654,6 +669,15 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     if (m == 0) return BIFROST_OK;
     cudaStream_t st = h.st;
     int32_t* seg = ctx->w_order + lo;
+    if (m <= ctx->small_m && m <= SUB_M) {
+        // the whole subtree below a small level in one single-CTA launch: no device -> host read, no further launches
+        const SubArgs sa{(int)m, seg, h.pos, h.vel, h.mass, ctx->w_dt0, h.dt_cap, h.G, soft2(h.eps_soft), h.eta_ff, h.eta_fb, tau,
+                         depth, h.max_depth, ctx->w_log, HHS_LOG_ROWS, ctx->w_log + 3 * HHS_LOG_ROWS};
+        hhs_subtree_kernel<<<1, SUB_M, 0, st>>>(sa);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+        return BIFROST_OK;
+    }
     const int all_slow = depth >= h.max_depth;
     if (!all_slow)   // time-steps of the level's particles among themselves (Eq. 21-22)
         RC_TRY(dtmin_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eta_ff, h.eta_fb, ctx->w_dtff, ctx->w_dtfb,
@@ -674,15 +698,11 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
         CU_TRY(ctx, cudaGetLastError());
         CU_TRY(ctx, cudaMemcpyAsync(seg, ctx->w_tmp, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
     }
+    hhs_log_kernel<<<1, 1, 0, st>>>(ctx->w_log, ctx->w_log + 3 * HHS_LOG_ROWS, HHS_LOG_ROWS, depth, ctx->w_nslow, (int)m);
+    ctx->launches++;
     CU_TRY(ctx, cudaMemcpyAsync(ctx->h_nslow, ctx->w_nslow, 4, cudaMemcpyDeviceToHost, st));
     CU_TRY(ctx, cudaStreamSynchronize(st));                // the host decides the recursion (as in the paper)
     const int64_t ns = *ctx->h_nslow, nf = m - ns;
-    if (h.log && h.n_levels < h.log_cap) {
-        int64_t* e = h.log + 3 * h.n_levels;
-        e[0] = depth; e[1] = ns; e[2] = nf;
-    }
-    h.n_levels++;
-    if (depth > h.deepest) h.deepest = depth;
     const int32_t* S = seg;
     const int32_t* F = seg + ns;
     if (nf == 0) {
@@ -826,8 +846,9 @@ int bifrost_destroy(bifrost_ctx* ctx) {
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
     cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_acc_s); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
-    cudaFree(ctx->w_order); cudaFree(ctx->w_tmp); cudaFree(ctx->w_bcount); cudaFree(ctx->w_nslow);
+    cudaFree(ctx->w_order); cudaFree(ctx->w_tmp); cudaFree(ctx->w_bcount); cudaFree(ctx->w_nslow); cudaFree(ctx->w_log);
     if (ctx->h_nslow) cudaFreeHost(ctx->h_nslow);
+    if (ctx->h_log) cudaFreeHost(ctx->h_log);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->h_stage_i) cudaFreeHost(ctx->h_stage_i);
     if (ctx->hstream) cudaStreamDestroy(ctx->hstream);
@@ -1215,11 +1236,22 @@ int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const
     fill_f64_kernel<<<ceil_div(n, 256), 256, 0, st>>>((int)n, HUGE_VAL, ctx->w_dt0);
     ctx->launches += 2;
     CU_TRY(ctx, cudaGetLastError());
+    long long* counters = ctx->w_log + 3 * HHS_LOG_ROWS;      // levels entered, deepest depth, FSI cycles of the subtree launches
+    CU_TRY(ctx, cudaMemsetAsync(counters, 0, 3 * sizeof(long long), st));
     Hhs h{ctx, n, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, dt_cap, max_depth, st, out_level_log, log_cap, 0, 0, 0};
     rc = hhs_level(h, 0, n, tau, 0);
-    if (out_summary) { out_summary[0] = h.n_levels; out_summary[1] = h.deepest; out_summary[2] = h.fsi_steps; }
     if (rc) return rc;
+    // the level log and the counters live on the device (host-steered levels and subtree launches append in stream order)
+    const long long want = std::min<long long>(log_cap, HHS_LOG_ROWS);
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->h_log + 3 * HHS_LOG_ROWS, counters, 3 * sizeof(long long), cudaMemcpyDeviceToHost, st));
+    if (out_level_log && want > 0)
+        CU_TRY(ctx, cudaMemcpyAsync(ctx->h_log, ctx->w_log, 3 * want * sizeof(long long), cudaMemcpyDeviceToHost, st));
     CU_TRY(ctx, cudaStreamSynchronize(st));
+    const long long* hc = ctx->h_log + 3 * HHS_LOG_ROWS;
+    if (out_level_log)
+        for (long long r = 0; r < std::min(want, hc[0]); ++r)
+            for (int q = 0; q < 3; ++q) out_level_log[3 * r + q] = ctx->h_log[3 * r + q];
+    if (out_summary) { out_summary[0] = hc[0]; out_summary[1] = hc[1]; out_summary[2] = h.fsi_steps + hc[2]; }
     return BIFROST_OK;
 }
 
