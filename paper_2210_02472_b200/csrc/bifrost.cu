@@ -991,10 +991,12 @@ int bifrost_acc_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
     if ((rc = ensure_host_mirrors(ctx))) return rc;
     H2D(ctx->d_pos, pos, 24 * (size_t)n);
     H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    // one list on both sides (same host pointer): one device copy, so that the call takes the symmetric kernels
+    const bool same = sink_idx && src_idx == sink_idx && n_src == n_sink;
     if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
-    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    if (src_idx && !same) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
     rc = acc_impl(ctx, n, ctx->d_pos, ctx->d_mass, sink_idx ? ctx->d_sink : nullptr, n_sink,
-                  src_idx ? ctx->d_src : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
+                  src_idx ? (same ? ctx->d_sink : ctx->d_src) : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
     if (rc) return rc;
     return fetch_rows(ctx, ctx->d_out, 24, sink_idx, n_sink, out_acc, ctx->h_stage);
 }
@@ -1011,10 +1013,11 @@ int bifrost_grad_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doub
     H2D(ctx->d_pos, pos, 24 * (size_t)n);
     H2D(ctx->d_mass, mass, 8 * (size_t)n);
     H2D(ctx->d_acc, acc, 24 * (size_t)n);
+    const bool same = sink_idx && src_idx == sink_idx && n_src == n_sink;
     if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
-    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    if (src_idx && !same) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
     rc = grad_impl(ctx, n, ctx->d_pos, ctx->d_mass, ctx->d_acc, sink_idx ? ctx->d_sink : nullptr, n_sink,
-                   src_idx ? ctx->d_src : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
+                   src_idx ? (same ? ctx->d_sink : ctx->d_src) : nullptr, n_src, G, eps, ctx->d_out, 1, ctx->hstream);
     if (rc) return rc;
     return fetch_rows(ctx, ctx->d_out, 24, sink_idx, n_sink, out_grad, ctx->h_stage);
 }

@@ -981,6 +981,19 @@ def test_integrator_refuses_subsystems(torch, ctx):
     ctx.fsi_step(pos, vel, mass, w.G, 0.0, 1e-4)      # fine again without subsystems
 
 
+def test_host_variants_take_the_symmetric_kernels_for_one_list(torch, ctx_sym):
+    """bifrost_acc_host / bifrost_grad_host with the SAME host list on both sides: one device copy of the list, so the
+    call qualifies for the symmetric kernels (3 launches), results equal to the oracle's."""
+    w = _small(6000, 21)
+    ids = np.random.default_rng(22).permutation(w.n)[:4000].astype(np.int32)
+    l0 = ctx_sym.launch_count
+    a = ctx_sym.acc_host(w.pos, w.mass, w.G, 1e-4, ids, ids)
+    assert ctx_sym.launch_count - l0 == 3
+    check_vec(a[ids], oracle.acc(w.pos, w.mass, w.G, 1e-4, ids, ids), "acc_host one list")
+    c = ctx_sym.grad_host(w.pos, w.mass, a, w.G, 1e-4, ids, ids)
+    check_vec(c[ids], oracle.grad(w.pos, w.mass, a, w.G, 1e-4, ids, ids), "grad_host one list")
+
+
 def test_reserve_and_tuning_api(torch):
     from paper_2210_02472_b200.binding import BifrostError, Context
     c = Context(5000)
