@@ -232,7 +232,11 @@ template <class P, class Huge, int HUGE_GAIN_PERMILLE, class Big, class F4, clas
 int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src,
              size_t partial_bytes_per_sink, int compact, cudaStream_t st) {
     Geom g;
-    if (n_sink < ctx->fused_max_sinks) {
+    // grad and dtmin (heavier records, more arithmetic per pair) gain from the packed path already at 2048 sinks when the
+    // source list is long (config 3, 2048 sinks x 131072 sources: grad 605 -> 518 us, dtmin 628 -> 568 us; config 2's 16384
+    // sources: the fused launch stays ahead) - profiles/r2_sweep_small_sets.md
+    const bool pack_early = P::PACK_EARLY && n_sink >= 2048 && (double)n_sink * (double)n_src >= 1e8 && ctx->fused_max_sinks >= 2048;
+    if (n_sink < ctx->fused_max_sinks && !pack_early) {
         const int64_t splits = std::max<int64_t>(1, std::min<int64_t>(ceil_div(n_src, TILE), MAX_SPLIT));
         const int64_t want = 4LL * ctx->num_sms;
         if ((int64_t)ceil_div(n_sink, 128 * 4) * splits >= want)

@@ -65,6 +65,7 @@ template <bool EXCL>
 struct AccPassT {
     using Short = AccPassT;
     static constexpr int REC = EXCL ? 8 : 6;   // x y z m 1.5m 1.875m [subsystem code (bits), pad]
+    static constexpr bool PACK_EARLY = false;  // (see run_pass)
     static constexpr int PHASED_MIN_S = EXCL ? 2 : 0;
     using Args = AccArgs;
     struct Sink { double x, y, z; int sub; };
@@ -164,6 +165,7 @@ template <bool EXCL, bool WITH_ACC = false>
 struct GradPassT {
     using Short = GradPassT;
     static constexpr int REC = 10;  // x y z ax ay az m 1.5m 1.875m [subsystem code (bits)]
+    static constexpr bool PACK_EARLY = true;
     static constexpr int PHASED_MIN_S = 5;   // measured: phase-major helps at S = 5 (+1.4 %), hurts at S = 4
     using Args = GradArgs;
     struct Sink { double x, y, z, ax, ay, az; int sub; };
@@ -405,6 +407,7 @@ template <bool EXCL, bool NGB = false, bool SHORT = false>
 struct DtPassT {
     using Short = DtPassT<EXCL, NGB, true>;
     static constexpr int REC = 8;   // x y z m vx vy vz {id (low word), subsystem code (high word)}
+    static constexpr bool PACK_EARLY = true;
     static constexpr int PHASED_MIN_S = 1;
     using Args = DtArgs;
     struct Sink { double x, y, z, m, vx, vy, vz; int id, sub; };
@@ -656,6 +659,7 @@ template <bool EXCL>
 struct PotPassT {
     using Short = PotPassT;
     static constexpr int REC = 8;   // x y z m 0.5m 0.375m {id, subsystem code}(bits) pad
+    static constexpr bool PACK_EARLY = false;
     static constexpr int PHASED_MIN_S = 2;
     using Args = PotArgs;
     struct Sink { double x, y, z; int id, sub; };
