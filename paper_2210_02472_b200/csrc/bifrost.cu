@@ -43,6 +43,7 @@
 #include "policies.cuh"
 #include "pair_kernels.cuh"
 #include "sym_kernels.cuh"
+#include "sym_dt.cuh"
 #include "epilogues.cuh"
 #include "pn1.cuh"
 #include "subsystems.cuh"
@@ -76,6 +77,7 @@ struct bifrost_ctx {
     size_t sym_ws_bytes = 0;
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
+    int64_t sym_min_dt = 65536;      // shortest list for the symmetric dtmin (BIFROST_TUNE_SYM_MIN_N sets it too)
     int64_t sym_min_acc = 16384, sym_min_grad = 12288;   // shortest list the symmetric kernels are used for (measured
                                      // crossover, profiles/r2_symmetric.md; BIFROST_TUNE_SYM_MIN_N sets both)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
@@ -446,6 +448,56 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
                : run_pass<GradPassT<false, true>, Huge, 40, Big, F4, F2, F1>(ctx, a, src, n_sink, n_src, 48, 0, st);
 }
 
+// dtmin over one list that is both sink and source set, every pair once (sym_dt.cuh).  Returns 1 when the call does not qualify.
+int sym_dt_impl(bifrost_ctx* ctx, const double* pos, const double* vel, const double* mass, const int32_t* idx, int64_t m, double G,
+                double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact, cudaStream_t st) {
+    constexpr int S = 6, T = 256, MINB = 1;
+    if (m < ctx->sym_min_dt || m < 2 || !ctx->sym_ws || ctx->shard_world > 1) return 1;
+    SymGeom g{};
+    g.m = (int)m;
+    g.n_tiles = ceil_div(m, TILE);
+    g.bs = T * S;
+    g.tb = g.bs / TILE;
+    g.n_blocks = ceil_div(m, g.bs);
+    g.compact = compact;
+    g.rank = 0; g.world = 1;
+    int64_t total = 0;
+    for (int b = 0; b < g.n_blocks; ++b) total += sym_range(g, b);
+    const int64_t slots = (int64_t)ctx->num_sms * MINB;
+    g.unit_tiles = (int)std::max<int64_t>(2, (total + 64 * slots - 1) / (64 * slots));
+    const int64_t max_pieces_ws = (int64_t)(ctx->partial_bytes / (sizeof(DtBest) * (size_t)m));
+    if (max_pieces_ws < 2) return 1;
+    while (sym_pieces(g, 0) > max_pieces_ws) g.unit_tiles *= 2;
+    // the symmetric workspace holds: best[m], lock[m], two counters, the candidate list (the rest)
+    char* ws = (char*)ctx->sym_ws;
+    const size_t off_lock = sizeof(DtBest) * (size_t)m, off_cnt = (off_lock + 4 * (size_t)m + 15) & ~(size_t)15, off_cand = off_cnt + 16;
+    if (ctx->sym_ws_bytes < off_cand + ((size_t)64 << 20)) return 1;
+    SymDtArgs a{};
+    a.d = DtArgs{pos, vel, mass, nullptr, idx, idx, (int)m, nullptr, nullptr, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
+    a.idx = idx;
+    a.pieces = (DtBest*)ctx->partial;
+    a.best = (DtBest*)ws;
+    a.lock = (int*)(ws + off_lock);
+    a.counters = (unsigned long long*)(ws + off_cnt);
+    a.cand = (DtCand*)(ws + off_cand);
+    a.cand_cap = (ctx->sym_ws_bytes - off_cand) / sizeof(DtCand);
+    a.hint_ff = ctx->smin;
+    a.hint_fb = (unsigned long long*)ctx->phi_scratch;
+    const int n_pad = g.n_tiles * TILE;
+    const SrcArrays src{pos, vel, mass, nullptr, idx};
+    pack_kernel<DtPassT<false>><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)m, n_pad, src, ctx->src_rec);
+    CU_TRY(ctx, cudaMemsetAsync(a.counters, 0, 16, st));
+    sym_dt_kernel<S, T, MINB><<<dim3(sym_diag_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 0);
+    sym_dt_hint_kernel<<<ceil_div(m, 256), 256, 0, st>>>(a, g);
+    sym_dt_kernel<S, T, MINB><<<dim3(sym_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 1);
+    sym_dt_merge_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);
+    sym_dt_apply_kernel<<<ctx->num_sms * 8, 256, 0, st>>>(a);
+    sym_dt_final_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);
+    ctx->launches += 7;
+    CU_TRY(ctx, cudaGetLastError());
+    return BIFROST_OK;
+}
+
 // ng == NULL: bifrost_dtmin; else the neighbour search of Eq. 18-19 rides on the same pass (bifrost_dtmin_neighbours)
 int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel, const double* mass,
                const int32_t* sink_idx, int64_t n_sink, const int32_t* src_idx, int64_t n_src, double G,
@@ -453,6 +505,10 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
                cudaStream_t st, const NgbArgs* ng = nullptr) {
     const int32_t* sub = (ctx->subsys && ctx->subsys_n == n) ? ctx->subsys : nullptr;   // NEXT-2
     if (n_sink == 0) return BIFROST_OK;
+    if (!ng && !sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
+        const int rc = sym_dt_impl(ctx, pos, vel, mass, sink_idx, n_sink, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, compact, st);
+        if (rc <= 0) return rc;
+    }
     // workspace per sink and split: 16 B of time-steps, 8 B of ids [, 4 B neighbour count + 4 cap B of list]; the regions
     // share ctx->partial in those proportions, so whatever split count fits the whole fits every region
     const size_t per_sink = 24 + (ng ? 4 * ((size_t)ng->cap + 1) : 0);
@@ -817,7 +873,7 @@ int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
             if (value > SMALL_M) return BIFROST_EINVAL;
             ctx->small_m = (int)value; return BIFROST_OK;
         case BIFROST_TUNE_SYM_MIN_N:
-            ctx->sym_min_acc = ctx->sym_min_grad = value; return BIFROST_OK;
+            ctx->sym_min_acc = ctx->sym_min_grad = ctx->sym_min_dt = value; return BIFROST_OK;
         case BIFROST_TUNE_MUTUAL_MIN_PAIRS:
             ctx->mutual_min_pairs = (double)value; ctx->mutual_min_b = value == 0 ? 1 : 512; return BIFROST_OK;
         default: return BIFROST_EINVAL;

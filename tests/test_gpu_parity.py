@@ -1210,3 +1210,45 @@ def test_mutual_inter_level_sums(torch, n_a, n_b, forced):
             assert (np.abs(tot) <= 1e-12 * scale).all()
     finally:
         c.close()
+
+
+@pytest.mark.parametrize("m", [2, 3, 129, 1537, 3073, 10000])
+def test_symmetric_dtmin_ragged_sizes(torch, ctx, ctx_sym, m):
+    """bifrost_dtmin over one list, every unordered pair once (sym_dt.cuh: hints, candidate list, per-particle merge): list
+    lengths around the tile and block sizes, indices and values bit-identical to the oracle's and to the plain kernel's;
+    repeats bit-identical although the candidate order is not."""
+    w = _small(m, 700 + m)
+    pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
+    l0 = ctx_sym.launch_count
+    d = ctx_sym.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+    assert ctx_sym.launch_count - l0 == 7
+    d2 = ctx_sym.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+    dp = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+    torch.cuda.synchronize()
+    assert all(torch.equal(x, y) for x, y in zip(d, d2)) and all(torch.equal(x, y) for x, y in zip(d, dp))
+    check_dt(tuple(t.cpu().numpy() for t in d), oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb), f"sym dtmin m={m}")
+
+
+def test_symmetric_dtmin_list_ties_and_zero_velocity(torch, ctx_sym):
+    """The symmetric dtmin through an unsorted index list (rows of the others untouched), on the exact-tie lattice (every
+    tie to the smaller id, whichever side of the pair found it) and with all velocities zero (+inf / -1)."""
+    w = _small(7000, 41)
+    ids = np.random.default_rng(42).permutation(w.n)[:4000].astype(np.int32)
+    pos, vel, mass, li = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), dev(torch, ids)
+    d = ctx_sym.dtmin(pos, vel, mass, w.G, 0.02, 0.03, li, li)
+    got = tuple(t.cpu().numpy() for t in d)
+    rest = np.ones(w.n, bool); rest[ids] = False
+    assert np.isinf(got[0][rest]).all() and (got[2][rest] == -1).all()
+    check_dt(tuple(x[ids] for x in got), oracle.dtmin(w.pos, w.vel, w.mass, w.G, 0.02, 0.03, ids, ids), "sym dtmin list")
+    g = np.arange(6)
+    lat = np.array([[x, y, z] for x in g for y in g for z in g], dtype=np.float64) * 0.25
+    lat = lat[np.random.default_rng(5).permutation(lat.shape[0])]
+    lv = np.sign(lat - 0.625) * lat * lat * 0.5
+    wl = W.Workload("lattice", lat, lv, np.full(lat.shape[0], 2.0 ** -7), 1.0, 0.0, 0.5, 0.25)
+    d = ctx_sym.dtmin(dev(torch, wl.pos), dev(torch, wl.vel), dev(torch, wl.mass), wl.G, wl.eta_ff, wl.eta_fb)
+    ref = oracle.dtmin(wl.pos, wl.vel, wl.mass, wl.G, wl.eta_ff, wl.eta_fb)
+    assert (ref["margin_ff"] == 0).any() and (ref["margin_fb"] == 0).any()
+    check_dt(tuple(t.cpu().numpy() for t in d), ref, "sym dtmin lattice")
+    d = ctx_sym.dtmin(dev(torch, wl.pos), torch.zeros_like(dev(torch, wl.vel)), dev(torch, wl.mass), wl.G, wl.eta_ff, wl.eta_fb)
+    assert torch.isinf(d[1]).all() and bool((d[3] == -1).all())
+    assert np.array_equal(d[2].cpu().numpy(), ref["j_ff"])
