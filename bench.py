@@ -50,8 +50,9 @@ UNIT = "interactions/s"
 #   grad 33 + 4.5/6 = 33.75 / 52.75 - i.e. half of that per interaction.
 #   dtmin: 17 instructions in the hot path (7 DADD + 6 DFMA + 4 DMUL = 23 flops: keys from the unrefined rsqrt seed; the
 #   refinement and the exact time-steps run in the rarely taken branch only).
-FP64_INSTR = {"plain": {"acc": 15, "grad": 28, "dtmin": 17}, "sym": {"acc": 20.5625 / 2, "grad": 33.75 / 2, "dtmin": 17}}
-FP64_FLOPS = {"plain": {"acc": 24, "grad": 44, "dtmin": 23}, "sym": {"acc": 32.5625 / 2, "grad": 52.75 / 2, "dtmin": 23}}
+#   Same-list dtmin evaluates every unordered pair once too (both keys are symmetric): 17 / 23 per unordered pair.
+FP64_INSTR = {"plain": {"acc": 15, "grad": 28, "dtmin": 17}, "sym": {"acc": 20.5625 / 2, "grad": 33.75 / 2, "dtmin": 17 / 2}}
+FP64_FLOPS = {"plain": {"acc": 24, "grad": 44, "dtmin": 23}, "sym": {"acc": 32.5625 / 2, "grad": 52.75 / 2, "dtmin": 23 / 2}}
 # SURVEY.md 8(d)'s budget for the minimal ONE-SIDED sequence: flops per ordered pair.  Against it the symmetric
 # kernels deliver more interactions than the executed flops alone would ("work-equivalent" fraction, may exceed 1).
 SURVEY_8D_FLOPS = {"acc": 26, "grad": 42}
@@ -373,13 +374,14 @@ def run_cuda(args):
                 ms, rate = ctx.fp64_probe(mix=mix, iters=(1 << 15) if mix < 2 else (1 << 16), ctas_per_sm=32)
                 probe[name] = {"ms": ms, "lane_instr_per_s": rate, "frac_of_derived_pipe_peak": rate / (peak * 1e12 / 2)}
         pairs_rank = float(n) * n / world                               # a rank's share of the ordered interactions
-        path = "sym" if world > 1 or n >= 16384 else "plain"            # which acc / grad kernels these sizes select
+        path_ag = path = "sym" if world > 1 or n >= 16384 else "plain"  # which acc / grad kernels these sizes select
         kernel_name = {"acc": {"sym": "sym_pair_kernel<SymAcc, 8, 256, 1>", "plain": "pair_kernel<AccPass, 8, 256, 1, 1>"},
                        "grad": {"sym": "sym_pair_kernel<SymGrad, 6, 256, 1>", "plain": "pair_kernel<GradPass, 5, 128, 2, 2>"},
-                       "dtmin": {"sym": "pair_kernel<DtPass, 4, 128, 3, 2>", "plain": "pair_kernel<DtPass, 4, 128, 3, 2>"}}
+                       "dtmin": {"sym": "sym_dt_kernel<4, 128, 3, 4>", "plain": "pair_kernel<DtPass, 4, 128, 3, 2>"}}
 
         def kern(name):
             ms = mean_ms[name]
+            path = path_ag if name != "dtmin" else ("sym" if world == 1 and n >= 40960 else "plain")   # dtmin is sink-sharded when world > 1
             tf = pairs_rank * FP64_FLOPS[path][name] / (ms * 1e-3) / 1e12
             pipe = pairs_rank * FP64_INSTR[path][name] / (ms * 1e-3) / (peak * 1e12 / 2)
             out = {"ms": ms, "kernel": kernel_name[name][path], "interactions_per_s": pairs_rank / (ms * 1e-3),
@@ -683,12 +685,13 @@ def run_sweep(args):
     ctx = Context(1 << 18)
     for m in (4096, 8192, 12288, 16384, 24576, 32768, 65536, 131072, 262144):
         w = W.config4(n=m, n_sbh=10)
-        pos, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.mass))
+        pos, vel, mass = (torch.from_numpy(x).to(dev) for x in (w.pos, w.vel, w.mass))
         rec = {"m": m}
         for mode, thr in (("sym", 0), ("plain", 1 << 40)):
             ctx.set_tuning(Context.TUNE_SYM_MIN_N, thr)
             a = ctx.acc(pos, mass, w.G, w.eps)
-            for name, fn in (("acc", lambda: ctx.acc(pos, mass, w.G, w.eps)), ("grad", lambda: ctx.grad(pos, mass, a, w.G, w.eps))):
+            for name, fn in (("acc", lambda: ctx.acc(pos, mass, w.G, w.eps)), ("grad", lambda: ctx.grad(pos, mass, a, w.G, w.eps)),
+                             ("dtmin", lambda: ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb))):
                 reps = 20 if m <= 65536 else 4
                 for _ in range(reps):
                     fn()

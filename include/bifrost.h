@@ -49,9 +49,10 @@
  *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
  *  - Launch shapes are chosen from the argument sizes alone: below 4096 sinks a call is one
  *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish;
- *    bifrost_acc / bifrost_grad whose sink and source lists are the SAME list (same pointer, or both
- *    NULL) of >= 16384 / 12288 entries evaluate every unordered pair once (symmetric kernels).  The
- *    thresholds are bifrost_set_tuning knobs; no environment variable or file is read.
+ *    bifrost_acc / bifrost_grad / bifrost_dtmin whose sink and source lists are the SAME list (same
+ *    pointer, or both NULL) of >= 16384 / 12288 / 40960 entries evaluate every unordered pair once
+ *    (symmetric kernels; results as before, in another summation order - dtmin's are bit-identical).
+ *    The thresholds are bifrost_set_tuning knobs; no environment variable or file is read.
  *  - Return value: BIFROST_OK (0) or a negative BIFROST_E* code.  Nothing is printed, nothing
  *    aborts.  On BIFROST_ECUDA, bifrost_last_cuda_error(ctx) holds the CUDA error string.
  */
@@ -105,7 +106,8 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
  *   BIFROST_TUNE_SMALL_M          largest particle set whose FSI cycle / level split is one single-CTA launch
  *                                 (default 128, 0..256; 0 disables)
  *   BIFROST_TUNE_SYM_MIN_N        shortest same-list call that takes the symmetric kernels (default 16384 for
- *                                 acc, 12288 for grad; this knob sets both; a value above max_n disables them) */
+ *                                 acc, 12288 for grad, 40960 for dtmin; this knob sets all three; a value above
+ *                                 max_n disables them) */
 #define BIFROST_TUNE_FUSED_MAX_SINKS 0
 #define BIFROST_TUNE_SMALL_M         1
 #define BIFROST_TUNE_SYM_MIN_N       2

@@ -77,7 +77,7 @@ struct bifrost_ctx {
     size_t sym_ws_bytes = 0;
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
-    int64_t sym_min_dt = 65536;      // shortest list for the symmetric dtmin (BIFROST_TUNE_SYM_MIN_N sets it too)
+    int64_t sym_min_dt = 40960;      // shortest list for the symmetric dtmin (cross-over near 32768; BIFROST_TUNE_SYM_MIN_N sets it too)
     int64_t sym_min_acc = 16384, sym_min_grad = 12288;   // shortest list the symmetric kernels are used for (measured
                                      // crossover, profiles/r2_symmetric.md; BIFROST_TUNE_SYM_MIN_N sets both)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
@@ -451,7 +451,9 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
 // dtmin over one list that is both sink and source set, every pair once (sym_dt.cuh).  Returns 1 when the call does not qualify.
 int sym_dt_impl(bifrost_ctx* ctx, const double* pos, const double* vel, const double* mass, const int32_t* idx, int64_t m, double G,
                 double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact, cudaStream_t st) {
-    constexpr int S = 6, T = 256, MINB = 1;
+    // 4 sinks x 128 threads x 3 CTAs/SM, unroll 4: 690 ms at N = 2^20 (before the sink side started from the hints: 728; 6 x 256 x 1:
+    // 772; 6 x 128 x 2: 743; profiles/r2_dtmin.md)
+    constexpr int S = 4, T = 128, MINB = 3, UNR = 4;
     if (m < ctx->sym_min_dt || m < 2 || !ctx->sym_ws || ctx->shard_world > 1) return 1;
     SymGeom g{};
     g.m = (int)m;
@@ -487,9 +489,9 @@ int sym_dt_impl(bifrost_ctx* ctx, const double* pos, const double* vel, const do
     const SrcArrays src{pos, vel, mass, nullptr, idx};
     pack_kernel<DtPassT<false>><<<ceil_div(n_pad, 256), 256, 0, st>>>((int)m, n_pad, src, ctx->src_rec);
     CU_TRY(ctx, cudaMemsetAsync(a.counters, 0, 16, st));
-    sym_dt_kernel<S, T, MINB><<<dim3(sym_diag_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 0);
+    sym_dt_kernel<S, T, MINB, UNR><<<dim3(sym_diag_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 0);
     sym_dt_hint_kernel<<<ceil_div(m, 256), 256, 0, st>>>(a, g);
-    sym_dt_kernel<S, T, MINB><<<dim3(sym_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 1);
+    sym_dt_kernel<S, T, MINB, UNR><<<dim3(sym_pieces(g, 0), g.n_blocks), T, 0, st>>>(a, g, ctx->src_rec, 1);
     sym_dt_merge_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);
     sym_dt_apply_kernel<<<ctx->num_sms * 8, 256, 0, st>>>(a);
     sym_dt_final_kernel<<<ceil_div(m, 128), 128, 0, st>>>(a, g);

@@ -35,7 +35,7 @@ struct SymDtArgs {
 };
 
 // phase = 0: the diagonal pieces only (one-sided; sets the hints);  phase = 1: the pieces beyond the block (both sides)
-template <int S, int T, int MINB>
+template <int S, int T, int MINB, int UNR = 2>
 __global__ void __launch_bounds__(T, MINB)
 sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ rec, int phase) {
     using D = DtPassT<false>;
@@ -64,6 +64,14 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
         const double* r = rec + (size_t)(live[s] ? k : g.m - 1) * REC;
         sink[s] = D::Sink{r[0], r[1], r[2], r[3], r[4], r[5], r[6], __double2loint(r[7]), 0};
         D::init(accu[s]);
+        // beyond the diagonal the sink side starts from the position's hint as well: a pair clearly below the best key
+        // already on record for this particle cannot be its minimum, in whichever piece it turns up (id -1 = "nothing in this
+        // piece reaches the record").  Without it every piece restarts its running maxima and takes the branch at most
+        // sources of a short piece.
+        if (!diag && live[s]) {
+            accu[s].thr_ff = __longlong_as_double((long long)__ldcg(a.hint_ff + k)) * KEY_PRE;
+            accu[s].thr_fb = __longlong_as_double((long long)__ldcg(a.hint_fb + k)) * KEY_PRE;
+        }
     }
 
     const int jb = sym_first(g, b);
@@ -95,7 +103,7 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
         __syncthreads();
         const double* __restrict__ tb = tile_sm[buf];
         const int cnt = min(TILE, g.m - tile * TILE);
-#pragma unroll 2
+#pragma unroll UNR
         for (int jj = 0; jj < cnt; ++jj) {
             double r[REC];
 #pragma unroll
@@ -154,6 +162,10 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
         if (!live[s]) continue;
         const DtBest o{accu[s].thr_ff * KEY_PRE_INV, accu[s].thr_fb * KEY_PRE_INV, accu[s].jff, accu[s].jfb};
         a.pieces[(size_t)piece * g.m + k] = o;
+        if (!diag) {                                            // what this piece found raises the particle's hints
+            if (accu[s].jff >= 0) atomicMax(a.hint_ff + k, (unsigned long long)__double_as_longlong(o.kff));
+            if (accu[s].jfb >= 0) atomicMax(a.hint_fb + k, (unsigned long long)__double_as_longlong(o.kfb));
+        }
     }
 }
 
