@@ -1097,14 +1097,15 @@ int bifrost_dtmin_host(bifrost_ctx* ctx, int64_t n, const double* pos, const dou
     H2D(ctx->d_pos, pos, 24 * (size_t)n);
     H2D(ctx->d_vel, vel, 24 * (size_t)n);
     H2D(ctx->d_mass, mass, 8 * (size_t)n);
+    const bool same = sink_idx && src_idx == sink_idx && n_src == n_sink;      // one list on both sides: one device copy
     if (sink_idx) H2D(ctx->d_sink, sink_idx, 4 * (size_t)n_sink);
-    if (src_idx) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
+    if (src_idx && !same) H2D(ctx->d_src, src_idx, 4 * (size_t)n_src);
     double* d_ff = ctx->d_dt;
     double* d_fb = ctx->d_dt + n_sink;
     int32_t* d_jff = ctx->d_j;
     int32_t* d_jfb = ctx->d_j + n_sink;
     rc = dtmin_impl(ctx, n, ctx->d_pos, ctx->d_vel, ctx->d_mass, sink_idx ? ctx->d_sink : nullptr, n_sink,
-                    src_idx ? ctx->d_src : nullptr, n_src, G, eta_ff, eta_fb, d_ff, d_fb, d_jff, d_jfb, 1, ctx->hstream);
+                    src_idx ? (same ? ctx->d_sink : ctx->d_src) : nullptr, n_src, G, eta_ff, eta_fb, d_ff, d_fb, d_jff, d_jfb, 1, ctx->hstream);
     if (rc) return rc;
     if ((rc = fetch_rows(ctx, d_ff, 8, sink_idx, n_sink, out_dt_ff, ctx->h_stage))) return rc;
     if ((rc = fetch_rows(ctx, d_fb, 8, sink_idx, n_sink, out_dt_fb, ctx->h_stage))) return rc;
