@@ -377,7 +377,7 @@ def run_cuda(args):
         path_ag = path = "sym" if world > 1 or n >= 16384 else "plain"  # which acc / grad kernels these sizes select
         kernel_name = {"acc": {"sym": "sym_pair_kernel<SymAcc, 8, 256, 1>", "plain": "pair_kernel<AccPass, 8, 256, 1, 1>"},
                        "grad": {"sym": "sym_pair_kernel<SymGrad, 6, 256, 1>", "plain": "pair_kernel<GradPass, 5, 128, 2, 2>"},
-                       "dtmin": {"sym": "sym_dt_kernel<4, 128, 3, 4>", "plain": "pair_kernel<DtPass, 4, 128, 3, 2>"}}
+                       "dtmin": {"sym": "sym_dt_kernel<6, 128, 2, 2>", "plain": "pair_kernel<DtPass, 4, 128, 3, 2>"}}
 
         def kern(name):
             ms = mean_ms[name]

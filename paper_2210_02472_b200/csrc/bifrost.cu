@@ -451,9 +451,9 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
 // dtmin over one list that is both sink and source set, every pair once (sym_dt.cuh).  Returns 1 when the call does not qualify.
 int sym_dt_impl(bifrost_ctx* ctx, const double* pos, const double* vel, const double* mass, const int32_t* idx, int64_t m, double G,
                 double eta_ff, double eta_fb, double* dt_ff, double* dt_fb, int32_t* j_ff, int32_t* j_fb, int compact, cudaStream_t st) {
-    // 4 sinks x 128 threads x 3 CTAs/SM, unroll 4: 690 ms at N = 2^20 (before the sink side started from the hints: 728; 6 x 256 x 1:
-    // 772; 6 x 128 x 2: 743; profiles/r2_dtmin.md)
-    constexpr int S = 4, T = 128, MINB = 3, UNR = 4;
+    // 6 sinks x 128 threads x 2 CTAs/SM, unroll 2 (254 registers, no spill): 665 ms at N = 2^20; 3 x 128 x 3 unroll 4: 681;
+    // 4 x 128 x 3 unroll 4 (168 registers, spills): 690; 6 x 256 x 1: 698; 4 x 128 x 2: 771 (profiles/r2_dtmin.md)
+    constexpr int S = 6, T = 128, MINB = 2, UNR = 2;
     if (m < ctx->sym_min_dt || m < 2 || !ctx->sym_ws || ctx->shard_world > 1) return 1;
     SymGeom g{};
     g.m = (int)m;
