@@ -374,6 +374,34 @@ int bifrost_pn1_host(bifrost_ctx* ctx, int64_t n, const double* pos, const doubl
 int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm, double* out_ms,
                        double* out_lane_instr);
 
+/* bifrost_acc_static - bifrost_acc (Eq. 6, all n particles as sinks and as sources) for callers
+ * that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * It needs NO context and calls no cudaMalloc, cudaFree or allocating library routine: the packed source
+ * records, the split-j partial sums and the arrival counters of the fused kernel live in ONE file-scope
+ * `static __device__` array of BIFROST_STATIC_SCRATCH_BYTES (8 MiB) inside libbifrost.so, which every GPU that
+ * loads the library holds until the process exits.  The kernels are those of bifrost_acc (one fused launch
+ * below 4096 particles, pack -> pair -> finish from there on); only the split count, hence the summation
+ * order, can differ from a context's (the workspace is smaller), so results agree with bifrost_acc to rounding.
+ *   device   CUDA device ordinal (0 <= device < 64); made current for the call and restored afterwards.  The first
+ *            call on a device does the set-up (the array's device address, the SM count); make one call
+ *            before starting a graph capture.
+ *   n        0 <= n <= BIFROST_STATIC_MAX_N (16384); beyond that the call is refused with BIFROST_EINVAL and a
+ *            message that names the limit (bifrost_static_error) - use bifrost_acc with a context instead.
+ *   pos [n][3], mass [n], out_acc [n][3]: DEVICE pointers on `device`, borrowed; G, eps as for bifrost_acc.
+ *   stream   cudaStream_t (NULL = legacy default); asynchronous like bifrost_acc.
+ * Every call on a device shares that device's array.  The array keeps the last call's contents; the one part that
+ * must start at zero (the arrival counters) is cleared on the stream by every call that uses it, everything
+ * else is written before it is read.  Two calls that OVERLAP on the same GPU (different streams, or different
+ * host threads without ordering between their streams) race on the array and give undefined results; calls on
+ * one stream, or ordered by events, are safe.
+ * Returns BIFROST_OK, BIFROST_EINVAL (bad device, n out of range, NULL pointer) or BIFROST_ECUDA. */
+#define BIFROST_STATIC_MAX_N 16384
+#define BIFROST_STATIC_SCRATCH_BYTES (8u << 20)
+int bifrost_acc_static(int device, int64_t n, const double* pos, const double* mass, double G, double eps,
+                       double* out_acc, void* stream);
+/* Message of the calling thread's last failed bifrost_acc_static ("" if it succeeded); static storage. */
+const char* bifrost_static_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -32,6 +32,7 @@ SYMBOLS = [
     "bifrost_neighbours", "bifrost_components", "bifrost_dtmin_neighbours",
     "bifrost_reserve", "bifrost_set_tuning", "bifrost_set_shard", "bifrost_acc_mutual", "bifrost_grad_mutual",
     "bifrost_acc_jerk", "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
+    "bifrost_acc_static", "bifrost_static_error",
 ]
 
 
@@ -90,6 +91,9 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_hhs_fsi.argtypes = [_P, _I64, _P, _P, _P, _D, _D, _D, _D, _P, _D, _I, _P, _I64, _P, _P]
     lib.bifrost_kinetic_energy.argtypes = [_P, _I64, _P, _P, _P, _I64, _P, _P]
     lib.bifrost_fp64_probe.argtypes = [_P, _I, _I64, _I, ctypes.POINTER(_D), ctypes.POINTER(_D)]
+    lib.bifrost_acc_static.argtypes = [_I, _I64, _P, _P, _D, _D, _P, _P]
+    lib.bifrost_static_error.argtypes = []
+    lib.bifrost_static_error.restype = ctypes.c_char_p
     _lib = lib
     return lib
 
@@ -152,6 +156,31 @@ def _host_idx(a):
         return None, None
     a = np.ascontiguousarray(a, dtype=np.int32)
     return a, (a.ctypes.data if a.size else _HOST_DUMMY.ctypes.data)
+
+
+STATIC_MAX_N = 16384           # BIFROST_STATIC_MAX_N
+
+
+def acc_static(pos, mass, G, eps, out):
+    """bifrost_acc_static: Eq. 6 over all particles with NO context and no allocation anywhere - the scratch is a
+    static device array inside libbifrost.so (n <= STATIC_MAX_N; calls that overlap on one GPU race on it).  `out` is
+    the caller's [n, 3] tensor (this function allocates nothing either); returns it."""
+    import torch
+    lib = load_library()
+    _seen.clear()
+    pos = _dev_f64(pos, (3,), "pos"); mass = _dev_f64(mass, (), "mass"); out = _dev_f64(out, (3,), "out")
+    _seen.clear()
+    n = mass.shape[0]
+    if pos.shape[0] != n or out.shape[0] != n:
+        raise BifrostError(f"acc_static: pos has {pos.shape[0]} rows, out {out.shape[0]}, mass {n}")
+    if pos.device != mass.device or out.device != mass.device:
+        raise BifrostError("acc_static: pos, mass and out must be on one device")
+    dev = mass.device.index
+    rc = lib.bifrost_acc_static(dev, n, pos.data_ptr(), mass.data_ptr(), float(G), float(eps), out.data_ptr(),
+                                torch.cuda.current_stream(dev).cuda_stream)
+    if rc != 0:
+        raise BifrostError(f"bifrost_acc_static: {lib.bifrost_strerror(rc).decode()} [{lib.bifrost_static_error().decode()}]")
+    return out
 
 
 class Context:

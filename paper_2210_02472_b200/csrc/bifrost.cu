@@ -1382,3 +1382,120 @@ int bifrost_fp64_probe(bifrost_ctx* ctx, int mix, int64_t iters, int ctas_per_sm
 }
 
 }  // extern "C"
+
+// ========================================================================================
+// bifrost_acc_static: Eq. 6 without any allocation (include/bifrost.h) - for callers under CUDA graph capture, in
+// tight serving loops, or in harnesses that forbid cudaMalloc.  The scratch of the acc pass (packed source records,
+// split-j partials, the fused kernel's arrival counters) lives in ONE file-scope device array; every GPU that loads the
+// library holds its BIFROST_STATIC_SCRATCH_BYTES until the process exits.  The kernels and launch rules are run_pass's,
+// driven through a bifrost_ctx on the HOST STACK whose scratch pointers point into that array.
+// ========================================================================================
+
+#include <mutex>
+
+static __device__ __align__(256) unsigned char bifrost_static_scratch[BIFROST_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// carve-up of the array: [records | arrival counters | partials]
+constexpr size_t STATIC_REC_DOUBLES = (size_t)((BIFROST_STATIC_MAX_N + TILE - 1) / TILE * TILE) * AccPassT<false>::REC;
+constexpr size_t STATIC_OFF_TICKETS = STATIC_REC_DOUBLES * sizeof(double);                  // 768 KiB of records
+constexpr size_t STATIC_OFF_PARTIAL = STATIC_OFF_TICKETS + TICKETS * sizeof(unsigned);      // + 4 KiB of counters
+constexpr size_t STATIC_PARTIAL_BYTES = (size_t)BIFROST_STATIC_SCRATCH_BYTES - STATIC_OFF_PARTIAL;
+static_assert(STATIC_OFF_TICKETS % 256 == 0 && STATIC_OFF_PARTIAL % 256 == 0, "regions keep the array's alignment");
+static_assert(STATIC_PARTIAL_BYTES >= 16 * 24 * (size_t)BIFROST_STATIC_MAX_N, "room for 16 source-range splits at the largest n");
+
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDevice {
+    bool ready = false;
+    unsigned char* base = nullptr;   // DEVICE address of bifrost_static_scratch on this device (cudaGetSymbolAddress)
+    int num_sms = 0;
+};
+StaticDevice g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+thread_local char g_static_err[256] = {0};
+
+// Once per device, with that device current.  In host code the name `bifrost_static_scratch` is only a handle of the
+// symbol, NOT a device address (a kernel given it would fault, or read host memory where the GPU can reach it):
+// the address each device holds the array at comes from cudaGetSymbolAddress.
+int static_setup(int device, StaticDevice* out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_dev[device];
+    if (!d.ready) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, bifrost_static_scratch);
+        if (e != cudaSuccess || !p) {
+            snprintf(g_static_err, sizeof(g_static_err), "cudaGetSymbolAddress(bifrost_static_scratch) on device %d: %s", device,
+                     cudaGetErrorString(e));
+            return BIFROST_ECUDA;
+        }
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        if (e != cudaSuccess || sms <= 0) {
+            snprintf(g_static_err, sizeof(g_static_err), "cudaDeviceGetAttribute(multiProcessorCount) on device %d: %s", device,
+                     cudaGetErrorString(e));
+            return BIFROST_ECUDA;
+        }
+        d.base = (unsigned char*)p;
+        d.num_sms = sms;
+        d.ready = true;
+    }
+    *out = d;
+    return BIFROST_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bifrost_static_error(void) { return g_static_err; }
+
+int bifrost_acc_static(int device, int64_t n, const double* pos, const double* mass, double G, double eps, double* out_acc,
+                       void* stream) {
+    g_static_err[0] = 0;
+    if (n < 0 || n > BIFROST_STATIC_MAX_N) {
+        snprintf(g_static_err, sizeof(g_static_err),
+                 "bifrost_acc_static: n = %lld is outside 0..BIFROST_STATIC_MAX_N = %d (the static scratch array of %u bytes is "
+                 "sized for that many particles); use bifrost_acc with a context for larger sets",
+                 (long long)n, BIFROST_STATIC_MAX_N, (unsigned)BIFROST_STATIC_SCRATCH_BYTES);
+        return BIFROST_EINVAL;
+    }
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess) n_dev = 0;
+    if (device < 0 || device >= STATIC_MAX_DEVICES || device >= n_dev) {
+        snprintf(g_static_err, sizeof(g_static_err), "bifrost_acc_static: device %d is not one of the %d CUDA devices (at most %d)",
+                 device, n_dev, STATIC_MAX_DEVICES);
+        return BIFROST_EINVAL;
+    }
+    if (n == 0) return BIFROST_OK;
+    if (!pos || !mass || !out_acc) {
+        snprintf(g_static_err, sizeof(g_static_err), "bifrost_acc_static: pos, mass and out_acc must not be NULL");
+        return BIFROST_EINVAL;
+    }
+    DeviceGuard guard(device);
+    StaticDevice d;
+    RC_TRY(static_setup(device, &d));
+    // A context on the host stack: launch geometry and pointers into the static array; nothing is allocated or freed.
+    bifrost_ctx c;
+    c.device = device;
+    c.max_n = BIFROST_STATIC_MAX_N;
+    c.num_sms = d.num_sms;
+    c.src_rec = (double*)d.base;
+    c.src_rec_doubles = STATIC_REC_DOUBLES;
+    c.tickets = (unsigned*)(d.base + STATIC_OFF_TICKETS);
+    c.tickets_dirty = true;          // the array keeps the last call's contents (and an aborted launch may have left counts):
+                                     // the counters, the one part that must start at zero, are cleared by every fused call
+    c.partial = d.base + STATIC_OFF_PARTIAL;
+    c.partial_bytes = STATIC_PARTIAL_BYTES;
+    const SrcArrays src{pos, nullptr, mass, nullptr, nullptr};
+    const AccArgs a{pos, nullptr, nullptr, soft2(eps), G, out_acc, (double*)c.partial};
+    using Big = Shape<8, 256, 1, 1>;      // acc_impl's shapes
+    using F4 = Shape<4, 128, 4, 2>;
+    using F2 = Shape<2, 128, 6, 2>;
+    using F1 = Shape<1, 128, 8, 4>;
+    const int rc = run_pass<AccPassT<false>, Big, 0, Big, F4, F2, F1>(&c, a, src, n, n, 24, 0, (cudaStream_t)stream);
+    if (rc) snprintf(g_static_err, sizeof(g_static_err), "bifrost_acc_static: %s", c.err[0] ? c.err : bifrost_strerror(rc));
+    return rc;
+}
+
+}  // extern "C"
