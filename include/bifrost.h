@@ -47,7 +47,8 @@
  *  - One context per stream; concurrent calls on one context are not allowed.
  *  - Results are bit-identical for identical inputs on the same GPU model: tiling is fixed by
  *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
- *  - Launch shapes are chosen from the argument sizes alone: below 4096 sinks a call is one
+ *  - Launch shapes are chosen from the argument sizes alone: at most 32 sinks (and a bounded number of
+ *    pairs) are one thread-block-cluster launch with the threads over the sources; below 4096 sinks a call is one
  *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish;
  *    bifrost_acc / bifrost_grad / bifrost_dtmin whose sink and source lists are the SAME list (same
  *    pointer, or both NULL) of >= 16384 / 12288 / 40960 entries evaluate every unordered pair once
@@ -113,6 +114,10 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
 #define BIFROST_TUNE_SYM_MIN_N       2
 #define BIFROST_TUNE_MUTUAL_MIN_PAIRS 3   /* bifrost_*_mutual: fewest n_a * n_b pairs for the two-list symmetric kernel
                                              (default 5e7, and >= 512 entries in the shorter list; 0 = always) */
+#define BIFROST_TUNE_FEW_MAX_SINKS 4      /* calls with at most this many sinks (default 32, 0..32; 0 disables) and at most */
+#define BIFROST_TUNE_FEW_MAX_PAIRS 5      /* this many sink-source pairs (default 2^19 for acc, 2^18 for grad and dtmin; the knob sets
+                                             all three; doubled for <= 8 sinks) run as ONE thread-block-cluster launch: threads
+                                             over the sources, results merged through distributed shared memory, no workspace */
 int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value);
 
 const char* bifrost_strerror(int code);                 /* static string */

@@ -44,6 +44,7 @@
 #include "pair_kernels.cuh"
 #include "sym_kernels.cuh"
 #include "sym_dt.cuh"
+#include "few_sinks.cuh"
 #include "epilogues.cuh"
 #include "pn1.cuh"
 #include "subsystems.cuh"
@@ -75,6 +76,11 @@ struct bifrost_ctx {
     int shard_rank = 0, shard_world = 1;   // bifrost_set_shard: which blocks of the symmetric kernels this context evaluates
     double* sym_ws = nullptr;        // source-side rows of the symmetric (every pair once) kernels, [block][source][3]
     size_t sym_ws_bytes = 0;
+    int64_t few_max_sinks = 32;      // at most this many sinks, and at most few_max_pairs pairs: ONE cluster launch of few_sinks_kernel
+    double few_max_pairs[3] = {524288.0, 262144.0, 262144.0};   // (acc, grad, dtmin; BIFROST_TUNE_FEW_MAX_SINKS / _FEW_MAX_PAIRS; 0 sinks
+                                     // disables; measured: profiles/r2_sweep_small_sets.md)
+    int few_pairs_per_thread = 4;    // the cluster grows (1, 2, .. few_max_cl CTAs) until a thread has at most this many pairs
+    int few_max_cl[3] = {0, 0, 0};   // largest cluster the device accepts for the acc / grad / dtmin instance (0: not asked yet)
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
     int64_t sym_min_dt = 40960;      // shortest list for the symmetric dtmin (cross-over near 32768; BIFROST_TUNE_SYM_MIN_N sets it too)
@@ -274,6 +280,49 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
     return BIFROST_OK;
 }
 
+// A handful of sinks (few_sinks.cuh): one thread-block cluster, threads over the sources, results merged through shared and
+// distributed shared memory - no workspace, one launch.  Returns 1 when the call does not qualify.
+template <class F, int WHICH>
+int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src, int compact,
+             cudaStream_t st) {
+    if (n_sink < 1 || n_sink > ctx->few_max_sinks || n_sink > FEW_MAX_SINKS || ctx->shard_world > 1) return 1;
+    // measured cross-over against the fused kernel (profiles/r2_sweep_small_sets.md): 2^19 pairs for acc, 2^18 for grad and dtmin,
+    // twice that for at most 8 sinks (long source lists, where the fused kernel's 128-way split pays its reduction)
+    if ((double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 2.0 : 1.0)) return 1;
+    auto kern = few_sinks_kernel<F>;
+    if (ctx->few_max_cl[WHICH] == 0) {          // once per context and instance: may a cluster have 16 CTAs here?
+        int max_cl = 8;                         // the portable size
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+            cudaLaunchConfig_t q = {};
+            q.gridDim = dim3(FEW_MAX_CL); q.blockDim = dim3(FEW_T);
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = FEW_MAX_CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            q.attrs = at; q.numAttrs = 1;
+            int n_clusters = 0;
+            if (cudaOccupancyMaxActiveClusters(&n_clusters, kern, &q) == cudaSuccess && n_clusters >= 1) max_cl = FEW_MAX_CL;
+        }
+        (void)cudaGetLastError();
+        ctx->few_max_cl[WHICH] = max_cl;
+    }
+    int nsp = 1;
+    while (nsp < n_sink) nsp *= 2;
+    const int n_tiles = ceil_div(n_src, FEW_T);
+    int cl = 1;
+    while (cl * 2 <= ctx->few_max_cl[WHICH] && cl * 2 <= n_tiles &&
+           (int64_t)cl * FEW_T * ctx->few_pairs_per_thread < (int64_t)nsp * n_src)
+        cl *= 2;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cl); cfg.blockDim = dim3(FEW_T); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    CU_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, a, src, (int)n_sink, (int)n_src, nsp, compact));
+    ctx->launches++;
+    return BIFROST_OK;
+}
+
 // acc / grad over one list that is both sink and source set, every pair once (sym_kernels.cuh).
 // Returns 1 when the call does not qualify (list too short, workspace too small): the caller then takes the plain path.
 constexpr int SYM_ACC_BS = 8 * 256, SYM_GRAD_BS = 6 * 256;   // sinks per CTA of the two symmetric shapes (sym_impl callers)
@@ -370,6 +419,10 @@ int acc_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass,
     }
     const SrcArrays src{pos, nullptr, mass, sub, src_idx};
     const AccArgs a{pos, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial};
+    if (!sub) {                                             // a handful of sinks: one cluster launch
+        const int rc = few_impl<FewAcc, 0>(ctx, a, src, n_sink, n_src, compact, st);
+        if (rc <= 0) return rc;
+    }
     using Big = Shape<8, 256, 1, 1>;
     using F4 = Shape<4, 128, 4, 2>;
     using F2 = Shape<2, 128, 6, 2>;
@@ -390,6 +443,10 @@ int grad_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* mass
     }
     const SrcArrays src{pos, acc, mass, sub, src_idx};
     const GradArgs a{pos, acc, sub, sink_idx, soft2(eps), G, out, (double*)ctx->partial, nullptr, nullptr};
+    if (!sub) {
+        const int rc = few_impl<FewGrad, 1>(ctx, a, src, n_sink, n_src, compact, st);
+        if (rc <= 0) return rc;
+    }
     using Huge = Shape<5, 128, 2, 2>;     // phase-major (GradPassT::pairs), 1.6 % faster per pair than Big
     using Big = Shape<4, 256, 1, 2>;
     using F4 = Shape<4, 128, 3, 2>;
@@ -509,6 +566,13 @@ int dtmin_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* vel
     if (n_sink == 0) return BIFROST_OK;
     if (!ng && !sub && sink_idx == src_idx && n_sink == n_src) {   // one list on both sides: every pair once
         const int rc = sym_dt_impl(ctx, pos, vel, mass, sink_idx, n_sink, G, eta_ff, eta_fb, dt_ff, dt_fb, j_ff, j_fb, compact, st);
+        if (rc <= 0) return rc;
+    }
+    if (!ng && !sub) {                                      // a handful of sinks: one cluster launch, exact time-steps for every pair
+        const DtArgs fa{pos, vel, mass, nullptr, sink_idx, src_idx, (int)n_src, nullptr, nullptr, G, eta_ff, eta_fb,
+                        dt_ff, dt_fb, j_ff, j_fb, NgbArgs{}};
+        const SrcArrays fsrc{pos, vel, mass, nullptr, src_idx};
+        const int rc = few_impl<FewDt, 2>(ctx, fa, fsrc, n_sink, n_src, compact, st);
         if (rc <= 0) return rc;
     }
     // workspace per sink and split: 16 B of time-steps, 8 B of ids [, 4 B neighbour count + 4 cap B of list]; the regions
@@ -878,6 +942,11 @@ int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
             ctx->sym_min_acc = ctx->sym_min_grad = ctx->sym_min_dt = value; return BIFROST_OK;
         case BIFROST_TUNE_MUTUAL_MIN_PAIRS:
             ctx->mutual_min_pairs = (double)value; ctx->mutual_min_b = value == 0 ? 1 : 512; return BIFROST_OK;
+        case BIFROST_TUNE_FEW_MAX_SINKS:
+            if (value > FEW_MAX_SINKS) return BIFROST_EINVAL;
+            ctx->few_max_sinks = value; return BIFROST_OK;
+        case BIFROST_TUNE_FEW_MAX_PAIRS:
+            ctx->few_max_pairs[0] = ctx->few_max_pairs[1] = ctx->few_max_pairs[2] = (double)value; return BIFROST_OK;
         default: return BIFROST_EINVAL;
     }
 }

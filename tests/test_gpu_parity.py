@@ -749,7 +749,8 @@ def test_small_level_single_launch_equals_the_general_path_bit_for_bit(torch, ct
     idx = rng.permutation(w.n)[:m].astype(np.int32)          # unsorted on purpose
     general = Context(w.n)
     general.set_tuning(Context.TUNE_SMALL_M, 0)
-    try:
+    general.set_tuning(Context.TUNE_FEW_MAX_SINKS, 0)        # the fused kernel's summation order (the cluster kernel for <= 32
+    try:                                                     # sinks adds in another order: equal to rounding, not to the bit)
         out = []
         for c in (ctx, general):
             pos, vel, mass = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass)
@@ -1252,3 +1253,112 @@ def test_symmetric_dtmin_list_ties_and_zero_velocity(torch, ctx_sym):
     d = ctx_sym.dtmin(dev(torch, wl.pos), torch.zeros_like(dev(torch, wl.vel)), dev(torch, wl.mass), wl.G, wl.eta_ff, wl.eta_fb)
     assert torch.isinf(d[1]).all() and bool((d[3] == -1).all())
     assert np.array_equal(d[2].cpu().numpy(), ref["j_ff"])
+
+
+# ---- a handful of sinks: one thread-block-cluster launch (few_sinks.cuh) -------------------------------------
+
+@pytest.fixture(scope="module")
+def ctx_nofew(torch):
+    """The same calls with the few-sinks kernel switched off (the fused kernel), for comparisons."""
+    from paper_2210_02472_b200.binding import Context
+    c = Context(1 << 17)
+    c.set_tuning(Context.TUNE_FEW_MAX_SINKS, 0)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("n_sink,n_src", [(1, 16384), (2, 16384), (3, 5000), (5, 257), (8, 256), (13, 1), (17, 16384),
+                                          (31, 777), (32, 16384), (1, 131072), (4, 131072), (7, 0)])
+def test_few_sinks_cluster_kernel(torch, ctx, ctx_nofew, n_sink, n_src):
+    """at most 32 sinks (and at most 2^19 pairs; 2^18 for grad) run as ONE cluster launch with the threads
+    over the sources.  Against the oracle at the gates (time-steps and argmin bit-identical), rows of other particles
+    untouched, one launch per call, and dtmin bit-identical to the fused kernel's."""
+    w = workload(3) if n_src > 16384 else workload(2)
+    rng = np.random.default_rng(1000 * n_sink + n_src)
+    sinks = np.sort(rng.choice(w.n, n_sink, replace=False)).astype(np.int32)
+    srcs = None if n_src == w.n else rng.permutation(w.n)[:n_src].astype(np.int32)
+    if srcs is not None and n_src >= 2:
+        srcs[: min(n_sink, n_src) // 2] = sinks[: min(n_sink, n_src) // 2]       # some sinks are their own sources
+    acc_full = oracle.acc(w.pos, w.mass, w.G, w.eps)
+    l0 = ctx.launch_count
+    a, c, d, _ = run_all(torch, ctx, w, sinks, srcs, acc_full=acc_full)
+    assert ctx.launch_count - l0 == 3        # acc, grad, dtmin: one launch each (grad beyond 2^18 pairs: the fused kernel)
+    if n_src == 0:
+        assert (a == 0).all() and (c == 0).all() and np.isinf(d[0]).all() and np.isinf(d[1]).all() and (d[2] == -1).all()
+        return
+    if n_sink * n_src >= 64:
+        check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), "few acc")
+        check_vec(c, oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sinks, srcs), "few grad")
+    else:                                  # a sum of one or a few terms: compare row by row
+        ra, rc = oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sinks, srcs)
+        assert np.abs(a - ra).max() <= 1e-12 * np.abs(ra).max() and np.abs(c - rc).max() <= 1e-12 * np.abs(rc).max()
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs), "few dtmin")
+    a2, c2, d2, _ = run_all(torch, ctx_nofew, w, sinks, srcs, acc_full=acc_full)
+    assert all(np.array_equal(x, y) for x, y in zip(d, d2))
+    assert np.abs(a - a2).max() <= 1e-13 * np.abs(a2).max() and np.abs(c - c2).max() <= 1e-13 * np.abs(c2).max()
+    # untouched rows and bit-reproducibility
+    pos, vel, mass, si = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    out = torch.full((w.n, 3), 7.0, dtype=torch.float64, device="cuda")
+    ctx.acc(pos, mass, w.G, w.eps, si, sj, out=out)
+    rest = np.ones(w.n, bool); rest[sinks] = False
+    assert (out.cpu().numpy()[rest] == 7.0).all() and np.array_equal(out.cpu().numpy()[sinks], a)
+
+
+@pytest.mark.parametrize("n_sink", [32, 33])
+def test_few_sinks_switch_points(torch, ctx, ctx_nofew, n_sink):
+    """32 sinks take the cluster kernel, 33 the fused kernel; 32 sinks x 16385 sources exceed the pair limit.  All agree."""
+    from paper_2210_02472_b200.binding import Context
+    w = workload(3)
+    sinks = np.sort(np.random.default_rng(n_sink).choice(w.n, n_sink, replace=False)).astype(np.int32)
+    for n_src in (8192, 16384, 16385):
+        srcs = np.arange(n_src, dtype=np.int32)
+        a, c, d, acc_in = run_all(torch, ctx, w, sinks, srcs)
+        a2, c2, d2, _ = run_all(torch, ctx_nofew, w, sinks, srcs, acc_full=acc_in)
+        check_vec(a, a2, "acc across the switch", tol=1e-13)
+        check_vec(c, c2, "grad across the switch", tol=1e-13)
+        assert all(np.array_equal(x, y) for x, y in zip(d, d2))
+    c3 = Context(w.n)
+    try:
+        c3.set_tuning(Context.TUNE_FEW_MAX_SINKS, 8)
+        with pytest.raises(Exception):
+            c3.set_tuning(Context.TUNE_FEW_MAX_SINKS, 33)
+    finally:
+        c3.close()
+
+
+def test_few_sinks_exact_ties_zero_velocity_and_coincident(torch, ctx):
+    """The cluster kernel on exactly tied inputs: a lattice (every tie to the smaller id - the flagged sinks are settled by
+    the exact scan), all velocities zero (+inf / -1 for Eq. 22), two coincident particles at eps = 0 (reading A3b)."""
+    g = np.arange(6)
+    lat = np.array([[x, y, z] for x in g for y in g for z in g], dtype=np.float64) * 0.25
+    lat = lat[np.random.default_rng(5).permutation(lat.shape[0])]
+    lv = np.sign(lat - 0.625) * lat * lat * 0.5
+    wl = W.Workload("lattice", lat, lv, np.full(lat.shape[0], 2.0 ** -7), 1.0, 0.0, 0.5, 0.25)
+    pos, vel, mass = dev(torch, wl.pos), dev(torch, wl.vel), dev(torch, wl.mass)
+    for n_sink in (1, 6, 32):
+        sinks = np.sort(np.random.default_rng(n_sink).choice(wl.n, n_sink, replace=False)).astype(np.int32)
+        ref = oracle.dtmin(wl.pos, wl.vel, wl.mass, wl.G, wl.eta_ff, wl.eta_fb, sinks, None)
+        assert n_sink == 1 or ((ref["margin_ff"] == 0).any() and (ref["margin_fb"] == 0).any())
+        d = ctx.dtmin(pos, vel, mass, wl.G, wl.eta_ff, wl.eta_fb, dev(torch, sinks))
+        check_dt(tuple(t.cpu().numpy()[sinks] for t in d), ref, f"few dtmin lattice {n_sink}")
+        d0 = ctx.dtmin(pos, torch.zeros_like(vel), mass, wl.G, wl.eta_ff, wl.eta_fb, dev(torch, sinks))
+        assert torch.isinf(d0[1][dev(torch, sinks).long()]).all() and bool((d0[3][dev(torch, sinks).long()] == -1).all())
+        assert np.array_equal(d0[2].cpu().numpy()[sinks], ref["j_ff"])
+    w = _small(600, 77)
+    w.pos[400] = w.pos[11]
+    sinks = np.array([3, 11, 250, 400], dtype=np.int32)
+    pos, vel, mass, si = dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), dev(torch, sinks)
+    a = ctx.acc(pos, mass, w.G, 0.0, si).cpu().numpy()
+    assert np.isfinite(a[sinks]).all()
+    with np.errstate(all="ignore"):
+        check_vec(a[[3, 250]], oracle.acc(w.pos, w.mass, w.G, 0.0, sink_idx=np.array([3, 250], dtype=np.int32)), "few acc, other sinks")
+    for i, j in ((11, 400), (400, 11)):           # the coincident pair contributes exactly 0
+        src = np.array([k for k in range(w.n) if k != j], dtype=np.int32)
+        ref = oracle.acc(w.pos, w.mass, w.G, 0.0, sink_idx=np.array([i], dtype=np.int32), src_idx=src)
+        assert np.abs(a[i] - ref[0]).max() <= 1e-12 * np.abs(ref[0]).max()
+    dff, dfb, jff, jfb = (t.cpu().numpy() for t in ctx.dtmin(pos, vel, mass, w.G, 0.02, 0.03, si))
+    assert dff[11] == 0.0 and dff[400] == 0.0 and jff[11] == 400 and jff[400] == 11 and dfb[11] == 0.0 and jfb[11] == 400
+    others = np.array([3, 250], dtype=np.int32)
+    check_dt(tuple(x[others] for x in (dff, dfb, jff, jfb)), oracle.dtmin(w.pos, w.vel, w.mass, w.G, 0.02, 0.03, sink_idx=others),
+             "few dtmin, other sinks")
