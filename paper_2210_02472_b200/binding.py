@@ -218,7 +218,7 @@ class Context:
             raise BifrostError(f"{what}: {msg}" + (f" [{cu}]" if cu else ""))
 
     RESERVE_HOST, RESERVE_INTEGRATOR = 1, 2
-    TUNE_FUSED_MAX_SINKS, TUNE_SMALL_M, TUNE_SYM_MIN_N, TUNE_MUTUAL_MIN_PAIRS, TUNE_FEW_MAX_SINKS, TUNE_FEW_MAX_PAIRS = 0, 1, 2, 3, 4, 5
+    TUNE_FUSED_MAX_SINKS, TUNE_SMALL_M, TUNE_SYM_MIN_N, TUNE_MUTUAL_MIN_PAIRS, TUNE_FEW_MAX_SINKS, TUNE_FEW_MAX_PAIRS, TUNE_FUSED_CLUSTER = 0, 1, 2, 3, 4, 5, 6
 
     def reserve(self, what: int):
         self._check(self._lib.bifrost_reserve(self._h, int(what)), "bifrost_reserve")

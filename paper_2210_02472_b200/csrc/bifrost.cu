@@ -81,6 +81,7 @@ struct bifrost_ctx {
                                      // disables; measured: profiles/r2_sweep_small_sets.md)
     int few_pairs_per_thread = 4;    // the cluster grows (1, 2, .. few_max_cl CTAs) until a thread has at most this many pairs
     int few_max_cl[3] = {0, 0, 0};   // largest cluster the device accepts for the acc / grad / dtmin instance (0: not asked yet)
+    bool fused_cluster = true;       // pair_fused_kernel as clusters with a DSMEM reduction (BIFROST_TUNE_FUSED_CLUSTER: 0 / 1)
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
     int64_t sym_min_dt = 40960;      // shortest list for the symmetric dtmin (cross-over near 32768; BIFROST_TUNE_SYM_MIN_N sets it too)
@@ -207,12 +208,29 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
         CU_TRY(ctx, cudaMemsetAsync(ctx->tickets, 0, TICKETS * sizeof(unsigned), st));
         ctx->tickets_dirty = false;
     }
+    // vec3 policies with a split source range: clusters of up to 8 CTAs along the split axis add their partials through
+    // distributed shared memory (pair_fused_kernel); grid.y is padded to a multiple of the cluster size with CTAs that find
+    // no tiles and add zeros
+    // Clusters hold their CTAs' slots until the whole cluster is done and need 8 free slots in one GPC at a time, which costs
+    // ~10-15 % of a long launch; they pay when the launch is short: at most 2 tiles per CTA, or no more CTAs than the
+    // GPU holds at once (measured: config 2, 33-4095 sinks acc -3 .. -10 us, grad -2 .. -9 us; config 3 beyond one wave: slower).
+    int cl = 1;
+    const bool short_launch = g.tiles_per_split <= 2 || (int64_t)grid.x * g.n_split <= (int64_t)ctx->num_sms * Sh::MINB;
+    if (P::CLUSTER_REDUCE && ctx->fused_cluster && g.n_split >= 2 && short_launch) {
+        cl = g.n_split >= 8 ? 8 : g.n_split >= 4 ? 4 : 2;
+        grid.y = (unsigned)(ceil_div(g.n_split, cl) * cl);
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(Sh::T); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = cl; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = cl > 1 ? 1 : 0;
     if (g.tiles_per_split < DT_SHORT_TILES)      // short source range per CTA: the policy's variant for it (dtmin)
-        pair_fused_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+        CU_TRY(ctx, cudaLaunchKernelEx(&cfg, pair_fused_kernel<typename P::Short, Sh::S, Sh::T, Sh::MINB, Sh::UNR>, a, g, src, ctx->tickets));
     else
-        pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR><<<grid, Sh::T, 0, st>>>(a, g, src, ctx->tickets);
+        CU_TRY(ctx, cudaLaunchKernelEx(&cfg, pair_fused_kernel<P, Sh::S, Sh::T, Sh::MINB, Sh::UNR>, a, g, src, ctx->tickets));
     ctx->launches++;
-    CU_TRY(ctx, cudaGetLastError());
     return BIFROST_OK;
 }
 
@@ -945,6 +963,9 @@ int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
         case BIFROST_TUNE_FEW_MAX_SINKS:
             if (value > FEW_MAX_SINKS) return BIFROST_EINVAL;
             ctx->few_max_sinks = value; return BIFROST_OK;
+        case BIFROST_TUNE_FUSED_CLUSTER:
+            if (value > 1) return BIFROST_EINVAL;
+            ctx->fused_cluster = value != 0; return BIFROST_OK;
         case BIFROST_TUNE_FEW_MAX_PAIRS:
             ctx->few_max_pairs[0] = ctx->few_max_pairs[1] = ctx->few_max_pairs[2] = (double)value; return BIFROST_OK;
         default: return BIFROST_EINVAL;

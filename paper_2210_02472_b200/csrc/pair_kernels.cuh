@@ -2,6 +2,8 @@
 // Part of the single translation unit bifrost.cu (see its header and DESIGN.md); not a public header.
 #pragma once
 
+#include <cooperative_groups.h>
+
 namespace {
 
 // All S sinks of a thread against one source record.  A policy may provide a phase-major
@@ -123,6 +125,13 @@ __global__ void finish_kernel(const typename P::Args a, const Geom g) {
 // partials in split order - so the result does not depend on which CTA that is (deterministic) and
 // no second or third launch is needed.
 // ----------------------------------------------------------------------------------------
+// shared memory for the cluster reduction of pair_fused_kernel: 3 doubles per sink of the CTA for the policies that use it
+template <class P, int S, int T>
+__device__ __forceinline__ double* part_sm_of() {
+    __shared__ double part_sm[P::CLUSTER_REDUCE ? 3 * T * S : 1];
+    return part_sm;
+}
+
 template <class P, int S, int T, int MINB, int UNR>
 __global__ void __launch_bounds__(T, MINB)
 pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, unsigned* __restrict__ ticket) {
@@ -178,10 +187,42 @@ pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, u
         if (more) emit_tile(buf ^ 1);
     }
 
+    // Launched as thread-block clusters along blockIdx.y (launch_fused, vec3 policies): the CTAs of a cluster add their
+    // partials through DISTRIBUTED SHARED MEMORY in rank order - CTA r takes every cl-th double of the block's n_local x 3 -
+    // and only one partial per cluster goes to global memory.  The last CTA's reduction, a chain of L2 round trips per
+    // split (10 us for 128 splits), then runs over gridDim.y / cl entries; with one cluster per sink block there is no
+    // global partial, no ticket and no fence at all.
+    int n_part = g.n_split;                    // entries of the [.][n_sink] partial workspace the last CTA adds
+    bool stored = false;
+    if constexpr (P::CLUSTER_REDUCE) {
+        cooperative_groups::cluster_group cluster = cooperative_groups::this_cluster();
+        const int cl = (int)cluster.dim_blocks().y;
+        if (cl > 1) {
+            stored = true;
+            double* part_sm = part_sm_of<P, S, T>();
 #pragma unroll
-    for (int s = 0; s < S; ++s) {
-        const int k = kbase + s * T;
-        if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
+            for (int s = 0; s < S; ++s) P::vec3(accu[s], part_sm + 3 * (threadIdx.x + s * T));
+            cluster.sync();
+            const int r = (int)cluster.block_rank(), base = blockIdx.x * (T * S);
+            const int n_doubles = 3 * min(T * S, g.n_sink - base);
+            n_part = gridDim.y / cl;
+            for (int e = r + cl * threadIdx.x; e < n_doubles; e += cl * T) {
+                double sum = 0.0;
+                for (int q = 0; q < cl; ++q) sum += *cluster.map_shared_rank(part_sm + e, q);
+                const int k = base + e / 3, c = e % 3;
+                if (n_part == 1) a.out[3 * (size_t)(g.compact ? k : (a.sink_idx ? a.sink_idx[k] : k)) + c] = a.G * sum;
+                else a.partial[3 * ((size_t)(blockIdx.y / cl) * g.n_sink + k) + c] = sum;
+            }
+            cluster.sync();                    // shared memory must outlive the other CTAs' reads
+            if (n_part == 1) return;
+        }
+    }
+    if (!stored) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const int k = kbase + s * T;
+            if (k < g.n_sink) P::store(a, g, blockIdx.y, k, ids[s], sink[s], accu[s]);
+        }
     }
     if (g.n_split == 1) {
         if (P::ALWAYS_FINISH) {                // a thread finishes the sinks it stored itself
@@ -203,6 +244,8 @@ pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, u
     if (!s_last) return;
     __threadfence();
     // the last CTA reduces: L lanes per sink when this CTA's sinks leave threads to spare
+    Geom gf = g;
+    gf.n_split = n_part;
     const int base = blockIdx.x * (T * S);
     const int n_local = min(T * S, g.n_sink - base);
     int L = 1;
@@ -211,13 +254,13 @@ pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, u
 #pragma unroll
         for (int s = 0; s < S; ++s) {
             const int k = kbase + s * T;
-            if (k < g.n_sink) P::finish(a, g, k, ids[s], 0, 1, true);
+            if (k < g.n_sink) P::finish(a, gf, k, ids[s], 0, 1, true);
         }
     } else {
         const int q = threadIdx.x / L;
         const bool live = q < n_local;
         const int k = base + (live ? q : 0);
-        P::finish(a, g, k, a.sink_idx ? a.sink_idx[k] : k, threadIdx.x % L, L, live);
+        P::finish(a, gf, k, a.sink_idx ? a.sink_idx[k] : k, threadIdx.x % L, L, live);
     }
     if (threadIdx.x == 0) ticket[blockIdx.x] = 0;
 }

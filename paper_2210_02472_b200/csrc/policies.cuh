@@ -140,6 +140,10 @@ struct AccPassT {
         }
     }
     static constexpr bool ALWAYS_FINISH = false;
+    // the split-j partial of a sink is three doubles that add: pair_fused_kernel may add the partials of the CTAs of a
+    // thread-block cluster through distributed shared memory before anything goes to global memory
+    static constexpr bool CLUSTER_REDUCE = true;
+    __device__ __forceinline__ static void vec3(const Acc& c, double* v) { v[0] = c.x; v[1] = c.y; v[2] = c.z; }
     __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
         finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
     }
@@ -264,6 +268,10 @@ struct GradPassT {
         }
     }
     static constexpr bool ALWAYS_FINISH = false;
+    static constexpr bool CLUSTER_REDUCE = !WITH_ACC;       // (see AccPassT; the acc + jerk pass has two partials per sink)
+    __device__ __forceinline__ static void vec3(const Acc& c, double* v) {
+        v[0] = fma(-3.0, c.wx, c.ux); v[1] = fma(-3.0, c.wy, c.uy); v[2] = fma(-3.0, c.wz, c.uz);     // as store()
+    }
     __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
         finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
         if (WITH_ACC) finish_vec3(a.partial2, a.out2, a.G, g, k, id, lane, L, write);
@@ -577,6 +585,8 @@ struct DtPassT {
     // decides, a near-tie is decided on the exact time-steps - then Eq. 21 / Eq. 22 for the winning pair in IEEE operations
     // in the oracle's order.  The winner is the exact (time-step, id) minimum, so the order of the splits does not matter.
     static constexpr bool ALWAYS_FINISH = true;
+    static constexpr bool CLUSTER_REDUCE = false;
+    __device__ __forceinline__ static void vec3(const Acc&, double*) {}
     __device__ __forceinline__ static void merge(const Args& a, int i, int w, double key, int j, double& kb, int& jb) {
         const bool clear = (j >= 0) & ((key * KEY_SLACK > kb) | (jb < 0));
         const bool near = (j >= 0) & !clear & (key >= kb * KEY_SLACK) & (j != jb);
@@ -726,6 +736,8 @@ struct PotPassT {
         else a.partial[(size_t)split * g.n_sink + k] = c.p;
     }
     static constexpr bool ALWAYS_FINISH = false;
+    static constexpr bool CLUSTER_REDUCE = false;
+    __device__ __forceinline__ static void vec3(const Acc&, double*) {}
     __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
         double s = 0.0;
         for (int q = lane; q < g.n_split; q += L) s += __ldcg(a.partial + (size_t)q * g.n_sink + k);     // fixed order

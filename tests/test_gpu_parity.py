@@ -1362,3 +1362,45 @@ def test_few_sinks_exact_ties_zero_velocity_and_coincident(torch, ctx):
     others = np.array([3, 250], dtype=np.int32)
     check_dt(tuple(x[others] for x in (dff, dfb, jff, jfb)), oracle.dtmin(w.pos, w.vel, w.mass, w.G, 0.02, 0.03, sink_idx=others),
              "few dtmin, other sinks")
+
+
+@pytest.mark.parametrize("n_sink,n_src", [(33, 16384), (100, 300), (129, 700), (500, 16384), (1024, 16384), (2048, 5000),
+                                          (4095, 16384), (128, 131072), (40, 129)])
+def test_fused_kernel_cluster_reduction(torch, ctx, n_sink, n_src):
+    """The fused launch of acc / grad as thread-block clusters along the split axis (partials added through distributed
+    shared memory; grid.y padded to a multiple of the cluster size with CTAs that add zeros) against the oracle, and
+    against the same launch without clusters (BIFROST_TUNE_FUSED_CLUSTER = 0): equal to rounding."""
+    from paper_2210_02472_b200.binding import Context
+    w = workload(3) if n_src > 16384 else workload(2)
+    rng = np.random.default_rng(n_sink + 7 * n_src)
+    sinks = np.sort(rng.choice(w.n, n_sink, replace=False)).astype(np.int32)
+    srcs = None if n_src == w.n else rng.permutation(w.n)[:n_src].astype(np.int32)
+    acc_full = oracle.acc(w.pos, w.mass, w.G, w.eps)
+    a, c, d, _ = run_all(torch, ctx, w, sinks, srcs, acc_full=acc_full)
+    check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), "fused cluster acc")
+    check_vec(c, oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sinks, srcs), "fused cluster grad")
+    plain = Context(w.n)
+    plain.set_tuning(Context.TUNE_FUSED_CLUSTER, 0)
+    try:
+        a2, c2, d2, _ = run_all(torch, plain, w, sinks, srcs, acc_full=acc_full)
+    finally:
+        plain.close()
+    check_vec(a, a2, "acc, clusters on / off", tol=1e-13)
+    check_vec(c, c2, "grad, clusters on / off", tol=1e-13)
+    assert all(np.array_equal(x, y) for x, y in zip(d, d2))
+    # bit-reproducible, also in a CUDA graph replay
+    pos, mass, si = dev(torch, w.pos), dev(torch, w.mass), dev(torch, sinks)
+    sj = None if srcs is None else dev(torch, srcs)
+    out = torch.zeros((w.n, 3), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        ctx.acc(pos, mass, w.G, w.eps, si, sj, out=out)
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            ctx.acc(pos, mass, w.G, w.eps, si, sj, out=out)
+        out.zero_()
+        g.replay(); g.replay()
+        st.synchronize()
+    assert np.array_equal(out.cpu().numpy()[sinks], a)
