@@ -211,11 +211,13 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     // vec3 policies with a split source range: clusters of up to 8 CTAs along the split axis add their partials through
     // distributed shared memory (pair_fused_kernel); grid.y is padded to a multiple of the cluster size with CTAs that find
     // no tiles and add zeros
-    // Clusters hold their CTAs' slots until the whole cluster is done and need 8 free slots in one GPC at a time, which costs
-    // ~10-15 % of a long launch; they pay when the launch is short: at most 2 tiles per CTA, or no more CTAs than the
-    // GPU holds at once (measured: config 2, 33-4095 sinks acc -3 .. -10 us, grad -2 .. -9 us; config 3 beyond one wave: slower).
+    // A cluster needs 8 free slots in ONE GPC at the same time (a GPC of 18 SMs x 4 slots holds 9 clusters, not 9.25), so a
+    // grid sized to fill the GPU in one wave spills into a second one (config 3, 1024 sinks, grad: 285 -> 338 us).  Clusters
+    // are used when the launch is short anyway (at most 2 tiles per CTA) or stays below 7/8 of the resident slots
+    // (measured: config 2, 33-4095 sinks: acc -3 .. -10 us, grad -2 .. -9 us; config 3, 128 sinks: acc 54.6 -> 41.3 us).
     int cl = 1;
-    const bool short_launch = g.tiles_per_split <= 2 || (int64_t)grid.x * g.n_split <= (int64_t)ctx->num_sms * Sh::MINB;
+    const int64_t ctas_padded = (int64_t)grid.x * ceil_div(g.n_split, 8) * 8;
+    const bool short_launch = g.tiles_per_split <= 2 || 8 * ctas_padded <= 7 * (int64_t)ctx->num_sms * Sh::MINB;
     if (P::CLUSTER_REDUCE && ctx->fused_cluster && g.n_split >= 2 && short_launch) {
         cl = g.n_split >= 8 ? 8 : g.n_split >= 4 ? 4 : 2;
         grid.y = (unsigned)(ceil_div(g.n_split, cl) * cl);
