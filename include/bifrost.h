@@ -118,9 +118,10 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
 #define BIFROST_TUNE_FEW_MAX_PAIRS 5      /* this many sink-source pairs (default 2^19 for acc, 2^18 for grad and dtmin; the knob sets
                                              all three; doubled for <= 8 sinks) run as ONE thread-block-cluster launch: threads
                                              over the sources, results merged through distributed shared memory, no workspace */
-#define BIFROST_TUNE_FUSED_CLUSTER 6      /* 1 (default): the fused launch of acc / grad / jerk runs as clusters of up to 8 CTAs that add
-                                             their split-j partials through distributed shared memory; 0: every CTA's partial
-                                             goes through global memory (the order of the additions differs, nothing else) */
+#define BIFROST_TUNE_FUSED_CLUSTER 6      /* 1 (default): the fused launch runs as clusters of up to 8 CTAs that combine their split-j
+                                             partials through distributed shared memory (sums for acc / grad / jerk, the winners'
+                                             merge for dtmin); 0: every CTA's partial goes through global memory (the order of
+                                             the additions differs, nothing else; dtmin is bit-identical) */
 int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value);
 
 const char* bifrost_strerror(int code);                 /* static string */

@@ -218,7 +218,7 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     int cl = 1;
     const int64_t ctas_padded = (int64_t)grid.x * ceil_div(g.n_split, 8) * 8;
     const bool short_launch = g.tiles_per_split <= 2 || 8 * ctas_padded <= 7 * (int64_t)ctx->num_sms * Sh::MINB;
-    if (P::CLUSTER_REDUCE && ctx->fused_cluster && g.n_split >= 2 && short_launch) {
+    if ((P::CLUSTER_REDUCE || P::CLUSTER_MERGE) && ctx->fused_cluster && g.n_split >= 2 && short_launch) {
         cl = g.n_split >= 8 ? 8 : g.n_split >= 4 ? 4 : 2;
         grid.y = (unsigned)(ceil_div(g.n_split, cl) * cl);
     }

@@ -128,7 +128,7 @@ __global__ void finish_kernel(const typename P::Args a, const Geom g) {
 // shared memory for the cluster reduction of pair_fused_kernel: 3 doubles per sink of the CTA for the policies that use it
 template <class P, int S, int T>
 __device__ __forceinline__ double* part_sm_of() {
-    __shared__ double part_sm[P::CLUSTER_REDUCE ? 3 * T * S : 1];
+    __shared__ double part_sm[(P::CLUSTER_REDUCE || P::CLUSTER_MERGE) ? 3 * T * S : 1];
     return part_sm;
 }
 
@@ -215,6 +215,51 @@ pair_fused_kernel(const typename P::Args a, const Geom g, const SrcArrays src, u
             }
             cluster.sync();                    // shared memory must outlive the other CTAs' reads
             if (n_part == 1) return;
+        }
+    }
+    // dtmin: the same with the policy's merge (a key clear of the other by the band decides, a near-tie is decided on the exact
+    // time-steps): CTA r of the cluster merges every cl-th sink of the block over the CTAs' winners and writes one entry per
+    // cluster; the last CTA's finish then runs over gridDim.y / cl entries (the exact minimum whatever the order).
+    if constexpr (P::CLUSTER_MERGE) {
+        cooperative_groups::cluster_group cluster = cooperative_groups::this_cluster();
+        const int cl = (int)cluster.dim_blocks().y;
+        if (cl > 1) {
+            stored = true;
+            double* part_sm = part_sm_of<P, S, T>();
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                double kf, kb;
+                int jf, jb;
+                P::partial_of(a, g, blockIdx.y, ids[s], accu[s], kf, kb, jf, jb);
+                double* o = part_sm + 3 * (threadIdx.x + s * T);
+                o[0] = kf; o[1] = kb; o[2] = __hiloint2double(jf, jb);
+            }
+            cluster.sync();
+            const int r = (int)cluster.block_rank(), base = blockIdx.x * (T * S);
+            const int n_local = min(T * S, g.n_sink - base);
+            n_part = gridDim.y / cl;
+            for (int kl = r + cl * threadIdx.x; kl < n_local; kl += cl * T) {
+                double v[8][3];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {                 // all remote reads in flight before the first merge
+                    const double* p = cluster.map_shared_rank(part_sm + 3 * kl, q < cl ? q : 0);
+                    v[q][0] = p[0]; v[q][1] = p[1]; v[q][2] = p[2];
+                }
+                const int k = base + kl, i = a.sink_idx ? a.sink_idx[k] : k;
+                double kb[2] = {0.0, 0.0};
+                int jb[2] = {-1, -1};
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    if (q < cl) {
+                        P::merge(a, i, 0, v[q][0], __double2hiint(v[q][2]), kb[0], jb[0]);
+                        P::merge(a, i, 1, v[q][1], __double2loint(v[q][2]), kb[1], jb[1]);
+                    }
+                }
+                const size_t o = (size_t)(blockIdx.y / cl) * 2 * g.n_sink + k;
+                a.pkey[o] = kb[0]; a.pkey[o + g.n_sink] = kb[1];
+                a.pid[o] = jb[0];  a.pid[o + g.n_sink] = jb[1];
+            }
+            cluster.sync();                    // shared memory must outlive the other CTAs' reads
         }
     }
     if (!stored) {

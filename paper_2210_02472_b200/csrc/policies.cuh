@@ -143,6 +143,7 @@ struct AccPassT {
     // the split-j partial of a sink is three doubles that add: pair_fused_kernel may add the partials of the CTAs of a
     // thread-block cluster through distributed shared memory before anything goes to global memory
     static constexpr bool CLUSTER_REDUCE = true;
+    static constexpr bool CLUSTER_MERGE = false;
     __device__ __forceinline__ static void vec3(const Acc& c, double* v) { v[0] = c.x; v[1] = c.y; v[2] = c.z; }
     __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
         finish_vec3(a.partial, a.out, a.G, g, k, id, lane, L, write);
@@ -269,6 +270,7 @@ struct GradPassT {
     }
     static constexpr bool ALWAYS_FINISH = false;
     static constexpr bool CLUSTER_REDUCE = !WITH_ACC;       // (see AccPassT; the acc + jerk pass has two partials per sink)
+    static constexpr bool CLUSTER_MERGE = false;
     __device__ __forceinline__ static void vec3(const Acc& c, double* v) {
         v[0] = fma(-3.0, c.wx, c.ux); v[1] = fma(-3.0, c.wy, c.uy); v[2] = fma(-3.0, c.wz, c.uz);     // as store()
     }
@@ -565,11 +567,12 @@ struct DtPassT {
         const double r[8] = {a.pos[o], a.pos[o + 1], a.pos[o + 2], a.mass[j], a.vel[o], a.vel[o + 1], a.vel[o + 2], 0.0};
         keys(s, r, kff, kfb);
     }
-    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
-        const size_t o = (size_t)split * 2 * g.n_sink + k;
+    // the split's winners: refined keys of the running bests (recovered from the thresholds, ~2 ulp) and their ids
+    __device__ __forceinline__ static void partial_of(const Args& a, const Geom& g, int split, int id, const Acc& c, double& kf, double& kb,
+                                                      int& jf, int& jb) {
         constexpr double UNSCALE = SHORT ? 1.0 / KEY_SLACK : KEY_PRE_INV;
-        double kf = c.thr_ff * UNSCALE, kb = c.thr_fb * UNSCALE;
-        int jf = c.jff, jb = c.jfb;
+        kf = c.thr_ff * UNSCALE; kb = c.thr_fb * UNSCALE;
+        jf = c.jff; jb = c.jfb;
         if (SHORT && __builtin_expect(c.amb != 0, 0)) {      // a near-tie in this range: settle it on the exact time-steps
             const int l0 = min(split * g.tiles_per_split * TILE, g.n_src), l1 = min(l0 + g.tiles_per_split * TILE, g.n_src);
             Sink t;
@@ -577,6 +580,12 @@ struct DtPassT {
             if (c.amb & 1) { jf = dt_rescan(a, 0, id, l0, l1); if (jf >= 0) { double d0, d1; key_of(a, t, jf, d0, d1); kf = d0; } }
             if (c.amb & 2) { jb = dt_rescan(a, 1, id, l0, l1); if (jb >= 0) { double d0, d1; key_of(a, t, jb, d0, d1); kb = d1; } }
         }
+    }
+    __device__ static void store(const Args& a, const Geom& g, int split, int k, int id, const Sink&, const Acc& c) {
+        const size_t o = (size_t)split * 2 * g.n_sink + k;
+        double kf, kb;
+        int jf, jb;
+        partial_of(a, g, split, id, c, kf, kb, jf, jb);
         a.pkey[o] = kf; a.pkey[o + g.n_sink] = kb;
         a.pid[o] = jf;  a.pid[o + g.n_sink] = jb;
         if (NGB) a.ng.pcount[(size_t)split * g.n_sink + k] = c.nc;
@@ -586,6 +595,9 @@ struct DtPassT {
     // in the oracle's order.  The winner is the exact (time-step, id) minimum, so the order of the splits does not matter.
     static constexpr bool ALWAYS_FINISH = true;
     static constexpr bool CLUSTER_REDUCE = false;
+    // pair_fused_kernel as clusters: the winners of the CTAs of a cluster are merged through distributed shared memory with
+    // merge() below, one entry per cluster goes to the workspace (not with the neighbour lists riding along)
+    static constexpr bool CLUSTER_MERGE = !NGB;
     __device__ __forceinline__ static void vec3(const Acc&, double*) {}
     __device__ __forceinline__ static void merge(const Args& a, int i, int w, double key, int j, double& kb, int& jb) {
         const bool clear = (j >= 0) & ((key * KEY_SLACK > kb) | (jb < 0));
@@ -737,6 +749,7 @@ struct PotPassT {
     }
     static constexpr bool ALWAYS_FINISH = false;
     static constexpr bool CLUSTER_REDUCE = false;
+    static constexpr bool CLUSTER_MERGE = false;
     __device__ __forceinline__ static void vec3(const Acc&, double*) {}
     __device__ static void finish(const Args& a, const Geom& g, int k, int id, int lane, int L, bool write) {
         double s = 0.0;

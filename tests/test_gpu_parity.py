@@ -1367,9 +1367,10 @@ def test_few_sinks_exact_ties_zero_velocity_and_coincident(torch, ctx):
 @pytest.mark.parametrize("n_sink,n_src", [(33, 16384), (100, 300), (129, 700), (500, 16384), (1024, 16384), (2048, 5000),
                                           (4095, 16384), (128, 131072), (40, 129)])
 def test_fused_kernel_cluster_reduction(torch, ctx, n_sink, n_src):
-    """The fused launch of acc / grad as thread-block clusters along the split axis (partials added through distributed
-    shared memory; grid.y padded to a multiple of the cluster size with CTAs that add zeros) against the oracle, and
-    against the same launch without clusters (BIFROST_TUNE_FUSED_CLUSTER = 0): equal to rounding."""
+    """The fused launch of acc / grad / dtmin as thread-block clusters along the split axis (partials added - dtmin: winners
+    merged - through distributed shared memory; grid.y padded to a multiple of the cluster size with CTAs that contribute
+    nothing) against the oracle, and against the same launch without clusters (BIFROST_TUNE_FUSED_CLUSTER = 0): equal to
+    rounding, dtmin bit-identical."""
     from paper_2210_02472_b200.binding import Context
     w = workload(3) if n_src > 16384 else workload(2)
     rng = np.random.default_rng(n_sink + 7 * n_src)
@@ -1379,6 +1380,7 @@ def test_fused_kernel_cluster_reduction(torch, ctx, n_sink, n_src):
     a, c, d, _ = run_all(torch, ctx, w, sinks, srcs, acc_full=acc_full)
     check_vec(a, oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), "fused cluster acc")
     check_vec(c, oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sinks, srcs), "fused cluster grad")
+    check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs), "fused cluster dtmin")
     plain = Context(w.n)
     plain.set_tuning(Context.TUNE_FUSED_CLUSTER, 0)
     try:
