@@ -116,7 +116,7 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
                                              (default 5e7, and >= 512 entries in the shorter list; 0 = always) */
 #define BIFROST_TUNE_FEW_MAX_SINKS 4      /* calls with at most this many sinks (default 32, 0..32; 0 disables) and at most */
 #define BIFROST_TUNE_FEW_MAX_PAIRS 5      /* this many sink-source pairs (default 2^19 for acc, 2^18 for grad and dtmin; the knob sets
-                                             all three; doubled for <= 8 sinks) run as ONE thread-block-cluster launch: threads
+                                             all three; four times that for <= 8 sinks) run as ONE thread-block-cluster launch: threads
                                              over the sources, results merged through distributed shared memory, no workspace */
 #define BIFROST_TUNE_FUSED_CLUSTER 6      /* 1 (default): the fused launch runs as clusters of up to 8 CTAs that combine their split-j
                                              partials through distributed shared memory (sums for acc / grad / jerk, the winners'

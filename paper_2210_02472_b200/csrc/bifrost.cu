@@ -307,8 +307,9 @@ int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, 
              cudaStream_t st) {
     if (n_sink < 1 || n_sink > ctx->few_max_sinks || n_sink > FEW_MAX_SINKS || ctx->shard_world > 1) return 1;
     // measured cross-over against the fused kernel (profiles/r2_sweep_small_sets.md): 2^19 pairs for acc, 2^18 for grad and dtmin,
-    // twice that for at most 8 sinks (long source lists, where the fused kernel's 128-way split pays its reduction)
-    if ((double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 2.0 : 1.0)) return 1;
+    // four times that for at most 8 sinks (long source lists, where one working thread per CTA of the fused kernel walks its
+    // tiles one source after the other: 1 sink x 2^20 sources 264 -> 105 us, 4 sinks x 2^18 sources 71 -> 47 us)
+    if ((double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 4.0 : 1.0)) return 1;
     auto kern = few_sinks_kernel<F>;
     if (ctx->few_max_cl[WHICH] == 0) {          // once per context and instance: may a cluster have 16 CTAs here?
         int max_cl = 8;                         // the portable size

@@ -1268,7 +1268,7 @@ def ctx_nofew(torch):
 
 
 @pytest.mark.parametrize("n_sink,n_src", [(1, 16384), (2, 16384), (3, 5000), (5, 257), (8, 256), (13, 1), (17, 16384),
-                                          (31, 777), (32, 16384), (1, 131072), (4, 131072), (7, 0)])
+                                          (31, 777), (32, 16384), (1, 131072), (4, 131072), (8, 131072), (7, 0)])
 def test_few_sinks_cluster_kernel(torch, ctx, ctx_nofew, n_sink, n_src):
     """at most 32 sinks (and at most 2^19 pairs; 2^18 for grad) run as ONE cluster launch with the threads
     over the sources.  Against the oracle at the gates (time-steps and argmin bit-identical), rows of other particles
