@@ -9,7 +9,8 @@
 // that source's minimum and is dropped by one more integer compare per key; a pair that reaches the hint (inside or above the
 // 1e-12 band) is a CANDIDATE: it is appended to a global list and raises the hint.  A stale hint only lets more candidates
 // through, never fewer, so the result does not depend on the order in which CTAs run.  Hints start from the block diagonal
-// (every particle against the 1536 members of its own block, evaluated one-sided by a first launch), so that even the first
+// (every particle against the 768 members of its own block - a short last block reaches back to a full block's worth -
+// evaluated one-sided by a first launch), so that even the first
 // off-diagonal CTAs see few candidates.  Afterwards: the sink-side pieces are merged per particle, the candidates are applied
 // under a per-particle lock with the same band rule as everywhere else (clear key decides, near-tie -> exact time-steps, ties ->
 // smaller id), and Eq. 21 / 22 are evaluated once for the winners.  The winner is the exact (time-step, id) minimum over all
@@ -34,6 +35,18 @@ struct SymDtArgs {
     unsigned long long cand_cap;
 };
 
+// The diagonal of a block for dtmin.  A short last block would take its first hints from its few members only, and its
+// positions then collect hundreds of candidates each (m = 16384: 256 members, 400-500 candidates per position, all fighting
+// for one lock per position: 3.2 ms instead of 1.0 ms per call).  Its diagonal pieces therefore reach back over a full
+// block's worth of tiles; a pair seen twice cannot change a maximum.
+__host__ __device__ inline bool sym_dt_short_last(const SymGeom& g, int b) { return b > 0 && sym_diag_tiles(g, b) < g.tb; }
+__host__ __device__ inline int sym_dt_diag_tiles(const SymGeom& g, int b) { return sym_dt_short_last(g, b) ? g.tb : sym_diag_tiles(g, b); }
+__host__ __device__ inline int sym_dt_diag_first(const SymGeom& g, int b) { return sym_dt_short_last(g, b) ? g.n_tiles - g.tb : b * g.tb; }
+__host__ __device__ inline int sym_dt_diag_pieces(const SymGeom& g, int b) { return (sym_dt_diag_tiles(g, b) + g.unit_tiles - 1) / g.unit_tiles; }
+__host__ __device__ inline int sym_dt_pieces(const SymGeom& g, int b) {
+    return sym_dt_diag_pieces(g, b) + (sym_range(g, b) + g.unit_tiles - 1) / g.unit_tiles;
+}
+
 // phase = 0: the diagonal pieces only (one-sided; sets the hints);  phase = 1: the pieces beyond the block (both sides)
 template <int S, int T, int MINB, int UNR = 2>
 __global__ void __launch_bounds__(T, MINB)
@@ -47,8 +60,8 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
     SymGeom g = g_in;
     g.mutual = 0;
     const int b = blockIdx.y, piece = blockIdx.x;
-    const int range = sym_range(g, b), np = sym_pieces(g, b);
-    const int nd = sym_diag_pieces(g, b), dt = sym_diag_tiles(g, b);
+    const int range = sym_range(g, b), np = sym_dt_pieces(g, b);
+    const int nd = sym_dt_diag_pieces(g, b), dt = sym_dt_diag_tiles(g, b), dfirst = sym_dt_diag_first(g, b);
     if (piece >= np) return;
     const bool diag = piece < nd;
     if (diag != (phase == 0)) return;
@@ -76,8 +89,8 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
 
     const int jb = sym_first(g, b);
     const int len = diag ? (dt + nd - 1) / nd : (range + (np - nd) - 1) / (np - nd);
-    const int t0 = diag ? b * g.tb + piece * len : jb + (piece - nd) * len;
-    const int t1 = min(t0 + len, diag ? b * g.tb + dt : jb + range);
+    const int t0 = diag ? dfirst + piece * len : jb + (piece - nd) * len;
+    const int t1 = min(t0 + len, diag ? dfirst + dt : jb + range);
     const int n_my = max(t1 - t0, 0);
 
     auto load_tile = [&](int tile, int buf) {
@@ -173,7 +186,7 @@ sym_dt_kernel(const SymDtArgs a, const SymGeom g_in, const double* __restrict__ 
 __global__ void sym_dt_hint_kernel(const SymDtArgs a, const SymGeom g) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= g.m) return;
-    const int nd = sym_diag_pieces(g, k / g.bs);
+    const int nd = sym_dt_diag_pieces(g, k / g.bs);
     double hf = 0.0, hb = 0.0;
     for (int p = 0; p < nd; ++p) {
         const DtBest o = a.pieces[(size_t)p * g.m + k];
@@ -190,7 +203,7 @@ __global__ void sym_dt_merge_kernel(const SymDtArgs a, const SymGeom g) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= g.m) return;
     const int i = a.idx ? a.idx[k] : k;
-    const int np = sym_pieces(g, k / g.bs);
+    const int np = sym_dt_pieces(g, k / g.bs);
     double kb[2] = {0.0, 0.0};
     int jb[2] = {-1, -1};
     for (int p = 0; p < np; ++p) {
@@ -202,14 +215,34 @@ __global__ void sym_dt_merge_kernel(const SymDtArgs a, const SymGeom g) {
     a.lock[k] = 0;
 }
 
-// every candidate into best[] under the position's lock (candidates are rare and spread: the lock is all but uncontended)
+// Every candidate into best[] under the position's lock.  Candidates of one source found by the sinks of one CTA sit next to
+// each other in the list, so the lanes of a warp would fight for one lock (a ragged last block, whose diagonal hints come from
+// few members, collected 400-500 candidates per position: 2.2 ms instead of 0.15 ms for 16384 entries).  The lanes of a warp
+// that hold the same (position, kind) elect a leader (__match_any_sync); it merges its group with the band rule first and
+// takes the lock once.
 __global__ void sym_dt_apply_kernel(const SymDtArgs a) {
     using D = DtPassT<false>;
     const unsigned long long n = min(a.counters[0], a.cand_cap);
-    for (unsigned long long c = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (unsigned long long)gridDim.x * blockDim.x) {
-        const DtCand cd = a.cand[c];
+    const int lane = threadIdx.x & 31;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31); base < n; base += stride) {
+        const unsigned long long c = base + lane;
+        const bool valid = c < n;
+        const DtCand cd = valid ? a.cand[c] : DtCand{0.0, -1 - lane, -1};
+        const unsigned peers = __match_any_sync(0xffffffffu, cd.pos2);
+        const bool leader = valid && lane == __ffs(peers) - 1;
         const int pos = cd.pos2 >> 1, w = cd.pos2 & 1;
-        const int i = a.idx ? a.idx[pos] : pos;
+        const int i = valid ? (a.idx ? a.idx[pos] : pos) : 0;
+        double kg = cd.key;                     // the group's best, formed by its leader
+        int jg = cd.id;
+        if (__any_sync(0xffffffffu, (peers & (peers - 1)) != 0)) {      // some group of this warp has more than one lane: only where candidates cluster
+            for (int src = 0; src < 32; ++src) {
+                const double ks = __shfl_sync(0xffffffffu, cd.key, src);
+                const int js = __shfl_sync(0xffffffffu, cd.id, src);
+                if (leader && src != lane && ((peers >> src) & 1)) D::merge(a.d, i, w, ks, js, kg, jg);
+            }
+        }
+        if (!leader) continue;
         bool done = false;
         while (!done) {
             if (atomicCAS(a.lock + pos, 0, 1) == 0) {
@@ -217,7 +250,7 @@ __global__ void sym_dt_apply_kernel(const SymDtArgs a) {
                 DtBest* o = a.best + pos;
                 double kb = w ? ((volatile DtBest*)o)->kfb : ((volatile DtBest*)o)->kff;
                 int jb = w ? ((volatile DtBest*)o)->jfb : ((volatile DtBest*)o)->jff;
-                D::merge(a.d, i, w, cd.key, cd.id, kb, jb);
+                D::merge(a.d, i, w, kg, jg, kb, jb);
                 if (w) { ((volatile DtBest*)o)->kfb = kb; ((volatile DtBest*)o)->jfb = jb; }
                 else { ((volatile DtBest*)o)->kff = kb; ((volatile DtBest*)o)->jff = jb; }
                 __threadfence();
