@@ -381,7 +381,7 @@ def run_cuda(args):
 
         def kern(name):
             ms = mean_ms[name]
-            path = path_ag if name != "dtmin" else ("sym" if world == 1 and n >= 40960 else "plain")   # dtmin is sink-sharded when world > 1
+            path = path_ag if name != "dtmin" else ("sym" if world == 1 and n >= 32768 else "plain")   # dtmin is sink-sharded when world > 1
             tf = pairs_rank * FP64_FLOPS[path][name] / (ms * 1e-3) / 1e12
             pipe = pairs_rank * FP64_INSTR[path][name] / (ms * 1e-3) / (peak * 1e12 / 2)
             out = {"ms": ms, "kernel": kernel_name[name][path], "interactions_per_s": pairs_rank / (ms * 1e-3),

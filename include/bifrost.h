@@ -51,7 +51,7 @@
  *    pairs) are one thread-block-cluster launch with the threads over the sources; below 4096 sinks a call is one
  *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish;
  *    bifrost_acc / bifrost_grad / bifrost_dtmin whose sink and source lists are the SAME list (same
- *    pointer, or both NULL) of >= 16384 / 12288 / 40960 entries evaluate every unordered pair once
+ *    pointer, or both NULL) of >= 16384 / 12288 / 32768 entries evaluate every unordered pair once
  *    (symmetric kernels; results as before, in another summation order - dtmin's are bit-identical).
  *    The thresholds are bifrost_set_tuning knobs; no environment variable or file is read.
  *  - Return value: BIFROST_OK (0) or a negative BIFROST_E* code.  Nothing is printed, nothing
@@ -107,7 +107,7 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
  *   BIFROST_TUNE_SMALL_M          largest particle set whose FSI cycle / level split is one single-CTA launch
  *                                 (default 128, 0..256; 0 disables)
  *   BIFROST_TUNE_SYM_MIN_N        shortest same-list call that takes the symmetric kernels (default 16384 for
- *                                 acc, 12288 for grad, 40960 for dtmin; this knob sets all three; a value above
+ *                                 acc, 12288 for grad, 32768 for dtmin; this knob sets all three; a value above
  *                                 max_n disables them) */
 #define BIFROST_TUNE_FUSED_MAX_SINKS 0
 #define BIFROST_TUNE_SMALL_M         1

@@ -84,7 +84,7 @@ struct bifrost_ctx {
     bool fused_cluster = true;       // pair_fused_kernel as clusters with a DSMEM reduction (BIFROST_TUNE_FUSED_CLUSTER: 0 / 1)
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
-    int64_t sym_min_dt = 40960;      // shortest list for the symmetric dtmin (cross-over near 32768; BIFROST_TUNE_SYM_MIN_N sets it too)
+    int64_t sym_min_dt = 32768;      // shortest list for the symmetric dtmin (cross-over near 28000; BIFROST_TUNE_SYM_MIN_N sets it too)
     int64_t sym_min_acc = 16384, sym_min_grad = 12288;   // shortest list the symmetric kernels are used for (measured
                                      // crossover, profiles/r2_symmetric.md; BIFROST_TUNE_SYM_MIN_N sets both)
     const int32_t* subsys = nullptr; // borrowed DEVICE pointer set by bifrost_set_subsystems (NEXT-2), or NULL
@@ -218,7 +218,9 @@ int launch_fused(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& s
     int cl = 1;
     const int64_t ctas_padded = (int64_t)grid.x * ceil_div(g.n_split, 8) * 8;
     const bool short_launch = g.tiles_per_split <= 2 || 8 * ctas_padded <= 7 * (int64_t)ctx->num_sms * Sh::MINB;
-    if ((P::CLUSTER_REDUCE || P::CLUSTER_MERGE) && ctx->fused_cluster && g.n_split >= 2 && short_launch) {
+    // (at most 32 sinks: the last CTA has 4-32 lanes per sink for its reduction and is as fast without clusters - the calls of
+    // few_sinks_kernel's size that cannot take it, e.g. with subsystems set: 1 sink dtmin 16.2 us against 22.6 with clusters)
+    if ((P::CLUSTER_REDUCE || P::CLUSTER_MERGE) && ctx->fused_cluster && g.n_split >= 2 && short_launch && n_sink > 32) {
         cl = g.n_split >= 8 ? 8 : g.n_split >= 4 ? 4 : 2;
         grid.y = (unsigned)(ceil_div(g.n_split, cl) * cl);
     }

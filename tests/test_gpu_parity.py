@@ -1406,3 +1406,20 @@ def test_fused_kernel_cluster_reduction(torch, ctx, n_sink, n_src):
         g.replay(); g.replay()
         st.synchronize()
     assert np.array_equal(out.cpu().numpy()[sinks], a)
+
+
+@pytest.mark.parametrize("m", [32767, 32768])
+def test_symmetric_dtmin_switch_point(torch, ctx, m):
+    """Default threshold: dtmin over one list switches to the symmetric kernel at 32768 entries (7 launches instead of 3);
+    both sides of the switch against the oracle on a sample, bit for bit."""
+    w = workload(3, n=40000)
+    pos, vel, mass = dev(torch, w.pos[:m].copy()), dev(torch, w.vel[:m].copy()), dev(torch, w.mass[:m].copy())
+    l0 = ctx.launch_count
+    d = ctx.dtmin(pos, vel, mass, w.G, w.eta_ff, w.eta_fb)
+    torch.cuda.synchronize()
+    assert ctx.launch_count - l0 == (7 if m >= 32768 else 3)
+    pick = np.sort(np.random.default_rng(m).choice(m, 2048, replace=False)).astype(np.int32)
+    pick[:8] = np.arange(8); pick[-8:] = np.arange(m - 8, m)
+    pick = np.unique(pick).astype(np.int32)
+    check_dt(tuple(t.cpu().numpy()[pick] for t in d), oracle.dtmin(w.pos[:m], w.vel[:m], w.mass[:m], w.G, w.eta_ff, w.eta_fb, sink_idx=pick),
+             f"dtmin at the switch, m = {m}")
