@@ -47,8 +47,8 @@
  *  - One context per stream; concurrent calls on one context are not allowed.
  *  - Results are bit-identical for identical inputs on the same GPU model: tiling is fixed by
  *    the argument sizes and every reduction runs in a fixed order (no floating-point atomics).
- *  - Launch shapes are chosen from the argument sizes alone: at most 32 sinks (and a bounded number of
- *    pairs) are one thread-block-cluster launch with the threads over the sources; below 4096 sinks a call is one
+ *  - Launch shapes are chosen from the argument sizes alone: at most 32 sinks and a bounded number of pairs
+ *    (128 sinks against at most 16384 sources) are one launch of thread-block clusters with the threads over the sources; below 4096 sinks a call is one
  *    fused launch (gather + pairs + last-CTA fixed-order reduction), above it is pack -> pair -> finish;
  *    bifrost_acc / bifrost_grad / bifrost_dtmin whose sink and source lists are the SAME list (same
  *    pointer, or both NULL) of >= 16384 / 12288 / 32768 entries evaluate every unordered pair once
@@ -117,7 +117,9 @@ int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world);
 #define BIFROST_TUNE_FEW_MAX_SINKS 4      /* calls with at most this many sinks (default 32, 0..32; 0 disables) and at most */
 #define BIFROST_TUNE_FEW_MAX_PAIRS 5      /* this many sink-source pairs (default 2^19 for acc, 2^18 for grad and dtmin; the knob sets
                                              all three; four times that for <= 8 sinks) run as ONE thread-block-cluster launch: threads
-                                             over the sources, results merged through distributed shared memory, no workspace */
+                                             over the sources, results merged through distributed shared memory, no workspace.
+                                             At the default 32, calls with 33-128 sinks and at most 16384 sources take the same
+                                             kernel with one cluster per 32 sinks. */
 #define BIFROST_TUNE_FUSED_CLUSTER 6      /* 1 (default): the fused launch runs as clusters of up to 8 CTAs that combine their split-j
                                              partials through distributed shared memory (sums for acc / grad / jerk, the winners'
                                              merge for dtmin); 0: every CTA's partial goes through global memory (the order of

@@ -307,11 +307,15 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
 template <class F, int WHICH>
 int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src, int compact,
              cudaStream_t st) {
-    if (n_sink < 1 || n_sink > ctx->few_max_sinks || n_sink > FEW_MAX_SINKS || ctx->shard_world > 1) return 1;
+    // 33-128 sinks against at most 16384 sources: one cluster per 32 sinks (config 2: acc 13.4-15.2 -> 11.0 us, grad 16.8-18.0 ->
+    // 15.8-16.1, dtmin 128 sinks 26.6 -> 23.4; from 256 sinks on, or with longer lists, the fused kernel's clusters are faster)
+    const bool groups = n_sink > FEW_MAX_SINKS;
+    if (n_sink < 1 || ctx->shard_world > 1 || ctx->few_max_sinks == 0) return 1;
+    if (groups ? (ctx->few_max_sinks < FEW_MAX_SINKS || n_sink > FEW_GROUP_MAX_SINKS || n_src > FEW_GROUP_MAX_SRC) : n_sink > ctx->few_max_sinks) return 1;
     // measured cross-over against the fused kernel (profiles/r2_sweep_small_sets.md): 2^19 pairs for acc, 2^18 for grad and dtmin,
     // four times that for at most 8 sinks (long source lists, where one working thread per CTA of the fused kernel walks its
     // tiles one source after the other: 1 sink x 2^20 sources 264 -> 105 us, 4 sinks x 2^18 sources 71 -> 47 us)
-    if ((double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 4.0 : 1.0)) return 1;
+    if (!groups && (double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 4.0 : 1.0)) return 1;
     auto kern = few_sinks_kernel<F>;
     if (ctx->few_max_cl[WHICH] == 0) {          // once per context and instance: may a cluster have 16 CTAs here?
         int max_cl = 8;                         // the portable size
@@ -329,14 +333,15 @@ int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, 
         ctx->few_max_cl[WHICH] = max_cl;
     }
     int nsp = 1;
-    while (nsp < n_sink) nsp *= 2;
+    while (nsp < n_sink && nsp < FEW_MAX_SINKS) nsp *= 2;
+    const int n_groups = ceil_div(n_sink, nsp);
     const int n_tiles = ceil_div(n_src, FEW_T);
     int cl = 1;
     while (cl * 2 <= ctx->few_max_cl[WHICH] && cl * 2 <= n_tiles &&
            (int64_t)cl * FEW_T * ctx->few_pairs_per_thread < (int64_t)nsp * n_src)
         cl *= 2;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(cl); cfg.blockDim = dim3(FEW_T); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cfg.gridDim = dim3(cl * n_groups); cfg.blockDim = dim3(FEW_T); cfg.dynamicSmemBytes = 0; cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;

@@ -5,7 +5,7 @@
 // pair_fused_kernel gives every thread one sink and walks the sources of its CTA one after the other: with one sink, one
 // thread per CTA works through 128 dependent iterations, then 128 CTAs meet at a global ticket and the last one reads 128
 // partials back through L2 (12 us for 1 sink x 16384 sources, of which < 1 us is arithmetic).  Here the THREADS GO OVER THE
-// SOURCES: the launch is ONE thread-block cluster of CL <= 16 CTAs of 256 threads; thread t of a CTA serves sink t mod NSP (NSP =
+// SOURCES: the launch is ONE thread-block cluster of CL <= 16 CTAs of 256 threads (one cluster per 32 sinks for 33-128 sinks); thread t of a CTA serves sink t mod NSP (NSP =
 // the sink count rounded up to a power of two) and every (256 / NSP)-th source of the CTA's tiles, so one sink x 16384
 // sources is 4 pairs per thread.  The per-thread results are merged in a FIXED order - xor-shuffles over the lanes that share
 // a sink, the 8 warps of the CTA through shared memory in warp order, the CL CTAs of the cluster through DISTRIBUTED shared
@@ -25,7 +25,9 @@ namespace cg = cooperative_groups;
 
 constexpr int FEW_T = 256;                 // threads per CTA = sources per tile
 constexpr int FEW_WARPS = FEW_T / 32;
-constexpr int FEW_MAX_SINKS = 32;
+constexpr int FEW_MAX_SINKS = 32;            // sinks per cluster
+constexpr int FEW_GROUP_MAX_SINKS = 128;     // several clusters of 32 sinks: up to this many sinks ..
+constexpr int FEW_GROUP_MAX_SRC = 16384;     // .. against at most this many sources (measured cross-over, launch rule in few_impl)
 constexpr int FEW_MAX_CL = 16;             // CTAs per cluster (16 = the non-portable maximum; every B200 GPC holds >= 16 SMs)
 
 struct FewVec3 {
@@ -51,7 +53,7 @@ struct FewAcc {
     __device__ __forceinline__ static Val value(const State& c) { return Val{c.x, c.y, c.z}; }
     __device__ __forceinline__ static Val identity() { return Val{0.0, 0.0, 0.0}; }
     __device__ __forceinline__ static void merge(const Args&, int, Val& c, const Val& o) { c.x += o.x; c.y += o.y; c.z += o.z; }
-    __device__ __forceinline__ static void settle(const Args&, const SrcArrays&, int, int, Val*, Val (*)[FEW_MAX_SINKS]) {}
+    __device__ __forceinline__ static void settle(const Args&, const SrcArrays&, int, int, int, Val*, Val (*)[FEW_MAX_SINKS]) {}
     static constexpr int PARTS = 1;          // threads that share the output of one sink
     __device__ __forceinline__ static void write(const Args& a, int row, int, const Val& v, int) {
         double* o = a.out + 3 * (size_t)row;
@@ -76,7 +78,7 @@ struct FewGrad {
     __device__ __forceinline__ static Val value(const State& c) { return Val{fma(-3.0, c.wx, c.ux), fma(-3.0, c.wy, c.uy), fma(-3.0, c.wz, c.uz)}; }
     __device__ __forceinline__ static Val identity() { return Val{0.0, 0.0, 0.0}; }
     __device__ __forceinline__ static void merge(const Args&, int, Val& c, const Val& o) { c.x += o.x; c.y += o.y; c.z += o.z; }
-    __device__ __forceinline__ static void settle(const Args&, const SrcArrays&, int, int, Val*, Val (*)[FEW_MAX_SINKS]) {}
+    __device__ __forceinline__ static void settle(const Args&, const SrcArrays&, int, int, int, Val*, Val (*)[FEW_MAX_SINKS]) {}
     static constexpr int PARTS = 1;          // threads that share the output of one sink
     __device__ __forceinline__ static void write(const Args& a, int row, int, const Val& v, int) {
         double* o = a.out + 3 * (size_t)row;
@@ -149,13 +151,13 @@ struct FewDt {
     // CTA 0, all threads: every flagged sink gets the exact (time-step, id) minimum over the WHOLE source list, by the
     // oracle's rule on dt_exact_ids (smaller time-step; equal -> smaller id; +inf never wins).  Rare and slow (an exact
     // evaluation per source), but parallel: n_src / 256 evaluations per thread.
-    __device__ static void settle(const Args& a, const SrcArrays& src, int n_sink, int n_src, Val* cta_sm, Val (*warp_sm)[FEW_MAX_SINKS]) {
+    __device__ static void settle(const Args& a, const SrcArrays& src, int k0, int n_here, int n_src, Val* cta_sm, Val (*warp_sm)[FEW_MAX_SINKS]) {
         const double inf = __longlong_as_double(0x7ff0000000000000LL);
         const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-        for (int q = 0; q < n_sink; ++q) {
+        for (int q = 0; q < n_here; ++q) {
             const int amb = cta_sm[q].amb;                    // the same for every thread
             if (!amb) continue;
-            const int i = a.sink_idx ? a.sink_idx[q] : q;
+            const int i = a.sink_idx ? a.sink_idx[k0 + q] : k0 + q;
             for (int w = 0; w < 2; ++w) {
                 if (!((amb >> w) & 1)) continue;
                 double tb = inf;
@@ -201,7 +203,8 @@ struct FewDt {
     }
 };
 
-// grid = cluster = CL CTAs of FEW_T threads.  nsp = n_sink rounded up to a power of two (<= 32).
+// grid = one cluster of CL CTAs of FEW_T threads per group of nsp sinks.  One group: nsp = n_sink rounded up to a power of two
+// (<= 32); several groups: nsp = 32.
 template <class F>
 __global__ void __launch_bounds__(FEW_T, 1)
 few_sinks_kernel(const typename F::Args a, const SrcArrays src, int n_sink, int n_src, int nsp, int compact) {
@@ -214,7 +217,8 @@ few_sinks_kernel(const typename F::Args a, const SrcArrays src, int n_sink, int 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const int s = t & (nsp - 1), rep = t / nsp, reps = FEW_T / nsp;   // this thread: sink s, sources rep, rep + reps, .. of a tile
 
-    const int k = s < n_sink ? s : n_sink - 1;                        // a shadow thread repeats the last sink; never merged
+    const int k0 = ((int)blockIdx.x / cl) * nsp;                      // first sink of this cluster (several clusters: nsp = 32)
+    const int k = k0 + s < n_sink ? k0 + s : n_sink - 1;              // a shadow thread repeats the last sink; never merged
     const int id = a.sink_idx ? a.sink_idx[k] : k;
     typename F::Sink sink;
     typename F::State st;
@@ -261,7 +265,7 @@ few_sinks_kernel(const typename F::Args a, const SrcArrays src, int n_sink, int 
         }
         __syncthreads();
     };
-    cta_reduce(s < n_sink ? F::value(st) : F::identity());
+    cta_reduce(k0 + s < n_sink ? F::value(st) : F::identity());
     cluster.sync();
     if (rank == 0) {
         // the CTAs of the cluster: thread (s, rep) of CTA 0 fetches the results of ranks rep, rep + reps, .. for its sink
@@ -269,8 +273,8 @@ few_sinks_kernel(const typename F::Args a, const SrcArrays src, int n_sink, int 
         typename F::Val v = F::identity();
         for (int q = rep; q < cl; q += reps) F::merge(a, id, v, *cluster.map_shared_rank(&cta_sm[s], q));
         cta_reduce(v);
-        F::settle(a, src, n_sink, n_src, cta_sm, warp_sm);
-        if (t < nsp * F::PARTS && s < n_sink) F::write(a, compact ? s : id, id, cta_sm[s], t / nsp);   // s = t mod nsp
+        F::settle(a, src, k0, min(nsp, n_sink - k0), n_src, cta_sm, warp_sm);
+        if (t < nsp * F::PARTS && k0 + s < n_sink) F::write(a, compact ? k0 + s : id, id, cta_sm[s], t / nsp);   // s = t mod nsp
     }
     cluster.sync();                             // a CTA's shared memory must outlive CTA 0's reads
 }

@@ -1268,10 +1268,11 @@ def ctx_nofew(torch):
 
 
 @pytest.mark.parametrize("n_sink,n_src", [(1, 16384), (2, 16384), (3, 5000), (5, 257), (8, 256), (13, 1), (17, 16384),
-                                          (31, 777), (32, 16384), (1, 131072), (4, 131072), (8, 131072), (7, 0)])
+                                          (31, 777), (32, 16384), (1, 131072), (4, 131072), (8, 131072), (7, 0),
+                                          (33, 16384), (64, 5000), (100, 300), (128, 16384), (97, 1)])
 def test_few_sinks_cluster_kernel(torch, ctx, ctx_nofew, n_sink, n_src):
-    """at most 32 sinks (and at most 2^19 pairs; 2^18 for grad) run as ONE cluster launch with the threads
-    over the sources.  Against the oracle at the gates (time-steps and argmin bit-identical), rows of other particles
+    """at most 32 sinks (and at most 2^19 pairs; 2^18 for grad), or 33-128 sinks against at most 16384
+    sources (one cluster per 32 sinks), run as ONE cluster launch with the threads over the sources.  Against the oracle at the gates (time-steps and argmin bit-identical), rows of other particles
     untouched, one launch per call, and dtmin bit-identical to the fused kernel's."""
     w = workload(3) if n_src > 16384 else workload(2)
     rng = np.random.default_rng(1000 * n_sink + n_src)
@@ -1307,7 +1308,8 @@ def test_few_sinks_cluster_kernel(torch, ctx, ctx_nofew, n_sink, n_src):
 
 @pytest.mark.parametrize("n_sink", [32, 33])
 def test_few_sinks_switch_points(torch, ctx, ctx_nofew, n_sink):
-    """32 sinks take the cluster kernel, 33 the fused kernel; 32 sinks x 16385 sources exceed the pair limit.  All agree."""
+    """32 sinks x 16384 sources take one cluster, 33 sinks two clusters of the same kernel; with 16385 sources both take the
+    fused kernel (pair limit / source limit).  All agree."""
     from paper_2210_02472_b200.binding import Context
     w = workload(3)
     sinks = np.sort(np.random.default_rng(n_sink).choice(w.n, n_sink, replace=False)).astype(np.int32)
