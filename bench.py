@@ -613,6 +613,17 @@ def run_extras(torch, ctx, w, pos, vel, mass, acc):
         rec8.update({"ms": 1e3 * (time.perf_counter() - t0), "launches": ctx8.launch_count - l0, **summ,
                      "rel_energy_error_of_the_interval": abs(energy() - e_before) / abs(e_before)})
     out["hhs_fsi_fig8"] = rec8
+    # the same interval (a third one, from the state the second left) with Eq. 24-29 evaluated at EVERY level over the
+    # level's own particles (bifrost_set_level_criteria) instead of only as dt_cap at level 0
+    ctx8.set_level_criteria(0.1, 0.1, 0.1)
+    e_before = energy()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    l0 = ctx8.launch_count
+    summ, _ = ctx8.hhs_fsi(p, v, m, w8.G, w8.eps, 0.2, 0.2, W.fig8_tau(), max_depth=40)
+    torch.cuda.synchronize()
+    out["hhs_fsi_fig8_level_criteria"] = {"ms": 1e3 * (time.perf_counter() - t0), "launches": ctx8.launch_count - l0, **summ,
+                                          "rel_energy_error_of_the_interval": abs(energy() - e_before) / abs(e_before)}
     ctx8.close()
     return out
 

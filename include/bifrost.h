@@ -346,6 +346,16 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
  *                   order they are entered;   out_summary : HOST int64[3] or NULL - levels entered, deepest
  *                   depth, FSI cycles run.  pos, vel : DEVICE double[n][3], updated in place.
  * BIFROST_EINVAL while bifrost_set_subsystems is active (as bifrost_fsi_step). */
+/* bifrost_set_level_criteria - bifrost_hhs_fsi evaluates the acceleration-based time-step criteria of Eq. 24, 26, 27, 29
+ * (bifrost_timestep_criteria's formulas with eta, eta_grad, eta_jerk) at EVERY level, over the level's
+ * own particles (accelerations, gradient sums and jerks of the level's particles among themselves), and takes
+ * eps_i = min(eps_ff, eps_fb, those four) before the level-0 cap: "the final time-step of a particle is the minimum of
+ * the set of its different time-steps" (L293), "eps_i = min(eps_i, eps_i^{level 0})" (L295).  Costs one acc+jerk pass and one
+ * grad pass per level, and levels of <= 128 particles then run host-steered instead of as one single-CTA launch.
+ * All three > 0 switches it on, all three 0 (the default) off: then only dt_cap carries such criteria, at level 0
+ * (reading H4).  Anything else is BIFROST_EINVAL. */
+int bifrost_set_level_criteria(bifrost_ctx* ctx, double eta, double eta_grad, double eta_jerk);
+
 int bifrost_hhs_fsi(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, const double* mass, double G,
                     double eps_soft, double eta_ff, double eta_fb, const double* dt_cap, double tau, int max_depth,
                     int64_t* out_level_log, int64_t log_cap, int64_t* out_summary, void* stream);

@@ -87,24 +87,43 @@ def level_timesteps(pos, vel, mass, idx, G, eta_ff, eta_fb):
     return np.minimum(d["dt_ff"], d["dt_fb"])
 
 
-def hhs_fsi(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, stats=None, dt_cap=None):
+def level_criteria_timesteps(pos, vel, mass, idx, G, eps_soft, eta, eta_grad, eta_jerk):
+    """PAPER.md:L293-295, per level: the acceleration-based criteria of Eq. 24, 26, 27, 29 of the
+    particles idx with the accelerations, gradient sums and jerks of the particles idx AMONG THEMSELVES (the sums of
+    a sparse faster level - the "pathological situations" L295 guards against with the level-0 cap); returns their
+    minimum per particle.  Built from the pinned routines only."""
+    n = mass.shape[0]
+    a = np.zeros((n, 3)); a[idx] = oracle.acc(pos, mass, G, eps_soft, idx, idx)
+    j = np.zeros((n, 3)); j[idx] = oracle.jerk(pos, vel, mass, G, eps_soft, idx, idx)
+    c = np.zeros((n, 3)); c[idx] = oracle.grad(pos, mass, a, G, eps_soft, idx, idx)
+    cr = oracle.criteria(vel, a, c, j, eta, eta_grad, eta_jerk, idx)
+    return np.minimum(np.minimum(cr["dt_va"], cr["dt_gradv"]), np.minimum(cr["dt_grada"], cr["dt_jerk"]))
+
+
+def hhs_fsi(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, stats=None, dt_cap=None, level_criteria=None):
     """One HHS-FSI integration interval of length tau (Eq. 11), in place.  stats (a dict, optional)
     receives 'levels' (list of (depth, n_slow, n_fast, tau)) in the order the levels are entered.
-    dt_cap (optional, [n]): further per-particle time-steps (e.g. Eq. 24-29) min'd into the level-0 value."""
+    dt_cap (optional, [n]): further per-particle time-steps (e.g. Eq. 24-29) min'd into the level-0 value.
+    level_criteria (optional, (eta, eta_grad, eta_jerk)): Eq. 24-29 are ALSO evaluated at every level over the level's
+    own particles and min'd into the level's time-steps ("the final time-step of a particle is the minimum of the set
+    of its different time-steps"), still capped by the level-0 value (L295)."""
     n = mass.shape[0]
     order = np.arange(n, dtype=np.int32)
     dt0 = np.full(n, np.inf) if dt_cap is None else np.array(dt_cap, dtype=np.float64)   # further criteria (L293)
     if stats is not None:
         stats["levels"] = []
-    _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, 0, n, tau, 0, max_depth, dt0, stats)
+    _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, 0, n, tau, 0, max_depth, dt0, stats, level_criteria)
 
 
-def _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, lo, hi, tau, depth, max_depth, dt0, stats):
+def _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, lo, hi, tau, depth, max_depth, dt0, stats,
+               level_criteria=None):
     idx = order[lo:hi].copy()
     if idx.size == 0:
         return
     if depth < max_depth:
         dt = level_timesteps(pos, vel, mass, idx, G, eta_ff, eta_fb)
+        if level_criteria is not None:
+            dt = np.minimum(dt, level_criteria_timesteps(pos, vel, mass, idx, G, eps_soft, *level_criteria))
         if depth == 0:
             dt0[idx] = np.minimum(dt, dt0[idx])             # level-0 value = minimum of all criteria (PAPER.md:L293)
         dt = np.minimum(dt, dt0[idx])                       # PAPER.md:L295
@@ -136,7 +155,7 @@ def _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, lo, hi, tau, 
 
     def H_F():
         _hhs_level(pos, vel, mass, G, eps_soft, eta_ff, eta_fb, order, mid, hi, tau / 2.0, depth + 1, max_depth, dt0,
-                   stats)
+                   stats, level_criteria)
 
     Fn = inter_level_acc()
     if S.size:

@@ -32,7 +32,7 @@ SYMBOLS = [
     "bifrost_neighbours", "bifrost_components", "bifrost_dtmin_neighbours",
     "bifrost_reserve", "bifrost_set_tuning", "bifrost_set_shard", "bifrost_acc_mutual", "bifrost_grad_mutual",
     "bifrost_acc_jerk", "bifrost_kick", "bifrost_drift", "bifrost_fsi_step", "bifrost_hhs_fsi", "bifrost_kinetic_energy",
-    "bifrost_acc_static", "bifrost_static_error",
+    "bifrost_acc_static", "bifrost_static_error", "bifrost_set_level_criteria",
 ]
 
 
@@ -76,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.bifrost_reserve.argtypes = [_P, _I]
     lib.bifrost_set_tuning.argtypes = [_P, _I, _I64]
     lib.bifrost_set_shard.argtypes = [_P, _I, _I]
+    lib.bifrost_set_level_criteria.argtypes = [_P, _D, _D, _D]
     lib.bifrost_acc_mutual.argtypes = [_P, _I64, _P, _P, *lists, _D, _D, _P, _P]
     lib.bifrost_grad_mutual.argtypes = [_P, _I64, _P, _P, _P, *lists, _D, _D, _P, _P]
     lib.bifrost_set_subsystems.argtypes = [_P, _P, _I64]
@@ -567,6 +568,11 @@ class Context:
                                         n if ix is None else ix.shape[0], float(G), float(eps_soft), float(eps),
                                         self._stream())
         self._check(rc, "bifrost_fsi_step")
+
+    def set_level_criteria(self, eta, eta_grad, eta_jerk):
+        """Eq. 24-29 at every level of hhs_fsi (all three > 0), or off (all three 0, the default)."""
+        self._check(self._lib.bifrost_set_level_criteria(self._h, float(eta), float(eta_grad), float(eta_jerk)),
+                    "bifrost_set_level_criteria")
 
     def hhs_fsi(self, pos, vel, mass, G, eps_soft, eta_ff, eta_fb, tau, max_depth=32, log_cap=0, dt_cap=None):
         """One HHS-FSI interval (Eq. 11) in place.  Returns (summary dict, level log as an int64 array [k, 3])."""

@@ -94,6 +94,8 @@ struct bifrost_ctx {
     // NEXT-4 integrator scratch (allocated on first use of bifrost_fsi_step / bifrost_hhs_fsi)
     bool integ_ready = false;
     double *w_acc = nullptr, *w_grad = nullptr, *w_dtff = nullptr, *w_dtfb = nullptr, *w_dt0 = nullptr;
+    double* w_jerk = nullptr;        // jerks of a level's particles (per-level criteria, bifrost_set_level_criteria)
+    double lvl_eta = 0.0, lvl_eta_grad = 0.0, lvl_eta_jerk = 0.0;   // Eq. 24-29 at every level of bifrost_hhs_fsi (all 0: off)
     double* w_acc_s = nullptr;       // accelerations of the FSI cycles (rows of a level's slow set), kept between the two H_S of a level
     int32_t *w_order = nullptr, *w_tmp = nullptr;
     int *w_bcount = nullptr, *w_nslow = nullptr;
@@ -744,6 +746,7 @@ int ensure_integrator(bifrost_ctx* ctx) {
     CU_TRY(ctx, cudaMalloc(&ctx->w_acc, 24 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_grad, 24 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_acc_s, 24 * n));
+    CU_TRY(ctx, cudaMalloc(&ctx->w_jerk, 24 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dtff, 8 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dtfb, 8 * n));
     CU_TRY(ctx, cudaMalloc(&ctx->w_dt0, 8 * n));
@@ -823,7 +826,8 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     if (m == 0) return BIFROST_OK;
     cudaStream_t st = h.st;
     int32_t* seg = ctx->w_order + lo;
-    if (m <= ctx->small_m && m <= SUB_M) {
+    const bool level_crit = ctx->lvl_eta > 0.0 || ctx->lvl_eta_grad > 0.0 || ctx->lvl_eta_jerk > 0.0;
+    if (!level_crit && m <= ctx->small_m && m <= SUB_M) {
         // the whole subtree below a small level in one single-CTA launch: no device -> host read, no further launches
         const SubArgs sa{(int)m, seg, h.pos, h.vel, h.mass, ctx->w_dt0, h.dt_cap, h.G, soft2(h.eps_soft), h.eta_ff, h.eta_fb, tau,
                          depth, h.max_depth, ctx->w_log, HHS_LOG_ROWS, ctx->w_log + 3 * HHS_LOG_ROWS};
@@ -836,6 +840,18 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     if (!all_slow)   // time-steps of the level's particles among themselves (Eq. 21-22)
         RC_TRY(dtmin_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eta_ff, h.eta_fb, ctx->w_dtff, ctx->w_dtfb,
                           nullptr, nullptr, 0, st));
+    if (!all_slow && level_crit) {
+        // "the final time-step of a particle is the minimum of the set of its different time-steps" - the
+        // acceleration-based criteria (Eq. 24-29) of the level's particles among themselves, folded into eps_ff's row; the
+        // level-0 cap of L295 is applied by the flag kernels as before.  w_acc / w_grad are free until the inter-level sums.
+        RC_TRY(acc_jerk_impl(ctx, h.n, h.pos, h.vel, h.mass, seg, m, seg, m, h.G, h.eps_soft, ctx->w_acc, ctx->w_jerk, st));
+        RC_TRY(grad_impl(ctx, h.n, h.pos, h.mass, ctx->w_acc, seg, m, seg, m, h.G, h.eps_soft, ctx->w_grad, 0, st));
+        criteria_kernel<<<ceil_div(m, 256), 256, 0, st>>>((int)m, seg, h.vel, ctx->w_acc, ctx->w_grad, ctx->w_jerk, ctx->lvl_eta,
+                                                         ctx->lvl_eta_grad, ctx->lvl_eta_jerk, nullptr, nullptr, nullptr, nullptr,
+                                                         ctx->w_dtff);
+        ctx->launches++;
+        CU_TRY(ctx, cudaGetLastError());
+    }
     if (m <= ctx->small_m) {
         level_split_small_kernel<<<1, SMALL_M, 0, st>>>((int)m, seg, ctx->w_dtff, ctx->w_dtfb, ctx->w_dt0, h.dt_cap, depth, tau, all_slow,
                                                         ctx->w_nslow);
@@ -982,6 +998,14 @@ int bifrost_set_tuning(bifrost_ctx* ctx, int knob, int64_t value) {
     }
 }
 
+int bifrost_set_level_criteria(bifrost_ctx* ctx, double eta, double eta_grad, double eta_jerk) {
+    if (!ctx || !(eta >= 0.0) || !(eta_grad >= 0.0) || !(eta_jerk >= 0.0)) return BIFROST_EINVAL;
+    ctx->err[0] = 0;
+    if ((eta > 0.0 || eta_grad > 0.0 || eta_jerk > 0.0) && !(eta > 0.0 && eta_grad > 0.0 && eta_jerk > 0.0)) return BIFROST_EINVAL;
+    ctx->lvl_eta = eta; ctx->lvl_eta_grad = eta_grad; ctx->lvl_eta_jerk = eta_jerk;
+    return BIFROST_OK;
+}
+
 int bifrost_set_shard(bifrost_ctx* ctx, int rank, int world) {
     if (!ctx || world < 1 || world > 1024 || rank < 0 || rank >= world) return BIFROST_EINVAL;
     ctx->err[0] = 0;
@@ -1007,7 +1031,7 @@ int bifrost_destroy(bifrost_ctx* ctx) {
     cudaFree(ctx->src_rec); cudaFree(ctx->partial); cudaFree(ctx->is_bh); cudaFree(ctx->phi_scratch); cudaFree(ctx->wpart); cudaFree(ctx->smin); cudaFree(ctx->tickets); cudaFree(ctx->sym_ws);
     cudaFree(ctx->d_pos); cudaFree(ctx->d_vel); cudaFree(ctx->d_mass); cudaFree(ctx->d_acc); cudaFree(ctx->d_out);
     cudaFree(ctx->d_dt); cudaFree(ctx->d_sink); cudaFree(ctx->d_src); cudaFree(ctx->d_j);
-    cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_acc_s); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
+    cudaFree(ctx->w_acc); cudaFree(ctx->w_grad); cudaFree(ctx->w_acc_s); cudaFree(ctx->w_jerk); cudaFree(ctx->w_dtff); cudaFree(ctx->w_dtfb); cudaFree(ctx->w_dt0);
     cudaFree(ctx->w_order); cudaFree(ctx->w_tmp); cudaFree(ctx->w_bcount); cudaFree(ctx->w_nslow); cudaFree(ctx->w_log);
     if (ctx->h_nslow) cudaFreeHost(ctx->h_nslow);
     if (ctx->h_log) cudaFreeHost(ctx->h_log);

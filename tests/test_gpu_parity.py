@@ -1425,3 +1425,39 @@ def test_symmetric_dtmin_switch_point(torch, ctx, m):
     pick = np.unique(pick).astype(np.int32)
     check_dt(tuple(t.cpu().numpy()[pick] for t in d), oracle.dtmin(w.pos[:m], w.vel[:m], w.mass[:m], w.G, w.eta_ff, w.eta_fb, sink_idx=pick),
              f"dtmin at the switch, m = {m}")
+
+
+def test_hhs_fsi_per_level_criteria(torch):
+    """bifrost_set_level_criteria (missing #3): Eq. 24-29 evaluated at every level over the
+    level's own particles.  Level log equal to the oracle's and state to 1e-12, with the criteria binding (the level-0 split
+    differs from the one without them); switched off again the context reproduces the plain interval bit for bit."""
+    from oracle import integrator as I
+    from paper_2210_02472_b200.binding import Context, BifrostError
+    pos0, vel0, mass = _binary_cluster()
+    G, eps_soft, eta, tau = 1.0, 1e-4, 0.05, 1e-3
+    crit = (0.02, 0.02, 0.02)
+    rp, rv = pos0.copy(), vel0.copy()
+    stats, plain = {}, {}
+    I.hhs_fsi(rp, rv, mass, G, eps_soft, eta, eta, tau, max_depth=6, stats=stats, level_criteria=crit)
+    ref = np.array([(d, s, f) for d, s, f, _ in stats["levels"]], dtype=np.int64)
+    I.hhs_fsi(pos0.copy(), vel0.copy(), mass, G, eps_soft, eta, eta, tau, max_depth=6, stats=plain)
+    assert stats["levels"][0][2] > plain["levels"][0][2]            # more fast particles at level 0: the criteria bind
+    c = Context(len(mass))
+    try:
+        m = dev(torch, mass)
+        pos, vel = dev(torch, pos0), dev(torch, vel0)
+        summ0, log0 = c.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=6, log_cap=len(ref) + 64)
+        p_plain, v_plain = pos.clone(), vel.clone()
+        c.set_level_criteria(*crit)
+        pos, vel = dev(torch, pos0), dev(torch, vel0)
+        summ, log = c.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=6, log_cap=len(ref) + 64)
+        assert summ["levels"] == len(ref) and np.array_equal(log, ref)
+        assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
+        with pytest.raises(BifrostError):
+            c.set_level_criteria(0.1, 0.0, 0.1)                        # all three or none
+        c.set_level_criteria(0.0, 0.0, 0.0)
+        pos, vel = dev(torch, pos0), dev(torch, vel0)
+        summ1, log1 = c.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=6, log_cap=len(ref) + 64)
+        assert summ1 == summ0 and np.array_equal(log1, log0) and torch.equal(pos, p_plain) and torch.equal(vel, v_plain)
+    finally:
+        c.close()

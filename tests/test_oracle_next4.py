@@ -254,3 +254,35 @@ def test_wrong_inter_level_gradient_coefficient_breaks_fourth_order(scale, fine_
     """Eq. 13's gradient kick between S and F with 0, 1/2, 1.1 or 2 times its weight: order 2."""
     e = [_hhs_fixed_partition_error(s, fine_reference, scale, monkeypatch) for s in (8, 16)]
     assert e[0] / e[1] < 6.0
+
+
+def test_hhs_level_criteria_enter_every_level_and_stay_under_the_level0_cap():
+    """with level_criteria the acceleration-based time-steps (Eq. 24-29) of the level's own particles
+    are min'd into the level's time-steps.  Pins: (i) criteria that never bind (huge eta) change nothing, bit for bit;
+    (ii) at level 0 the fast set is exactly {min(pairwise, criteria) < tau}, recomputed here from the pinned routines;
+    (iii) a particle that is slow by its level-0 value can only get FASTER at depth (the cap of L295), so the level
+    structure refines the one without criteria; (iv) momentum is still conserved to round-off."""
+    tau = 2e-3
+    base, with_c, huge = {}, {}, {}
+    pos0, vel0, mass, _ = binary_in_cluster()
+    p, v = pos0.copy(), vel0.copy()
+    I.hhs_fsi(p, v, mass, G, 0.0, 0.02, 0.02, tau, stats=base)
+    p2, v2 = pos0.copy(), vel0.copy()
+    I.hhs_fsi(p2, v2, mass, G, 0.0, 0.02, 0.02, tau, stats=huge, level_criteria=(1e30, 1e30, 1e30))
+    assert huge["levels"] == base["levels"] and np.array_equal(p, p2) and np.array_equal(v, v2)
+    eta = (0.01, 0.01, 0.01)
+    p3, v3 = pos0.copy(), vel0.copy()
+    mom0 = (mass[:, None] * v3).sum(0)
+    I.hhs_fsi(p3, v3, mass, G, 0.0, 0.02, 0.02, tau, stats=with_c, level_criteria=eta)
+    n = mass.shape[0]
+    idx = np.arange(n, dtype=np.int32)
+    d = oracle.dtmin(pos0, vel0, mass, G, 0.02, 0.02)
+    a = oracle.acc(pos0, mass, G, 0.0)
+    cr = oracle.criteria(vel0, a, oracle.grad(pos0, mass, a, G, 0.0), oracle.jerk(pos0, vel0, mass, G, 0.0), *eta)
+    dt = np.minimum.reduce([d["dt_ff"], d["dt_fb"], cr["dt_va"], cr["dt_gradv"], cr["dt_grada"], cr["dt_jerk"]])
+    assert with_c["levels"][0][:3] == (0, int((dt >= tau).sum()), int((dt < tau).sum()))
+    assert with_c["levels"][0][2] > base["levels"][0][2]                 # the criteria bind for some particles here
+    assert max(x[0] for x in with_c["levels"]) >= max(x[0] for x in base["levels"])
+    assert np.abs((mass[:, None] * v3).sum(0) - mom0).max() < 1e-15
+    assert np.array_equal(I.level_criteria_timesteps(pos0, vel0, mass, idx, G, 0.0, *eta),
+                          np.minimum.reduce([cr["dt_va"], cr["dt_gradv"], cr["dt_grada"], cr["dt_jerk"]]))
