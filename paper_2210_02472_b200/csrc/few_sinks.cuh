@@ -1,16 +1,17 @@
-// few_sinks.cuh - acc (Eq. 6/12), grad (Eq. 9/13) and dtmin (Eq. 21/22) for a HANDFUL of sinks (at most 32) against a source
-// list: the fastest levels of the hierarchy, where a call is latency, not arithmetic.
+// few_sinks.cuh - acc (Eq. 6/12), grad (Eq. 9/13) and dtmin (Eq. 21/22) for a HANDFUL of sinks (at most 32 per cluster; up to 128
+// in all) against a source list: the fastest levels of the hierarchy, where a call is latency, not arithmetic.
 // Part of the single translation unit bifrost.cu (see its header and DESIGN.md); not a public header.
 //
 // pair_fused_kernel gives every thread one sink and walks the sources of its CTA one after the other: with one sink, one
 // thread per CTA works through 128 dependent iterations, then 128 CTAs meet at a global ticket and the last one reads 128
 // partials back through L2 (12 us for 1 sink x 16384 sources, of which < 1 us is arithmetic).  Here the THREADS GO OVER THE
-// SOURCES: the launch is ONE thread-block cluster of CL <= 16 CTAs of 256 threads (one cluster per 32 sinks for 33-128 sinks); thread t of a CTA serves sink t mod NSP (NSP =
-// the sink count rounded up to a power of two) and every (256 / NSP)-th source of the CTA's tiles, so one sink x 16384
-// sources is 4 pairs per thread.  The per-thread results are merged in a FIXED order - xor-shuffles over the lanes that share
-// a sink, the 8 warps of the CTA through shared memory in warp order, the CL CTAs of the cluster through DISTRIBUTED shared
-// memory in rank order - and CTA 0 writes the outputs: no workspace in global memory, no ticket, no fence, no second
-// launch; bit-reproducible.
+// SOURCES: the launch is ONE thread-block cluster of CL <= 16 CTAs of 256 threads (33-128 sinks against a short source list:
+// one such cluster per 32 sinks); thread t of a CTA serves sink t mod NSP (NSP = the sink count rounded up to a power of
+// two) and every (256 / NSP)-th source of the CTA's tiles, so one sink x 16384 sources is 4 pairs per thread.  The per-thread
+// results are merged in a FIXED order - xor-shuffles over the lanes that share a sink, the 8 warps of the CTA through shared
+// memory in warp order, the CL CTAs of the cluster through DISTRIBUTED shared memory (CTA 0 reads the other CTAs' results,
+// spread over its threads, and merges them the same way) - and CTA 0 writes the outputs: no workspace in global memory, no
+// ticket, no fence, no second launch; bit-reproducible.
 //   acc, grad : the pair arithmetic of AccPassT / GradPassT (policies.cuh), partial sums added in the order above;
 //   dtmin     : DtPassT's refined keys for every pair, merged by selects (a key clear of the other by the band decides); a
 //               near-tie anywhere flags the sink, and a flagged sink is settled by an exact scan: the exact (time-step, id)
