@@ -351,7 +351,7 @@ int bifrost_fsi_step(bifrost_ctx* ctx, int64_t n, double* pos, double* vel, cons
  * own particles (accelerations, gradient sums and jerks of the level's particles among themselves), and takes
  * eps_i = min(eps_ff, eps_fb, those four) before the level-0 cap: "the final time-step of a particle is the minimum of
  * the set of its different time-steps" (L293), "eps_i = min(eps_i, eps_i^{level 0})" (L295).  Costs one acc+jerk pass and one
- * grad pass per level, and levels of <= 128 particles then run host-steered instead of as one single-CTA launch.
+ * grad pass per level.
  * All three > 0 switches it on, all three 0 (the default) off: then only dt_cap carries such criteria, at level 0
  * (reading H4).  Anything else is BIFROST_EINVAL. */
 int bifrost_set_level_criteria(bifrost_ctx* ctx, double eta, double eta_grad, double eta_jerk);

@@ -827,10 +827,10 @@ int hhs_level(Hhs& h, int64_t lo, int64_t hi, double tau, int depth) {
     cudaStream_t st = h.st;
     int32_t* seg = ctx->w_order + lo;
     const bool level_crit = ctx->lvl_eta > 0.0 || ctx->lvl_eta_grad > 0.0 || ctx->lvl_eta_jerk > 0.0;
-    if (!level_crit && m <= ctx->small_m && m <= SUB_M) {
+    if (m <= ctx->small_m && m <= SUB_M) {
         // the whole subtree below a small level in one single-CTA launch: no device -> host read, no further launches
         const SubArgs sa{(int)m, seg, h.pos, h.vel, h.mass, ctx->w_dt0, h.dt_cap, h.G, soft2(h.eps_soft), h.eta_ff, h.eta_fb, tau,
-                         depth, h.max_depth, ctx->w_log, HHS_LOG_ROWS, ctx->w_log + 3 * HHS_LOG_ROWS};
+                         level_crit ? ctx->lvl_eta : 0.0, ctx->lvl_eta_grad, ctx->lvl_eta_jerk, depth, h.max_depth, ctx->w_log, HHS_LOG_ROWS, ctx->w_log + 3 * HHS_LOG_ROWS};
         hhs_subtree_kernel<<<1, SUB_M, 0, st>>>(sa);
         ctx->launches++;
         CU_TRY(ctx, cudaGetLastError());

@@ -23,6 +23,7 @@ struct SubArgs {
     double* dt0;                     // per-particle level-0 time-step; written when depth0 == 0
     const double* dt_cap;            // optional further criteria at level 0 (reading H4)
     double G, eps2, eta_ff, eta_fb, tau;
+    double crit_eta, crit_eta_grad, crit_eta_jerk;   // Eq. 24-29 at every level (bifrost_set_level_criteria); all 0: off
     int depth0, max_depth;
     long long* log;                  // device log [log_cap][3] of (depth, |S|, |F|), in the order the levels are entered
     long long log_cap;
@@ -33,6 +34,7 @@ struct SubState {                    // shared memory; indexed by SLOT = positio
     double x[SUB_M], y[SUB_M], z[SUB_M], vx[SUB_M], vy[SUB_M], vz[SUB_M], ms[SUB_M], dt0[SUB_M];
     double ax[SUB_M], ay[SUB_M], az[SUB_M];         // inter-level accelerations (Eq. 12), rows of the current level
     double gx[SUB_M], gy[SUB_M], gz[SUB_M];         // inter-level gradient sums (Eq. 13)
+    double jx[SUB_M], jy[SUB_M], jz[SUB_M];         // jerks of the level's particles (per-level criteria only)
     double rec[SUB_M * 10];                         // packed records of the current operation, by list position
     int id[SUB_M];                                  // particle id of a slot
     int ord[SUB_M];                                 // slot at list position k (the order list, local copy)
@@ -82,6 +84,7 @@ __global__ void __launch_bounds__(SUB_M)
 hhs_subtree_kernel(const SubArgs a) {
     using PA = AccPassT<false>;
     using PG = GradPassT<false>;
+    using PJ = GradPassT<false, true>;      // acceleration + jerk in one pass (bifrost_acc_jerk's policy)
     __shared__ SubState s;
     const int t = threadIdx.x;
     const int lane = t & 31, warp = t >> 5;
@@ -166,6 +169,31 @@ hhs_subtree_kernel(const SubArgs a) {
             rx[i] = a.G * fma(-3.0, c.wx, c.ux); ry[i] = a.G * fma(-3.0, c.wy, c.uy); rz[i] = a.G * fma(-3.0, c.wz, c.uz);
         }
     };
+    // Eq. 6 and Eq. 28 of the positions [lo, hi) among themselves in one pass (acc_jerk_impl's arithmetic): accelerations into
+    // (ax, ay, az), jerks into (jx, jy, jz) of their slots
+    auto acc_jerk_set = [&](int lo, int hi) {
+        const int m = hi - lo;
+        __syncthreads();
+        if (t < m) {
+            const int i = s.ord[lo + t];
+            PJ::Raw w{s.x[i], s.y[i], s.z[i], s.vx[i], s.vy[i], s.vz[i], s.ms[i], -1};
+            PJ::emit(w, reinterpret_cast<double2*>(s.rec + t * PJ::REC));
+        }
+        __syncthreads();
+        if (t < m) {
+            const int i = s.ord[lo + t];
+            PJ::Sink sk{s.x[i], s.y[i], s.z[i], s.vx[i], s.vy[i], s.vz[i], 0};
+            PJ::Acc c; PJ::init(c);
+            for (int j = 0; j < m; ++j) {
+                double r[PJ::REC];
+#pragma unroll
+                for (int q = 0; q < PJ::REC; ++q) r[q] = s.rec[j * PJ::REC + q];
+                PJ::pair(ga, sk, c, r);
+            }
+            s.jx[i] = a.G * fma(-3.0, c.wx, c.ux); s.jy[i] = a.G * fma(-3.0, c.wy, c.uy); s.jz[i] = a.G * fma(-3.0, c.wz, c.uz);
+            s.ax[i] = a.G * c.ax; s.ay[i] = a.G * c.ay; s.az[i] = a.G * c.az;
+        }
+    };
     // v += h (acc + c grad) for the positions [lo, hi) (kick_kernel's operations)
     auto kick = [&](int lo, int hi, const double* qx, const double* qy, const double* qz, const double* hx, const double* hy,
                     const double* hz, double h, double cc) {
@@ -213,11 +241,28 @@ hhs_subtree_kernel(const SubArgs a) {
         if (stage == 0) {
             // time-steps of the level's particles among themselves, slow / fast split (stable, S first)
             const bool all_slow = depth >= a.max_depth;
+            const bool crit = a.crit_eta > 0.0 && !all_slow;
+            if (crit) {     // Eq. 24-29 over the level's own particles: (ax..), (jx..), then C into (gx..)
+                acc_jerk_set(lo, hi);
+                grad_rows(lo, hi, hi, false, s.ax, s.ay, s.az, bx, by, bz);
+                __syncthreads();
+            }
             int fast = 0, slot = 0;
             if (t < m) {
                 slot = s.ord[lo + t];
                 if (!all_slow) {
                     double dt = sub_dtmin(s, a, slot, lo, hi);
+                    if (crit) {     // criteria_kernel's operations
+                        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+                        auto norm = [](double p0, double p1, double p2) {
+                            return sqrt(__dadd_rn(__dadd_rn(__dmul_rn(p0, p0), __dmul_rn(p1, p1)), __dmul_rn(p2, p2)));
+                        };
+                        const double v = norm(s.vx[slot], s.vy[slot], s.vz[slot]), ac = norm(s.ax[slot], s.ay[slot], s.az[slot]);
+                        const double gp = norm(bx[slot], by[slot], bz[slot]) / 24.0, jk = norm(s.jx[slot], s.jy[slot], s.jz[slot]);
+                        dt = fmin(dt, (ac == 0.0) ? inf : __dmul_rn(a.crit_eta, v) / ac);
+                        dt = fmin(dt, fmin((gp == 0.0) ? inf : a.crit_eta_grad * cbrt(v / gp), (gp == 0.0) ? inf : a.crit_eta_grad * sqrt(ac / gp)));
+                        dt = fmin(dt, (jk == 0.0) ? inf : __dmul_rn(a.crit_eta_jerk, ac) / jk);
+                    }
                     if (depth == 0) { if (a.dt_cap) dt = fmin(dt, a.dt_cap[s.id[slot]]); s.dt0[slot] = dt; }
                     dt = fmin(dt, s.dt0[slot]);
                     fast = dt < tau ? 1 : 0;

@@ -1453,6 +1453,13 @@ def test_hhs_fsi_per_level_criteria(torch):
         summ, log = c.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=6, log_cap=len(ref) + 64)
         assert summ["levels"] == len(ref) and np.array_equal(log, ref)
         assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
+        # the same with every level steered from the host (no single-CTA subtree launches): same hierarchy, same state
+        c.set_tuning(Context.TUNE_SMALL_M, 0)
+        pos, vel = dev(torch, pos0), dev(torch, vel0)
+        summ_h, log_h = c.hhs_fsi(pos, vel, m, G, eps_soft, eta, eta, tau, max_depth=6, log_cap=len(ref) + 64)
+        assert summ_h == summ and np.array_equal(log_h, ref)
+        assert _state_err(pos.cpu().numpy(), vel.cpu().numpy(), rp, rv) < 1e-12
+        c.set_tuning(Context.TUNE_SMALL_M, 128)
         with pytest.raises(BifrostError):
             c.set_level_criteria(0.1, 0.0, 0.1)                        # all three or none
         c.set_level_criteria(0.0, 0.0, 0.0)
