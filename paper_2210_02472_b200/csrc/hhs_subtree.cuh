@@ -8,7 +8,9 @@
 // recursion as an explicit stack of frames, a barrier between the stages.  Arithmetic and summation order are those of
 // the general path (AccPass / GradPass ::pair over the level's list in list order; kicks and drifts in the same IEEE
 // operations; the same stable partitions of the order list), and the time-steps are the exact Eq. 21-22 minima, so the
-// state after the interval and the level log are bit-identical to the host-steered path (tested).
+// state after the interval and the level log are bit-identical to the host-steered path (tested).  With
+// bifrost_set_level_criteria the level's own accelerations, jerks (acc_jerk's pair arithmetic) and gradient sums are formed at
+// every level as well and Eq. 24-29 enter the level's time-steps in criteria_kernel's operations.
 #pragma once
 
 namespace {
