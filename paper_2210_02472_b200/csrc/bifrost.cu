@@ -80,7 +80,7 @@ struct bifrost_ctx {
     double few_max_pairs[3] = {524288.0, 262144.0, 262144.0};   // (acc, grad, dtmin; BIFROST_TUNE_FEW_MAX_SINKS / _FEW_MAX_PAIRS; 0 sinks
                                      // disables; measured: profiles/r2_sweep_small_sets.md)
     int few_pairs_per_thread = 4;    // the cluster grows (1, 2, .. few_max_cl CTAs) until a thread has at most this many pairs
-    int few_max_cl[3] = {0, 0, 0};   // largest cluster the device accepts for the acc / grad / dtmin instance (0: not asked yet)
+    int few_max_cl[4] = {0, 0, 0, 0};   // largest cluster the device accepts for the acc / grad / dtmin / acc+jerk instance (0: not asked yet)
     bool fused_cluster = true;       // pair_fused_kernel as clusters with a DSMEM reduction (BIFROST_TUNE_FUSED_CLUSTER: 0 / 1)
     int64_t mutual_min_b = 512;      // bifrost_*_mutual: shortest shorter list / fewest pairs for the two-list symmetric kernel
     double mutual_min_pairs = 5e7;   // (below: two plain calls)
@@ -306,7 +306,7 @@ int run_pass(bifrost_ctx* ctx, const typename P::Args& a, const SrcArrays& src, 
 
 // A handful of sinks (few_sinks.cuh): one thread-block cluster, threads over the sources, results merged through shared and
 // distributed shared memory - no workspace, one launch.  Returns 1 when the call does not qualify.
-template <class F, int WHICH>
+template <class F, int WHICH, int CLIDX = WHICH>
 int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, int64_t n_sink, int64_t n_src, int compact,
              cudaStream_t st) {
     // 33-128 sinks against at most 16384 sources: one cluster per 32 sinks (config 2: acc 13.4-15.2 -> 11.0 us, grad 16.8-18.0 ->
@@ -319,7 +319,7 @@ int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, 
     // tiles one source after the other: 1 sink x 2^20 sources 264 -> 105 us, 4 sinks x 2^18 sources 71 -> 47 us)
     if (!groups && (double)n_sink * (double)n_src > ctx->few_max_pairs[WHICH] * (n_sink <= 8 ? 4.0 : 1.0)) return 1;
     auto kern = few_sinks_kernel<F>;
-    if (ctx->few_max_cl[WHICH] == 0) {          // once per context and instance: may a cluster have 16 CTAs here?
+    if (ctx->few_max_cl[CLIDX] == 0) {          // once per context and instance: may a cluster have 16 CTAs here?
         int max_cl = 8;                         // the portable size
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
             cudaLaunchConfig_t q = {};
@@ -332,14 +332,14 @@ int few_impl(bifrost_ctx* ctx, const typename F::Args& a, const SrcArrays& src, 
             if (cudaOccupancyMaxActiveClusters(&n_clusters, kern, &q) == cudaSuccess && n_clusters >= 1) max_cl = FEW_MAX_CL;
         }
         (void)cudaGetLastError();
-        ctx->few_max_cl[WHICH] = max_cl;
+        ctx->few_max_cl[CLIDX] = max_cl;
     }
     int nsp = 1;
     while (nsp < n_sink && nsp < FEW_MAX_SINKS) nsp *= 2;
     const int n_groups = ceil_div(n_sink, nsp);
     const int n_tiles = ceil_div(n_src, FEW_T);
     int cl = 1;
-    while (cl * 2 <= ctx->few_max_cl[WHICH] && cl * 2 <= n_tiles &&
+    while (cl * 2 <= ctx->few_max_cl[CLIDX] && cl * 2 <= n_tiles &&
            (int64_t)cl * FEW_T * ctx->few_pairs_per_thread < (int64_t)nsp * n_src)
         cl *= 2;
     cudaLaunchConfig_t cfg = {};
@@ -526,6 +526,10 @@ int acc_jerk_impl(bifrost_ctx* ctx, int64_t n, const double* pos, const double* 
     double* p1 = (double*)ctx->partial;
     double* p2 = (double*)((char*)ctx->partial + ctx->partial_bytes / 2);
     const GradArgs a{pos, vel, sub, sink_idx, soft2(eps), G, out_jerk, p1, out_acc, p2};
+    if (!sub) {                                             // a handful of sinks: one cluster launch (grad's thresholds)
+        const int rc = few_impl<FewAccJerk, 1, 3>(ctx, a, src, n_sink, n_src, 0, st);
+        if (rc <= 0) return rc;
+    }
     using Big = Shape<4, 256, 1, 2>;
     using F4 = Shape<4, 128, 2, 2>;       // 9 accumulators per sink: two CTAs per SM keep it out of local memory
     using F2 = Shape<2, 128, 4, 2>;

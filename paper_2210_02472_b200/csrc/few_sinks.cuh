@@ -12,7 +12,7 @@
 // memory in warp order, the CL CTAs of the cluster through DISTRIBUTED shared memory (CTA 0 reads the other CTAs' results,
 // spread over its threads, and merges them the same way) - and CTA 0 writes the outputs: no workspace in global memory, no
 // ticket, no fence, no second launch; bit-reproducible.
-//   acc, grad : the pair arithmetic of AccPassT / GradPassT (policies.cuh), partial sums added in the order above;
+//   acc, grad, jerk, acc + jerk : the pair arithmetic of AccPassT / GradPassT (policies.cuh), partial sums added in the order above;
 //   dtmin     : DtPassT's refined keys for every pair, merged by selects (a key clear of the other by the band decides); a
 //               near-tie anywhere flags the sink, and a flagged sink is settled by an exact scan: the exact (time-step, id)
 //               minimum, whatever the order.
@@ -84,6 +84,44 @@ struct FewGrad {
     __device__ __forceinline__ static void write(const Args& a, int row, int, const Val& v, int) {
         double* o = a.out + 3 * (size_t)row;
         o[0] = a.G * v.x; o[1] = a.G * v.y; o[2] = a.G * v.z;
+    }
+};
+
+// acceleration (Eq. 6) and jerk (Eq. 28) in one pass (bifrost_acc_jerk): GradPassT<false, true> over (x, v, m) records
+struct FewVec6 {
+    double x, y, z, u, v, w;
+    __device__ __forceinline__ FewVec6 shfl_xor(int off) const {
+        return FewVec6{__shfl_xor_sync(0xffffffffu, x, off), __shfl_xor_sync(0xffffffffu, y, off), __shfl_xor_sync(0xffffffffu, z, off),
+                       __shfl_xor_sync(0xffffffffu, u, off), __shfl_xor_sync(0xffffffffu, v, off), __shfl_xor_sync(0xffffffffu, w, off)};
+    }
+};
+
+struct FewAccJerk {
+    using P = GradPassT<false, true>;
+    using Args = GradArgs;
+    static constexpr int REC = P::REC;
+    using Raw = P::Raw;
+    using Sink = P::Sink;
+    using State = P::Acc;
+    using Val = FewVec6;                     // jerk (x, y, z), acceleration (u, v, w)
+    __device__ __forceinline__ static void fetch(const SrcArrays& s, int j, Raw& w) { P::fetch(s, j, w); }
+    __device__ __forceinline__ static void emit(const Raw& w, double2* o) { P::emit(w, o); }
+    __device__ __forceinline__ static void load_sink(const Args& a, int id, Sink& s) { P::load_sink(a, id, s); }
+    __device__ __forceinline__ static void init(State& c) { P::init(c); }
+    __device__ __forceinline__ static void pair(const Args& a, const Sink& s, State& c, const double* __restrict__ r) { P::pair(a, s, c, r); }
+    __device__ __forceinline__ static Val value(const State& c) {
+        return Val{fma(-3.0, c.wx, c.ux), fma(-3.0, c.wy, c.uy), fma(-3.0, c.wz, c.uz), c.ax, c.ay, c.az};
+    }
+    __device__ __forceinline__ static Val identity() { return Val{0.0, 0.0, 0.0, 0.0, 0.0, 0.0}; }
+    __device__ __forceinline__ static void merge(const Args&, int, Val& c, const Val& o) {
+        c.x += o.x; c.y += o.y; c.z += o.z; c.u += o.u; c.v += o.v; c.w += o.w;
+    }
+    __device__ __forceinline__ static void settle(const Args&, const SrcArrays&, int, int, int, Val*, Val (*)[FEW_MAX_SINKS]) {}
+    static constexpr int PARTS = 2;          // one thread writes the jerk, one the acceleration
+    __device__ __forceinline__ static void write(const Args& a, int row, int, const Val& v, int part) {
+        double* o = (part == 0 ? a.out : a.out2) + 3 * (size_t)row;
+        if (part == 0) { o[0] = a.G * v.x; o[1] = a.G * v.y; o[2] = a.G * v.z; }
+        else { o[0] = a.G * v.u; o[1] = a.G * v.v; o[2] = a.G * v.w; }
     }
 };
 

@@ -1294,6 +1294,19 @@ def test_few_sinks_cluster_kernel(torch, ctx, ctx_nofew, n_sink, n_src):
         ra, rc = oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), oracle.grad(w.pos, w.mass, acc_full, w.G, w.eps, sinks, srcs)
         assert np.abs(a - ra).max() <= 1e-12 * np.abs(ra).max() and np.abs(c - rc).max() <= 1e-12 * np.abs(rc).max()
     check_dt(d, oracle.dtmin(w.pos, w.vel, w.mass, w.G, w.eta_ff, w.eta_fb, sinks, srcs), "few dtmin")
+    # acceleration + jerk in one pass takes the same kernel (grad's limits)
+    l0 = ctx.launch_count
+    aj, jj = ctx.acc_jerk(dev(torch, w.pos), dev(torch, w.vel), dev(torch, w.mass), w.G, w.eps, dev(torch, sinks),
+                          None if srcs is None else dev(torch, srcs))
+    torch.cuda.synchronize()
+    assert ctx.launch_count - l0 == 1
+    ra, rj = oracle.acc(w.pos, w.mass, w.G, w.eps, sinks, srcs), oracle.jerk(w.pos, w.vel, w.mass, w.G, w.eps, sinks, srcs)
+    aj, jj = aj.cpu().numpy()[sinks], jj.cpu().numpy()[sinks]
+    if n_sink * n_src >= 64:
+        check_vec(aj, ra, "few acc (acc+jerk)")
+        check_vec(jj, rj, "few jerk (acc+jerk)")
+    else:
+        assert np.abs(aj - ra).max() <= 1e-12 * np.abs(ra).max() and np.abs(jj - rj).max() <= 1e-12 * np.abs(rj).max()
     a2, c2, d2, _ = run_all(torch, ctx_nofew, w, sinks, srcs, acc_full=acc_full)
     assert all(np.array_equal(x, y) for x, y in zip(d, d2))
     assert np.abs(a - a2).max() <= 1e-13 * np.abs(a2).max() and np.abs(c - c2).max() <= 1e-13 * np.abs(c2).max()
